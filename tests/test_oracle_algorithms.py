@@ -1,0 +1,254 @@
+"""Pins of the oracle's Algorithm 1 / Algorithm 2 against the paper's worked example, brute force,
+HiGHS, hand-computed constants and equivariances (CPU only).  P:<line> = /root/reference/PAPER.md."""
+import itertools
+import os
+
+import numpy as np
+import pytest
+import scipy.optimize as so
+import scipy.sparse as sp
+
+import oracle
+from paper_2103_00736_b200 import workloads as W
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _golden(name):
+    out = {}
+    with open(os.path.join(HERE, "golden", name)) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                out[k] = float(v)
+    return out
+
+
+def brute_force_lp(A, b, c):
+    """min c'x s.t. Ax=b, x>=0 by enumerating all bases (tiny problems only)."""
+    m, n = A.shape
+    best = None
+    for B in itertools.combinations(range(n), m):
+        AB = A[:, B]
+        if abs(np.linalg.det(AB)) < 1e-12:
+            continue
+        xB = np.linalg.solve(AB, b)
+        if (xB < -1e-10).any():
+            continue
+        val = c[list(B)] @ xB
+        if best is None or val < best[0] - 1e-12:
+            x = np.zeros(n)
+            x[list(B)] = xB
+            y = np.linalg.solve(AB.T, c[list(B)])
+            best = (val, x, y, c - A.T @ y)
+    return best
+
+
+def _problem_from_dense(A, b, c, n_lin, soc, **kw):
+    S = sp.csr_matrix(A)
+    S.sort_indices()
+    nanv = lambda k: np.full(k, np.nan)
+    return W.Problem(name="adhoc", m=A.shape[0], n=A.shape[1], row_ptr=S.indptr.astype(np.int32),
+                     col_idx=S.indices.astype(np.int32), val=S.data.copy(), b=b, c=c, n_lin=n_lin,
+                     soc_size=np.asarray(soc, np.int32), x0=nanv(A.shape[1]), y0=nanv(A.shape[0]),
+                     s0=nanv(A.shape[1]), **kw)
+
+
+# ------------------------------------------------------------------ worked example
+def test_worked_example_condition_numbers_and_optimum():
+    g = _golden("worked_example.txt")
+    A = W.WORKED_A
+    assert np.isclose(np.linalg.cond(A), g["cond_A"], rtol=1e-4)
+    ASK = np.diag(W.WORKED_D_SK) @ A @ np.diag(W.WORKED_E_SK)      # A_hat = D A E, eq.(4)
+    assert np.isclose(np.linalg.cond(ASK), g["cond_A_SK"], rtol=1e-3)  # D,E printed to 4 digits
+    assert np.isclose(np.linalg.cond(A @ np.diag(W.WORKED_E_AC)), g["cond_A_AC"], rtol=1e-4)
+
+    val, xs, ys, zs = brute_force_lp(A, W.WORKED_B, W.WORKED_C)
+    res = so.linprog(W.WORKED_C, A_eq=A, b_eq=W.WORKED_B, bounds=(0, None), method="highs")
+    assert np.isclose(res.fun, val, rtol=1e-8)
+
+    p = W.worked_example()
+    # Algorithm 1 (mu=1, s0=0): O = I throughout
+    o = oracle.Oracle.from_problem(p)
+    o.run(3000)
+    gt = o.get()
+    assert np.allclose(gt["x"], xs, atol=1e-8) and np.allclose(gt["z"], zs, atol=1e-8)
+    assert np.allclose(gt["y"], ys, atol=1e-6)
+    assert o.residuals()["kkt_rel"] < 1e-10
+    # E^AC as a FIXED column scaling (eq.(4)-(5) with D=I, E=E^AC): same optimum, much faster (Fig.1(c))
+    its = {}
+    for name, E in (("none", np.ones(5)), ("ac", W.WORKED_E_AC)):
+        o = oracle.Oracle.from_problem(p)
+        o.set_point(np.zeros(5), np.zeros(5))     # s0 = 0 in either scaling
+        o.set_scaling(E)
+        k = 0
+        while np.linalg.norm(o.get()["x"] - xs) > 1e-4 and k < 2000:
+            o.run_fixed(1)
+            k += 1
+        its[name] = k
+        assert k < 2000
+    assert its["ac"] <= 5 and its["ac"] * 5 < its["none"]
+
+
+# ------------------------------------------------------------------ tiny LPs vs brute force and HiGHS
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_tiny_lp_matches_vertex_enumeration(seed):
+    rng = np.random.default_rng(seed)
+    m, n = 4, 9
+    A = rng.standard_normal((m, n))
+    x0, s0 = rng.random(n), np.zeros(n)
+    zero = rng.permutation(n)[: n - m]         # non-degenerate vertex: exactly m positive entries
+    x0[zero] = 0.0
+    s0[zero] = rng.random(n - m) + 0.1
+    b, c = A @ x0, A.T @ rng.standard_normal(m) + s0
+    val, xs, ys, zs = brute_force_lp(A, b, c)
+    p = _problem_from_dense(A, b, c, n, [])
+    for L in ((), (50, 100, 150)):
+        o = oracle.Oracle.from_problem(p)
+        o.run(4000, L=L)
+        g, r = o.get(), o.residuals()
+        assert r["kkt_rel"] < 1e-9
+        assert np.isclose(r["pobj"], val, atol=1e-8) and np.isclose(r["dobj"], val, atol=1e-8)
+        assert np.allclose(g["x"], xs, atol=1e-7) and np.allclose(g["z"], zs, atol=1e-7)
+        assert np.allclose(g["y"], ys, atol=1e-6)
+
+
+def test_config0_reaches_constructed_optimum_and_highs_value():
+    p = W.config(0)
+    res = so.linprog(p.c, A_eq=p.csr().toarray(), b_eq=p.b, bounds=(0, None), method="highs")
+    assert np.isclose(res.fun, p.opt_value(), rtol=1e-9)
+    ends = {}
+    for mode in (1, 2):
+        o = oracle.Oracle.from_problem(p, solve_mode=mode)
+        o.run(500, L=p.schedule(500))
+        g, r = o.get(), o.residuals()
+        assert r["kkt_rel"] < 1e-8
+        assert np.isclose(r["pobj"], p.opt_value(), atol=1e-7)
+        assert np.allclose(g["z"], p.s0, atol=1e-6) and np.allclose(g["y"], p.y0, atol=1e-6)  # unique
+        ends[mode] = g
+    assert np.linalg.norm(ends[1]["x"] - ends[2]["x"]) <= 1e-8 * np.linalg.norm(ends[1]["x"])  # Cholesky == PCG
+
+
+# ------------------------------------------------------------------ conditioning rule, hand-computed
+def test_conditioning_rule_hand_example():
+    """K = R_+ x K_3.  x=(4 | 6,3,4), z=(0.5 | 2,.,.): o = (4/0.5, (6-5)/2) = (8, 0.5);
+    spread = ln 16; t = ln 4 => alpha = 1/2 => O = (sqrt 8 | sqrt .5 x3)."""
+    rng = np.random.default_rng(0)
+    A = rng.standard_normal((2, 4))
+    x = np.array([4.0, 6.0, 3.0, 4.0])
+    z = np.array([0.5, 2.0, 0.3, -0.1])
+    p = _problem_from_dense(A, A @ x, rng.standard_normal(4), 1, [3], t=np.log(4.0))
+    o = oracle.Oracle.from_problem(p)
+    o.set_point(x, z)
+    o.run(1)
+    O = o.get()["O"]
+    assert np.allclose(O, [np.sqrt(8.0)] + [np.sqrt(0.5)] * 3, rtol=1e-14)
+    # cap not active (t large): O = o exactly
+    p2 = _problem_from_dense(A, A @ x, p.c, 1, [3], t=50.0)
+    o2 = oracle.Oracle.from_problem(p2)
+    o2.set_point(x, z)
+    o2.run(1)
+    assert np.allclose(o2.get()["O"], [8.0, 0.5, 0.5, 0.5], rtol=1e-14)
+    # default start e_K gives O = I (reading (j),(h))
+    o3 = oracle.Oracle.from_problem(p)
+    o3.run(1)
+    assert np.array_equal(o3.get()["O"], np.ones(4))
+
+
+def test_step14_recast_keeps_xz_and_cap_holds():
+    """Step 14 s = O^-1 x - mu O z continues 'current progress': right after a
+    conditioning, abs_K(s) and s give back the same proj_K parts; and ln(max O/min O) <= t."""
+    p = W.gaussian_dense_lp(3)
+    o = oracle.Oracle.from_problem(p)
+    o.run(40, L=[40])
+    g = o.get()
+    assert np.log(g["O"].max() / g["O"].min()) <= p.t * (1 + 1e-12)
+    assert g["O"].min() > 0
+
+
+# ------------------------------------------------------------------ row-scaling invariance (derived)
+def test_row_scaling_is_inert():
+    p = W.sparse_lp(21, 25, 60, 4)
+    D = 10.0 ** np.random.default_rng(1).uniform(-2, 2, p.m)
+    A = p.csr().toarray()
+    p2 = _problem_from_dense(D[:, None] * A, D * p.b, p.c, p.n, [])
+    runs = []
+    for q in (p, p2):
+        o = oracle.Oracle.from_problem(q)
+        o.run(60, L=[30])
+        runs.append(o.get())
+    for k in ("s", "x", "z", "O"):
+        assert np.linalg.norm(runs[0][k] - runs[1][k]) <= 1e-9 * np.linalg.norm(runs[0][k])
+
+
+# ------------------------------------------------------------------ size-2 cones = rotated orthant
+def test_size2_soc_equals_rotated_lp():
+    """K_2 = {x1 >= |x2|} = Q R^2_+ with Q = [[1,1],[1,-1]]/sqrt2; Algorithm 1 is equivariant under the
+    orthogonal change x -> Qx, A -> AQ', c -> Qc, so Q s_soc^l = s_lp^l for all l (L = {})."""
+    rng = np.random.default_rng(5)
+    m, n = 5, 12
+    A = rng.standard_normal((m, n))
+    Q = np.kron(np.eye(n // 2), np.array([[1.0, 1.0], [1.0, -1.0]]) / np.sqrt(2.0))
+    xl = rng.random(n)                          # LP-feasible point => SOC-feasible Q'xl
+    c_lp = (A @ Q.T).T @ rng.standard_normal(m) + rng.random(n)   # dual feasible => bounded LP
+    c = Q.T @ c_lp
+    # SOC problem (A, b, c, K_2^6) ; LP problem (A Q', b, Q c, R^12_+) with x_lp = Q x_soc
+    ps = _problem_from_dense(A, A @ (Q.T @ xl), c, 0, [2] * 6)
+    pl = _problem_from_dense(A @ Q.T, A @ (Q.T @ xl), Q @ c, n, [])
+    os_, ol = oracle.Oracle.from_problem(ps), oracle.Oracle.from_problem(pl)
+    # same start in both coordinate systems: s = 0  (x=z=e_K maps differently, so set points explicitly)
+    x_soc = np.tile([1.0, 0.0], 6)
+    os_.set_point(x_soc, x_soc)
+    ol.set_point(Q @ x_soc, Q @ x_soc)
+    os_.set_scaling(np.ones(n))
+    ol.set_scaling(np.ones(n))
+    for l in range(200):
+        os_.run_fixed(1)
+        ol.run_fixed(1)
+        if l % 20 == 0 or l == 199:
+            a, bq = Q @ os_.get()["s"], ol.get()["s"]
+            assert np.linalg.norm(a - bq) <= 1e-10 * (1 + np.linalg.norm(bq))
+    val = brute_force_lp(pl.csr().toarray(), pl.b, pl.c)[0]
+    os_.run_fixed(5000)
+    assert np.isclose(os_.residuals()["pobj"], val, atol=1e-7)
+
+
+# ------------------------------------------------------------------ qualitative claims
+def test_section4a_one_conditioning_helps():
+    """L={} stalls, L={300} 'significant improvement', L={1..50} fast (Fig.2)."""
+    worse = 0
+    for seed in range(3):
+        p = W.gaussian_dense_lp(100 + seed)
+        res = {}
+        for name, L, k in (("none", (), 1500), ("one", (300,), 1500), ("cont", tuple(range(1, 51)), 300)):
+            o = oracle.Oracle.from_problem(p)
+            ones = np.ones(p.n)
+            o.set_point(ones, ones)
+            o.run(k, L=L)
+            res[name] = o.residuals()["pres_abs"]
+        assert res["one"] < 1e-2 * res["none"]
+        assert res["cont"] < 1e-2 * res["none"]
+
+
+@pytest.mark.parametrize("h", [4, 10])
+def test_section5d_socp_converges_with_and_without_conditioning(h):
+    """P:364-377 shape (n=100): both schedules reach the same optimal value, KKT -> 0."""
+    p = W.dense_socp_sec5d(7, n=100, h=h)
+    vals = []
+    for L in ((), tuple(range(200, 3001, 100))):
+        o = oracle.Oracle.from_problem(p)
+        o.run(3000, L=L)
+        r = o.residuals()
+        assert r["kkt_rel"] < 1e-7
+        vals.append(r["pobj"])
+    assert np.isclose(vals[0], vals[1], rtol=1e-6, atol=1e-7)
+
+
+def test_constructed_socp_reaches_known_value():
+    p = W.sparse_socp(9, 60, 160, 16, 5, n_lin=0, lo=3, hi=20)
+    o = oracle.Oracle.from_problem(p)
+    o.run(3000, L=p.schedule(3000))
+    r = o.residuals()
+    assert r["kkt_rel"] < 1e-7
+    assert np.isclose(r["pobj"], p.opt_value(), rtol=1e-6, atol=1e-6)
+    assert np.isclose(r["dobj"], p.opt_value(), rtol=1e-6, atol=1e-6)
