@@ -1,0 +1,272 @@
+#!/usr/bin/env python
+"""bench.py -- outer iterations/s of Algorithm 2 (arXiv 2103.00736) through libcs.so on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4] [--k 5]
+
+A *step* is one pass of the whole hot path over one resident problem:
+    cs_condition()  ->  cs_iterate(k)  ->  cs_residuals()
+i.e. steps 5-14, k x steps 16-18 (each with its inner CG solve) and the KKT norms with their single
+read-back.  `value` = outer iterations/s with the problem resident in HBM; `e2e` = the same metric with
+cs_create from pinned HOST buffers (H2D of A, b, c), the same calls, and cs_solution to HOST buffers
+inside the timed region.  Multi-GPU: "replicas only" (the path does not shard without a per-CG-step
+all-reduce): rank r runs an independent replica on GPU r, value = sum over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2103_00736_b200 import workloads as W  # noqa: E402
+
+METRIC = "outer_iterations_per_s"
+UNIT = "iterations/s"
+
+
+def algorithmic_bytes(p, k_iter, cg_steps, n_cond):
+    """Bytes the method must move: int32 indices, fp64 values, each
+    gathered vector counted once per pass."""
+    nnz, n, m = p.nnz, p.n, p.m
+    cg = 24 * nnz + 28 * n + 60 * m          # K1 (CSC pass) + K2 (CSR pass) of one CG step
+    outer = 24 * nnz + 92 * n + 24 * m       # cone reflect + rhs pass + final A'w pass with the s-update
+    cond = 64 * nnz + 80 * n + 40 * m        # row norms, rescale of both copies, d/s recast (solve counted in cg)
+    return cg * cg_steps + outer * k_iter + cond * n_cond, cg
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.idx = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(cfg, scale, steps, warmup):
+    """The oracle as it stands on a bounded sample: the same recipe at `scale`, one pass per step;
+    iterations/s extrapolated to full size linearly in nnz (stated in `sample`)."""
+    import oracle
+    full_nnz = {0: 999, 1: 250_000, 2: 2_000_000, 3: 4_000_000, 4: 33_000_000}[cfg]
+    p = W.config(cfg, scale)
+    O = oracle.Oracle.from_problem(p)
+    O.run(max(1, warmup))
+    t0 = time.perf_counter()
+    O.run(max(1, steps))
+    dt = time.perf_counter() - t0
+    its = max(1, steps) / dt
+    ratio = min(1.0, p.nnz / full_nnz)
+    return {"value": its * ratio, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{p.name}: m={p.m} n={p.n} nnz={p.nnz}, {max(1, steps)} passes in {dt:.2f}s = {its:.3f} it/s on the "
+                      f"replica, scaled by nnz ratio {ratio:.4g} to the full config (CG-step growth with size ignored)",
+            "pcg_steps_per_pass": O.counters()["pcg_steps_total"] / (max(1, warmup) + max(1, steps))}, dt
+
+
+ORACLE_SCALE = {0: 1.0, 1: 1.0, 2: 0.05, 3: 0.1, 4: 0.02}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--scale", type=float, default=1.0)
+    ap.add_argument("--k", type=int, default=5, help="outer iterations per step")
+    ap.add_argument("--e2e-steps", type=int, default=1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    a = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if a.impl == "reference":
+        if rank != 0:
+            return 0
+        base, dt = oracle_sample(a.config, ORACLE_SCALE[a.config] * a.scale, a.steps, a.warmup)
+        line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": a.gpus,
+                "steps": a.steps, "warmup": a.warmup, "ms_per_step": 1e3 * dt / max(1, a.steps),
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"cfg{a.config}"}, "cpu_baseline": base,
+                "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return 0
+
+    import torch
+    from paper_2103_00736_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    t_gen = time.perf_counter()
+    p = W.config(a.config, a.scale)
+    t_gen = time.perf_counter() - t_gen
+    stream = torch.cuda.current_stream()
+    S = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
+
+    def step():
+        S.condition()
+        S.iterate(a.k)
+        return S.residuals()
+
+    for _ in range(a.warmup):
+        step()
+    r0 = S.residuals()
+    l0 = S.kernel_launches()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(a.steps)]
+    e_all = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    torch.cuda.synchronize()
+    e_all[0].record(stream)
+    for i in range(a.steps):
+        S.condition()
+        ev[i][0].record(stream)
+        S.iterate(a.k)           # ONE launch of the dominant kernel k_iterate
+        ev[i][1].record(stream)
+        r1 = S.residuals()
+    e_all[1].record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clk = clocks.stop()
+    ms_total = e_all[0].elapsed_time(e_all[1])
+    ms_iter = sum(x.elapsed_time(y) for x, y in ev)
+    launches = S.kernel_launches() - l0
+    t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    n_it = a.steps * a.k
+    value = world * n_it / (ms_max * 1e-3)
+
+    # ---- roofline of the dominant kernel (k_iterate, one launch per step): algorithmic bytes of the K
+    # timed launches / their summed CUDA-event durations.  CG steps are data dependent, so they are read
+    # from the device counters (total minus those spent inside cs_condition).
+    cg_steps = r1["cg_steps_total"] - r0["cg_steps_total"]
+    cg_iter = cg_steps - (r1["cg_steps_cond"] - r0["cg_steps_cond"])
+    it_bytes, cg_bytes = algorithmic_bytes(p, n_it, cg_iter, 0)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    achieved = it_bytes / (ms_iter * 1e-3) / 1e9
+    roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+            "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
+            "cg_steps_per_launch": cg_iter / a.steps, "bytes_per_cg_step": cg_bytes,
+            "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "frac_of_8TBs": achieved / 8000.0,
+            "kernel_share_of_step": ms_iter / ms_total}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": p.name, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "k_per_step": a.k,
+                       "step": "cs_condition + cs_iterate(k) + cs_residuals", "multi_gpu": "replicas only",
+                       "l2": "inputs larger than L2" if 24 * p.nnz > 126e6 else "matrix fits in L2 (flagged)",
+                       "gen_s": round(t_gen, 2)},
+            "clocks": clk, "gpu_launches": int(launches), "kkt_rel": r1["kkt_rel"], "iter_total": r1["iter"],
+            "cg_steps_timed": int(cg_steps), "cg_steps_per_iter": cg_iter / n_it, "roofline": roof}
+    return finish(a, p, S, line, rank, world, dev, stream)
+
+
+def finish(a, p, S, line, rank, world, dev, stream):
+    import torch
+    from paper_2103_00736_b200 import binding
+    S.destroy()
+
+    # ---- e2e: host buffers in, host buffers out, everything inside the timed region
+    pin = lambda x: torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
+    hin = [pin(x) for x in (p.row_ptr, p.col_idx, p.val, p.b, p.c)]
+    hx, hz = torch.empty(p.n, dtype=torch.float64).pin_memory(), torch.empty(p.n, dtype=torch.float64).pin_memory()
+    h2d = sum(t.numel() * t.element_size() for t in hin)
+    d2h = 16 * p.n + 128
+    def e2e_step():
+        S2 = binding.Solver(p.m, p.n, hin[0].numpy(), hin[1].numpy(), hin[2].numpy(), hin[3].numpy(), hin[4].numpy(),
+                            p.n_lin, p.soc_size, stream=stream.cuda_stream)
+        S2.set_params(mu=p.mu, t=p.t)
+        S2.iterate(a.k)
+        S2.condition()
+        S2.residuals()
+        S2.solution_into(x=hx.numpy(), z=hz.numpy())
+        S2.destroy()
+    e2e_step()  # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(a.e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    tt = torch.tensor([dt], device=dev, dtype=torch.float64)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    line["e2e"] = {"value": world * a.e2e_steps * a.k / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                   "d2h_bytes_per_step": int(d2h), "steps": a.e2e_steps,
+                   "step": "cs_create(host A,b,c) + cs_iterate(k) + cs_condition + cs_residuals + cs_solution(host x,z)"}
+    if rank == 0:
+        if not a.no_cpu_baseline and world == 1:
+            base, _ = oracle_sample(a.config, ORACLE_SCALE[a.config] * a.scale, 2, 1)
+            line["cpu_baseline"] = base
+        else:
+            line["cpu_baseline"] = None
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,146 @@
+/*
+ * cs.h -- C ABI of libcs.so: the B200 (sm_100a) hot path of arXiv 2103.00736, Algorithm 2
+ * (operator-splitting conic solver with adaptive conditioning).
+ *
+ *      minimise c'x  s.t.  Ax = b,  x in K = R^{n_lin}_+ x K_{q_1} x ... x K_{q_k}      (1) PAPER.md:41-56
+ *
+ * Citations "P:<line>" refer to /root/reference/PAPER.md.  Every step of the path (sparse products,
+ * cone reflections, the normal-equation solve hidden in A^dagger, the averaged update, residual norms,
+ * the conditioning rescale) runs in CUDA kernels on ONE device; there is no CPU fallback.
+ *
+ * Conventions
+ *   - All floating point is IEEE fp64.  Indices are int32, sizes int64.
+ *   - Every array argument is a plain pointer; where an argument can be host or device memory the
+ *     call takes a cs_mem tag saying which.  Host arrays may be pageable or pinned.
+ *   - Ownership: the library copies what it needs during the call and never keeps a caller pointer.
+ *     Outputs are written into caller-owned buffers.  The handle owns all its device memory.
+ *   - A handle is bound to the device that is current at cs_create and to the CUDA stream passed
+ *     there (NULL = legacy default stream).  It is not thread-safe.
+ *   - Errors: every call returns a cs_status; nothing throws or aborts across the ABI.  The text of
+ *     the last error of a handle is available from cs_last_error.
+ *   - Calls are asynchronous on the handle's stream unless stated otherwise.
+ */
+#ifndef CS_H_
+#define CS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cs_solver cs_solver; /* opaque */
+
+typedef enum {
+    CS_OK = 0,
+    CS_EINVAL = 1, /* NULL / shape / unsorted or duplicate CSR indices / cone sizes do not sum to n / empty row */
+    CS_ENOMEM = 2, /* host or device allocation failed                                                           */
+    CS_ECUDA = 3,  /* a CUDA runtime call failed; text in cs_last_error                                          */
+    CS_ESTATE = 4, /* call not valid in the current state                                                        */
+    CS_ECGMAX = 5  /* an inner CG solve hit cg_max_iter since the last cs_residuals (not fatal)                  */
+} cs_status;
+
+typedef enum { CS_HOST = 0, CS_DEVICE = 1 } cs_mem;
+
+/* A in CSR.  row_ptr[0] = 0, non-decreasing, row_ptr[m] = nnz; col_idx sorted and unique within a row;
+ * every row must hold at least one entry (A is assumed to have full row rank: the proofs use
+ * A A^dagger = I).  All three arrays live in the memory space named by `where`. */
+typedef struct {
+    int64_t m, n, nnz;
+    const int32_t *row_ptr; /* [m+1] */
+    const int32_t *col_idx; /* [nnz] */
+    const double *val;      /* [nnz] */
+    cs_mem where;
+} cs_csr;
+
+/* K: n_lin leading orthant coordinates (Lorentz cones of size 1) followed by n_soc Lorentz
+ * cones of sizes soc_size[i] >= 1; n_lin + sum soc_size == n.  soc_size is a HOST array (may be NULL
+ * when n_soc == 0). */
+typedef struct {
+    int64_t n_lin;
+    int64_t n_soc;
+    const int32_t *soc_size;
+} cs_cones;
+
+/* Parameters of Algorithm 2 (input line P:214-215) and of the inner solve.
+ *   mu       fixed mu > 0; the experiments use 1
+ *   t        cap on ln(max O / min O) in step 11; 9.2 for LP, 1.7 for SOCP
+ *   o_floor  absolute floor of numerator and denominator of o_i in step 7 (paper silent on 0/0)
+ *   cg_tol   inner solve stops when ||residual||_2 <= cg_tol * ||rhs||_2, both measured on the
+ *            row-equilibrated system (D A_hat)(D A_hat)' with D = diag(1/||row_i(A_hat)||_2)
+ *   cg_max_iter  cap on CG steps per solve
+ * cs_set_params may be called at any time; mu, t, o_floor take effect at the next cs_condition
+ * (or at the implicit first conditioning), cg_* at the next solve. */
+typedef struct {
+    double mu, t, o_floor, cg_tol;
+    int32_t cg_max_iter;
+    int32_t reserved;
+} cs_params;
+
+/* Residuals of the KKT conditions (24) P:480-487 in ORIGINAL coordinates, for the current iterate
+ * x = O(p+s)/2, z = O^{-1}(p-s)/(2mu) (steps 19-20) and y = D(w_d - w)/mu:
+ *   pres_abs = ||Ax-b||_2 (16a)      pres_rel = pres_abs/(1+||b||_2)
+ *   dres_abs = ||c-z-A'y||_2                dres_rel = dres_abs/(1+||c||_2)
+ *   gap_abs  = |c'x-b'y|  (cf. 16b)  gap_rel  = gap_abs/(1+|c'x|+|b'y|)
+ *   cone_viol_rel = (||x-proj_K x||_2+||z-proj_K z||_2)/(1+||x||_2+||z||_2)
+ *   kkt_rel  = max(pres_rel, dres_rel, gap_rel, cone_viol_rel)
+ *   pobj = c'x, dobj = b'y, fp_res = ||s_new - s||_2 of the last pass (Lemma 3b). */
+typedef struct {
+    int64_t iter;           /* passes of steps 16-18 done so far (l of Algorithm 2) */
+    int64_t cg_steps_total; /* CG steps over all solves so far                       */
+    int64_t cg_steps_cond;  /* ... of which inside cs_condition's solve for d         */
+    int32_t cg_steps_last;  /* CG steps of the most recent solve                     */
+    int32_t n_conditionings;
+    int32_t cg_hit_max;     /* 1 if some solve hit cg_max_iter since the last cs_residuals */
+    int32_t reserved;
+    double pres_abs, pres_rel, dres_abs, dres_rel, gap_abs, gap_rel, cone_viol_rel, kkt_rel, pobj, dobj, fp_res;
+} cs_resid;
+
+/* Build a solver for (A,b,c,K): validates the input, copies it to the device, builds the CSC copy of A
+ * and the work partitions.  b[m], c[n] live in `vec_where`.  Parameters start at mu=1, t=9.2 (n_soc=0)
+ * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-13, cg_max_iter=20000; the starting point is x=z=e_K
+ * (1 on each cone's first coordinate), which makes the mandatory first conditioning (l=1) the
+ * identity and s=0.  Synchronous.  On failure *out is NULL. */
+cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
+                    const cs_cones *K, void *cuda_stream);
+
+cs_status cs_set_params(cs_solver *S, const cs_params *p);
+cs_status cs_get_params(const cs_solver *S, cs_params *p);
+
+/* Starting point (x,z) of Algorithm 2, each [n] in `where`.  Only before the first
+ * cs_iterate / cs_condition (else CS_ESTATE). */
+cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem where);
+
+/* k passes of steps 16-18: p = abs_K(s); r = abs_{A_hat}(p); s = s/2 - r/2 + d.
+ * x,z of steps 19-20 are formed lazily by cs_condition / cs_residuals / cs_solution.  If no
+ * conditioning has happened yet, the l=1 conditioning of step 4 runs first.  One kernel launch for
+ * all k passes; no host synchronisation. */
+cs_status cs_iterate(cs_solver *S, int64_t k);
+
+/* Steps 5-14 from the current (x,z): o per cone, O = o^alpha, A_hat = D A O (D = row
+ * equilibration, mathematically inert), c_hat = O c, d, and the recast s = O^{-1}x - mu O z.
+ * The schedule L is the caller's: L = {300,400,...} is cs_iterate(299); cs_condition(); cs_iterate(100); ... */
+cs_status cs_condition(cs_solver *S);
+
+/* Replace step 5-11's rule by a caller-given positive diagonal O[n] (a FIXED preconditioner E of
+ * eq.(4)-(5)), then steps 12-14.  Block-constant O is the caller's responsibility. */
+cs_status cs_set_scaling(cs_solver *S, const double *O, cs_mem where);
+
+/* Residual norms of the current iterate; ONE device->host copy and a stream synchronisation.
+ * Returns CS_ECGMAX (with *out filled) if a solve hit cg_max_iter since the previous call. */
+cs_status cs_residuals(cs_solver *S, cs_resid *out);
+
+/* Copy out the current x[n], z[n], y[m], s[n], O[n] (original coordinates for x,z,y; scaled for s).
+ * Any pointer may be NULL.  Synchronous when where == CS_HOST. */
+cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where);
+
+/* Number of kernels the library has launched on this handle so far (for bench accounting). */
+int64_t cs_kernel_launches(const cs_solver *S);
+
+const char *cs_last_error(const cs_solver *S);
+void cs_destroy(cs_solver *S);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CS_H_ */

@@ -1,0 +1,214 @@
+"""ctypes binding of libcs.so (include/cs.h): same names, argument marshalling only.
+
+Arrays may be numpy arrays (host memory) or torch tensors (host or CUDA memory); the binding passes
+their raw pointers with the matching ``cs_mem`` tag.  There is NO fallback: if ``libcs.so`` is missing
+or cannot be loaded, importing the symbols raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcs.so")
+
+CS_OK, CS_EINVAL, CS_ENOMEM, CS_ECUDA, CS_ESTATE, CS_ECGMAX = range(6)
+CS_HOST, CS_DEVICE = 0, 1
+STATUS_NAMES = {0: "CS_OK", 1: "CS_EINVAL", 2: "CS_ENOMEM", 3: "CS_ECUDA", 4: "CS_ESTATE", 5: "CS_ECGMAX"}
+
+
+class cs_csr(C.Structure):
+    _fields_ = [("m", C.c_int64), ("n", C.c_int64), ("nnz", C.c_int64), ("row_ptr", C.c_void_p),
+                ("col_idx", C.c_void_p), ("val", C.c_void_p), ("where", C.c_int)]
+
+
+class cs_cones(C.Structure):
+    _fields_ = [("n_lin", C.c_int64), ("n_soc", C.c_int64), ("soc_size", C.c_void_p)]
+
+
+class cs_params(C.Structure):
+    _fields_ = [("mu", C.c_double), ("t", C.c_double), ("o_floor", C.c_double), ("cg_tol", C.c_double),
+                ("cg_max_iter", C.c_int32), ("reserved", C.c_int32)]
+
+
+class cs_resid(C.Structure):
+    _fields_ = [("iter", C.c_int64), ("cg_steps_total", C.c_int64), ("cg_steps_cond", C.c_int64), ("cg_steps_last", C.c_int32),
+                ("n_conditionings", C.c_int32), ("cg_hit_max", C.c_int32), ("reserved", C.c_int32)] + \
+               [(k, C.c_double) for k in ("pres_abs", "pres_rel", "dres_abs", "dres_rel", "gap_abs", "gap_rel",
+                                          "cone_viol_rel", "kkt_rel", "pobj", "dobj", "fp_res")]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+EXPORTS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
+           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_kernel_launches", "cs_last_error", "cs_destroy")
+
+_lib = None
+
+
+def lib():
+    """Load libcs.so (fails loudly when it has not been built: run ``__graft_entry__.build()``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2103_00736_b200.build`; "
+                               "there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp = C.c_void_p
+        L.cs_create.argtypes = [C.POINTER(vp), C.POINTER(cs_csr), vp, vp, C.c_int, C.POINTER(cs_cones), vp]
+        L.cs_set_params.argtypes = [vp, C.POINTER(cs_params)]
+        L.cs_get_params.argtypes = [vp, C.POINTER(cs_params)]
+        L.cs_set_point.argtypes = [vp, vp, vp, C.c_int]
+        L.cs_iterate.argtypes = [vp, C.c_int64]
+        L.cs_condition.argtypes = [vp]
+        L.cs_set_scaling.argtypes = [vp, vp, C.c_int]
+        L.cs_residuals.argtypes = [vp, C.POINTER(cs_resid)]
+        L.cs_solution.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
+        L.cs_kernel_launches.argtypes = [vp]
+        L.cs_kernel_launches.restype = C.c_int64
+        L.cs_last_error.argtypes = [vp]
+        L.cs_last_error.restype = C.c_char_p
+        L.cs_destroy.argtypes = [vp]
+        L.cs_destroy.restype = None
+        for name in EXPORTS[:9]:
+            getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+class CsError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {text}")
+        self.status = status
+
+
+def _ptr(a, dtype=None):
+    """(pointer, cs_mem) of a numpy array or torch tensor; None -> (None, host)."""
+    if a is None:
+        return None, CS_HOST
+    if isinstance(a, np.ndarray):
+        if dtype is not None and a.dtype != dtype:
+            raise TypeError(f"expected {dtype}, got {a.dtype}")
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be contiguous")
+        return a.ctypes.data, CS_HOST
+    # torch tensor (duck-typed so that torch stays optional for host-only use)
+    if not a.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    if dtype is not None and np.dtype(str(a.dtype).replace("torch.", "")) != dtype:
+        raise TypeError(f"expected {dtype}, got {a.dtype}")
+    return a.data_ptr(), (CS_DEVICE if a.is_cuda else CS_HOST)
+
+
+def _same_space(*tags):
+    tags = [t for p, t in tags if p is not None]
+    if tags and any(t != tags[0] for t in tags):
+        raise ValueError("all arrays of one call must live in the same memory space")
+    return tags[0] if tags else CS_HOST
+
+
+class Solver:
+    """One ``cs_solver`` handle.  Method names mirror the C ABI without the ``cs_`` prefix."""
+
+    def __init__(self, m, n, row_ptr, col_idx, val, b, c, n_lin, soc_size=None, stream=None):
+        L = lib()
+        rp, ci, va = _ptr(row_ptr, np.int32), _ptr(col_idx, np.int32), _ptr(val, np.float64)
+        where_A = _same_space(rp, ci, va)
+        bp, cp = _ptr(b, np.float64), _ptr(c, np.float64)
+        where_v = _same_space(bp, cp)
+        nnz = int(val.shape[0])
+        A = cs_csr(int(m), int(n), nnz, rp[0], ci[0], va[0], where_A)
+        soc = np.ascontiguousarray(soc_size if soc_size is not None else [], dtype=np.int32)
+        K = cs_cones(int(n_lin), int(soc.shape[0]), soc.ctypes.data if soc.size else None)
+        h = C.c_void_p()
+        st = L.cs_create(C.byref(h), C.byref(A), bp[0], cp[0], where_v, C.byref(K),
+                         C.c_void_p(int(stream)) if stream else None)
+        if st != CS_OK:
+            raise CsError(st, L.cs_last_error(None).decode())
+        self._h, self.m, self.n = h, int(m), int(n)
+
+    @classmethod
+    def from_problem(cls, p, device=None, stream=None):
+        """Build from a ``workloads.Problem``; ``device`` = torch device to stage the inputs on first
+        (inputs resident in HBM), None = pass the host arrays."""
+        arrs = [p.row_ptr, p.col_idx, p.val, p.b, p.c]
+        if device is not None:
+            import torch
+            arrs = [torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in arrs]
+        S = cls(p.m, p.n, arrs[0], arrs[1], arrs[2], arrs[3], arrs[4], p.n_lin, p.soc_size, stream=stream)
+        S.set_params(mu=p.mu, t=p.t)
+        return S
+
+    def _check(self, st, ok=(CS_OK,)):
+        if st not in ok:
+            raise CsError(st, lib().cs_last_error(self._h).decode())
+        return st
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().cs_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def get_params(self):
+        p = cs_params()
+        self._check(lib().cs_get_params(self._h, C.byref(p)))
+        return {k: getattr(p, k) for k, _ in p._fields_ if k != "reserved"}
+
+    def set_params(self, **kw):
+        cur = self.get_params()
+        cur.update(kw)
+        p = cs_params(cur["mu"], cur["t"], cur["o_floor"], cur["cg_tol"], int(cur["cg_max_iter"]), 0)
+        self._check(lib().cs_set_params(self._h, C.byref(p)))
+
+    def set_point(self, x, z):
+        xp, zp = _ptr(x, np.float64), _ptr(z, np.float64)
+        self._check(lib().cs_set_point(self._h, xp[0], zp[0], _same_space(xp, zp)))
+
+    def iterate(self, k):
+        self._check(lib().cs_iterate(self._h, int(k)))
+
+    def condition(self):
+        self._check(lib().cs_condition(self._h))
+
+    def set_scaling(self, O):
+        op = _ptr(O, np.float64)
+        self._check(lib().cs_set_scaling(self._h, op[0], op[1]))
+
+    def residuals(self, strict=False):
+        r = cs_resid()
+        self._check(lib().cs_residuals(self._h, C.byref(r)), ok=(CS_OK,) if strict else (CS_OK, CS_ECGMAX))
+        return r.as_dict()
+
+    def solution_into(self, x=None, z=None, y=None, s=None, O=None):
+        ps = [_ptr(a, np.float64) for a in (x, z, y, s, O)]
+        self._check(lib().cs_solution(self._h, *[p[0] for p in ps], _same_space(*ps)))
+
+    def solution(self):
+        """x, z, y, s, O as host numpy arrays."""
+        out = {k: np.empty(self.n) for k in ("x", "z", "s", "O")}
+        out["y"] = np.empty(self.m)
+        self.solution_into(out["x"], out["z"], out["y"], out["s"], out["O"])
+        return out
+
+    def kernel_launches(self):
+        return int(lib().cs_kernel_launches(self._h))
+
+    def run(self, k, L=()):
+        """Algorithm 2 with the schedule L: continues the iteration counter kept by the caller
+        in ``self.l``.  cs_iterate / cs_condition calls only."""
+        l = getattr(self, "l", 0)
+        end = l + int(k)
+        for cond_at in sorted(x for x in L if l < x <= end):
+            if cond_at - 1 > l:
+                self.iterate(cond_at - 1 - l)
+                l = cond_at - 1
+            if cond_at > 1:
+                self.condition()
+        if end > l:
+            self.iterate(end - l)
+        self.l = end

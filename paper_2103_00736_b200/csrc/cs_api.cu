@@ -1,0 +1,419 @@
+// cs_api.cu -- host side of libcs.so: the C ABI of include/cs.h.
+// Validation, CSR->CSC transposition and the work partition are one-off host work at cs_create;
+// every step of the iteration itself is a kernel in cs_kernels*.cuh.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/cs.h"
+#include "cs_kernels_cond.cuh"
+
+using namespace csd;
+
+struct cs_solver {
+    Ctx ctx{};
+    cudaStream_t stream = nullptr;
+    int device = 0;
+    int grid = 0;
+    std::vector<void *> allocs;
+    cs_params prm{};
+    bool conditioned = false;  // the l=1 conditioning of step 4 has run
+    bool xz_stale = false;     // xb, zb older than (p, s)
+    bool started = false;      // some pass or conditioning has run (cs_set_point no longer allowed)
+    int64_t launches = 0;
+    std::string err;
+};
+
+namespace {
+
+thread_local std::string g_create_err;
+
+#define CS_CUDA(S, call)                                                                         \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess) {                                                                 \
+            (S)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                       \
+            return e_ == cudaErrorMemoryAllocation ? CS_ENOMEM : CS_ECUDA;                       \
+        }                                                                                        \
+    } while (0)
+
+template <class T>
+cs_status dev_alloc(cs_solver *S, T **out, size_t count) {
+    void *p = nullptr;
+    CS_CUDA(S, cudaMalloc(&p, std::max<size_t>(count, 1) * sizeof(T)));
+    S->allocs.push_back(p);
+    *out = static_cast<T *>(p);
+    return CS_OK;
+}
+
+template <class T>
+cs_status dev_upload(cs_solver *S, T **out, const T *host, size_t count) {
+    cs_status st = dev_alloc(S, out, count);
+    if (st != CS_OK) return st;
+    if (count) CS_CUDA(S, cudaMemcpyAsync(*out, host, count * sizeof(T), cudaMemcpyHostToDevice, S->stream));
+    return CS_OK;
+}
+
+template <class T>
+cs_status dev_zeros(cs_solver *S, T **out, size_t count) {
+    cs_status st = dev_alloc(S, out, count);
+    if (st != CS_OK) return st;
+    CS_CUDA(S, cudaMemsetAsync(*out, 0, std::max<size_t>(count, 1) * sizeof(T), S->stream));
+    return CS_OK;
+}
+
+// Fetch an input array to the host (inputs may live in device memory).
+template <class T>
+cs_status fetch(cs_solver *S, std::vector<T> &dst, const T *src, size_t count, cs_mem where) {
+    dst.resize(count);
+    if (!count) return CS_OK;
+    if (where == CS_HOST) std::memcpy(dst.data(), src, count * sizeof(T));
+    else CS_CUDA(S, cudaMemcpy(dst.data(), src, count * sizeof(T), cudaMemcpyDeviceToHost));
+    return CS_OK;
+}
+
+struct HostBins {
+    std::vector<int> short_ids;
+    std::vector<int4> chunks, multi;
+    int n_short = 0, G = 8, n_slots = 0;
+    bool identity = false;
+};
+
+HostBins make_bins(const std::vector<int> &ptr) {
+    HostBins hb;
+    const int nseg = (int)ptr.size() - 1;
+    long long short_nnz = 0;
+    for (int s = 0; s < nseg; ++s) {
+        const int len = ptr[s + 1] - ptr[s];
+        if (len <= kShortMax) {
+            hb.short_ids.push_back(s);
+            short_nnz += len;
+        } else if (len <= kChunk) {
+            hb.chunks.push_back(make_int4(s, ptr[s], len, -1));
+        } else {
+            const int nch = (len + kChunk - 1) / kChunk;
+            hb.multi.push_back(make_int4(s, hb.n_slots, nch, 0));
+            for (int q = 0; q < nch; ++q) {
+                const int a = ptr[s] + q * kChunk;
+                hb.chunks.push_back(make_int4(s, a, std::min(kChunk, ptr[s + 1] - a), hb.n_slots++));
+            }
+        }
+    }
+    hb.n_short = (int)hb.short_ids.size();
+    hb.identity = hb.n_short == nseg;
+    const double avg = hb.n_short ? (double)short_nnz / hb.n_short : 1.0;
+    hb.G = 4;
+    while (hb.G < 32 && hb.G < avg) hb.G *= 2;
+    return hb;
+}
+
+cs_status upload_bins(cs_solver *S, const HostBins &hb, Bins *out) {
+    out->n_short = hb.n_short;
+    out->G = hb.G;
+    out->short_ids = nullptr;
+    cs_status st;
+    if (!hb.identity) {
+        int *p;
+        if ((st = dev_upload(S, &p, hb.short_ids.data(), hb.short_ids.size())) != CS_OK) return st;
+        out->short_ids = p;
+    }
+    int4 *c4, *m4;
+    if ((st = dev_upload(S, &c4, hb.chunks.data(), hb.chunks.size())) != CS_OK) return st;
+    if ((st = dev_upload(S, &m4, hb.multi.data(), hb.multi.size())) != CS_OK) return st;
+    out->n_chunk = (int)hb.chunks.size();
+    out->chunks = c4;
+    out->n_multi = (int)hb.multi.size();
+    out->multi = m4;
+    return dev_zeros(S, &out->partial, (size_t)hb.n_slots * 2);
+}
+
+cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
+    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, 0, S->stream));
+    S->launches += 1;
+    return CS_OK;
+}
+
+cs_status ensure_xz(cs_solver *S) {
+    if (!S->xz_stale) return CS_OK;
+    const int blocks = std::min((S->ctx.n + 255) / 256, 148 * 8);
+    k_materialize_xz<<<blocks, 256, 0, S->stream>>>(S->ctx);
+    CS_CUDA(S, cudaGetLastError());
+    S->launches += 1;
+    S->xz_stale = false;
+    return CS_OK;
+}
+
+void sync_params(cs_solver *S) {
+    S->ctx.cg_tol = S->prm.cg_tol;
+    S->ctx.cg_max_iter = S->prm.cg_max_iter;
+}
+
+cs_status do_condition(cs_solver *S, int use_rule) {
+    cs_status st = ensure_xz(S);
+    if (st != CS_OK) return st;
+    S->ctx.mu = S->prm.mu;  // mu, t, o_floor take effect here (cs.h)
+    S->ctx.t = S->prm.t;
+    S->ctx.o_floor = S->prm.o_floor;
+    sync_params(S);
+    void *args[] = {&S->ctx, &use_rule};
+    st = launch_coop(S, (const void *)k_condition, args);
+    if (st != CS_OK) return st;
+    S->conditioned = true;
+    S->started = true;
+    return CS_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char *cs_last_error(const cs_solver *S) { return S ? S->err.c_str() : g_create_err.c_str(); }
+
+void cs_destroy(cs_solver *S) {
+    if (!S) return;
+    cudaSetDevice(S->device);
+    cudaStreamSynchronize(S->stream);
+    for (void *p : S->allocs) cudaFree(p);
+    delete S;
+}
+
+int64_t cs_kernel_launches(const cs_solver *S) { return S ? S->launches : 0; }
+
+static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
+                             const cs_cones *K) {
+    const int64_t m64 = A->m, n64 = A->n, nnz64 = A->nnz;
+    if (m64 <= 0 || n64 <= 0 || nnz64 <= 0 || m64 >= INT32_MAX || n64 >= INT32_MAX || nnz64 >= INT32_MAX) {
+        S->err = "sizes must be positive and below 2^31";
+        return CS_EINVAL;
+    }
+    const int m = (int)m64, n = (int)n64, nnz = (int)nnz64;
+    // ---- cones
+    if (K->n_lin < 0 || K->n_soc < 0 || (K->n_soc > 0 && !K->soc_size)) { S->err = "bad cone spec"; return CS_EINVAL; }
+    std::vector<int> cone_off((size_t)K->n_soc + 1);
+    int64_t off = K->n_lin;
+    for (int64_t i = 0; i < K->n_soc; ++i) {
+        if (K->soc_size[i] < 1) { S->err = "soc_size entries must be >= 1"; return CS_EINVAL; }
+        cone_off[i] = (int)off;
+        off += K->soc_size[i];
+        if (off > n64) break;
+    }
+    if (off != n64) { S->err = "n_lin + sum(soc_size) != n"; return CS_EINVAL; }
+    cone_off[K->n_soc] = n;
+    // ---- fetch and validate A
+    std::vector<int> rptr, cidx;
+    std::vector<double> val, hb, hc;
+    cs_status st;
+    if ((st = fetch(S, rptr, A->row_ptr, (size_t)m + 1, A->where)) != CS_OK) return st;
+    if ((st = fetch(S, cidx, A->col_idx, (size_t)nnz, A->where)) != CS_OK) return st;
+    if ((st = fetch(S, val, A->val, (size_t)nnz, A->where)) != CS_OK) return st;
+    if ((st = fetch(S, hb, b, (size_t)m, vec_where)) != CS_OK) return st;
+    if ((st = fetch(S, hc, c, (size_t)n, vec_where)) != CS_OK) return st;
+    if (rptr[0] != 0 || rptr[m] != nnz) { S->err = "row_ptr[0] != 0 or row_ptr[m] != nnz"; return CS_EINVAL; }
+    for (int i = 0; i < m; ++i) {
+        if (rptr[i + 1] <= rptr[i]) { S->err = "row_ptr not increasing (empty rows are not allowed)"; return CS_EINVAL; }
+        if (rptr[i + 1] > nnz) { S->err = "row_ptr out of range"; return CS_EINVAL; }
+        for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
+            if (cidx[k] < 0 || cidx[k] >= n || (k > rptr[i] && cidx[k] <= cidx[k - 1])) {
+                S->err = "col_idx out of range, unsorted or duplicated within a row";
+                return CS_EINVAL;
+            }
+            if (!std::isfinite(val[k])) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
+        }
+    }
+    double nb = 0.0, nc = 0.0;
+    for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
+    for (int j = 0; j < n; ++j) { if (!std::isfinite(hc[j])) { S->err = "non-finite c"; return CS_EINVAL; } nc += hc[j] * hc[j]; }
+    // ---- CSC copy (counting sort by column; rows come out sorted within a column)
+    std::vector<int> cptr((size_t)n + 1, 0), ridx((size_t)nnz);
+    std::vector<double> cval((size_t)nnz);
+    for (int k = 0; k < nnz; ++k) cptr[(size_t)cidx[k] + 1]++;
+    for (int j = 0; j < n; ++j) cptr[(size_t)j + 1] += cptr[j];
+    {
+        std::vector<int> fill(cptr.begin(), cptr.end() - 1);
+        for (int i = 0; i < m; ++i)
+            for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
+                const int q = fill[cidx[k]]++;
+                ridx[q] = i;
+                cval[q] = val[k];
+            }
+    }
+    // ---- device state
+    Ctx &x = S->ctx;
+    x.m = m; x.n = n; x.n_lin = (int)K->n_lin; x.n_soc = (int)K->n_soc;
+    x.norm_b = std::sqrt(nb); x.norm_c = std::sqrt(nc);
+    int *ip; double *dp;
+    if ((st = dev_upload(S, &ip, cone_off.data(), cone_off.size())) != CS_OK) return st; x.cone_off = ip;
+    if ((st = dev_upload(S, &ip, rptr.data(), rptr.size())) != CS_OK) return st; x.R.ptr = ip;
+    if ((st = dev_upload(S, &ip, cidx.data(), cidx.size())) != CS_OK) return st; x.R.idx = ip;
+    if ((st = dev_upload(S, &dp, val.data(), val.size())) != CS_OK) return st; x.R.val0 = dp;
+    if ((st = dev_upload(S, &x.R.val, val.data(), val.size())) != CS_OK) return st;
+    if ((st = dev_upload(S, &ip, cptr.data(), cptr.size())) != CS_OK) return st; x.C.ptr = ip;
+    if ((st = dev_upload(S, &ip, ridx.data(), ridx.size())) != CS_OK) return st; x.C.idx = ip;
+    if ((st = dev_upload(S, &dp, cval.data(), cval.size())) != CS_OK) return st; x.C.val0 = dp;
+    if ((st = dev_upload(S, &x.C.val, cval.data(), cval.size())) != CS_OK) return st;
+    if ((st = upload_bins(S, make_bins(rptr), &x.R.bins)) != CS_OK) return st;
+    if ((st = upload_bins(S, make_bins(cptr), &x.C.bins)) != CS_OK) return st;
+    if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
+    if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
+    double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.d, &x.chat};
+    for (double **q : nv) if ((st = dev_zeros(S, q, (size_t)n)) != CS_OK) return st;
+    double **mv[] = {&x.w, &x.r, &x.v, &x.wd, &x.btil};
+    for (double **q : mv) if ((st = dev_zeros(S, q, (size_t)m)) != CS_OK) return st;
+    {   // O = 1, D = 1, x = z = e_K
+        std::vector<double> ones((size_t)std::max(m, n), 1.0), ek((size_t)n, 0.0);
+        for (int j = 0; j < x.n_lin; ++j) ek[j] = 1.0;
+        for (int i = 0; i < x.n_soc; ++i) ek[cone_off[i]] = 1.0;
+        if ((st = dev_upload(S, &x.O, ones.data(), (size_t)n)) != CS_OK) return st;
+        if ((st = dev_upload(S, &x.D, ones.data(), (size_t)m)) != CS_OK) return st;
+        if ((st = dev_upload(S, &x.xb, ek.data(), (size_t)n)) != CS_OK) return st;
+        if ((st = dev_upload(S, &x.zb, ek.data(), (size_t)n)) != CS_OK) return st;
+        CS_CUDA(S, cudaStreamSynchronize(S->stream));  // host staging buffers die at scope end
+    }
+    if ((st = dev_zeros(S, &x.sc, 1)) != CS_OK) return st;
+    // ---- cooperative grid: as many CTAs as can be co-resident
+    int sms = 0, occ = 0, occ_min = 1 << 30;
+    CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
+    const void *kernels[] = {(const void *)k_iterate, (const void *)k_condition, (const void *)k_residuals};
+    for (const void *k : kernels) {
+        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, 0));
+        occ_min = std::min(occ_min, occ);
+    }
+    if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
+    S->grid = sms * occ_min;
+    if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * S->grid)) != CS_OK) return st;
+    // ---- defaults (cs.h)
+    S->prm.mu = 1.0;
+    S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
+    S->prm.o_floor = 1e-16;
+    S->prm.cg_tol = 1e-13;
+    S->prm.cg_max_iter = 20000;
+    x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
+    sync_params(S);
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    return CS_OK;
+}
+
+cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
+                    const cs_cones *K, void *cuda_stream) {
+    if (!out) return CS_EINVAL;
+    *out = nullptr;
+    if (!A || !b || !c || !K || !A->row_ptr || !A->col_idx || !A->val) { g_create_err = "NULL argument"; return CS_EINVAL; }
+    cs_solver *S = new (std::nothrow) cs_solver;
+    if (!S) return CS_ENOMEM;
+    S->stream = static_cast<cudaStream_t>(cuda_stream);
+    cs_status st = CS_OK;
+    if (cudaGetDevice(&S->device) != cudaSuccess) { S->err = "no CUDA device"; st = CS_ECUDA; }
+    if (st == CS_OK) {
+        try { st = create_impl(S, A, b, c, vec_where, K); }
+        catch (const std::bad_alloc &) { S->err = "host allocation failed"; st = CS_ENOMEM; }
+    }
+    if (st != CS_OK) { g_create_err = S->err; cs_destroy(S); return st; }
+    *out = S;
+    return CS_OK;
+}
+
+cs_status cs_set_params(cs_solver *S, const cs_params *p) {
+    if (!S || !p) return CS_EINVAL;
+    if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || p->cg_max_iter < 1) {
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, cg_max_iter >= 1";
+        return CS_EINVAL;
+    }
+    S->prm = *p;
+    sync_params(S);
+    return CS_OK;
+}
+
+cs_status cs_get_params(const cs_solver *S, cs_params *p) {
+    if (!S || !p) return CS_EINVAL;
+    *p = S->prm;
+    return CS_OK;
+}
+
+cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem where) {
+    if (!S || !x || !z) return CS_EINVAL;
+    if (S->started) { S->err = "cs_set_point after the iteration has started"; return CS_ESTATE; }
+    const cudaMemcpyKind kind = where == CS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    CS_CUDA(S, cudaMemcpyAsync(S->ctx.xb, x, sizeof(double) * S->ctx.n, kind, S->stream));
+    CS_CUDA(S, cudaMemcpyAsync(S->ctx.zb, z, sizeof(double) * S->ctx.n, kind, S->stream));
+    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    return CS_OK;
+}
+
+cs_status cs_condition(cs_solver *S) {
+    if (!S) return CS_EINVAL;
+    return do_condition(S, 1);
+}
+
+cs_status cs_set_scaling(cs_solver *S, const double *O, cs_mem where) {
+    if (!S || !O) return CS_EINVAL;
+    cs_status st = ensure_xz(S);  // x,z of the OLD scaling, before O is overwritten
+    if (st != CS_OK) return st;
+    const cudaMemcpyKind kind = where == CS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    CS_CUDA(S, cudaMemcpyAsync(S->ctx.O, O, sizeof(double) * S->ctx.n, kind, S->stream));
+    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    return do_condition(S, 0);
+}
+
+cs_status cs_iterate(cs_solver *S, int64_t k) {
+    if (!S || k < 0) return CS_EINVAL;
+    if (k == 0) return CS_OK;
+    cs_status st;
+    if (!S->conditioned && (st = do_condition(S, 1)) != CS_OK) return st;  // step 4: l = 1
+    sync_params(S);
+    long long kk = k;
+    void *args[] = {&S->ctx, &kk};
+    if ((st = launch_coop(S, (const void *)k_iterate, args)) != CS_OK) return st;
+    S->xz_stale = true;
+    S->started = true;
+    return CS_OK;
+}
+
+cs_status cs_residuals(cs_solver *S, cs_resid *out) {
+    if (!S || !out) return CS_EINVAL;
+    cs_status st;
+    if (!S->conditioned && (st = do_condition(S, 1)) != CS_OK) return st;
+    if ((st = ensure_xz(S)) != CS_OK) return st;
+    void *args[] = {&S->ctx};
+    if ((st = launch_coop(S, (const void *)k_residuals, args)) != CS_OK) return st;
+    Scalars h;
+    CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
+    CS_CUDA(S, cudaMemsetAsync(&S->ctx.sc->cg_hit_max, 0, sizeof(int), S->stream));
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    out->iter = h.iter; out->cg_steps_total = h.cg_steps_total; out->cg_steps_cond = h.cg_steps_cond; out->cg_steps_last = h.cg_steps_last;
+    out->n_conditionings = h.n_cond; out->cg_hit_max = h.cg_hit_max; out->reserved = 0;
+    out->pres_abs = h.resid[0]; out->pres_rel = h.resid[1]; out->dres_abs = h.resid[2]; out->dres_rel = h.resid[3];
+    out->gap_abs = h.resid[4]; out->gap_rel = h.resid[5]; out->cone_viol_rel = h.resid[6]; out->kkt_rel = h.resid[7];
+    out->pobj = h.resid[8]; out->dobj = h.resid[9]; out->fp_res = h.resid[10];
+    return h.cg_hit_max ? CS_ECGMAX : CS_OK;
+}
+
+cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where) {
+    if (!S) return CS_EINVAL;
+    cs_status st;
+    if ((st = ensure_xz(S)) != CS_OK) return st;
+    const Ctx &c = S->ctx;
+    const cudaMemcpyKind kind = where == CS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    const size_t nb = sizeof(double) * c.n;
+    if (x) CS_CUDA(S, cudaMemcpyAsync(x, c.xb, nb, kind, S->stream));
+    if (z) CS_CUDA(S, cudaMemcpyAsync(z, c.zb, nb, kind, S->stream));
+    if (s) CS_CUDA(S, cudaMemcpyAsync(s, c.s, nb, kind, S->stream));
+    if (O) CS_CUDA(S, cudaMemcpyAsync(O, c.O, nb, kind, S->stream));
+    if (y) {
+        double *ydev = where == CS_DEVICE ? y : c.r;  // r is scratch between solves
+        k_dual_y<<<std::min((c.m + 255) / 256, 148 * 8), 256, 0, S->stream>>>(c, ydev);
+        CS_CUDA(S, cudaGetLastError());
+        S->launches += 1;
+        if (where == CS_HOST) CS_CUDA(S, cudaMemcpyAsync(y, ydev, sizeof(double) * c.m, kind, S->stream));
+    }
+    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    return CS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,196 @@
+// cs_kernels.cuh -- the persistent cooperative kernels of libcs.so.
+//
+//   k_iterate   : k passes of Algorithm 2 steps 16-18 incl. the inner CG on (A~ A~')
+//   k_condition : Algorithm 2 steps 5-14 incl. the solve for d
+//   k_residuals : KKT residual norms of the current iterate
+//
+// A~ = D A O is the row-equilibrated, column-conditioned matrix; D = diag(1/||row_i(A O)||_2) is
+// mathematically inert for the iterates ((DA)^dagger(DA) = A^dagger A) and makes diag(A~A~') = I,
+// i.e. it IS the Jacobi preconditioner in split form.
+#pragma once
+#include "cs_device.cuh"
+
+namespace csd {
+
+// ---------------------------------------------------------------------------------------------
+// abs_K on one Lorentz block handled by kConeLanes lanes (Def.1; closed form of the
+// projection onto {t >= ||u||}):  ||u|| <= t : v ;  ||u|| <= -t : -v ;  else (||u||, (t/||u||) u).
+// `f(j, s_j, p_j)` receives every coordinate.  All 32 lanes of a warp must call this together.
+// ---------------------------------------------------------------------------------------------
+template <class F>
+__device__ __forceinline__ void soc_abs_block(const double *s, int a, int b, int sl, bool active, F &f) {
+    double t = 0.0, nu2 = 0.0;
+    if (active) {
+        t = s[a];
+        for (int j = a + 1 + sl; j < b; j += kConeLanes) { const double x = s[j]; nu2 += x * x; }
+    }
+    nu2 = group_reduce<kConeLanes>(nu2);
+    if (!active) return;
+    const double nu = sqrt(nu2);
+    if (nu <= t) {
+        for (int j = a + sl; j < b; j += kConeLanes) f(j, s[j], s[j]);
+    } else if (nu <= -t) {
+        for (int j = a + sl; j < b; j += kConeLanes) f(j, s[j], -s[j]);
+    } else {
+        const double sc = t / nu;
+        if (sl == 0) f(a, t, nu);
+        for (int j = a + 1 + sl; j < b; j += kConeLanes) f(j, s[j], sc * s[j]);
+    }
+}
+
+// step 16: p = abs_K(s) ; also e = p - g (the warm-start difference, g = A~' w of the previous pass)
+__device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    for (int j = tid; j < c.n_lin; j += nth) {
+        const double pj = fabs(c.s[j]);
+        c.p[j] = pj;
+        c.e[j] = pj - c.g[j];
+    }
+    if (c.n_soc) {
+        const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
+        constexpr int CPW = 32 / kConeLanes;
+        const int gwarp = tid >> 5, nwarps = nth >> 5;
+        auto put = [&](int j, double, double pj) { c.p[j] = pj; c.e[j] = pj - c.g[j]; };
+        for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
+            const int ci = base + sub;
+            const bool act = ci < c.n_soc;
+            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
+            soc_abs_block(c.s, a, b, sl, act, put);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Inner solve: CG on (A~ A~') w = q, started from the current w with residual r already in c.r and
+// rho = ||r||^2, qq = ||q||^2 known.  Two sparse passes and two grid reductions per step:
+//   K1 (columns, CSC):  u = A~' r + beta u          sigma = ||u||^2       (u == A~' v by induction)
+//   K2 (rows,    CSR):  v = r + beta v ; w += alpha v ; r -= alpha (A~ u) ; rho' = ||r||^2
+// with alpha = rho/sigma (v'A~A~'v = ||A~'v||^2) and beta = rho'/rho.  Returns the steps done.
+// ---------------------------------------------------------------------------------------------
+struct TermCscR {   // A~' r
+    const double *val; const int *idx; const double *r;
+    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * r[__ldg(idx + k)]; }
+};
+struct TermCsrU {   // A~ u
+    const double *val; const int *idx; const double *u;
+    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * u[__ldg(idx + k)]; }
+};
+struct EpiK1 {
+    double *u; double beta; double sigma;
+    __device__ void operator()(int j, const double (&a)[1]) {
+        const double uj = a[0] + beta * u[j];
+        u[j] = uj;
+        sigma += uj * uj;
+    }
+};
+struct EpiK2 {
+    double *v, *w, *r; double alpha, beta; double rho;
+    __device__ void operator()(int i, const double (&a)[1]) {
+        const double ri = r[i];
+        const double vi = ri + beta * v[i];
+        v[i] = vi;
+        w[i] += alpha * vi;
+        const double rn = ri - alpha * a[0];
+        r[i] = rn;
+        rho += rn * rn;
+    }
+};
+
+__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, double qq, bool &hit_max) {
+    const double thresh = c.cg_tol * c.cg_tol * qq;
+    double beta = 0.0;
+    int steps = 0;
+    hit_max = false;
+    while (rho > thresh) {
+        if (steps >= c.cg_max_iter) { hit_max = true; break; }
+        TermCscR t1{c.C.val, c.C.idx, c.r};
+        EpiK1 e1{c.u, beta, 0.0};
+        seg_reduce<1>(c.C, t1, e1, gc);
+        double red[1] = {e1.sigma};
+        grid_reduce<1>(red, gc);
+        const double sigma = red[0];
+        if (!(sigma > 0.0)) break;
+        const double alpha = rho / sigma;
+        TermCsrU t2{c.R.val, c.R.idx, c.u};
+        EpiK2 e2{c.v, c.w, c.r, alpha, beta, 0.0};
+        seg_reduce<1>(c.R, t2, e2, gc);
+        red[0] = e2.rho;
+        grid_reduce<1>(red, gc);
+        beta = red[0] / rho;
+        rho = red[0];
+        ++steps;
+    }
+    return steps;
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_iterate
+// ---------------------------------------------------------------------------------------------
+struct TermCsrPE {  // (A~ p, A~ (p - g))
+    const double *val; const int *idx; const double *p, *e;
+    __device__ void operator()(int k, double (&a)[2]) const {
+        const int j = __ldg(idx + k);
+        const double vk = val[k];
+        a[0] += vk * p[j];
+        a[1] += vk * e[j];
+    }
+};
+struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r||^2
+    double *r; double qq, rho;
+    __device__ void operator()(int i, const double (&a)[2]) {
+        r[i] = a[1];
+        qq += a[0] * a[0];
+        rho += a[1] * a[1];
+    }
+};
+struct TermCscW {   // A~' w
+    const double *val; const int *idx; const double *w;
+    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * w[__ldg(idx + k)]; }
+};
+struct EpiUpdate {  // steps 17-18: r = 2 A~'w - p ; s <- s/2 - r/2 + d = (s+p)/2 - A~'w + d
+    double *s, *g; const double *p, *d; double fp2;
+    __device__ void operator()(int j, const double (&a)[1]) {
+        const double sj = s[j];
+        const double sn = 0.5 * (sj + p[j]) - a[0] + d[j];
+        g[j] = a[0];
+        s[j] = sn;
+        fp2 += (sn - sj) * (sn - sj);
+    }
+};
+
+__global__ void __launch_bounds__(kBlock, 2) k_iterate(Ctx c, long long k_iter) {
+    __shared__ double smem[kMaxRed * kWarps];
+    GridCtl gc(c.partials, smem);
+    long long cg_total = 0;
+    int cg_last = 0;
+    bool any_max = false;
+    double fp2 = 0.0;
+    for (long long it = 0; it < k_iter; ++it) {
+        phase_cone_reflect(c);                                   // step 16
+        gc.sync();
+        TermCsrPE tq{c.R.val, c.R.idx, c.p, c.e};
+        EpiRhs eq{c.r, 0.0, 0.0};
+        seg_reduce<2>(c.R, tq, eq, gc);
+        double red[2] = {eq.qq, eq.rho};
+        grid_reduce<2>(red, gc);
+        bool hm;
+        cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
+        any_max |= hm;
+        cg_total += cg_last;
+        TermCscW tw{c.C.val, c.C.idx, c.w};
+        EpiUpdate eu{c.s, c.g, c.p, c.d, 0.0};
+        seg_reduce<1>(c.C, tw, eu, gc);                          // steps 17-18
+        double rf[1] = {eu.fp2};
+        grid_reduce<1>(rf, gc);
+        fp2 = rf[0];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0 && k_iter > 0) {
+        c.sc->iter += k_iter;
+        c.sc->cg_steps_total += cg_total;
+        c.sc->cg_steps_last = cg_last;
+        c.sc->fp_res2 = fp2;
+        if (any_max) c.sc->cg_hit_max = 1;
+    }
+}
+
+}  // namespace csd

@@ -1,0 +1,238 @@
+// cs_kernels_cond.cuh -- k_condition (Algorithm 2 steps 5-14), k_residuals, and the small
+// element-wise kernels around them.
+#pragma once
+#include "cs_kernels.cuh"
+
+namespace csd {
+
+// steps 19-20: x = O(p+s)/2, z = O^{-1}(p-s)/(2 mu) into xb, zb (original coordinates)
+__global__ void k_materialize_xz(Ctx c) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int j = tid; j < c.n; j += nth) {
+        const double pj = c.p[j], sj = c.s[j], Oj = c.O[j];
+        c.xb[j] = Oj * (pj + sj) * 0.5;
+        c.zb[j] = (pj - sj) / (2.0 * c.mu) / Oj;
+    }
+}
+
+// y = D (w_d - w) / mu  (derived multiplier; s+ = x~ - mu(c^ - A~'y'), y' = (w_d - w)/mu)
+__global__ void k_dual_y(Ctx c, double *y) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int i = tid; i < c.m; i += nth) y[i] = c.D[i] * (c.wd[i] - c.w[i]) / c.mu;
+}
+
+// ---- steps 5-9: o per cone (stored as ln o in c.O), then max / min of ln o -------------------
+__device__ __forceinline__ void phase_cone_ratio(const Ctx &c, double &lmax, double &lmin_neg) {
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    const double fl = c.o_floor;
+    for (int j = tid; j < c.n_lin; j += nth) {
+        const double lo = log(fmax(fabs(c.xb[j]), fl) / fmax(fabs(c.zb[j]), fl));
+        c.O[j] = lo;
+        lmax = fmax(lmax, lo);
+        lmin_neg = fmax(lmin_neg, -lo);
+    }
+    if (c.n_soc) {
+        const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
+        constexpr int CPW = 32 / kConeLanes;
+        const int gwarp = tid >> 5, nwarps = nth >> 5;
+        for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
+            const int ci = base + sub;
+            const bool act = ci < c.n_soc;
+            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
+            double nu2 = 0.0;
+            for (int j = a + 1 + sl; j < b; j += kConeLanes) { const double x = c.xb[j]; nu2 += x * x; }
+            nu2 = group_reduce<kConeLanes>(nu2);
+            if (act) {
+                const double num = fmax(fabs(c.xb[a] - sqrt(nu2)), fl), den = fmax(fabs(c.zb[a]), fl);
+                const double lo = log(num / den);
+                for (int j = a + sl; j < b; j += kConeLanes) c.O[j] = lo;
+                lmax = fmax(lmax, lo);
+                lmin_neg = fmax(lmin_neg, -lo);
+            }
+        }
+    }
+}
+
+struct TermRowNorm {  // sum_j (A_ij O_j)^2
+    const double *val0; const int *idx; const double *O;
+    __device__ void operator()(int k, double (&a)[1]) const {
+        const double x = val0[k] * O[__ldg(idx + k)];
+        a[0] += x * x;
+    }
+};
+struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b
+    double *D, *btil; const double *b;
+    __device__ void operator()(int i, const double (&a)[1]) {
+        const double di = 1.0 / sqrt(a[0]);
+        D[i] = di;
+        btil[i] = di * b[i];
+    }
+};
+struct ScaleCsr {     // A~_ij = D_i A_ij O_j on the row-major copy
+    double *val; const double *val0; const int *idx; const double *O, *D;
+    __device__ void operator()(int i, int k) const { val[k] = val0[k] * O[__ldg(idx + k)] * D[i]; }
+};
+struct ScaleCsc {     // same on the column-major copy
+    double *val; const double *val0; const int *idx; const double *O, *D;
+    __device__ void operator()(int j, int k) const { val[k] = val0[k] * O[j] * D[__ldg(idx + k)]; }
+};
+struct TermCsrChat {  // A~ c^
+    const double *val; const int *idx; const double *chat;
+    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * chat[__ldg(idx + k)]; }
+};
+struct EpiRhsD {      // q = b~ + mu A~ c^ ; w = 0 => r = q
+    double *r, *w; const double *btil; double mu; double qq;
+    __device__ void operator()(int i, const double (&a)[1]) {
+        const double q = btil[i] + mu * a[0];
+        r[i] = q;
+        w[i] = 0.0;
+        qq += q * q;
+    }
+};
+struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu O z ; g = 0
+    double *d, *s, *g; const double *chat, *xb, *zb, *O; double mu;
+    __device__ void operator()(int j, const double (&a)[1]) {
+        d[j] = a[0] - mu * chat[j];
+        s[j] = xb[j] / O[j] - mu * O[j] * zb[j];
+        g[j] = 0.0;
+    }
+};
+
+// use_rule = 1: O from steps 5-11 applied to (xb, zb); 0: O already in c.O (cs_set_scaling)
+__global__ void __launch_bounds__(kBlock, 2) k_condition(Ctx c, int use_rule) {
+    __shared__ double smem[kMaxRed * kWarps];
+    GridCtl gc(c.partials, smem);
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    if (use_rule) {
+        double mm[2] = {-INFINITY, -INFINITY};
+        phase_cone_ratio(c, mm[0], mm[1]);
+        grid_reduce<2, OpMax>(mm, gc, -INFINITY);
+        const double spread = mm[0] + mm[1];                      // ln max o - ln min o
+        const double alpha = (spread <= c.t) ? 1.0 : c.t / spread; // step 11; spread 0 => 1
+        for (int j = tid; j < c.n; j += nth) c.O[j] = exp(alpha * c.O[j]);
+    }
+    for (int j = tid; j < c.n; j += nth) c.chat[j] = c.O[j] * c.c[j];   // each thread reads its own O[j]
+    gc.sync();
+    {   // row equilibration D
+        TermRowNorm t{c.R.val0, c.R.idx, c.O};
+        EpiRowScale e{c.D, c.btil, c.b};
+        seg_reduce<1>(c.R, t, e, gc);
+    }
+    gc.sync();
+    {   // A~ = D A O on both copies
+        ScaleCsr f1{c.R.val, c.R.val0, c.R.idx, c.O, c.D};
+        seg_foreach(c.R, f1);
+        ScaleCsc f2{c.C.val, c.C.val0, c.C.idx, c.O, c.D};
+        seg_foreach(c.C, f2);
+    }
+    gc.sync();
+    // d = A~^dagger b~ + (mu/2)(abs_{A~}(c^) - c^) = A~'w_d - mu c^  with (A~A~') w_d = b~ + mu A~ c^
+    TermCsrChat tq{c.R.val, c.R.idx, c.chat};
+    EpiRhsD eq{c.r, c.w, c.btil, c.mu, 0.0};
+    seg_reduce<1>(c.R, tq, eq, gc);
+    double red[1] = {eq.qq};
+    grid_reduce<1>(red, gc);
+    bool hm;
+    const int steps = cg_solve(c, gc, red[0], red[0], hm);
+    TermCscW tw{c.C.val, c.C.idx, c.w};
+    EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
+    seg_reduce<1>(c.C, tw, ed, gc);
+    gc.sync();
+    for (int i = tid; i < c.m; i += nth) { c.wd[i] = c.w[i]; c.w[i] = 0.0; }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        c.sc->n_cond += 1;
+        c.sc->cg_steps_total += steps;
+        c.sc->cg_steps_cond += steps;
+        c.sc->cg_steps_last = steps;
+        if (hm) c.sc->cg_hit_max = 1;
+    }
+}
+
+// ---- residuals (original coordinates; xb, zb must be current) --------------------------------
+struct TermCsrX {     // A~ x^ with x^ = x/O
+    const double *val; const int *idx; const double *xb, *O;
+    __device__ void operator()(int k, double (&a)[1]) const {
+        const int j = __ldg(idx + k);
+        a[0] += val[k] * (xb[j] / O[j]);
+    }
+};
+struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
+    const double *btil, *D, *wd, *w; double mu; double pres2, by;
+    __device__ void operator()(int i, const double (&a)[1]) {
+        const double e = (a[0] - btil[i]) / D[i];
+        pres2 += e * e;
+        by += btil[i] * (wd[i] - w[i]) / mu;
+    }
+};
+struct TermCscY {     // A~' y'
+    const double *val; const int *idx; const double *wd, *w; double mu;
+    __device__ void operator()(int k, double (&a)[1]) const {
+        const int i = __ldg(idx + k);
+        a[0] += val[k] * ((wd[i] - w[i]) / mu);
+    }
+};
+struct EpiDres {      // (c - z - A'y)_j = c_j - z_j - (A~'y')_j / O_j
+    const double *cc, *xb, *zb, *O; double dres2, cx, nx2, nz2;
+    __device__ void operator()(int j, const double (&a)[1]) {
+        const double e = cc[j] - zb[j] - a[0] / O[j];
+        dres2 += e * e;
+        cx += cc[j] * xb[j];
+        nx2 += xb[j] * xb[j];
+        nz2 += zb[j] * zb[j];
+    }
+};
+
+// squared distance of one Lorentz block to the cone: 0 | ||v||^2 | (||u|| - t)^2 / 2
+__device__ __forceinline__ double soc_dist2(double t, double nu2) {
+    const double nu = sqrt(nu2);
+    if (nu <= t) return 0.0;
+    if (nu <= -t) return t * t + nu2;
+    return 0.5 * (nu - t) * (nu - t);
+}
+
+__global__ void __launch_bounds__(kBlock, 2) k_residuals(Ctx c) {
+    __shared__ double smem[kMaxRed * kWarps];
+    GridCtl gc(c.partials, smem);
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    TermCsrX t1{c.R.val, c.R.idx, c.xb, c.O};
+    EpiPres e1{c.btil, c.D, c.wd, c.w, c.mu, 0.0, 0.0};
+    seg_reduce<1>(c.R, t1, e1, gc);
+    TermCscY t2{c.C.val, c.C.idx, c.wd, c.w, c.mu};
+    EpiDres e2{c.c, c.xb, c.zb, c.O, 0.0, 0.0, 0.0, 0.0};
+    seg_reduce<1>(c.C, t2, e2, gc);
+    double vx = 0.0, vz = 0.0;
+    for (int j = tid; j < c.n_lin; j += nth) {
+        const double a = fmin(c.xb[j], 0.0), b = fmin(c.zb[j], 0.0);
+        vx += a * a;
+        vz += b * b;
+    }
+    if (c.n_soc) {
+        const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
+        constexpr int CPW = 32 / kConeLanes;
+        const int gwarp = tid >> 5, nwarps = nth >> 5;
+        for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
+            const int ci = base + sub;
+            const bool act = ci < c.n_soc;
+            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
+            double nx = 0.0, nz = 0.0;
+            for (int j = a + 1 + sl; j < b; j += kConeLanes) { nx += c.xb[j] * c.xb[j]; nz += c.zb[j] * c.zb[j]; }
+            nx = group_reduce<kConeLanes>(nx);
+            nz = group_reduce<kConeLanes>(nz);
+            if (act && sl == 0) { vx += soc_dist2(c.xb[a], nx); vz += soc_dist2(c.zb[a], nz); }
+        }
+    }
+    double red[8] = {e1.pres2, e1.by, e2.dres2, e2.cx, e2.nx2, e2.nz2, vx, vz};
+    grid_reduce<8>(red, gc);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        double *o = c.sc->resid;
+        const double pres = sqrt(red[0]), by = red[1], dres = sqrt(red[2]), cx = red[3];
+        o[0] = pres; o[1] = pres / (1.0 + c.norm_b);
+        o[2] = dres; o[3] = dres / (1.0 + c.norm_c);
+        o[4] = fabs(cx - by); o[5] = o[4] / (1.0 + fabs(cx) + fabs(by));
+        o[6] = (sqrt(red[6]) + sqrt(red[7])) / (1.0 + sqrt(red[4]) + sqrt(red[5]));
+        o[7] = fmax(fmax(o[1], o[3]), fmax(o[5], o[6]));
+        o[8] = cx; o[9] = by; o[10] = sqrt(c.sc->fp_res2);
+    }
+}
+
+}  // namespace csd

@@ -66,17 +66,23 @@ class Problem:
 # sparse patterns
 # --------------------------------------------------------------------------------------------
 
-def _finish_csr(rows, cols, vals, m, n, rng):
-    """COO -> canonical CSR (sorted, unique); every empty row gets one N(0,1) entry in a uniform
-    random column (SURVEY 8(d) cfg 4 policy, applied to every generator)."""
+def _finish_csr(rows, cols, vals, m, n, rng, min_row_nnz=1):
+    """COO -> canonical CSR (sorted, unique).  Every row is topped up to at least `min_row_nnz` entries
+    with N(0,1) values in uniform random columns (BASELINE.json is silent on empty / very short rows;
+    DESIGN.md "Input recipe": with fewer than ~3 entries per row the Zipf matrices are rank-deficient
+    w.h.p. -- singleton rows sharing a column -- which breaks the paper's full-row-rank assumption)."""
     A = sp.csr_matrix((vals, (rows, cols)), shape=(m, n))
     A.sum_duplicates()
-    counts = np.diff(A.indptr)
-    empty = np.flatnonzero(counts == 0)
-    if empty.size:
-        ec = rng.integers(0, n, size=empty.size)
-        ev = rng.standard_normal(empty.size)
-        A = (A + sp.csr_matrix((ev, (empty, ec)), shape=(m, n))).tocsr()
+    for _ in range(50):
+        counts = np.diff(A.indptr)
+        short = np.flatnonzero(counts < min_row_nnz)
+        if not short.size:
+            break
+        rr = np.repeat(short, min_row_nnz - counts[short])
+        cc = rng.integers(0, n, size=rr.size)
+        vv = rng.standard_normal(rr.size)
+        A = (A + sp.csr_matrix((vv, (rr, cc)), shape=(m, n))).tocsr()
+        A.sum_duplicates()
     A.sort_indices()
     A.eliminate_zeros()
     return A
@@ -119,11 +125,11 @@ def _distinct_rows_zipf(rng, m, n, k, s_exp):
     return perm[r]
 
 
-def sparse_fixed_per_column(rng, m, n, k, zipf=None):
+def sparse_fixed_per_column(rng, m, n, k, zipf=None, min_row_nnz=1):
     rows = _distinct_rows_zipf(rng, m, n, k, zipf) if zipf else _distinct_rows_uniform(rng, m, n, k)
     cols = np.repeat(np.arange(n, dtype=np.int64), k)
     vals = rng.standard_normal(n * k)
-    return _finish_csr(rows.reshape(-1), cols, vals, m, n, rng)
+    return _finish_csr(rows.reshape(-1), cols, vals, m, n, rng, min_row_nnz)
 
 
 # --------------------------------------------------------------------------------------------
@@ -205,11 +211,11 @@ def tiny_dense_lp(seed, m=50, n=100, density=0.2, zero_frac=0.4, name="cfg0_tiny
 
 
 def sparse_lp(seed, m, n, per_col, zero_frac=0.5, zipf=None, row_log10=None, col_log10=None,
-              name="sparse_lp"):
+              min_row_nnz=1, name="sparse_lp"):
     """BASELINE.json configs 1, 2, 4: fixed non-zeros per column at uniform (or Zipf) rows, N(0,1);
     optional row/column scaling 10^U(-a,a) (config 2); optimum built on the scaled matrix."""
     rng = np.random.default_rng(seed)
-    A = sparse_fixed_per_column(rng, m, n, per_col, zipf=zipf)
+    A = sparse_fixed_per_column(rng, m, n, per_col, zipf=zipf, min_row_nnz=min_row_nnz)
     if row_log10 is not None:
         A = sp.diags(10.0 ** rng.uniform(-row_log10, row_log10, size=m)) @ A
     if col_log10 is not None:
@@ -321,7 +327,7 @@ def config(idx: int, scale: float = 1.0, seed: int | None = None) -> Problem:
         n = int(round(nc * 20))  # 400,000 / 20,000
         return sparse_socp(seed, sc(sh["m"]), n, nc, sh["per_col"], name=f"cfg3_sparse_socp_x{scale:g}")
     if idx == 4:
-        return sparse_lp(seed, sc(sh["m"]), sc(sh["n"]), sh["per_col"], zipf=1.1,
+        return sparse_lp(seed, sc(sh["m"]), sc(sh["n"]), sh["per_col"], zipf=1.1, min_row_nnz=4,
                          name=f"cfg4_zipf_lp_x{scale:g}")
     raise KeyError(idx)
 
