@@ -137,6 +137,15 @@ static int build_cholesky(orc_solver *S) {
         for (int32_t k = S->row_ptr[i]; k < S->row_ptr[i + 1]; ++k) dense_row[S->col_idx[k]] = 0.0;
     }
     free(dense_row);
+    /* symmetric diagonal equilibration G <- E G E, E = diag(G)^{-1/2} (kept in S->jac as G_ii): the
+     * same solve, w = E (EGE)^{-1} E rhs, but the factorisation error is governed by cond(EGE)
+     * instead of cond(G) (van der Sluis); matters for the badly row-scaled config 2. */
+    for (int64_t i = 0; i < m; ++i) {
+        if (!(G[i * m + i] > 0.0)) return 3;
+        S->jac[i] = G[i * m + i];
+    }
+    for (int64_t i = 0; i < m; ++i)
+        for (int64_t q = 0; q <= i; ++q) G[i * m + q] = G[i * m + q] / (sqrt(S->jac[i]) * sqrt(S->jac[q]));
     /* textbook Cholesky-Banachiewicz, in place on the lower triangle */
     for (int64_t i = 0; i < m; ++i) {
         for (int64_t j = 0; j <= i; ++j) {
@@ -156,8 +165,8 @@ static int build_cholesky(orc_solver *S) {
 static void cholesky_solve(const orc_solver *S, const double *rhs, double *w) {
     const int64_t m = S->m;
     const double *Lc = S->chol;
-    for (int64_t i = 0; i < m; ++i) {                          /* L t = rhs */
-        double acc = rhs[i];
+    for (int64_t i = 0; i < m; ++i) {                          /* L t = E rhs */
+        double acc = rhs[i] / sqrt(S->jac[i]);
         for (int64_t k = 0; k < i; ++k) acc -= Lc[i * m + k] * w[k];
         w[i] = acc / Lc[i * m + i];
     }
@@ -166,22 +175,22 @@ static void cholesky_solve(const orc_solver *S, const double *rhs, double *w) {
         for (int64_t k = i + 1; k < m; ++k) acc -= Lc[k * m + i] * w[k];
         w[i] = acc / Lc[i * m + i];
     }
+    for (int64_t i = 0; i < m; ++i) w[i] = w[i] / sqrt(S->jac[i]);   /* w = E (.) */
 }
 
 /* Jacobi-preconditioned CG on (A_hat A_hat') w = rhs from w = 0 (textbook PCG).  Stops when
- * sqrt(r'M^{-1}r) <= pcg_tol * sqrt(rhs'M^{-1}rhs), on stagnation (no new best for 100 steps) or at
- * pcg_max.  Returns the number of steps. */
+ * sqrt(r'M^{-1}r) <= pcg_tol * sqrt(rhs'M^{-1}rhs) or at pcg_max (flagged in pcg_fail).  Returns the
+ * number of steps. */
 static int64_t pcg_solve(orc_solver *S, const double *rhs, double *w) {
     const int64_t m = S->m, n = S->n;
     double *r = (double *)malloc(sizeof(double) * (size_t)m), *zv = (double *)malloc(sizeof(double) * (size_t)m);
     double *pv = (double *)malloc(sizeof(double) * (size_t)m), *q = (double *)malloc(sizeof(double) * (size_t)m);
-    double *u = (double *)malloc(sizeof(double) * (size_t)n), *best = (double *)malloc(sizeof(double) * (size_t)m);
+    double *u = (double *)malloc(sizeof(double) * (size_t)n);
     double rz = 0.0, ref = 0.0;
-    for (int64_t i = 0; i < m; ++i) { w[i] = 0.0; r[i] = rhs[i]; zv[i] = r[i] / S->jac[i]; pv[i] = zv[i]; best[i] = 0.0; }
+    for (int64_t i = 0; i < m; ++i) { w[i] = 0.0; r[i] = rhs[i]; zv[i] = r[i] / S->jac[i]; pv[i] = zv[i]; }
     for (int64_t i = 0; i < m; ++i) rz += r[i] * zv[i];
     ref = rz;
-    double best_rz = rz;
-    int64_t since_best = 0, it = 0;
+    int64_t it = 0;
     const double thresh = S->pcg_tol * S->pcg_tol * ref;
     while (rz > thresh && it < S->pcg_max) {
         mat_tvec(S, S->val_hat, pv, u);                        /* u = A_hat' p          */
@@ -197,11 +206,9 @@ static int64_t pcg_solve(orc_solver *S, const double *rhs, double *w) {
         for (int64_t i = 0; i < m; ++i) pv[i] = zv[i] + beta * pv[i];
         rz = rz_new;
         ++it;
-        if (rz < best_rz) { best_rz = rz; since_best = 0; memcpy(best, w, sizeof(double) * (size_t)m); }
-        else if (++since_best >= 100) { memcpy(w, best, sizeof(double) * (size_t)m); S->pcg_fail |= 1; break; }
     }
     if (it >= S->pcg_max && rz > thresh) S->pcg_fail |= 2;
-    free(r); free(zv); free(pv); free(q); free(u); free(best);
+    free(r); free(zv); free(pv); free(q); free(u);
     S->pcg_steps_last = it;
     S->pcg_steps_total += it;
     return it;

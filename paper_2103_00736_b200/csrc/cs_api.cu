@@ -292,7 +292,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.mu = 1.0;
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
     S->prm.o_floor = 1e-16;
-    S->prm.cg_tol = 1e-13;
+    S->prm.cg_tol = 1e-15;
     S->prm.cg_max_iter = 20000;
     x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
     sync_params(S);
