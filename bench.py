@@ -117,6 +117,7 @@ def main():
     ap.add_argument("--k", type=int, default=5, help="outer iterations per step")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cg-max-iter", type=int, default=0, help="profiling only: cap CG steps per solve (0 = library default)")
     a = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -149,6 +150,8 @@ def main():
     t_gen = time.perf_counter() - t_gen
     stream = torch.cuda.current_stream()
     S = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
+    if a.cg_max_iter:
+        S.set_params(cg_max_iter=a.cg_max_iter)
 
     def step():
         S.condition()
@@ -212,7 +215,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": p.name, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "k_per_step": a.k,
+            "config": {"workload": p.name, "cg_max_iter_cap": a.cg_max_iter or None, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "k_per_step": a.k,
                        "step": "cs_condition + cs_iterate(k) + cs_residuals", "multi_gpu": "replicas only",
                        "l2": "inputs larger than L2" if 24 * p.nnz > 126e6 else "matrix fits in L2 (flagged)",
                        "gen_s": round(t_gen, 2)},
@@ -235,19 +238,21 @@ def finish(a, p, S, line, rank, world, dev, stream):
     def e2e_step():
         S2 = binding.Solver(p.m, p.n, hin[0].numpy(), hin[1].numpy(), hin[2].numpy(), hin[3].numpy(), hin[4].numpy(),
                             p.n_lin, p.soc_size, stream=stream.cuda_stream)
-        S2.set_params(mu=p.mu, t=p.t)
+        S2.set_params(mu=p.mu, t=p.t, **({"cg_max_iter": a.cg_max_iter} if a.cg_max_iter else {}))
         S2.iterate(a.k)
         S2.condition()
         S2.residuals()
         S2.solution_into(x=hx.numpy(), z=hz.numpy())
         S2.destroy()
-    e2e_step()  # warm-up
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for _ in range(a.e2e_steps):
-        e2e_step()
-    torch.cuda.synchronize()
-    dt = time.perf_counter() - t0
+    dt = float("nan")
+    if a.e2e_steps > 0:
+        e2e_step()  # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(a.e2e_steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
     tt = torch.tensor([dt], device=dev, dtype=torch.float64)
     if world > 1:
         import torch.distributed as dist

@@ -78,59 +78,90 @@ cs_status fetch(cs_solver *S, std::vector<T> &dst, const T *src, size_t count, c
     return CS_OK;
 }
 
-struct HostBins {
-    std::vector<int> short_ids;
-    std::vector<int4> chunks, multi;
-    int n_short = 0, G = 8, n_slots = 0;
-    bool identity = false;
+// Host image of one Sparse (cs_device.cuh): ELL slices for the short segments, chunks for the long ones.
+struct HostSparse {
+    std::vector<int4> slices, chunks, multi;
+    std::vector<int> eidx, lidx;
+    std::vector<double> eval, lval;
+    int n_slots = 0;
 };
 
-HostBins make_bins(const std::vector<int> &ptr) {
-    HostBins hb;
+// ptr/idx/val: compressed segments in INTERNAL numbering (segment s = entries [ptr[s], ptr[s+1])).
+HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx, const std::vector<double> &val) {
+    HostSparse h;
     const int nseg = (int)ptr.size() - 1;
-    long long short_nnz = 0;
-    for (int s = 0; s < nseg; ++s) {
-        const int len = ptr[s + 1] - ptr[s];
-        if (len <= kShortMax) {
-            hb.short_ids.push_back(s);
-            short_nnz += len;
-        } else if (len <= kChunk) {
-            hb.chunks.push_back(make_int4(s, ptr[s], len, -1));
-        } else {
-            const int nch = (len + kChunk - 1) / kChunk;
-            hb.multi.push_back(make_int4(s, hb.n_slots, nch, 0));
-            for (int q = 0; q < nch; ++q) {
-                const int a = ptr[s] + q * kChunk;
-                hb.chunks.push_back(make_int4(s, a, std::min(kChunk, ptr[s + 1] - a), hb.n_slots++));
+    auto flush_run = [&](int a, int b) {  // consecutive short segments [a,b) -> slices of 32
+        for (int s0 = a; s0 < b; s0 += 32) {
+            const int cnt = std::min(32, b - s0);
+            int width = 0;
+            for (int q = 0; q < cnt; ++q) width = std::max(width, ptr[s0 + q + 1] - ptr[s0 + q]);
+            const int off = (int)h.eval.size();
+            h.slices.push_back(make_int4(off, s0, cnt, width));
+            h.eval.resize((size_t)off + 32u * width, 0.0);
+            h.eidx.resize((size_t)off + 32u * width, 0);
+            for (int q = 0; q < 32; ++q) {
+                const int seg = s0 + std::min(q, cnt - 1);      // padding lanes replicate a valid index
+                const int len = ptr[seg + 1] - ptr[seg];
+                for (int k = 0; k < width; ++k) {
+                    const int src = ptr[seg] + std::min(k, len - 1);
+                    h.eidx[(size_t)off + 32u * k + q] = idx[src];
+                    if (q < cnt && k < len) h.eval[(size_t)off + 32u * k + q] = val[src];
+                }
             }
         }
+    };
+    int run = 0;
+    for (int s = 0; s < nseg; ++s) {
+        const int len = ptr[s + 1] - ptr[s];
+        if (len <= kShortMax) continue;
+        flush_run(run, s);
+        run = s + 1;
+        const int base = (int)h.lval.size();
+        h.lval.insert(h.lval.end(), val.begin() + ptr[s], val.begin() + ptr[s + 1]);
+        h.lidx.insert(h.lidx.end(), idx.begin() + ptr[s], idx.begin() + ptr[s + 1]);
+        if (len <= kChunk) {
+            h.chunks.push_back(make_int4(s, base, len, -1));
+        } else {
+            const int nch = (len + kChunk - 1) / kChunk;
+            h.multi.push_back(make_int4(s, h.n_slots, nch, 0));
+            for (int q = 0; q < nch; ++q)
+                h.chunks.push_back(make_int4(s, base + q * kChunk, std::min(kChunk, len - q * kChunk), h.n_slots++));
+        }
     }
-    hb.n_short = (int)hb.short_ids.size();
-    hb.identity = hb.n_short == nseg;
-    const double avg = hb.n_short ? (double)short_nnz / hb.n_short : 1.0;
-    hb.G = 4;
-    while (hb.G < 32 && hb.G < avg) hb.G *= 2;
-    return hb;
+    flush_run(run, nseg);
+    return h;
 }
 
-cs_status upload_bins(cs_solver *S, const HostBins &hb, Bins *out) {
-    out->n_short = hb.n_short;
-    out->G = hb.G;
-    out->short_ids = nullptr;
+cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     cs_status st;
-    if (!hb.identity) {
-        int *p;
-        if ((st = dev_upload(S, &p, hb.short_ids.data(), hb.short_ids.size())) != CS_OK) return st;
-        out->short_ids = p;
-    }
-    int4 *c4, *m4;
-    if ((st = dev_upload(S, &c4, hb.chunks.data(), hb.chunks.size())) != CS_OK) return st;
-    if ((st = dev_upload(S, &m4, hb.multi.data(), hb.multi.size())) != CS_OK) return st;
-    out->n_chunk = (int)hb.chunks.size();
-    out->chunks = c4;
-    out->n_multi = (int)hb.multi.size();
-    out->multi = m4;
-    return dev_zeros(S, &out->partial, (size_t)hb.n_slots * 2);
+    int4 *p4; int *pi; double *pd;
+    if ((st = dev_upload(S, &p4, h.slices.data(), h.slices.size())) != CS_OK) return st; out->slices = p4;
+    if ((st = dev_upload(S, &p4, h.chunks.data(), h.chunks.size())) != CS_OK) return st; out->chunks = p4;
+    if ((st = dev_upload(S, &p4, h.multi.data(), h.multi.size())) != CS_OK) return st; out->multi = p4;
+    if ((st = dev_upload(S, &pi, h.eidx.data(), h.eidx.size())) != CS_OK) return st; out->eidx = pi;
+    if ((st = dev_upload(S, &pi, h.lidx.data(), h.lidx.size())) != CS_OK) return st; out->lidx = pi;
+    if ((st = dev_upload(S, &pd, h.eval.data(), h.eval.size())) != CS_OK) return st; out->eval0 = pd;
+    if ((st = dev_upload(S, &out->eval, h.eval.data(), h.eval.size())) != CS_OK) return st;
+    if ((st = dev_upload(S, &pd, h.lval.data(), h.lval.size())) != CS_OK) return st; out->lval0 = pd;
+    if ((st = dev_upload(S, &out->lval, h.lval.data(), h.lval.size())) != CS_OK) return st;
+    out->n_slice = (int)h.slices.size();
+    out->n_chunk = (int)h.chunks.size();
+    out->n_multi = (int)h.multi.size();
+    return dev_zeros(S, &out->partial, (size_t)h.n_slots * 2);
+}
+
+// Stable sort of segment ids by decreasing length (counting sort); ids >= n_sort keep their place.
+std::vector<int> order_by_length(const std::vector<int> &len, int n_sort) {
+    const int n = (int)len.size();
+    std::vector<int> perm(n);
+    int maxlen = 0;
+    for (int i = 0; i < n_sort; ++i) maxlen = std::max(maxlen, len[i]);
+    std::vector<int> start((size_t)maxlen + 2, 0);
+    for (int i = 0; i < n_sort; ++i) start[(size_t)(maxlen - len[i]) + 1]++;
+    for (int q = 0; q <= maxlen; ++q) start[(size_t)q + 1] += start[q];
+    for (int i = 0; i < n_sort; ++i) perm[start[maxlen - len[i]]++] = i;
+    for (int i = n_sort; i < n; ++i) perm[i] = i;
+    return perm;
 }
 
 cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
@@ -141,8 +172,7 @@ cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
 
 cs_status ensure_xz(cs_solver *S) {
     if (!S->xz_stale) return CS_OK;
-    const int blocks = std::min((S->ctx.n + 255) / 256, 148 * 8);
-    k_materialize_xz<<<blocks, 256, 0, S->stream>>>(S->ctx);
+    k_materialize_xz<<<std::max(1, std::min((S->ctx.n + 255) / 256, 148 * 8)), 256, 0, S->stream>>>(S->ctx);
     CS_CUDA(S, cudaGetLastError());
     S->launches += 1;
     S->xz_stale = false;
@@ -166,6 +196,34 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     if (st != CS_OK) return st;
     S->conditioned = true;
     S->started = true;
+    return CS_OK;
+}
+
+int ew_blocks(int n) { return std::max(1, std::min((n + 255) / 256, 148 * 8)); }
+
+// caller's n-vector (host or device) -> internal order, into dst (device)
+cs_status import_cols(cs_solver *S, double *dst, const double *src, cs_mem where) {
+    const Ctx &c = S->ctx;
+    const double *dsrc = src;
+    if (where == CS_HOST) {
+        CS_CUDA(S, cudaMemcpyAsync(c.e, src, sizeof(double) * c.n, cudaMemcpyHostToDevice, S->stream));  // e = scratch
+        dsrc = c.e;
+    }
+    k_gather_perm<<<ew_blocks(c.n), 256, 0, S->stream>>>(dst, dsrc, c.perm_c, c.n);
+    CS_CUDA(S, cudaGetLastError());
+    S->launches += 1;
+    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    return CS_OK;
+}
+
+// internal n-vector -> caller's order and memory space
+cs_status export_cols(cs_solver *S, double *dst, const double *src, cs_mem where) {
+    const Ctx &c = S->ctx;
+    double *ddst = where == CS_HOST ? c.e : dst;
+    k_scatter_perm<<<ew_blocks(c.n), 256, 0, S->stream>>>(ddst, src, c.perm_c, c.n);
+    CS_CUDA(S, cudaGetLastError());
+    S->launches += 1;
+    if (where == CS_HOST) CS_CUDA(S, cudaMemcpyAsync(dst, c.e, sizeof(double) * c.n, cudaMemcpyDeviceToHost, S->stream));
     return CS_OK;
 }
 
@@ -230,19 +288,49 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     double nb = 0.0, nc = 0.0;
     for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
     for (int j = 0; j < n; ++j) { if (!std::isfinite(hc[j])) { S->err = "non-finite c"; return CS_EINVAL; } nc += hc[j] * hc[j]; }
-    // ---- CSC copy (counting sort by column; rows come out sorted within a column)
-    std::vector<int> cptr((size_t)n + 1, 0), ridx((size_t)nnz);
-    std::vector<double> cval((size_t)nnz);
-    for (int k = 0; k < nnz; ++k) cptr[(size_t)cidx[k] + 1]++;
-    for (int j = 0; j < n; ++j) cptr[(size_t)j + 1] += cptr[j];
+    // ---- internal ordering: rows sorted by decreasing length, orthant columns likewise (Lorentz blocks
+    //      keep their place so that cones stay contiguous).  perm[internal] = caller's index.
+    std::vector<int> rlen((size_t)m), clen((size_t)n, 0);
+    for (int i = 0; i < m; ++i) rlen[i] = rptr[i + 1] - rptr[i];
+    for (int k = 0; k < nnz; ++k) clen[cidx[k]]++;
+    const std::vector<int> perm_r = order_by_length(rlen, m), perm_c = order_by_length(clen, (int)K->n_lin);
+    std::vector<int> inv_c((size_t)n);
+    for (int j = 0; j < n; ++j) inv_c[perm_c[j]] = j;
+    // row-major copy in internal numbering (entries of a row sorted by internal column)
+    std::vector<int> rp2((size_t)m + 1, 0), ci2((size_t)nnz);
+    std::vector<double> va2((size_t)nnz);
     {
-        std::vector<int> fill(cptr.begin(), cptr.end() - 1);
+        std::vector<std::pair<int, double>> tmp;
+        for (int i = 0; i < m; ++i) {
+            const int src = perm_r[i], a0 = rptr[src], len = rlen[src];
+            tmp.resize(len);
+            for (int k = 0; k < len; ++k) tmp[k] = {inv_c[cidx[a0 + k]], val[a0 + k]};
+            std::sort(tmp.begin(), tmp.end(), [](const std::pair<int, double> &u, const std::pair<int, double> &v) { return u.first < v.first; });
+            const int dst = rp2[i];
+            rp2[(size_t)i + 1] = dst + len;
+            for (int k = 0; k < len; ++k) { ci2[dst + k] = tmp[k].first; va2[dst + k] = tmp[k].second; }
+        }
+    }
+    // column-major copy (counting sort by internal column; rows come out sorted within a column)
+    std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
+    std::vector<double> cv2((size_t)nnz);
+    for (int k = 0; k < nnz; ++k) cp2[(size_t)ci2[k] + 1]++;
+    for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] += cp2[j];
+    {
+        std::vector<int> fill(cp2.begin(), cp2.end() - 1);
         for (int i = 0; i < m; ++i)
-            for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
-                const int q = fill[cidx[k]]++;
-                ridx[q] = i;
-                cval[q] = val[k];
+            for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
+                const int q = fill[ci2[k]]++;
+                ri2[q] = i;
+                cv2[q] = va2[k];
             }
+    }
+    {   // b, c in internal order
+        std::vector<double> t((size_t)std::max(m, n));
+        for (int i = 0; i < m; ++i) t[i] = hb[perm_r[i]];
+        std::copy(t.begin(), t.begin() + m, hb.begin());
+        for (int j = 0; j < n; ++j) t[j] = hc[perm_c[j]];
+        std::copy(t.begin(), t.begin() + n, hc.begin());
     }
     // ---- device state
     Ctx &x = S->ctx;
@@ -250,16 +338,10 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     x.norm_b = std::sqrt(nb); x.norm_c = std::sqrt(nc);
     int *ip; double *dp;
     if ((st = dev_upload(S, &ip, cone_off.data(), cone_off.size())) != CS_OK) return st; x.cone_off = ip;
-    if ((st = dev_upload(S, &ip, rptr.data(), rptr.size())) != CS_OK) return st; x.R.ptr = ip;
-    if ((st = dev_upload(S, &ip, cidx.data(), cidx.size())) != CS_OK) return st; x.R.idx = ip;
-    if ((st = dev_upload(S, &dp, val.data(), val.size())) != CS_OK) return st; x.R.val0 = dp;
-    if ((st = dev_upload(S, &x.R.val, val.data(), val.size())) != CS_OK) return st;
-    if ((st = dev_upload(S, &ip, cptr.data(), cptr.size())) != CS_OK) return st; x.C.ptr = ip;
-    if ((st = dev_upload(S, &ip, ridx.data(), ridx.size())) != CS_OK) return st; x.C.idx = ip;
-    if ((st = dev_upload(S, &dp, cval.data(), cval.size())) != CS_OK) return st; x.C.val0 = dp;
-    if ((st = dev_upload(S, &x.C.val, cval.data(), cval.size())) != CS_OK) return st;
-    if ((st = upload_bins(S, make_bins(rptr), &x.R.bins)) != CS_OK) return st;
-    if ((st = upload_bins(S, make_bins(cptr), &x.C.bins)) != CS_OK) return st;
+    if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
+    if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
+    if ((st = upload_sparse(S, make_sparse(rp2, ci2, va2), &x.R)) != CS_OK) return st;
+    if ((st = upload_sparse(S, make_sparse(cp2, ri2, cv2), &x.C)) != CS_OK) return st;
     if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
     if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
     double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.d, &x.chat};
@@ -339,11 +421,9 @@ cs_status cs_get_params(const cs_solver *S, cs_params *p) {
 cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem where) {
     if (!S || !x || !z) return CS_EINVAL;
     if (S->started) { S->err = "cs_set_point after the iteration has started"; return CS_ESTATE; }
-    const cudaMemcpyKind kind = where == CS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
-    CS_CUDA(S, cudaMemcpyAsync(S->ctx.xb, x, sizeof(double) * S->ctx.n, kind, S->stream));
-    CS_CUDA(S, cudaMemcpyAsync(S->ctx.zb, z, sizeof(double) * S->ctx.n, kind, S->stream));
-    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));
-    return CS_OK;
+    cs_status st;
+    if ((st = import_cols(S, S->ctx.xb, x, where)) != CS_OK) return st;
+    return import_cols(S, S->ctx.zb, z, where);
 }
 
 cs_status cs_condition(cs_solver *S) {
@@ -355,9 +435,7 @@ cs_status cs_set_scaling(cs_solver *S, const double *O, cs_mem where) {
     if (!S || !O) return CS_EINVAL;
     cs_status st = ensure_xz(S);  // x,z of the OLD scaling, before O is overwritten
     if (st != CS_OK) return st;
-    const cudaMemcpyKind kind = where == CS_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
-    CS_CUDA(S, cudaMemcpyAsync(S->ctx.O, O, sizeof(double) * S->ctx.n, kind, S->stream));
-    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    if ((st = import_cols(S, S->ctx.O, O, where)) != CS_OK) return st;
     return do_condition(S, 0);
 }
 
@@ -400,14 +478,13 @@ cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, 
     if ((st = ensure_xz(S)) != CS_OK) return st;
     const Ctx &c = S->ctx;
     const cudaMemcpyKind kind = where == CS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
-    const size_t nb = sizeof(double) * c.n;
-    if (x) CS_CUDA(S, cudaMemcpyAsync(x, c.xb, nb, kind, S->stream));
-    if (z) CS_CUDA(S, cudaMemcpyAsync(z, c.zb, nb, kind, S->stream));
-    if (s) CS_CUDA(S, cudaMemcpyAsync(s, c.s, nb, kind, S->stream));
-    if (O) CS_CUDA(S, cudaMemcpyAsync(O, c.O, nb, kind, S->stream));
+    if (x && (st = export_cols(S, x, c.xb, where)) != CS_OK) return st;
+    if (z && (st = export_cols(S, z, c.zb, where)) != CS_OK) return st;
+    if (s && (st = export_cols(S, s, c.s, where)) != CS_OK) return st;
+    if (O && (st = export_cols(S, O, c.O, where)) != CS_OK) return st;
     if (y) {
         double *ydev = where == CS_DEVICE ? y : c.r;  // r is scratch between solves
-        k_dual_y<<<std::min((c.m + 255) / 256, 148 * 8), 256, 0, S->stream>>>(c, ydev);
+        k_dual_y<<<ew_blocks(c.m), 256, 0, S->stream>>>(c, ydev);
         CS_CUDA(S, cudaGetLastError());
         S->launches += 1;
         if (where == CS_HOST) CS_CUDA(S, cudaMemcpyAsync(y, ydev, sizeof(double) * c.m, kind, S->stream));

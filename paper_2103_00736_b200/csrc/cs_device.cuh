@@ -18,24 +18,28 @@ constexpr int kShortMax = 64;        // segments up to this many non-zeros are "
 constexpr int kChunk = 1024;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
 
-// Work partition of one sparse format (rows of the CSR copy or columns of the CSC copy).
-struct Bins {
-    int n_short;            // number of short segments
-    const int *short_ids;   // their ids, or nullptr when every segment is short (identity)
-    int G;                  // lanes per short segment: 4, 8, 16 or 32
-    int n_chunk;            // chunks of long segments, one warp each
-    const int4 *chunks;     // {segment id, first nnz, length, slot}; slot < 0: chunk == whole segment
-    int n_multi;            // long segments spanning several chunks
+// One sparse format (rows of the CSR-like copy or columns of the CSC-like copy), stored in two parts:
+//  * ELL part: runs of consecutive short segments cut into slices of 32; slice s holds 32 x width
+//    entries laid out [k][lane] so that lane l reads entry k of segment seg0+l at off + 32k + l
+//    (fully coalesced, one thread per segment, no shuffles).  Padding entries have val = 0 and a valid
+//    index.  Rows (and orthant columns) are physically sorted by length at cs_create, so padding is
+//    negligible.
+//  * long part: segments longer than kShortMax, cut into chunks of kChunk entries, one warp each;
+//    segments spanning several chunks are finished from per-chunk partial sums in fixed order.
+struct Sparse {
+    int n_slice;
+    const int4 *slices;     // {offset into e*, first segment id, segments in the slice (<=32), width}
+    const int *eidx;
+    double *eval;           // scaled values (D A O)
+    const double *eval0;    // pristine values (A)
+    int n_chunk;
+    const int4 *chunks;     // {segment id, first entry in l*, length, slot}; slot < 0: chunk == whole segment
+    const int *lidx;
+    double *lval;
+    const double *lval0;
+    int n_multi;
     const int4 *multi;      // {segment id, first slot, number of slots, 0}
-    double *partial;        // one partial sum per slot
-};
-
-struct Sparse {             // one compressed format: segment pointers, minor indices, values
-    const int *ptr;
-    const int *idx;
-    double *val;            // scaled values  (D A O)
-    const double *val0;     // pristine values (A)
-    Bins bins;
+    double *partial;        // [slots][2]
 };
 
 struct Scalars {            // device-resident state scalars (read back only by cs_residuals)
@@ -48,7 +52,8 @@ struct Scalars {            // device-resident state scalars (read back only by 
 struct Ctx {
     int m, n, n_lin, n_soc;
     const int *cone_off;    // [n_soc+1] absolute offsets of the Lorentz blocks (cone_off[0] = n_lin)
-    Sparse R, C;            // CSR (segments = rows) and CSC (segments = columns) copies of A
+    const int *perm_r, *perm_c;  // internal index -> caller's index (rows / columns sorted by length)
+    Sparse R, C;            // row-major (segments = rows) and column-major (segments = columns) copies of A
     // n-vectors
     double *s, *p, *g, *e, *u, *d, *chat, *O, *xb, *zb;
     const double *c;
@@ -117,59 +122,75 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Segment traversals.  `term(k, out)` adds the contribution of non-zero k to out[NV];
-// `epi(seg, sums)` is called by ONE lane per segment with the complete sums.
-// Long segments first (warp per chunk), then short segments (G lanes each), then the segments that
-// span several chunks (after a grid barrier, from their per-chunk partial sums, in fixed order).
+// Segment traversals.  `term(a, j, acc)` adds the contribution of one entry (value a, minor index j)
+// to acc[NV]; `epi(seg, sums)` is called once per segment with the complete sums.
+// Long segments first (warp per chunk), then the ELL slices (thread per segment), then the segments
+// that span several chunks (after a grid barrier, from their partial sums, in fixed order).
+// The matrix streams use ld.global.cs (evict-first) so that the gathered vectors stay in L2.
 // ---------------------------------------------------------------------------------------------
-template <int NV, int G, class Term, class Epi>
-__device__ __forceinline__ void seg_reduce_G(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
-    const Bins &B = S.bins;
+template <int NV, bool PRISTINE, class Term, class Epi>
+__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
     const int lane = threadIdx.x & 31;
     const int gwarp = (blockIdx.x * kBlock + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * kBlock) >> 5;
-    for (int c = gwarp; c < B.n_chunk; c += nwarps) {
-        const int4 ch = __ldg(B.chunks + c);
-        double acc[NV];
+    {
+        const double *lv = PRISTINE ? S.lval0 : S.lval;
+        for (int c = gwarp; c < S.n_chunk; c += nwarps) {
+            const int4 ch = __ldg(S.chunks + c);
+            double acc[NV];
 #pragma unroll
-        for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-        for (int k = ch.y + lane; k < ch.y + ch.z; k += 32) term(k, acc);
+            for (int i = 0; i < NV; ++i) acc[i] = 0.0;
+            int k = ch.y + lane;
+            const int end = ch.y + ch.z;
+            for (; k + 96 < end; k += 128) {
+                double a[4]; int j[4];
 #pragma unroll
-        for (int i = 0; i < NV; ++i) acc[i] = group_reduce<32>(acc[i]);
-        if (lane == 0) {
-            if (ch.w < 0) epi(ch.x, acc);
-            else {
+                for (int q = 0; q < 4; ++q) { a[q] = __ldcs(lv + k + 32 * q); j[q] = __ldcs(S.lidx + k + 32 * q); }
 #pragma unroll
-                for (int i = 0; i < NV; ++i) B.partial[(size_t)ch.w * NV + i] = acc[i];
+                for (int q = 0; q < 4; ++q) term(a[q], j[q], acc);
+            }
+            for (; k < end; k += 32) term(__ldcs(lv + k), __ldcs(S.lidx + k), acc);
+#pragma unroll
+            for (int i = 0; i < NV; ++i) acc[i] = group_reduce<32>(acc[i]);
+            if (lane == 0) {
+                if (ch.w < 0) epi(ch.x, acc);
+                else {
+#pragma unroll
+                    for (int i = 0; i < NV; ++i) S.partial[(size_t)ch.w * 2 + i] = acc[i];
+                }
             }
         }
     }
-    constexpr int SPW = 32 / G;
-    const int sub = lane / G, sl = lane % G;
-    for (int base = gwarp * SPW; base < B.n_short; base += nwarps * SPW) {
-        const int si = base + sub;
-        int seg = -1;
-        double acc[NV];
+    {
+        const double *ev = PRISTINE ? S.eval0 : S.eval;
+        for (int s = gwarp; s < S.n_slice; s += nwarps) {
+            const int4 sl = __ldg(S.slices + s);
+            const double *vp = ev + sl.x + lane;
+            const int *ip = S.eidx + sl.x + lane;
+            double acc[NV];
 #pragma unroll
-        for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-        if (si < B.n_short) {
-            seg = B.short_ids ? __ldg(B.short_ids + si) : si;
-            const int a = __ldg(S.ptr + seg), b = __ldg(S.ptr + seg + 1);
-            for (int k = a + sl; k < b; k += G) term(k, acc);
+            for (int i = 0; i < NV; ++i) acc[i] = 0.0;
+            int k = 0;
+            for (; k + 4 <= sl.w; k += 4) {
+                double a[4]; int j[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) { a[q] = __ldcs(vp + 32 * (k + q)); j[q] = __ldcs(ip + 32 * (k + q)); }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) term(a[q], j[q], acc);
+            }
+            for (; k < sl.w; ++k) term(__ldcs(vp + 32 * k), __ldcs(ip + 32 * k), acc);
+            if (lane < sl.z) epi(sl.y + lane, acc);
         }
-#pragma unroll
-        for (int i = 0; i < NV; ++i) acc[i] = group_reduce<G>(acc[i]);
-        if (seg >= 0 && sl == 0) epi(seg, acc);
     }
-    if (B.n_multi) {
+    if (S.n_multi) {
         gc.sync();
-        for (int r = gwarp; r < B.n_multi; r += nwarps) {
-            const int4 mr = __ldg(B.multi + r);
+        for (int r = gwarp; r < S.n_multi; r += nwarps) {
+            const int4 mr = __ldg(S.multi + r);
             double acc[NV];
 #pragma unroll
             for (int i = 0; i < NV; ++i) {
                 double a = 0.0;
-                for (int k = lane; k < mr.z; k += 32) a += __ldcg(B.partial + (size_t)(mr.y + k) * NV + i);
+                for (int k = lane; k < mr.z; k += 32) a += __ldcg(S.partial + (size_t)(mr.y + k) * 2 + i);
                 acc[i] = group_reduce<32>(a);
             }
             if (lane == 0) epi(mr.x, acc);
@@ -177,35 +198,21 @@ __device__ __forceinline__ void seg_reduce_G(const Sparse &S, Term &term, Epi &e
     }
 }
 
-template <int NV, class Term, class Epi>
-__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
-    switch (S.bins.G) {
-        case 4: seg_reduce_G<NV, 4>(S, term, epi, gc); break;
-        case 8: seg_reduce_G<NV, 8>(S, term, epi, gc); break;
-        case 16: seg_reduce_G<NV, 16>(S, term, epi, gc); break;
-        default: seg_reduce_G<NV, 32>(S, term, epi, gc); break;
-    }
-}
-
-// Visit every non-zero once with its segment id: f(seg, k).  Same partition as seg_reduce.
+// Rewrite every stored entry: val = f(seg, val0, idx).  Same partition as seg_reduce.
 template <class F>
-__device__ __forceinline__ void seg_foreach(const Sparse &S, F &f) {
-    const Bins &B = S.bins;
+__device__ __forceinline__ void seg_rescale(const Sparse &S, F &f) {
     const int lane = threadIdx.x & 31;
     const int gwarp = (blockIdx.x * kBlock + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * kBlock) >> 5;
-    for (int c = gwarp; c < B.n_chunk; c += nwarps) {
-        const int4 ch = __ldg(B.chunks + c);
-        for (int k = ch.y + lane; k < ch.y + ch.z; k += 32) f(ch.x, k);
+    for (int c = gwarp; c < S.n_chunk; c += nwarps) {
+        const int4 ch = __ldg(S.chunks + c);
+        for (int k = ch.y + lane; k < ch.y + ch.z; k += 32) S.lval[k] = f(ch.x, S.lval0[k], __ldg(S.lidx + k));
     }
-    const int G = B.G, SPW = 32 / G;
-    const int sub = lane / G, sl = lane % G;
-    for (int base = gwarp * SPW; base < B.n_short; base += nwarps * SPW) {
-        const int si = base + sub;
-        if (si < B.n_short) {
-            const int seg = B.short_ids ? __ldg(B.short_ids + si) : si;
-            const int a = __ldg(S.ptr + seg), b = __ldg(S.ptr + seg + 1);
-            for (int k = a + sl; k < b; k += G) f(seg, k);
+    for (int s = gwarp; s < S.n_slice; s += nwarps) {
+        const int4 sl = __ldg(S.slices + s);
+        if (lane < sl.z) {
+            const int base = sl.x + lane;
+            for (int k = 0; k < sl.w; ++k) S.eval[base + 32 * k] = f(sl.y + lane, S.eval0[base + 32 * k], __ldg(S.eidx + base + 32 * k));
         }
     }
 }

@@ -67,13 +67,9 @@ __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
 //   K2 (rows,    CSR):  v = r + beta v ; w += alpha v ; r -= alpha (A~ u) ; rho' = ||r||^2
 // with alpha = rho/sigma (v'A~A~'v = ||A~'v||^2) and beta = rho'/rho.  Returns the steps done.
 // ---------------------------------------------------------------------------------------------
-struct TermCscR {   // A~' r
-    const double *val; const int *idx; const double *r;
-    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * r[__ldg(idx + k)]; }
-};
-struct TermCsrU {   // A~ u
-    const double *val; const int *idx; const double *u;
-    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * u[__ldg(idx + k)]; }
+struct TermDot {    // sum_k a_k x[j_k]  (A~' r, A~ u, A~' w, A~ c^ ...)
+    const double *x;
+    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * x[j]; }
 };
 struct EpiK1 {
     double *u; double beta; double sigma;
@@ -103,17 +99,17 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, d
     hit_max = false;
     while (rho > thresh) {
         if (steps >= c.cg_max_iter) { hit_max = true; break; }
-        TermCscR t1{c.C.val, c.C.idx, c.r};
+        TermDot t1{c.r};
         EpiK1 e1{c.u, beta, 0.0};
-        seg_reduce<1>(c.C, t1, e1, gc);
+        seg_reduce<1, false>(c.C, t1, e1, gc);
         double red[1] = {e1.sigma};
         grid_reduce<1>(red, gc);
         const double sigma = red[0];
         if (!(sigma > 0.0)) break;
         const double alpha = rho / sigma;
-        TermCsrU t2{c.R.val, c.R.idx, c.u};
+        TermDot t2{c.u};
         EpiK2 e2{c.v, c.w, c.r, alpha, beta, 0.0};
-        seg_reduce<1>(c.R, t2, e2, gc);
+        seg_reduce<1, false>(c.R, t2, e2, gc);
         red[0] = e2.rho;
         grid_reduce<1>(red, gc);
         beta = red[0] / rho;
@@ -127,12 +123,10 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, d
 // k_iterate
 // ---------------------------------------------------------------------------------------------
 struct TermCsrPE {  // (A~ p, A~ (p - g))
-    const double *val; const int *idx; const double *p, *e;
-    __device__ void operator()(int k, double (&a)[2]) const {
-        const int j = __ldg(idx + k);
-        const double vk = val[k];
-        a[0] += vk * p[j];
-        a[1] += vk * e[j];
+    const double *p, *e;
+    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[2]) const {
+        acc[0] += a * p[j];
+        acc[1] += a * e[j];
     }
 };
 struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r||^2
@@ -142,10 +136,6 @@ struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r
         qq += a[0] * a[0];
         rho += a[1] * a[1];
     }
-};
-struct TermCscW {   // A~' w
-    const double *val; const int *idx; const double *w;
-    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * w[__ldg(idx + k)]; }
 };
 struct EpiUpdate {  // steps 17-18: r = 2 A~'w - p ; s <- s/2 - r/2 + d = (s+p)/2 - A~'w + d
     double *s, *g; const double *p, *d; double fp2;
@@ -168,18 +158,18 @@ __global__ void __launch_bounds__(kBlock, 2) k_iterate(Ctx c, long long k_iter) 
     for (long long it = 0; it < k_iter; ++it) {
         phase_cone_reflect(c);                                   // step 16
         gc.sync();
-        TermCsrPE tq{c.R.val, c.R.idx, c.p, c.e};
+        TermCsrPE tq{c.p, c.e};
         EpiRhs eq{c.r, 0.0, 0.0};
-        seg_reduce<2>(c.R, tq, eq, gc);
+        seg_reduce<2, false>(c.R, tq, eq, gc);
         double red[2] = {eq.qq, eq.rho};
         grid_reduce<2>(red, gc);
         bool hm;
         cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
         any_max |= hm;
         cg_total += cg_last;
-        TermCscW tw{c.C.val, c.C.idx, c.w};
+        TermDot tw{c.w};
         EpiUpdate eu{c.s, c.g, c.p, c.d, 0.0};
-        seg_reduce<1>(c.C, tw, eu, gc);                          // steps 17-18
+        seg_reduce<1, false>(c.C, tw, eu, gc);                   // steps 17-18
         double rf[1] = {eu.fp2};
         grid_reduce<1>(rf, gc);
         fp2 = rf[0];

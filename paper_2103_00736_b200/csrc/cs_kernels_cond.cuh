@@ -16,9 +16,19 @@ __global__ void k_materialize_xz(Ctx c) {
 }
 
 // y = D (w_d - w) / mu  (derived multiplier; s+ = x~ - mu(c^ - A~'y'), y' = (w_d - w)/mu)
-__global__ void k_dual_y(Ctx c, double *y) {
+__global__ void k_dual_y(Ctx c, double *y) {   // written in the caller's (original) row order
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
-    for (int i = tid; i < c.m; i += nth) y[i] = c.D[i] * (c.wd[i] - c.w[i]) / c.mu;
+    for (int i = tid; i < c.m; i += nth) y[c.perm_r[i]] = c.D[i] * (c.wd[i] - c.w[i]) / c.mu;
+}
+
+// internal (sorted) order <-> caller's order: dst[i] = src[perm[i]]  /  dst[perm[i]] = src[i]
+__global__ void k_gather_perm(double *dst, const double *src, const int *perm, int n) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int i = tid; i < n; i += nth) dst[i] = src[perm[i]];
+}
+__global__ void k_scatter_perm(double *dst, const double *src, const int *perm, int n) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int i = tid; i < n; i += nth) dst[perm[i]] = src[i];
 }
 
 // ---- steps 5-9: o per cone (stored as ln o in c.O), then max / min of ln o -------------------
@@ -53,11 +63,11 @@ __device__ __forceinline__ void phase_cone_ratio(const Ctx &c, double &lmax, dou
     }
 }
 
-struct TermRowNorm {  // sum_j (A_ij O_j)^2
-    const double *val0; const int *idx; const double *O;
-    __device__ void operator()(int k, double (&a)[1]) const {
-        const double x = val0[k] * O[__ldg(idx + k)];
-        a[0] += x * x;
+struct TermRowNorm {  // sum_j (A_ij O_j)^2   (traversed over the PRISTINE values)
+    const double *O;
+    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const {
+        const double x = a * O[j];
+        acc[0] += x * x;
     }
 };
 struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b
@@ -68,17 +78,13 @@ struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b
         btil[i] = di * b[i];
     }
 };
-struct ScaleCsr {     // A~_ij = D_i A_ij O_j on the row-major copy
-    double *val; const double *val0; const int *idx; const double *O, *D;
-    __device__ void operator()(int i, int k) const { val[k] = val0[k] * O[__ldg(idx + k)] * D[i]; }
+struct ScaleCsr {     // A~_ij = D_i A_ij O_j on the row-major copy (segment = row i, minor = column j)
+    const double *O, *D;
+    __device__ __forceinline__ double operator()(int i, double a0, int j) const { return a0 * O[j] * D[i]; }
 };
-struct ScaleCsc {     // same on the column-major copy
-    double *val; const double *val0; const int *idx; const double *O, *D;
-    __device__ void operator()(int j, int k) const { val[k] = val0[k] * O[j] * D[__ldg(idx + k)]; }
-};
-struct TermCsrChat {  // A~ c^
-    const double *val; const int *idx; const double *chat;
-    __device__ void operator()(int k, double (&a)[1]) const { a[0] += val[k] * chat[__ldg(idx + k)]; }
+struct ScaleCsc {     // same on the column-major copy (segment = column j, minor = row i)
+    const double *O, *D;
+    __device__ __forceinline__ double operator()(int j, double a0, int i) const { return a0 * O[j] * D[i]; }
 };
 struct EpiRhsD {      // q = b~ + mu A~ c^ ; w = 0 => r = q
     double *r, *w; const double *btil; double mu; double qq;
@@ -114,29 +120,29 @@ __global__ void __launch_bounds__(kBlock, 2) k_condition(Ctx c, int use_rule) {
     for (int j = tid; j < c.n; j += nth) c.chat[j] = c.O[j] * c.c[j];   // each thread reads its own O[j]
     gc.sync();
     {   // row equilibration D
-        TermRowNorm t{c.R.val0, c.R.idx, c.O};
+        TermRowNorm t{c.O};
         EpiRowScale e{c.D, c.btil, c.b};
-        seg_reduce<1>(c.R, t, e, gc);
+        seg_reduce<1, true>(c.R, t, e, gc);
     }
     gc.sync();
     {   // A~ = D A O on both copies
-        ScaleCsr f1{c.R.val, c.R.val0, c.R.idx, c.O, c.D};
-        seg_foreach(c.R, f1);
-        ScaleCsc f2{c.C.val, c.C.val0, c.C.idx, c.O, c.D};
-        seg_foreach(c.C, f2);
+        ScaleCsr f1{c.O, c.D};
+        seg_rescale(c.R, f1);
+        ScaleCsc f2{c.O, c.D};
+        seg_rescale(c.C, f2);
     }
     gc.sync();
     // d = A~^dagger b~ + (mu/2)(abs_{A~}(c^) - c^) = A~'w_d - mu c^  with (A~A~') w_d = b~ + mu A~ c^
-    TermCsrChat tq{c.R.val, c.R.idx, c.chat};
+    TermDot tq{c.chat};
     EpiRhsD eq{c.r, c.w, c.btil, c.mu, 0.0};
-    seg_reduce<1>(c.R, tq, eq, gc);
+    seg_reduce<1, false>(c.R, tq, eq, gc);
     double red[1] = {eq.qq};
     grid_reduce<1>(red, gc);
     bool hm;
     const int steps = cg_solve(c, gc, red[0], red[0], hm);
-    TermCscW tw{c.C.val, c.C.idx, c.w};
+    TermDot tw{c.w};
     EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
-    seg_reduce<1>(c.C, tw, ed, gc);
+    seg_reduce<1, false>(c.C, tw, ed, gc);
     gc.sync();
     for (int i = tid; i < c.m; i += nth) { c.wd[i] = c.w[i]; c.w[i] = 0.0; }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -150,11 +156,8 @@ __global__ void __launch_bounds__(kBlock, 2) k_condition(Ctx c, int use_rule) {
 
 // ---- residuals (original coordinates; xb, zb must be current) --------------------------------
 struct TermCsrX {     // A~ x^ with x^ = x/O
-    const double *val; const int *idx; const double *xb, *O;
-    __device__ void operator()(int k, double (&a)[1]) const {
-        const int j = __ldg(idx + k);
-        a[0] += val[k] * (xb[j] / O[j]);
-    }
+    const double *xb, *O;
+    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * (xb[j] / O[j]); }
 };
 struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
     const double *btil, *D, *wd, *w; double mu; double pres2, by;
@@ -165,11 +168,8 @@ struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
     }
 };
 struct TermCscY {     // A~' y'
-    const double *val; const int *idx; const double *wd, *w; double mu;
-    __device__ void operator()(int k, double (&a)[1]) const {
-        const int i = __ldg(idx + k);
-        a[0] += val[k] * ((wd[i] - w[i]) / mu);
-    }
+    const double *wd, *w; double mu;
+    __device__ __forceinline__ void operator()(double a, int i, double (&acc)[1]) const { acc[0] += a * ((wd[i] - w[i]) / mu); }
 };
 struct EpiDres {      // (c - z - A'y)_j = c_j - z_j - (A~'y')_j / O_j
     const double *cc, *xb, *zb, *O; double dres2, cx, nx2, nz2;
@@ -194,12 +194,12 @@ __global__ void __launch_bounds__(kBlock, 2) k_residuals(Ctx c) {
     __shared__ double smem[kMaxRed * kWarps];
     GridCtl gc(c.partials, smem);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
-    TermCsrX t1{c.R.val, c.R.idx, c.xb, c.O};
+    TermCsrX t1{c.xb, c.O};
     EpiPres e1{c.btil, c.D, c.wd, c.w, c.mu, 0.0, 0.0};
-    seg_reduce<1>(c.R, t1, e1, gc);
-    TermCscY t2{c.C.val, c.C.idx, c.wd, c.w, c.mu};
+    seg_reduce<1, false>(c.R, t1, e1, gc);
+    TermCscY t2{c.wd, c.w, c.mu};
     EpiDres e2{c.c, c.xb, c.zb, c.O, 0.0, 0.0, 0.0, 0.0};
-    seg_reduce<1>(c.C, t2, e2, gc);
+    seg_reduce<1, false>(c.C, t2, e2, gc);
     double vx = 0.0, vz = 0.0;
     for (int j = tid; j < c.n_lin; j += nth) {
         const double a = fmin(c.xb[j], 0.0), b = fmin(c.zb[j], 0.0);
