@@ -161,6 +161,7 @@ def main():
     for _ in range(a.warmup):
         step()
     r0 = S.residuals()
+    ph0 = S.phase_times()
     l0 = S.kernel_launches()
     torch.cuda.synchronize()
     if world > 1:
@@ -206,12 +207,19 @@ def main():
     peak = float(peaks.get("hbm_gbs", 6650.0))
     peak_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     achieved = it_bytes / (ms_iter * 1e-3) / 1e9
+    ph1 = S.phase_times()
+    ph = {k: (ph1[k] - ph0[k]) * 1e-6 for k in ph1 if k not in ("r6", "r7")}   # ms, device globaltimer
+    k1_b, k2_b = 12 * p.nnz + 8 * p.m + 16 * p.n, 12 * p.nnz + 8 * p.n + 52 * p.m
+    phases = {"ms": {k: round(v, 3) for k, v in ph.items()},
+              "K1_GBs": k1_b * cg_iter / max(ph["K1"], 1e-9) / 1e6, "K2_GBs": k2_b * cg_iter / max(ph["K2"], 1e-9) / 1e6,
+              "K1_us": 1e3 * ph["K1"] / max(1, cg_iter), "K2_us": 1e3 * ph["K2"] / max(1, cg_iter),
+              "reduce_us_per_cg": 1e3 * ph["reduce"] / max(1, cg_iter)}
     roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
             "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
             "cg_steps_per_launch": cg_iter / a.steps, "bytes_per_cg_step": cg_bytes,
             "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "frac_of_8TBs": achieved / 8000.0,
-            "kernel_share_of_step": ms_iter / ms_total}
+            "kernel_share_of_step": ms_iter / ms_total, "phases": phases}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",

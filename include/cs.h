@@ -134,6 +134,11 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out);
  * Any pointer may be NULL.  Synchronous when where == CS_HOST. */
 cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where);
 
+/* Device time per phase of k_iterate so far, in ns, measured on the device between grid barriers:
+ * out[0] cone reflect, [1] rhs pass, [2] CG pass K1 (A~'r, columns), [3] CG pass K2 (A~u, rows),
+ * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6], [7] reserved.  One D2H copy + sync. */
+cs_status cs_phase_times(cs_solver *S, double out[8]);
+
 /* Number of kernels the library has launched on this handle so far (for bench accounting). */
 int64_t cs_kernel_launches(const cs_solver *S);
 

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcs.so")
+LIB_PATH = os.environ.get("CS_LIB") or os.path.join(_HERE, "libcs.so")  # CS_LIB: alternative build (tuning only)
 
 CS_OK, CS_EINVAL, CS_ENOMEM, CS_ECUDA, CS_ESTATE, CS_ECGMAX = range(6)
 CS_HOST, CS_DEVICE = 0, 1
@@ -44,7 +44,8 @@ class cs_resid(C.Structure):
 
 
 EXPORTS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
-           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_kernel_launches", "cs_last_error", "cs_destroy")
+           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_phase_times", "cs_kernel_launches", "cs_last_error",
+           "cs_destroy")
 
 _lib = None
 
@@ -73,7 +74,8 @@ def lib():
         L.cs_last_error.restype = C.c_char_p
         L.cs_destroy.argtypes = [vp]
         L.cs_destroy.restype = None
-        for name in EXPORTS[:9]:
+        L.cs_phase_times.argtypes = [vp, C.POINTER(C.c_double)]
+        for name in EXPORTS[:10]:
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -194,6 +196,13 @@ class Solver:
         out["y"] = np.empty(self.m)
         self.solution_into(out["x"], out["z"], out["y"], out["s"], out["O"])
         return out
+
+    def phase_times(self):
+        """Device time per phase of k_iterate so far (ns): cone, rhs, K1, K2, update, reduce."""
+        a = (C.c_double * 8)()
+        self._check(lib().cs_phase_times(self._h, a))
+        names = ("cone", "rhs", "K1", "K2", "update", "reduce", "r6", "r7")
+        return dict(zip(names, [float(x) for x in a]))
 
     def kernel_launches(self):
         return int(lib().cs_kernel_launches(self._h))

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -21,6 +22,7 @@ struct cs_solver {
     cudaStream_t stream = nullptr;
     int device = 0;
     int grid = 0;
+    size_t dyn_smem = 0;       // bytes of dynamic shared memory of k_iterate / k_condition (hot-row cache)
     std::vector<void *> allocs;
     cs_params prm{};
     bool conditioned = false;  // the l=1 conditioning of step 4 has run
@@ -90,24 +92,34 @@ struct HostSparse {
 HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx, const std::vector<double> &val) {
     HostSparse h;
     const int nseg = (int)ptr.size() - 1;
-    auto flush_run = [&](int a, int b) {  // consecutive short segments [a,b) -> slices of 32
-        for (int s0 = a; s0 < b; s0 += 32) {
-            const int cnt = std::min(32, b - s0);
-            int width = 0;
-            for (int q = 0; q < cnt; ++q) width = std::max(width, ptr[s0 + q + 1] - ptr[s0 + q]);
+    // several lanes per segment only pay when there are too few segments to fill the machine (measured:
+    // T>1 is slower once every warp has >= 2 thread-per-segment slices)
+    const bool split = nseg < 300000;
+    auto lg_lanes = [split](int len) { return (!split || len <= 8) ? 0 : len <= 16 ? 1 : len <= 32 ? 2 : 3; };  // T = 1,2,4,8 lanes
+    auto flush_run = [&](int a, int b) {  // consecutive short segments [a,b) -> slices (32 lanes, T lanes per segment)
+        int s0 = a;
+        while (s0 < b) {
+            const int lgT = lg_lanes(ptr[s0 + 1] - ptr[s0]), T = 1 << lgT, cap = 32 / T;
+            int cnt = 1, maxlen = ptr[s0 + 1] - ptr[s0];
+            while (cnt < cap && s0 + cnt < b && lg_lanes(ptr[s0 + cnt + 1] - ptr[s0 + cnt]) <= lgT) {
+                maxlen = std::max(maxlen, ptr[s0 + cnt + 1] - ptr[s0 + cnt]);
+                ++cnt;
+            }
+            const int width = (maxlen + T - 1) / T;
             const int off = (int)h.eval.size();
-            h.slices.push_back(make_int4(off, s0, cnt, width));
+            h.slices.push_back(make_int4(off, s0, cnt | (lgT << 8), width));
             h.eval.resize((size_t)off + 32u * width, 0.0);
             h.eidx.resize((size_t)off + 32u * width, 0);
-            for (int q = 0; q < 32; ++q) {
-                const int seg = s0 + std::min(q, cnt - 1);      // padding lanes replicate a valid index
-                const int len = ptr[seg + 1] - ptr[seg];
+            for (int lane = 0; lane < 32; ++lane) {
+                const int seg = s0 + std::min(lane / T, cnt - 1);   // padding lanes replicate a valid index
+                const int len = ptr[seg + 1] - ptr[seg], t = lane % T;
                 for (int k = 0; k < width; ++k) {
-                    const int src = ptr[seg] + std::min(k, len - 1);
-                    h.eidx[(size_t)off + 32u * k + q] = idx[src];
-                    if (q < cnt && k < len) h.eval[(size_t)off + 32u * k + q] = val[src];
+                    const int e = k * T + t;
+                    h.eidx[(size_t)off + 32u * k + lane] = idx[ptr[seg] + std::min(e, len - 1)];
+                    if (lane / T < cnt && e < len) h.eval[(size_t)off + 32u * k + lane] = val[ptr[seg] + e];
                 }
             }
+            s0 += cnt;
         }
     };
     int run = 0;
@@ -164,8 +176,8 @@ std::vector<int> order_by_length(const std::vector<int> &len, int n_sort) {
     return perm;
 }
 
-cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
-    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, 0, S->stream));
+cs_status launch_coop(cs_solver *S, const void *fn, void **args, size_t smem = 0) {
+    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, smem, S->stream));
     S->launches += 1;
     return CS_OK;
 }
@@ -192,7 +204,7 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     S->ctx.o_floor = S->prm.o_floor;
     sync_params(S);
     void *args[] = {&S->ctx, &use_rule};
-    st = launch_coop(S, (const void *)k_condition, args);
+    st = launch_coop(S, (const void *)k_condition, args, S->dyn_smem);
     if (st != CS_OK) return st;
     S->conditioned = true;
     S->started = true;
@@ -293,7 +305,35 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     std::vector<int> rlen((size_t)m), clen((size_t)n, 0);
     for (int i = 0; i < m; ++i) rlen[i] = rptr[i + 1] - rptr[i];
     for (int k = 0; k < nnz; ++k) clen[cidx[k]]++;
-    const std::vector<int> perm_r = order_by_length(rlen, m), perm_c = order_by_length(clen, (int)K->n_lin);
+    const std::vector<int> perm_r = order_by_length(rlen, m);
+    std::vector<int> perm_c = order_by_length(clen, (int)K->n_lin);
+    {   // Within each length class, order the orthant columns lexicographically by the (internal, i.e.
+        // hottest-first) rows they touch.  Columns sharing the heavy rows of a power-law matrix become
+        // neighbours, so a heavy row's gathers from u run over a few contiguous stretches (coalesced
+        // L1 wavefronts) instead of one sector per entry.  Pure relabelling: results are unchanged.
+        std::vector<int> inv_r((size_t)m);
+        for (int i = 0; i < m; ++i) inv_r[perm_r[i]] = i;
+        std::vector<int> cp0((size_t)n + 1, 0), cr0((size_t)nnz);
+        for (int k = 0; k < nnz; ++k) cp0[(size_t)cidx[k] + 1]++;
+        for (int j = 0; j < n; ++j) cp0[(size_t)j + 1] += cp0[j];
+        std::vector<int> fill(cp0.begin(), cp0.end() - 1);
+        for (int i = 0; i < m; ++i) {           // internal row order => every column list comes out ascending
+            const int src = perm_r[i];
+            for (int k = rptr[src]; k < rptr[src + 1]; ++k) cr0[fill[cidx[k]]++] = i;
+        }
+        constexpr int kDepth = 4;
+        auto less = [&](int a, int b) {
+            const int la = clen[a], lb = clen[b];
+            if (la != lb) return la > lb;
+            const int d = std::min(la, kDepth);
+            for (int q = 0; q < d; ++q) {
+                const int ra = cr0[cp0[a] + q], rb = cr0[cp0[b] + q];
+                if (ra != rb) return ra < rb;
+            }
+            return a < b;
+        };
+        if (rlen[perm_r[0]] > kShortMax) std::sort(perm_c.begin(), perm_c.begin() + K->n_lin, less);
+    }
     std::vector<int> inv_c((size_t)n);
     for (int j = 0; j < n; ++j) inv_c[perm_c[j]] = j;
     // row-major copy in internal numbering (entries of a row sorted by internal column)
@@ -363,14 +403,25 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
     const void *kernels[] = {(const void *)k_iterate, (const void *)k_condition, (const void *)k_residuals};
+    {   // heavy rows (longer than kShortMax) come first in the internal order: cache up to 8192 of them
+        int n_long = 0;
+        while (n_long < m && n_long < 8192 && rp2[(size_t)n_long + 1] - rp2[n_long] > kShortMax) ++n_long;
+        x.hot_rows = n_long;
+        S->dyn_smem = sizeof(double) * (size_t)n_long;
+        if (S->dyn_smem > 48 * 1024) {
+            CS_CUDA(S, cudaFuncSetAttribute((const void *)k_iterate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S->dyn_smem));
+            CS_CUDA(S, cudaFuncSetAttribute((const void *)k_condition, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S->dyn_smem));
+        }
+    }
     for (const void *k : kernels) {
-        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, 0));
+        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, k == (const void *)k_residuals ? 0 : S->dyn_smem));
         occ_min = std::min(occ_min, occ);
     }
     if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
     S->grid = sms * occ_min;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * S->grid)) != CS_OK) return st;
     // ---- defaults (cs.h)
+    x.dbg = getenv("CS_DEBUG") ? atoi(getenv("CS_DEBUG")) : 0;
     S->prm.mu = 1.0;
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
     S->prm.o_floor = 1e-16;
@@ -447,7 +498,7 @@ cs_status cs_iterate(cs_solver *S, int64_t k) {
     sync_params(S);
     long long kk = k;
     void *args[] = {&S->ctx, &kk};
-    if ((st = launch_coop(S, (const void *)k_iterate, args)) != CS_OK) return st;
+    if ((st = launch_coop(S, (const void *)k_iterate, args, S->dyn_smem)) != CS_OK) return st;
     S->xz_stale = true;
     S->started = true;
     return CS_OK;
@@ -470,6 +521,15 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     out->gap_abs = h.resid[4]; out->gap_rel = h.resid[5]; out->cone_viol_rel = h.resid[6]; out->kkt_rel = h.resid[7];
     out->pobj = h.resid[8]; out->dobj = h.resid[9]; out->fp_res = h.resid[10];
     return h.cg_hit_max ? CS_ECGMAX : CS_OK;
+}
+
+cs_status cs_phase_times(cs_solver *S, double out[8]) {
+    if (!S || !out) return CS_EINVAL;
+    Scalars h;
+    CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    for (int i = 0; i < 8; ++i) out[i] = (double)h.phase_ns[i];
+    return CS_OK;
 }
 
 cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where) {

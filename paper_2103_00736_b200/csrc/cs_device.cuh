@@ -11,6 +11,12 @@ namespace cg = cooperative_groups;
 
 namespace csd {
 
+#ifndef CS_UN
+#define CS_UN 8
+#endif
+#ifndef CS_MINB
+#define CS_MINB 2
+#endif
 constexpr int kBlock = 512;          // threads per CTA (16 warps)
 constexpr int kWarps = kBlock / 32;
 constexpr int kMaxRed = 8;           // scalars per grid reduction
@@ -28,7 +34,8 @@ constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
 //    segments spanning several chunks are finished from per-chunk partial sums in fixed order.
 struct Sparse {
     int n_slice;
-    const int4 *slices;     // {offset into e*, first segment id, segments in the slice (<=32), width}
+    const int4 *slices;     // {offset into e*, first segment id, segments in the slice | log2(T) << 8, width};
+                            // T = lanes per segment (1,2,4,8): entry e of segment r sits at lane r*T + e%T, row e/T
     const int *eidx;
     double *eval;           // scaled values (D A O)
     const double *eval0;    // pristine values (A)
@@ -47,7 +54,10 @@ struct Scalars {            // device-resident state scalars (read back only by 
     long long iter, cg_steps_total, cg_steps_cond;
     int cg_steps_last, n_cond, cg_hit_max, pad;
     double fp_res2;         // ||s_new - s||^2 of the last pass
+    unsigned long long phase_ns[8];  // time spent per phase id (kPh*), measured by CTA 0 between grid barriers
 };
+
+enum { kPhCone = 0, kPhRhs = 1, kPhK1 = 2, kPhK2 = 3, kPhUpdate = 4, kPhReduce = 5, kPhCondition = 6, kPhResid = 7 };
 
 struct Ctx {
     int m, n, n_lin, n_soc;
@@ -65,6 +75,8 @@ struct Ctx {
     double mu, t, o_floor, cg_tol;
     int cg_max_iter;
     double norm_b, norm_c;
+    int dbg;                // TEMP debug flags
+    int hot_rows;           // leading (longest) rows whose r / w entries are cached in shared memory for the column passes
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -85,8 +97,32 @@ struct GridCtl {            // per-thread view of the grid barrier state (unifor
     int parity;
     double *partials;
     double *smem;           // [kMaxRed * kWarps]
-    __device__ GridCtl(double *partials_, double *smem_) : grid(cg::this_grid()), parity(0), partials(partials_), smem(smem_) {}
+    unsigned long long t_last, ns[8];
+    __device__ GridCtl(double *partials_, double *smem_) : grid(cg::this_grid()), parity(0), partials(partials_), smem(smem_) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) ns[i] = 0;
+        t_last = now();
+    }
     __device__ void sync() { grid.sync(); }
+    __device__ static unsigned long long now() {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        return t;
+    }
+    // charge the time since the previous lap to phase `id` (only CTA 0 / thread 0 keeps the books)
+    __device__ void lap(int id) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            const unsigned long long t = now();
+            ns[id] += t - t_last;
+            t_last = t;
+        }
+    }
+    __device__ void flush(Scalars *sc) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) sc->phase_ns[i] += ns[i];
+        }
+    }
 };
 
 // Deterministic grid-wide reduction of NR per-thread values; includes ONE grid barrier.
@@ -129,31 +165,34 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
 // The matrix streams use ld.global.cs (evict-first) so that the gathered vectors stay in L2.
 // ---------------------------------------------------------------------------------------------
 template <int NV, bool PRISTINE, class Term, class Epi>
-__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
+__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc, int dbg = 0) {
     const int lane = threadIdx.x & 31;
     const int gwarp = (blockIdx.x * kBlock + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * kBlock) >> 5;
     {
         const double *lv = PRISTINE ? S.lval0 : S.lval;
-        for (int c = gwarp; c < S.n_chunk; c += nwarps) {
+        for (int c = gwarp; c < ((dbg & 2) ? 0 : S.n_chunk); c += nwarps) {
             const int4 ch = __ldg(S.chunks + c);
             double acc[NV];
 #pragma unroll
             for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-            int k = ch.y + lane;
             const int end = ch.y + ch.z;
-            for (; k + 96 < end; k += 128) {
-                double a[4]; int j[4];
+            constexpr int CU = 8;
+            for (int k = ch.y + lane; k < end; k += 32 * CU) {
+                double a[CU]; int j[CU];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) { a[q] = __ldcs(lv + k + 32 * q); j[q] = __ldcs(S.lidx + k + 32 * q); }
+                for (int q = 0; q < CU; ++q) {
+                    const bool ok = k + 32 * q < end;
+                    a[q] = ok ? __ldcs(lv + k + 32 * q) : 0.0;
+                    j[q] = ok ? __ldcs(S.lidx + k + 32 * q) : -1;
+                }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) term(a[q], j[q], acc);
+                for (int q = 0; q < CU; ++q) if (j[q] >= 0) term(a[q], j[q], acc);
             }
-            for (; k < end; k += 32) term(__ldcs(lv + k), __ldcs(S.lidx + k), acc);
 #pragma unroll
             for (int i = 0; i < NV; ++i) acc[i] = group_reduce<32>(acc[i]);
             if (lane == 0) {
-                if (ch.w < 0) epi(ch.x, acc);
+                if (ch.w < 0) epi(ch.x, acc, epi.pre(ch.x));
                 else {
 #pragma unroll
                     for (int i = 0; i < NV; ++i) S.partial[(size_t)ch.w * 2 + i] = acc[i];
@@ -162,27 +201,48 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
         }
     }
     {
+        // ELL slices: one thread per segment.  All loads of a slice row-block are issued before the
+        // first use (predicated 8-wide unroll), the operands of the epilogue are fetched up front
+        // (epi.pre) and the next slice descriptor is prefetched, so that a warp keeps ~20 independent
+        // loads in flight instead of a chain of dependent round trips.
+        constexpr int UN = CS_UN;
         const double *ev = PRISTINE ? S.eval0 : S.eval;
-        for (int s = gwarp; s < S.n_slice; s += nwarps) {
-            const int4 sl = __ldg(S.slices + s);
+        int s = gwarp;
+        int4 sl = s < S.n_slice ? __ldg(S.slices + s) : make_int4(0, 0, 0, 0);
+        if (dbg & 4) s = S.n_slice;
+        while (s < S.n_slice) {
+            const int sn = s + nwarps;
+            const int4 nxt = sn < S.n_slice ? __ldg(S.slices + sn) : make_int4(0, 0, 0, 0);
             const double *vp = ev + sl.x + lane;
             const int *ip = S.eidx + sl.x + lane;
+            const int lgT = sl.z >> 8, T = 1 << lgT;              // lanes per segment in this slice
+            const int seg = sl.y + (lane >> lgT);
+            const bool head = (lane >> lgT) < (sl.z & 255) && (lane & (T - 1)) == 0;
+            typename Epi::Pre pre = epi.pre(head ? seg : sl.y);
             double acc[NV];
 #pragma unroll
             for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-            int k = 0;
-            for (; k + 4 <= sl.w; k += 4) {
-                double a[4]; int j[4];
+            for (int k = 0; k < sl.w; k += UN) {
+                double a[UN]; int j[UN];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) { a[q] = __ldcs(vp + 32 * (k + q)); j[q] = __ldcs(ip + 32 * (k + q)); }
+                for (int q = 0; q < UN; ++q) {
+                    const bool ok = k + q < sl.w;
+                    a[q] = ok ? __ldcs(vp + 32 * (k + q)) : 0.0;
+                    j[q] = ok ? __ldcs(ip + 32 * (k + q)) : -1;
+                }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) term(a[q], j[q], acc);
+                for (int q = 0; q < UN; ++q) if (j[q] >= 0) term(a[q], j[q], acc);
             }
-            for (; k < sl.w; ++k) term(__ldcs(vp + 32 * k), __ldcs(ip + 32 * k), acc);
-            if (lane < sl.z) epi(sl.y + lane, acc);
+            for (int o = T >> 1; o > 0; o >>= 1) {
+#pragma unroll
+                for (int i = 0; i < NV; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
+            }
+            if (head) epi(seg, acc, pre);
+            s = sn;
+            sl = nxt;
         }
     }
-    if (S.n_multi) {
+    if (S.n_multi && !(dbg & 8)) {
         gc.sync();
         for (int r = gwarp; r < S.n_multi; r += nwarps) {
             const int4 mr = __ldg(S.multi + r);
@@ -190,10 +250,19 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
 #pragma unroll
             for (int i = 0; i < NV; ++i) {
                 double a = 0.0;
-                for (int k = lane; k < mr.z; k += 32) a += __ldcg(S.partial + (size_t)(mr.y + k) * 2 + i);
+                const double *pp = S.partial + (size_t)mr.y * 2 + i;
+                int k = lane;
+                for (; k + 224 < mr.z; k += 256) {       // 8 independent loads in flight
+                    double t[8];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) t[q] = __ldcg(pp + (size_t)(k + 32 * q) * 2);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) a += t[q];
+                }
+                for (; k < mr.z; k += 32) a += __ldcg(pp + (size_t)k * 2);
                 acc[i] = group_reduce<32>(a);
             }
-            if (lane == 0) epi(mr.x, acc);
+            if (lane == 0) epi(mr.x, acc, epi.pre(mr.x));
         }
     }
 }
@@ -210,9 +279,10 @@ __device__ __forceinline__ void seg_rescale(const Sparse &S, F &f) {
     }
     for (int s = gwarp; s < S.n_slice; s += nwarps) {
         const int4 sl = __ldg(S.slices + s);
-        if (lane < sl.z) {
-            const int base = sl.x + lane;
-            for (int k = 0; k < sl.w; ++k) S.eval[base + 32 * k] = f(sl.y + lane, S.eval0[base + 32 * k], __ldg(S.eidx + base + 32 * k));
+        const int lgT = sl.z >> 8;
+        if ((lane >> lgT) < (sl.z & 255)) {
+            const int base = sl.x + lane, seg = sl.y + (lane >> lgT);
+            for (int k = 0; k < sl.w; ++k) S.eval[base + 32 * k] = f(seg, S.eval0[base + 32 * k], __ldg(S.eidx + base + 32 * k));
         }
     }
 }

@@ -71,47 +71,77 @@ struct TermDot {    // sum_k a_k x[j_k]  (A~' r, A~ u, A~' w, A~ c^ ...)
     const double *x;
     __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * x[j]; }
 };
+struct NoPre {};
+struct TermNoGather { const double *x; __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * (double)j; } };
+struct TermDotHot { // same, with x[0..H) served from shared memory (the heavy rows of a power-law matrix)
+    const double *x; const double *hot; int H;
+    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const {
+        acc[0] += a * (j < H ? hot[j] : x[j]);
+    }
+};
+__device__ __forceinline__ void fill_hot(double *hot, const double *x, int H) {
+    for (int i = threadIdx.x; i < H; i += kBlock) hot[i] = x[i];
+    __syncthreads();
+}
 struct EpiK1 {
     double *u; double beta; double sigma;
-    __device__ void operator()(int j, const double (&a)[1]) {
-        const double uj = a[0] + beta * u[j];
+    struct Pre { double u; };
+    __device__ __forceinline__ Pre pre(int j) const { return Pre{u[j]}; }
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &q) {
+        const double uj = a[0] + beta * q.u;
         u[j] = uj;
         sigma += uj * uj;
     }
 };
 struct EpiK2 {
     double *v, *w, *r; double alpha, beta; double rho;
-    __device__ void operator()(int i, const double (&a)[1]) {
-        const double ri = r[i];
-        const double vi = ri + beta * v[i];
+    struct Pre { double r, v, w; };
+    __device__ __forceinline__ Pre pre(int i) const { return Pre{r[i], v[i], w[i]}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &q) {
+        const double vi = q.r + beta * q.v;
         v[i] = vi;
-        w[i] += alpha * vi;
-        const double rn = ri - alpha * a[0];
+        w[i] = q.w + alpha * vi;
+        const double rn = q.r - alpha * a[0];
         r[i] = rn;
         rho += rn * rn;
     }
 };
 
-__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, double qq, bool &hit_max) {
+__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double *hot, double rho, double qq, bool &hit_max) {
     const double thresh = c.cg_tol * c.cg_tol * qq;
     double beta = 0.0;
     int steps = 0;
     hit_max = false;
     while (rho > thresh) {
         if (steps >= c.cg_max_iter) { hit_max = true; break; }
-        TermDot t1{c.r};
         EpiK1 e1{c.u, beta, 0.0};
-        seg_reduce<1, false>(c.C, t1, e1, gc);
+        if (c.hot_rows) {
+            fill_hot(hot, c.r, c.hot_rows);
+            TermDotHot t1{c.r, hot, c.hot_rows};
+            seg_reduce<1, false>(c.C, t1, e1, gc);
+        } else {
+            TermDot t1{c.r};
+            seg_reduce<1, false>(c.C, t1, e1, gc);
+        }
+        gc.lap(kPhK1);
         double red[1] = {e1.sigma};
         grid_reduce<1>(red, gc);
+        gc.lap(kPhReduce);
         const double sigma = red[0];
         if (!(sigma > 0.0)) break;
         const double alpha = rho / sigma;
-        TermDot t2{c.u};
         EpiK2 e2{c.v, c.w, c.r, alpha, beta, 0.0};
-        seg_reduce<1, false>(c.R, t2, e2, gc);
+        if (c.dbg & 1) {
+            TermNoGather t2{c.u};
+            seg_reduce<1, false>(c.R, t2, e2, gc, c.dbg);
+        } else {
+            TermDot t2{c.u};
+            seg_reduce<1, false>(c.R, t2, e2, gc, c.dbg);
+        }
+        gc.lap(kPhK2);
         red[0] = e2.rho;
         grid_reduce<1>(red, gc);
+        gc.lap(kPhReduce);
         beta = red[0] / rho;
         rho = red[0];
         ++steps;
@@ -131,7 +161,9 @@ struct TermCsrPE {  // (A~ p, A~ (p - g))
 };
 struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r||^2
     double *r; double qq, rho;
-    __device__ void operator()(int i, const double (&a)[2]) {
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[2], const Pre &) {
         r[i] = a[1];
         qq += a[0] * a[0];
         rho += a[1] * a[1];
@@ -139,41 +171,57 @@ struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r
 };
 struct EpiUpdate {  // steps 17-18: r = 2 A~'w - p ; s <- s/2 - r/2 + d = (s+p)/2 - A~'w + d
     double *s, *g; const double *p, *d; double fp2;
-    __device__ void operator()(int j, const double (&a)[1]) {
-        const double sj = s[j];
-        const double sn = 0.5 * (sj + p[j]) - a[0] + d[j];
+    struct Pre { double s, p, d; };
+    __device__ __forceinline__ Pre pre(int j) const { return Pre{s[j], p[j], d[j]}; }
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &q) {
+        const double sj = q.s;
+        const double sn = 0.5 * (sj + q.p) - a[0] + q.d;
         g[j] = a[0];
         s[j] = sn;
         fp2 += (sn - sj) * (sn - sj);
     }
 };
 
-__global__ void __launch_bounds__(kBlock, 2) k_iterate(Ctx c, long long k_iter) {
+__global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_iter) {
     __shared__ double smem[kMaxRed * kWarps];
+    extern __shared__ double hot[];
     GridCtl gc(c.partials, smem);
     long long cg_total = 0;
     int cg_last = 0;
     bool any_max = false;
     double fp2 = 0.0;
     for (long long it = 0; it < k_iter; ++it) {
+        gc.lap(kPhReduce);
         phase_cone_reflect(c);                                   // step 16
         gc.sync();
+        gc.lap(kPhCone);
         TermCsrPE tq{c.p, c.e};
         EpiRhs eq{c.r, 0.0, 0.0};
         seg_reduce<2, false>(c.R, tq, eq, gc);
+        gc.lap(kPhRhs);
         double red[2] = {eq.qq, eq.rho};
         grid_reduce<2>(red, gc);
+        gc.lap(kPhReduce);
         bool hm;
-        cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
+        cg_last = cg_solve(c, gc, hot, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
         any_max |= hm;
         cg_total += cg_last;
-        TermDot tw{c.w};
         EpiUpdate eu{c.s, c.g, c.p, c.d, 0.0};
-        seg_reduce<1, false>(c.C, tw, eu, gc);                   // steps 17-18
+        if (c.hot_rows) {
+            fill_hot(hot, c.w, c.hot_rows);
+            TermDotHot tw{c.w, hot, c.hot_rows};
+            seg_reduce<1, false>(c.C, tw, eu, gc);               // steps 17-18
+        } else {
+            TermDot tw{c.w};
+            seg_reduce<1, false>(c.C, tw, eu, gc);
+        }
+        gc.lap(kPhUpdate);
         double rf[1] = {eu.fp2};
         grid_reduce<1>(rf, gc);
+        gc.lap(kPhReduce);
         fp2 = rf[0];
     }
+    gc.flush(c.sc);
     if (blockIdx.x == 0 && threadIdx.x == 0 && k_iter > 0) {
         c.sc->iter += k_iter;
         c.sc->cg_steps_total += cg_total;

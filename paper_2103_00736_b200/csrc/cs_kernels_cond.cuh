@@ -72,7 +72,9 @@ struct TermRowNorm {  // sum_j (A_ij O_j)^2   (traversed over the PRISTINE value
 };
 struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b
     double *D, *btil; const double *b;
-    __device__ void operator()(int i, const double (&a)[1]) {
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
         const double di = 1.0 / sqrt(a[0]);
         D[i] = di;
         btil[i] = di * b[i];
@@ -88,7 +90,9 @@ struct ScaleCsc {     // same on the column-major copy (segment = column j, mino
 };
 struct EpiRhsD {      // q = b~ + mu A~ c^ ; w = 0 => r = q
     double *r, *w; const double *btil; double mu; double qq;
-    __device__ void operator()(int i, const double (&a)[1]) {
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
         const double q = btil[i] + mu * a[0];
         r[i] = q;
         w[i] = 0.0;
@@ -97,7 +101,9 @@ struct EpiRhsD {      // q = b~ + mu A~ c^ ; w = 0 => r = q
 };
 struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu O z ; g = 0
     double *d, *s, *g; const double *chat, *xb, *zb, *O; double mu;
-    __device__ void operator()(int j, const double (&a)[1]) {
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) {
         d[j] = a[0] - mu * chat[j];
         s[j] = xb[j] / O[j] - mu * O[j] * zb[j];
         g[j] = 0.0;
@@ -105,8 +111,9 @@ struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu
 };
 
 // use_rule = 1: O from steps 5-11 applied to (xb, zb); 0: O already in c.O (cs_set_scaling)
-__global__ void __launch_bounds__(kBlock, 2) k_condition(Ctx c, int use_rule) {
+__global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_rule) {
     __shared__ double smem[kMaxRed * kWarps];
+    extern __shared__ double hot[];
     GridCtl gc(c.partials, smem);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     if (use_rule) {
@@ -139,7 +146,7 @@ __global__ void __launch_bounds__(kBlock, 2) k_condition(Ctx c, int use_rule) {
     double red[1] = {eq.qq};
     grid_reduce<1>(red, gc);
     bool hm;
-    const int steps = cg_solve(c, gc, red[0], red[0], hm);
+    const int steps = cg_solve(c, gc, hot, red[0], red[0], hm);
     TermDot tw{c.w};
     EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
     seg_reduce<1, false>(c.C, tw, ed, gc);
@@ -161,7 +168,9 @@ struct TermCsrX {     // A~ x^ with x^ = x/O
 };
 struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
     const double *btil, *D, *wd, *w; double mu; double pres2, by;
-    __device__ void operator()(int i, const double (&a)[1]) {
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
         const double e = (a[0] - btil[i]) / D[i];
         pres2 += e * e;
         by += btil[i] * (wd[i] - w[i]) / mu;
@@ -173,7 +182,9 @@ struct TermCscY {     // A~' y'
 };
 struct EpiDres {      // (c - z - A'y)_j = c_j - z_j - (A~'y')_j / O_j
     const double *cc, *xb, *zb, *O; double dres2, cx, nx2, nz2;
-    __device__ void operator()(int j, const double (&a)[1]) {
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) {
         const double e = cc[j] - zb[j] - a[0] / O[j];
         dres2 += e * e;
         cx += cc[j] * xb[j];
@@ -190,7 +201,7 @@ __device__ __forceinline__ double soc_dist2(double t, double nu2) {
     return 0.5 * (nu - t) * (nu - t);
 }
 
-__global__ void __launch_bounds__(kBlock, 2) k_residuals(Ctx c) {
+__global__ void __launch_bounds__(kBlock, CS_MINB) k_residuals(Ctx c) {
     __shared__ double smem[kMaxRed * kWarps];
     GridCtl gc(c.partials, smem);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
