@@ -22,7 +22,7 @@ struct cs_solver {
     cudaStream_t stream = nullptr;
     int device = 0;
     int grid = 0;
-    size_t dyn_smem = 0;       // bytes of dynamic shared memory of k_iterate / k_condition (hot-row cache)
+    size_t dyn_smem = 0;       // bytes of dynamic shared memory of the cooperative kernels (cp.async staging)
     std::vector<void *> allocs;
     cs_params prm{};
     bool conditioned = false;  // the l=1 conditioning of step 4 has run
@@ -80,12 +80,13 @@ cs_status fetch(cs_solver *S, std::vector<T> &dst, const T *src, size_t count, c
     return CS_OK;
 }
 
-// Host image of one Sparse (cs_device.cuh): ELL slices for the short segments, chunks for the long ones.
+// Host image of one Sparse (cs_device.cuh): chunk slices of the long segments first, then the slices of
+// the short ones, all in one pair of arrays.
 struct HostSparse {
-    std::vector<int4> slices, chunks, multi;
-    std::vector<int> eidx, lidx;
-    std::vector<double> eval, lval;
-    int n_slots = 0;
+    std::vector<int4> slices, multi;
+    std::vector<int> chunk_slot, idx;
+    std::vector<double> val;
+    int n_chunk = 0, n_slots = 0;
 };
 
 // ptr/idx/val: compressed segments in INTERNAL numbering (segment s = entries [ptr[s], ptr[s+1])).
@@ -96,7 +97,32 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
     // T>1 is slower once every warp has >= 2 thread-per-segment slices)
     const bool split = nseg < 300000;
     auto lg_lanes = [split](int len) { return (!split || len <= 8) ? 0 : len <= 16 ? 1 : len <= 32 ? 2 : 3; };  // T = 1,2,4,8 lanes
-    auto flush_run = [&](int a, int b) {  // consecutive short segments [a,b) -> slices (32 lanes, T lanes per segment)
+    auto new_slice = [&](int seg0, int meta, int width) {
+        const int off = (int)h.val.size();
+        h.slices.push_back(make_int4(off, seg0, meta, width));
+        h.val.resize((size_t)off + 32u * width, 0.0);
+        h.idx.resize((size_t)off + 32u * width, 0);
+        return off;
+    };
+    // pass 1: chunks of the long segments (T = 32: entry e of the chunk at lane e%32, row e/32)
+    for (int s = 0; s < nseg; ++s) {
+        const int len = ptr[s + 1] - ptr[s];
+        if (len <= kShortMax) continue;
+        const int nch = (len + kChunk - 1) / kChunk;
+        if (nch > 1) h.multi.push_back(make_int4(s, h.n_slots, nch, 0));
+        for (int q = 0; q < nch; ++q) {
+            const int a = ptr[s] + q * kChunk, clen = std::min(kChunk, ptr[s + 1] - a), width = (clen + 31) / 32;
+            const int off = new_slice(s, 1 | (5 << 8), width);
+            for (int e = 0; e < 32 * width; ++e) {
+                h.idx[(size_t)off + e] = idx[a + std::min(e, clen - 1)];
+                if (e < clen) h.val[(size_t)off + e] = val[a + e];
+            }
+            h.chunk_slot.push_back(nch > 1 ? h.n_slots++ : -1);
+        }
+    }
+    h.n_chunk = (int)h.slices.size();
+    // pass 2: runs of consecutive short segments -> slices of 32 lanes, T lanes per segment
+    auto flush_run = [&](int a, int b) {
         int s0 = a;
         while (s0 < b) {
             const int lgT = lg_lanes(ptr[s0 + 1] - ptr[s0]), T = 1 << lgT, cap = 32 / T;
@@ -106,17 +132,14 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 ++cnt;
             }
             const int width = (maxlen + T - 1) / T;
-            const int off = (int)h.eval.size();
-            h.slices.push_back(make_int4(off, s0, cnt | (lgT << 8), width));
-            h.eval.resize((size_t)off + 32u * width, 0.0);
-            h.eidx.resize((size_t)off + 32u * width, 0);
+            const int off = new_slice(s0, cnt | (lgT << 8), width);
             for (int lane = 0; lane < 32; ++lane) {
                 const int seg = s0 + std::min(lane / T, cnt - 1);   // padding lanes replicate a valid index
                 const int len = ptr[seg + 1] - ptr[seg], t = lane % T;
                 for (int k = 0; k < width; ++k) {
                     const int e = k * T + t;
-                    h.eidx[(size_t)off + 32u * k + lane] = idx[ptr[seg] + std::min(e, len - 1)];
-                    if (lane / T < cnt && e < len) h.eval[(size_t)off + 32u * k + lane] = val[ptr[seg] + e];
+                    h.idx[(size_t)off + 32u * k + lane] = idx[ptr[seg] + std::min(e, len - 1)];
+                    if (lane / T < cnt && e < len) h.val[(size_t)off + 32u * k + lane] = val[ptr[seg] + e];
                 }
             }
             s0 += cnt;
@@ -124,21 +147,9 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
     };
     int run = 0;
     for (int s = 0; s < nseg; ++s) {
-        const int len = ptr[s + 1] - ptr[s];
-        if (len <= kShortMax) continue;
+        if (ptr[s + 1] - ptr[s] <= kShortMax) continue;
         flush_run(run, s);
         run = s + 1;
-        const int base = (int)h.lval.size();
-        h.lval.insert(h.lval.end(), val.begin() + ptr[s], val.begin() + ptr[s + 1]);
-        h.lidx.insert(h.lidx.end(), idx.begin() + ptr[s], idx.begin() + ptr[s + 1]);
-        if (len <= kChunk) {
-            h.chunks.push_back(make_int4(s, base, len, -1));
-        } else {
-            const int nch = (len + kChunk - 1) / kChunk;
-            h.multi.push_back(make_int4(s, h.n_slots, nch, 0));
-            for (int q = 0; q < nch; ++q)
-                h.chunks.push_back(make_int4(s, base + q * kChunk, std::min(kChunk, len - q * kChunk), h.n_slots++));
-        }
     }
     flush_run(run, nseg);
     return h;
@@ -148,16 +159,13 @@ cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     cs_status st;
     int4 *p4; int *pi; double *pd;
     if ((st = dev_upload(S, &p4, h.slices.data(), h.slices.size())) != CS_OK) return st; out->slices = p4;
-    if ((st = dev_upload(S, &p4, h.chunks.data(), h.chunks.size())) != CS_OK) return st; out->chunks = p4;
     if ((st = dev_upload(S, &p4, h.multi.data(), h.multi.size())) != CS_OK) return st; out->multi = p4;
-    if ((st = dev_upload(S, &pi, h.eidx.data(), h.eidx.size())) != CS_OK) return st; out->eidx = pi;
-    if ((st = dev_upload(S, &pi, h.lidx.data(), h.lidx.size())) != CS_OK) return st; out->lidx = pi;
-    if ((st = dev_upload(S, &pd, h.eval.data(), h.eval.size())) != CS_OK) return st; out->eval0 = pd;
-    if ((st = dev_upload(S, &out->eval, h.eval.data(), h.eval.size())) != CS_OK) return st;
-    if ((st = dev_upload(S, &pd, h.lval.data(), h.lval.size())) != CS_OK) return st; out->lval0 = pd;
-    if ((st = dev_upload(S, &out->lval, h.lval.data(), h.lval.size())) != CS_OK) return st;
+    if ((st = dev_upload(S, &pi, h.chunk_slot.data(), h.chunk_slot.size())) != CS_OK) return st; out->chunk_slot = pi;
+    if ((st = dev_upload(S, &pi, h.idx.data(), h.idx.size())) != CS_OK) return st; out->idx = pi;
+    if ((st = dev_upload(S, &pd, h.val.data(), h.val.size())) != CS_OK) return st; out->val0 = pd;
+    if ((st = dev_upload(S, &out->val, h.val.data(), h.val.size())) != CS_OK) return st;
     out->n_slice = (int)h.slices.size();
-    out->n_chunk = (int)h.chunks.size();
+    out->n_chunk = h.n_chunk;
     out->n_multi = (int)h.multi.size();
     return dev_zeros(S, &out->partial, (size_t)h.n_slots * 2);
 }
@@ -403,25 +411,15 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
     const void *kernels[] = {(const void *)k_iterate, (const void *)k_condition, (const void *)k_residuals};
-    {   // heavy rows (longer than kShortMax) come first in the internal order: cache up to 8192 of them
-        int n_long = 0;
-        while (n_long < m && n_long < 8192 && rp2[(size_t)n_long + 1] - rp2[n_long] > kShortMax) ++n_long;
-        x.hot_rows = n_long;
-        S->dyn_smem = sizeof(double) * (size_t)n_long;
-        if (S->dyn_smem > 48 * 1024) {
-            CS_CUDA(S, cudaFuncSetAttribute((const void *)k_iterate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S->dyn_smem));
-            CS_CUDA(S, cudaFuncSetAttribute((const void *)k_condition, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S->dyn_smem));
-        }
-    }
+    S->dyn_smem = 0;
     for (const void *k : kernels) {
-        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, k == (const void *)k_residuals ? 0 : S->dyn_smem));
+        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, S->dyn_smem));
         occ_min = std::min(occ_min, occ);
     }
     if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
     S->grid = sms * occ_min;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * S->grid)) != CS_OK) return st;
     // ---- defaults (cs.h)
-    x.dbg = getenv("CS_DEBUG") ? atoi(getenv("CS_DEBUG")) : 0;
     S->prm.mu = 1.0;
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
     S->prm.o_floor = 1e-16;
@@ -510,7 +508,7 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     if (!S->conditioned && (st = do_condition(S, 1)) != CS_OK) return st;
     if ((st = ensure_xz(S)) != CS_OK) return st;
     void *args[] = {&S->ctx};
-    if ((st = launch_coop(S, (const void *)k_residuals, args)) != CS_OK) return st;
+    if ((st = launch_coop(S, (const void *)k_residuals, args, S->dyn_smem)) != CS_OK) return st;
     Scalars h;
     CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
     CS_CUDA(S, cudaMemsetAsync(&S->ctx.sc->cg_hit_max, 0, sizeof(int), S->stream));

@@ -11,9 +11,6 @@ namespace cg = cooperative_groups;
 
 namespace csd {
 
-#ifndef CS_UN
-#define CS_UN 8
-#endif
 #ifndef CS_MINB
 #define CS_MINB 2
 #endif
@@ -23,29 +20,28 @@ constexpr int kMaxRed = 8;           // scalars per grid reduction
 constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (sub-warp groups)
 constexpr int kChunk = 1024;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
+constexpr int kRoundK = 8;           // slice rows loaded per batch (8 values + 8 indices + 8 gathers in flight per lane)
 
-// One sparse format (rows of the CSR-like copy or columns of the CSC-like copy), stored in two parts:
-//  * ELL part: runs of consecutive short segments cut into slices of 32; slice s holds 32 x width
-//    entries laid out [k][lane] so that lane l reads entry k of segment seg0+l at off + 32k + l
-//    (fully coalesced, one thread per segment, no shuffles).  Padding entries have val = 0 and a valid
-//    index.  Rows (and orthant columns) are physically sorted by length at cs_create, so padding is
-//    negligible.
-//  * long part: segments longer than kShortMax, cut into chunks of kChunk entries, one warp each;
-//    segments spanning several chunks are finished from per-chunk partial sums in fixed order.
+// One sparse format (rows of the row-major copy or columns of the column-major copy): a list of SLICES.
+// A slice is 32 lanes x width entries stored [k][lane] (entry k of lane l at off + 32k + l), so that a
+// warp reads it fully coalesced; the lanes of a slice are split over its segments T lanes at a time:
+//   T = 1      32 short segments, one thread each (the bulk of every workload)
+//   T = 2,4,8  fewer segments per slice, several lanes each: only when the problem is too small to
+//              fill the machine with one thread per segment
+//   T = 32     one CHUNK (<= kChunk entries) of a long segment; these slices come first, and chunk c
+//              either completes its segment (chunk_slot[c] < 0) or writes a partial sum to a slot.
+// Padding entries have val = 0 and a valid index.  Rows (and orthant columns) are physically sorted by
+// length at cs_create, so padding is negligible.
 struct Sparse {
     int n_slice;
-    const int4 *slices;     // {offset into e*, first segment id, segments in the slice | log2(T) << 8, width};
-                            // T = lanes per segment (1,2,4,8): entry e of segment r sits at lane r*T + e%T, row e/T
-    const int *eidx;
-    double *eval;           // scaled values (D A O)
-    const double *eval0;    // pristine values (A)
-    int n_chunk;
-    const int4 *chunks;     // {segment id, first entry in l*, length, slot}; slot < 0: chunk == whole segment
-    const int *lidx;
-    double *lval;
-    const double *lval0;
+    const int4 *slices;     // {off, first segment id, segments in the slice | log2(T) << 8, width}
+    int n_chunk;            // slices [0, n_chunk) are chunks of long segments
+    const int *chunk_slot;  // [n_chunk]
+    const int *idx;
+    double *val;            // scaled values (D A O)
+    const double *val0;     // pristine values (A)
     int n_multi;
-    const int4 *multi;      // {segment id, first slot, number of slots, 0}
+    const int4 *multi;      // long segments spanning several chunks: {segment id, first slot, number of slots, 0}
     double *partial;        // [slots][2]
 };
 
@@ -75,8 +71,6 @@ struct Ctx {
     double mu, t, o_floor, cg_tol;
     int cg_max_iter;
     double norm_b, norm_c;
-    int dbg;                // TEMP debug flags
-    int hot_rows;           // leading (longest) rows whose r / w entries are cached in shared memory for the column passes
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -158,95 +152,74 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Segment traversals.  `term(a, j, acc)` adds the contribution of one entry (value a, minor index j)
-// to acc[NV]; `epi(seg, sums)` is called once per segment with the complete sums.
-// Long segments first (warp per chunk), then the ELL slices (thread per segment), then the segments
-// that span several chunks (after a grid barrier, from their partial sums, in fixed order).
-// The matrix streams use ld.global.cs (evict-first) so that the gathered vectors stay in L2.
+// Segment traversal.  `g = term.fetch(j)` gathers the operand(s) of minor index j and
+// `term.fma(a, g, acc)` adds the contribution of one entry of value a to acc[NV];
+// `epi(seg, sums, pre)` is called once per segment with the complete sums, where
+// `pre = epi.pre(seg)` holds whatever the epilogue reads from memory (fetched early).
+//
+// Every warp walks its slices (s = gwarp, gwarp + nwarps, ...).  Per slice, rows are consumed 8 at a
+// time: 8 value + 8 index loads (ld.global.cs: streamed, evict-first, so that the gathered vectors stay
+// in L2), then 8 gathers, then the FMAs -- all loads of a batch are in flight before the first use.
+// The epilogue operands and the next slice descriptor are fetched before the batch loop.
+// (A cp.async-staged variant of this loop was measured SLOWER on B200 -- the LDGSTS instructions add
+// to the L1TEX load that already bounds the gathers; see profiles/r01_ncu_notes.md.)
+// Long segments (chunks) leave partial sums; they are finished after a grid barrier in fixed order.
 // ---------------------------------------------------------------------------------------------
 template <int NV, bool PRISTINE, class Term, class Epi>
-__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc, int dbg = 0) {
+__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
     const int lane = threadIdx.x & 31;
     const int gwarp = (blockIdx.x * kBlock + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * kBlock) >> 5;
-    {
-        const double *lv = PRISTINE ? S.lval0 : S.lval;
-        for (int c = gwarp; c < ((dbg & 2) ? 0 : S.n_chunk); c += nwarps) {
-            const int4 ch = __ldg(S.chunks + c);
-            double acc[NV];
+    const double *gval = PRISTINE ? S.val0 : S.val;
+    constexpr int UN = NV == 1 ? kRoundK : kRoundK / 2;   // two-operand gathers: half the batch, same registers
+    int s = gwarp;
+    int4 sl = s < S.n_slice ? __ldg(S.slices + s) : make_int4(0, 0, 0, 0);
+    while (s < S.n_slice) {
+        const int sn = s + nwarps;
+        const int4 nxt = sn < S.n_slice ? __ldg(S.slices + sn) : make_int4(0, 0, 0, 0);
+        const double *vp = gval + sl.x + lane;
+        const int *ip = S.idx + sl.x + lane;
+        const int lgT = sl.z >> 8, T = 1 << lgT;              // lanes per segment in this slice
+        const int seg = sl.y + (lane >> lgT);
+        const bool head = (lane >> lgT) < (sl.z & 255) && (lane & (T - 1)) == 0;
+        typename Epi::Pre pre = epi.pre(head ? seg : sl.y);
+        double acc[NV];
 #pragma unroll
-            for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-            const int end = ch.y + ch.z;
-            constexpr int CU = 8;
-            for (int k = ch.y + lane; k < end; k += 32 * CU) {
-                double a[CU]; int j[CU];
+        for (int i = 0; i < NV; ++i) acc[i] = 0.0;
+        for (int k = 0; k < sl.w; k += UN) {
+            double a[UN]; int j[UN];
 #pragma unroll
-                for (int q = 0; q < CU; ++q) {
-                    const bool ok = k + 32 * q < end;
-                    a[q] = ok ? __ldcs(lv + k + 32 * q) : 0.0;
-                    j[q] = ok ? __ldcs(S.lidx + k + 32 * q) : -1;
-                }
-#pragma unroll
-                for (int q = 0; q < CU; ++q) if (j[q] >= 0) term(a[q], j[q], acc);
+            for (int q = 0; q < UN; ++q) {                   // predicated: no traffic for rows past the end
+                const bool ok = k + q < sl.w;
+                a[q] = ok ? __ldcs(vp + 32 * (k + q)) : 0.0;
+                j[q] = ok ? __ldcs(ip + 32 * (k + q)) : -1;
             }
+            typename Term::G g[UN];
 #pragma unroll
-            for (int i = 0; i < NV; ++i) acc[i] = group_reduce<32>(acc[i]);
-            if (lane == 0) {
-                if (ch.w < 0) epi(ch.x, acc, epi.pre(ch.x));
-                else {
+            for (int q = 0; q < UN; ++q) g[q] = term.fetch(j[q] >= 0 ? j[q] : 0);   // index 0: one broadcast wavefront
 #pragma unroll
-                    for (int i = 0; i < NV; ++i) S.partial[(size_t)ch.w * 2 + i] = acc[i];
-                }
+            for (int q = 0; q < UN; ++q) if (j[q] >= 0) term.fma(a[q], g[q], acc);
+        }
+        for (int o = T >> 1; o > 0; o >>= 1) {
+#pragma unroll
+            for (int i = 0; i < NV; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
+        }
+        if (head) {
+            const int slot = s < S.n_chunk ? __ldg(S.chunk_slot + s) : -1;
+            if (slot < 0) epi(seg, acc, pre);
+            else {
+#pragma unroll
+                for (int i = 0; i < NV; ++i) S.partial[(size_t)slot * 2 + i] = acc[i];
             }
         }
+        s = sn;
+        sl = nxt;
     }
-    {
-        // ELL slices: one thread per segment.  All loads of a slice row-block are issued before the
-        // first use (predicated 8-wide unroll), the operands of the epilogue are fetched up front
-        // (epi.pre) and the next slice descriptor is prefetched, so that a warp keeps ~20 independent
-        // loads in flight instead of a chain of dependent round trips.
-        constexpr int UN = CS_UN;
-        const double *ev = PRISTINE ? S.eval0 : S.eval;
-        int s = gwarp;
-        int4 sl = s < S.n_slice ? __ldg(S.slices + s) : make_int4(0, 0, 0, 0);
-        if (dbg & 4) s = S.n_slice;
-        while (s < S.n_slice) {
-            const int sn = s + nwarps;
-            const int4 nxt = sn < S.n_slice ? __ldg(S.slices + sn) : make_int4(0, 0, 0, 0);
-            const double *vp = ev + sl.x + lane;
-            const int *ip = S.eidx + sl.x + lane;
-            const int lgT = sl.z >> 8, T = 1 << lgT;              // lanes per segment in this slice
-            const int seg = sl.y + (lane >> lgT);
-            const bool head = (lane >> lgT) < (sl.z & 255) && (lane & (T - 1)) == 0;
-            typename Epi::Pre pre = epi.pre(head ? seg : sl.y);
-            double acc[NV];
-#pragma unroll
-            for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-            for (int k = 0; k < sl.w; k += UN) {
-                double a[UN]; int j[UN];
-#pragma unroll
-                for (int q = 0; q < UN; ++q) {
-                    const bool ok = k + q < sl.w;
-                    a[q] = ok ? __ldcs(vp + 32 * (k + q)) : 0.0;
-                    j[q] = ok ? __ldcs(ip + 32 * (k + q)) : -1;
-                }
-#pragma unroll
-                for (int q = 0; q < UN; ++q) if (j[q] >= 0) term(a[q], j[q], acc);
-            }
-            for (int o = T >> 1; o > 0; o >>= 1) {
-#pragma unroll
-                for (int i = 0; i < NV; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
-            }
-            if (head) epi(seg, acc, pre);
-            s = sn;
-            sl = nxt;
-        }
-    }
-    if (S.n_multi && !(dbg & 8)) {
+    if (S.n_multi) {
         gc.sync();
         for (int r = gwarp; r < S.n_multi; r += nwarps) {
             const int4 mr = __ldg(S.multi + r);
-            double acc[NV];
+            double tot[NV];
 #pragma unroll
             for (int i = 0; i < NV; ++i) {
                 double a = 0.0;
@@ -260,29 +233,25 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
                     for (int q = 0; q < 8; ++q) a += t[q];
                 }
                 for (; k < mr.z; k += 32) a += __ldcg(pp + (size_t)k * 2);
-                acc[i] = group_reduce<32>(a);
+                tot[i] = group_reduce<32>(a);
             }
-            if (lane == 0) epi(mr.x, acc, epi.pre(mr.x));
+            if (lane == 0) epi(mr.x, tot, epi.pre(mr.x));
         }
     }
 }
 
-// Rewrite every stored entry: val = f(seg, val0, idx).  Same partition as seg_reduce.
+// Rewrite every stored entry: val = f(seg, val0, idx).
 template <class F>
 __device__ __forceinline__ void seg_rescale(const Sparse &S, F &f) {
     const int lane = threadIdx.x & 31;
     const int gwarp = (blockIdx.x * kBlock + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * kBlock) >> 5;
-    for (int c = gwarp; c < S.n_chunk; c += nwarps) {
-        const int4 ch = __ldg(S.chunks + c);
-        for (int k = ch.y + lane; k < ch.y + ch.z; k += 32) S.lval[k] = f(ch.x, S.lval0[k], __ldg(S.lidx + k));
-    }
     for (int s = gwarp; s < S.n_slice; s += nwarps) {
         const int4 sl = __ldg(S.slices + s);
         const int lgT = sl.z >> 8;
         if ((lane >> lgT) < (sl.z & 255)) {
             const int base = sl.x + lane, seg = sl.y + (lane >> lgT);
-            for (int k = 0; k < sl.w; ++k) S.eval[base + 32 * k] = f(seg, S.eval0[base + 32 * k], __ldg(S.eidx + base + 32 * k));
+            for (int k = 0; k < sl.w; ++k) S.val[base + 32 * k] = f(seg, S.val0[base + 32 * k], __ldg(S.idx + base + 32 * k));
         }
     }
 }

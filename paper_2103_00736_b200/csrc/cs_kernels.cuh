@@ -69,20 +69,11 @@ __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
 // ---------------------------------------------------------------------------------------------
 struct TermDot {    // sum_k a_k x[j_k]  (A~' r, A~ u, A~' w, A~ c^ ...)
     const double *x;
-    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * x[j]; }
+    typedef double G;
+    __device__ __forceinline__ G fetch(int j) const { return x[j]; }
+    __device__ __forceinline__ void fma(double a, G g, double (&acc)[1]) const { acc[0] += a * g; }
 };
 struct NoPre {};
-struct TermNoGather { const double *x; __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * (double)j; } };
-struct TermDotHot { // same, with x[0..H) served from shared memory (the heavy rows of a power-law matrix)
-    const double *x; const double *hot; int H;
-    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const {
-        acc[0] += a * (j < H ? hot[j] : x[j]);
-    }
-};
-__device__ __forceinline__ void fill_hot(double *hot, const double *x, int H) {
-    for (int i = threadIdx.x; i < H; i += kBlock) hot[i] = x[i];
-    __syncthreads();
-}
 struct EpiK1 {
     double *u; double beta; double sigma;
     struct Pre { double u; };
@@ -107,22 +98,16 @@ struct EpiK2 {
     }
 };
 
-__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double *hot, double rho, double qq, bool &hit_max) {
+__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, double qq, bool &hit_max) {
     const double thresh = c.cg_tol * c.cg_tol * qq;
     double beta = 0.0;
     int steps = 0;
     hit_max = false;
     while (rho > thresh) {
         if (steps >= c.cg_max_iter) { hit_max = true; break; }
+        TermDot t1{c.r};
         EpiK1 e1{c.u, beta, 0.0};
-        if (c.hot_rows) {
-            fill_hot(hot, c.r, c.hot_rows);
-            TermDotHot t1{c.r, hot, c.hot_rows};
-            seg_reduce<1, false>(c.C, t1, e1, gc);
-        } else {
-            TermDot t1{c.r};
-            seg_reduce<1, false>(c.C, t1, e1, gc);
-        }
+        seg_reduce<1, false>(c.C, t1, e1, gc);
         gc.lap(kPhK1);
         double red[1] = {e1.sigma};
         grid_reduce<1>(red, gc);
@@ -130,14 +115,9 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double *hot, 
         const double sigma = red[0];
         if (!(sigma > 0.0)) break;
         const double alpha = rho / sigma;
+        TermDot t2{c.u};
         EpiK2 e2{c.v, c.w, c.r, alpha, beta, 0.0};
-        if (c.dbg & 1) {
-            TermNoGather t2{c.u};
-            seg_reduce<1, false>(c.R, t2, e2, gc, c.dbg);
-        } else {
-            TermDot t2{c.u};
-            seg_reduce<1, false>(c.R, t2, e2, gc, c.dbg);
-        }
+        seg_reduce<1, false>(c.R, t2, e2, gc);
         gc.lap(kPhK2);
         red[0] = e2.rho;
         grid_reduce<1>(red, gc);
@@ -154,9 +134,11 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double *hot, 
 // ---------------------------------------------------------------------------------------------
 struct TermCsrPE {  // (A~ p, A~ (p - g))
     const double *p, *e;
-    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[2]) const {
-        acc[0] += a * p[j];
-        acc[1] += a * e[j];
+    typedef double2 G;
+    __device__ __forceinline__ G fetch(int j) const { return make_double2(p[j], e[j]); }
+    __device__ __forceinline__ void fma(double a, G g, double (&acc)[2]) const {
+        acc[0] += a * g.x;
+        acc[1] += a * g.y;
     }
 };
 struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r||^2
@@ -184,7 +166,6 @@ struct EpiUpdate {  // steps 17-18: r = 2 A~'w - p ; s <- s/2 - r/2 + d = (s+p)/
 
 __global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_iter) {
     __shared__ double smem[kMaxRed * kWarps];
-    extern __shared__ double hot[];
     GridCtl gc(c.partials, smem);
     long long cg_total = 0;
     int cg_last = 0;
@@ -203,18 +184,12 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_
         grid_reduce<2>(red, gc);
         gc.lap(kPhReduce);
         bool hm;
-        cg_last = cg_solve(c, gc, hot, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
+        cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
         any_max |= hm;
         cg_total += cg_last;
+        TermDot tw{c.w};
         EpiUpdate eu{c.s, c.g, c.p, c.d, 0.0};
-        if (c.hot_rows) {
-            fill_hot(hot, c.w, c.hot_rows);
-            TermDotHot tw{c.w, hot, c.hot_rows};
-            seg_reduce<1, false>(c.C, tw, eu, gc);               // steps 17-18
-        } else {
-            TermDot tw{c.w};
-            seg_reduce<1, false>(c.C, tw, eu, gc);
-        }
+        seg_reduce<1, false>(c.C, tw, eu, gc);                   // steps 17-18
         gc.lap(kPhUpdate);
         double rf[1] = {eu.fp2};
         grid_reduce<1>(rf, gc);

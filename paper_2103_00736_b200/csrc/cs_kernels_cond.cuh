@@ -65,8 +65,10 @@ __device__ __forceinline__ void phase_cone_ratio(const Ctx &c, double &lmax, dou
 
 struct TermRowNorm {  // sum_j (A_ij O_j)^2   (traversed over the PRISTINE values)
     const double *O;
-    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const {
-        const double x = a * O[j];
+    typedef double G;
+    __device__ __forceinline__ G fetch(int j) const { return O[j]; }
+    __device__ __forceinline__ void fma(double a, G g, double (&acc)[1]) const {
+        const double x = a * g;
         acc[0] += x * x;
     }
 };
@@ -113,7 +115,6 @@ struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu
 // use_rule = 1: O from steps 5-11 applied to (xb, zb); 0: O already in c.O (cs_set_scaling)
 __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_rule) {
     __shared__ double smem[kMaxRed * kWarps];
-    extern __shared__ double hot[];
     GridCtl gc(c.partials, smem);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     if (use_rule) {
@@ -146,7 +147,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     double red[1] = {eq.qq};
     grid_reduce<1>(red, gc);
     bool hm;
-    const int steps = cg_solve(c, gc, hot, red[0], red[0], hm);
+    const int steps = cg_solve(c, gc, red[0], red[0], hm);
     TermDot tw{c.w};
     EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
     seg_reduce<1, false>(c.C, tw, ed, gc);
@@ -164,7 +165,9 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
 // ---- residuals (original coordinates; xb, zb must be current) --------------------------------
 struct TermCsrX {     // A~ x^ with x^ = x/O
     const double *xb, *O;
-    __device__ __forceinline__ void operator()(double a, int j, double (&acc)[1]) const { acc[0] += a * (xb[j] / O[j]); }
+    typedef double G;
+    __device__ __forceinline__ G fetch(int j) const { return xb[j] / O[j]; }
+    __device__ __forceinline__ void fma(double a, G g, double (&acc)[1]) const { acc[0] += a * g; }
 };
 struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
     const double *btil, *D, *wd, *w; double mu; double pres2, by;
@@ -178,7 +181,9 @@ struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
 };
 struct TermCscY {     // A~' y'
     const double *wd, *w; double mu;
-    __device__ __forceinline__ void operator()(double a, int i, double (&acc)[1]) const { acc[0] += a * ((wd[i] - w[i]) / mu); }
+    typedef double G;
+    __device__ __forceinline__ G fetch(int i) const { return (wd[i] - w[i]) / mu; }
+    __device__ __forceinline__ void fma(double a, G g, double (&acc)[1]) const { acc[0] += a * g; }
 };
 struct EpiDres {      // (c - z - A'y)_j = c_j - z_j - (A~'y')_j / O_j
     const double *cc, *xb, *zb, *O; double dres2, cx, nx2, nz2;
