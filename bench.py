@@ -106,6 +106,24 @@ def oracle_sample(cfg, scale, steps, warmup):
 ORACLE_SCALE = {0: 1.0, 1: 1.0, 2: 0.05, 3: 0.1, 4: 0.02}
 
 
+def max_over_ranks(x: float, device="cpu") -> float:
+    """MAX of a per-rank scalar over the job (identity without a process group).  Used for the timed
+    region: the job is as slow as its slowest replica."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(iters_per_rank: int, world: int, ms_max: float) -> float:
+    """Replicas only (weak scaling): every rank ran `iters_per_rank` outer iterations on its own
+    instance; the job's throughput is the total over the slowest rank's time."""
+    return world * iters_per_rank / (ms_max * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -186,12 +204,9 @@ def main():
     ms_total = e_all[0].elapsed_time(e_all[1])
     ms_iter = sum(x.elapsed_time(y) for x, y in ev)
     launches = S.kernel_launches() - l0
-    t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = max_over_ranks(ms_total, dev)
     n_it = a.steps * a.k
-    value = world * n_it / (ms_max * 1e-3)
+    value = whole_job_value(n_it, world, ms_max)
 
     # ---- roofline of the dominant kernel (k_iterate, one launch per step): algorithmic bytes of the K
     # timed launches / their summed CUDA-event durations.  CG steps are data dependent, so they are read
@@ -261,11 +276,8 @@ def finish(a, p, S, line, rank, world, dev, stream):
             e2e_step()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-    tt = torch.tensor([dt], device=dev, dtype=torch.float64)
-    if world > 1:
-        import torch.distributed as dist
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    line["e2e"] = {"value": world * a.e2e_steps * a.k / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+    dt_max = max_over_ranks(dt, dev)
+    line["e2e"] = {"value": whole_job_value(a.e2e_steps * a.k, world, dt_max * 1e3) if a.e2e_steps else None, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                    "d2h_bytes_per_step": int(d2h), "steps": a.e2e_steps,
                    "step": "cs_create(host A,b,c) + cs_iterate(k) + cs_condition + cs_residuals + cs_solution(host x,z)"}
     if rank == 0:

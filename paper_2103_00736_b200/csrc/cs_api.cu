@@ -394,7 +394,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
     double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.d, &x.chat};
     for (double **q : nv) if ((st = dev_zeros(S, q, (size_t)n)) != CS_OK) return st;
-    double **mv[] = {&x.w, &x.r, &x.v, &x.wd, &x.btil};
+    double **mv[] = {&x.w, &x.r, &x.v, &x.wd, &x.btil, &x.wsave};
     for (double **q : mv) if ((st = dev_zeros(S, q, (size_t)m)) != CS_OK) return st;
     {   // O = 1, D = 1, x = z = e_K
         std::vector<double> ones((size_t)std::max(m, n), 1.0), ek((size_t)n, 0.0);

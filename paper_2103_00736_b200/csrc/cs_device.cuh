@@ -64,7 +64,7 @@ struct Ctx {
     double *s, *p, *g, *e, *u, *d, *chat, *O, *xb, *zb;
     const double *c;
     // m-vectors
-    double *w, *r, *v, *wd, *D, *btil;
+    double *w, *r, *v, *wd, *D, *btil, *wsave;
     const double *b;
     double *partials;       // [2][kMaxRed][gridDim]
     Scalars *sc;

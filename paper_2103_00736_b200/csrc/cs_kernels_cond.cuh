@@ -72,14 +72,18 @@ struct TermRowNorm {  // sum_j (A_ij O_j)^2   (traversed over the PRISTINE value
         acc[0] += x * x;
     }
 };
-struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b
-    double *D, *btil; const double *b;
+struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b ; the multipliers follow the change of row scaling:
+                      // w_true = D w is what carries over, so w <- (D_old/D_new) w is the warm start (wsave), same for w_d (w)
+    double *D, *btil, *w, *wd, *wsave; const double *b;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
         const double di = 1.0 / sqrt(a[0]);
+        const double ratio = D[i] / di;
         D[i] = di;
         btil[i] = di * b[i];
+        wsave[i] = ratio * w[i];
+        w[i] = ratio * wd[i];       // the solve for w_d below runs in c.w
     }
 };
 struct ScaleCsr {     // A~_ij = D_i A_ij O_j on the row-major copy (segment = row i, minor = column j)
@@ -90,25 +94,40 @@ struct ScaleCsc {     // same on the column-major copy (segment = column j, mino
     const double *O, *D;
     __device__ __forceinline__ double operator()(int j, double a0, int i) const { return a0 * O[j] * D[i]; }
 };
-struct EpiRhsD {      // q = b~ + mu A~ c^ ; w = 0 => r = q
-    double *r, *w; const double *btil; double mu; double qq;
+struct EpiWarmE {     // e = mu c^ - A~'w_d(guess): the rhs pass below then gives the warm-start residual
+    double *e; const double *chat; double mu;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
-    __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
-        const double q = btil[i] + mu * a[0];
-        r[i] = q;
-        w[i] = 0.0;
-        qq += q * q;
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) { e[j] = mu * chat[j] - a[0]; }
+};
+struct TermTwo {      // (sum a x[j], sum a y[j])
+    const double *x, *y;
+    typedef double2 G;
+    __device__ __forceinline__ G fetch(int j) const { return make_double2(x[j], y[j]); }
+    __device__ __forceinline__ void fma(double a, G g, double (&acc)[2]) const {
+        acc[0] += a * g.x;
+        acc[1] += a * g.y;
     }
 };
-struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu O z ; g = 0
+struct EpiRhsD {      // q = b~ + mu A~ c^ ; r = q - A~A~'w_d(guess) = b~ + A~ e
+    double *r; const double *btil; double mu; double qq, rho;
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[2], const Pre &) {
+        const double q = btil[i] + mu * a[0], ri = btil[i] + a[1];
+        r[i] = ri;
+        qq += q * q;
+        rho += ri * ri;
+    }
+};
+struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu O z ; g = A~'w (warm start of the next pass)
     double *d, *s, *g; const double *chat, *xb, *zb, *O; double mu;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
-    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) {
+    __device__ __forceinline__ void operator()(int j, const double (&a)[2], const Pre &) {
         d[j] = a[0] - mu * chat[j];
         s[j] = xb[j] / O[j] - mu * O[j] * zb[j];
-        g[j] = 0.0;
+        g[j] = a[1];
     }
 };
 
@@ -129,7 +148,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     gc.sync();
     {   // row equilibration D
         TermRowNorm t{c.O};
-        EpiRowScale e{c.D, c.btil, c.b};
+        EpiRowScale e{c.D, c.btil, c.w, c.wd, c.wsave, c.b};
         seg_reduce<1, true>(c.R, t, e, gc);
     }
     gc.sync();
@@ -141,18 +160,26 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     }
     gc.sync();
     // d = A~^dagger b~ + (mu/2)(abs_{A~}(c^) - c^) = A~'w_d - mu c^  with (A~A~') w_d = b~ + mu A~ c^
-    TermDot tq{c.chat};
-    EpiRhsD eq{c.r, c.w, c.btil, c.mu, 0.0};
-    seg_reduce<1, false>(c.R, tq, eq, gc);
-    double red[1] = {eq.qq};
-    grid_reduce<1>(red, gc);
-    bool hm;
-    const int steps = cg_solve(c, gc, red[0], red[0], hm);
-    TermDot tw{c.w};
-    EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
-    seg_reduce<1, false>(c.C, tw, ed, gc);
+    // The solve is warm-started from the previous w_d carried over in true (unscaled) coordinates.
+    {
+        TermDot tg{c.w};
+        EpiWarmE ee{c.e, c.chat, c.mu};
+        seg_reduce<1, false>(c.C, tg, ee, gc);
+    }
     gc.sync();
-    for (int i = tid; i < c.m; i += nth) { c.wd[i] = c.w[i]; c.w[i] = 0.0; }
+    TermTwo tq{c.chat, c.e};
+    EpiRhsD eq{c.r, c.btil, c.mu, 0.0, 0.0};
+    seg_reduce<2, false>(c.R, tq, eq, gc);
+    double red[2] = {eq.qq, eq.rho};
+    grid_reduce<2>(red, gc);
+    bool hm;
+    const int steps = cg_solve(c, gc, red[1], red[0], hm);
+    for (int i = tid; i < c.m; i += nth) c.wd[i] = c.w[i];           // own elements only; w is gathered below
+    TermTwo tw{c.w, c.wsave};
+    EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
+    seg_reduce<2, false>(c.C, tw, ed, gc);
+    gc.sync();
+    for (int i = tid; i < c.m; i += nth) c.w[i] = c.wsave[i];        // the iterate's multiplier, rescaled
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         c.sc->n_cond += 1;
         c.sc->cg_steps_total += steps;

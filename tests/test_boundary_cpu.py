@@ -1,0 +1,125 @@
+"""CPU-side checks of the boundary: libcs.so loads and exports every symbol include/cs.h declares (no
+compute calls without a GPU), the binding's schedule logic, bench.py's multi-rank aggregation (gloo,
+world_size 2) and its byte accounting."""
+import ctypes
+import os
+import re
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_2103_00736_b200 import binding, build
+    path = build.build()
+    lib = ctypes.CDLL(path)
+    header = open(os.path.join(ROOT, "include", "cs.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(cs_[a-z_]+)\s*\(", header))
+    assert {"cs_create", "cs_set_params", "cs_iterate", "cs_condition", "cs_residuals", "cs_solution"} <= declared
+    for name in declared:
+        assert getattr(lib, name) is not None, name
+    assert declared == set(binding.EXPORTS)
+    # struct layouts agree with the header (sizes the C side would compute)
+    assert ctypes.sizeof(binding.cs_params) == 40
+    assert ctypes.sizeof(binding.cs_resid) == 3 * 8 + 4 * 4 + 11 * 8
+    assert ctypes.sizeof(binding.cs_csr) == 56 and ctypes.sizeof(binding.cs_cones) == 24
+
+
+def test_no_cuda_device_is_an_error_not_a_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("has a GPU")
+    from paper_2103_00736_b200 import binding, workloads as W
+    p = W.config(0)
+    with pytest.raises(binding.CsError) as ei:
+        binding.Solver.from_problem(p)
+    assert ei.value.status in (binding.CS_ECUDA, binding.CS_ENOMEM)
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    from paper_2103_00736_b200 import binding
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libcs.so")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.lib()
+
+
+def test_product_path_does_not_touch_the_oracle():
+    for rel in ("paper_2103_00736_b200/binding.py", "paper_2103_00736_b200/build.py",
+                "paper_2103_00736_b200/workloads.py", "paper_2103_00736_b200/__init__.py"):
+        src = open(os.path.join(ROOT, rel)).read()
+        assert "import oracle" not in src and "from oracle" not in src, rel
+    for f in os.listdir(os.path.join(ROOT, "paper_2103_00736_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_2103_00736_b200", "csrc", f)).read().lower(), f
+    osrc = open(os.path.join(ROOT, "oracle", "cs_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "paper_2103_00736_b200" not in osrc.replace("paper_2103_00736_b200/csrc/", "").replace("``paper_2103_00736_b200``", "")
+
+
+def test_schedule_decomposition_matches_algorithm2_step4():
+    """Solver.run(k, L): conditioning at the START of iteration l in L = iterate(l-1-l0); condition()."""
+    from paper_2103_00736_b200 import binding
+    calls = []
+
+    class Fake(binding.Solver):
+        def __init__(self):
+            pass
+        def iterate(self, k):
+            calls.append(("it", k))
+        def condition(self):
+            calls.append(("cond",))
+        def destroy(self):
+            pass
+
+    S = Fake()
+    S.run(450, L=[300, 400, 500])
+    assert calls == [("it", 299), ("cond",), ("it", 100), ("cond",), ("it", 51)]
+    calls.clear()
+    S.run(100, L=[300, 400, 500])          # continues at l = 450
+    assert calls == [("it", 49), ("cond",), ("it", 51)]
+    calls.clear()
+    S2 = Fake()
+    S2.run(5, L=[1, 2, 3])                 # l=1 is the implicit conditioning
+    assert calls == [("it", 1), ("cond",), ("it", 1), ("cond",), ("it", 3)]
+
+
+def _rank_main(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = bench.max_over_ranks(100.0 + 50.0 * rank)          # rank 1 is the slow replica
+    q.put((rank, ms, bench.whole_job_value(10, world, ms)))
+    dist.destroy_process_group()
+
+
+def test_multi_rank_aggregation_gloo_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    out = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, val in out:
+        assert ms == 150.0                                   # MAX over ranks
+        assert val == pytest.approx(2 * 10 / 0.150)          # whole-job aggregate, weak scaling
+
+
+def test_bench_byte_accounting():
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2103_00736_b200 import workloads as W
+    p = W.config(1, 0.05)
+    total, per_cg = bench.algorithmic_bytes(p, k_iter=2, cg_steps=10, n_cond=0)
+    assert per_cg == 24 * p.nnz + 28 * p.n + 60 * p.m
+    assert total == 10 * per_cg + 2 * (24 * p.nnz + 92 * p.n + 24 * p.m)
+    assert bench.max_over_ranks(3.5) == 3.5                  # no process group: identity
