@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- outer iterations/s of Algorithm 2 (arXiv 2103.00736) through libcs.so on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4] [--k 5]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4] [--k 1]
 
 A *step* is one pass of the whole hot path over one resident problem:
     cs_condition()  ->  cs_iterate(k)  ->  cs_residuals()
@@ -132,7 +132,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--scale", type=float, default=1.0)
-    ap.add_argument("--k", type=int, default=5, help="outer iterations per step")
+    ap.add_argument("--k", type=int, default=1, help="outer iterations per step (1 = continuous conditioning, P:313)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cg-max-iter", type=int, default=0, help="profiling only: cap CG steps per solve (0 = library default)")
@@ -229,8 +229,14 @@ def main():
               "K1_GBs": k1_b * cg_iter / max(ph["K1"], 1e-9) / 1e6, "K2_GBs": k2_b * cg_iter / max(ph["K2"], 1e-9) / 1e6,
               "K1_us": 1e3 * ph["K1"] / max(1, cg_iter), "K2_us": 1e3 * ph["K2"] / max(1, cg_iter),
               "reduce_us_per_cg": 1e3 * ph["reduce"] / max(1, cg_iter)}
+    # DRAM bytes of k_iterate from the ncu --set full captures in profiles/r01_ncu_notes.md, as a ratio to
+    # the algorithmic bytes of the captured launch (dram__bytes_read.sum + dram__bytes_write.sum) / bytes
+    ncu_ratio = {3: 0.826, 4: 0.902}.get(a.config if a.scale == 1.0 else -1)
     roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+            "frac": achieved / peak, "traffic": ncu_ratio * it_bytes / a.steps if ncu_ratio else None,
+            "traffic_source": "profiles/r01_ncu_notes.md (v3 capture: DRAM bytes / algorithmic bytes of the captured "
+                              "launch, applied to this launch)" if ncu_ratio else None,
+            "peak_source": peak_src,
             "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
             "cg_steps_per_launch": cg_iter / a.steps, "bytes_per_cg_step": cg_bytes,
             "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "frac_of_8TBs": achieved / 8000.0,

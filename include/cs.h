@@ -139,6 +139,10 @@ cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, 
  * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6], [7] reserved.  One D2H copy + sync. */
 cs_status cs_phase_times(cs_solver *S, double out[8]);
 
+/* Diagnostic: run n empty grid barriers (each a 1-value all-reduce over all CTAs, result checked) in one
+ * launch and report the mean latency in microseconds.  Synchronous. */
+cs_status cs_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier);
+
 /* Number of kernels the library has launched on this handle so far (for bench accounting). */
 int64_t cs_kernel_launches(const cs_solver *S);
 

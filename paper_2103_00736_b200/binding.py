@@ -44,7 +44,7 @@ class cs_resid(C.Structure):
 
 
 EXPORTS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
-           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_phase_times", "cs_kernel_launches", "cs_last_error",
+           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_phase_times", "cs_barrier_probe", "cs_kernel_launches", "cs_last_error",
            "cs_destroy")
 
 _lib = None
@@ -75,7 +75,8 @@ def lib():
         L.cs_destroy.argtypes = [vp]
         L.cs_destroy.restype = None
         L.cs_phase_times.argtypes = [vp, C.POINTER(C.c_double)]
-        for name in EXPORTS[:10]:
+        L.cs_barrier_probe.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
+        for name in EXPORTS[:11]:
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -203,6 +204,11 @@ class Solver:
         self._check(lib().cs_phase_times(self._h, a))
         names = ("cone", "rhs", "K1", "K2", "update", "reduce", "r6", "r7")
         return dict(zip(names, [float(x) for x in a]))
+
+    def barrier_probe(self, n=1000):
+        us = C.c_double()
+        self._check(lib().cs_barrier_probe(self._h, int(n), C.byref(us)))
+        return us.value
 
     def kernel_launches(self):
         return int(lib().cs_kernel_launches(self._h))

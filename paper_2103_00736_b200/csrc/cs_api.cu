@@ -407,6 +407,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         CS_CUDA(S, cudaStreamSynchronize(S->stream));  // host staging buffers die at scope end
     }
     if ((st = dev_zeros(S, &x.sc, 1)) != CS_OK) return st;
+    if ((st = dev_zeros(S, &x.partial_probe, 1)) != CS_OK) return st;
     // ---- cooperative grid: as many CTAs as can be co-resident
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
@@ -417,8 +418,9 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         occ_min = std::min(occ_min, occ);
     }
     if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
-    S->grid = sms * occ_min;
-    if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * S->grid)) != CS_OK) return st;
+    S->grid = std::min(sms * occ_min, kMaxGrid);
+    if ((st = dev_zeros(S, &x.bar, 1)) != CS_OK) return st;
+    if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * kMaxGrid)) != CS_OK) return st;
     // ---- defaults (cs.h)
     S->prm.mu = 1.0;
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
@@ -527,6 +529,31 @@ cs_status cs_phase_times(cs_solver *S, double out[8]) {
     CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
     for (int i = 0; i < 8; ++i) out[i] = (double)h.phase_ns[i];
+    return CS_OK;
+}
+
+cs_status cs_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier) {
+    if (!S || n < 1 || !us_per_barrier) return CS_EINVAL;
+    cudaEvent_t e0, e1;
+    CS_CUDA(S, cudaEventCreate(&e0));
+    CS_CUDA(S, cudaEventCreate(&e1));
+    double *out = S->ctx.partial_probe;
+    int nn = n;
+    void *args[] = {&S->ctx, &nn, &out};
+    cs_status st = launch_coop(S, (const void *)k_barrier_probe, args);   // warm-up
+    if (st != CS_OK) return st;
+    CS_CUDA(S, cudaEventRecord(e0, S->stream));
+    if ((st = launch_coop(S, (const void *)k_barrier_probe, args)) != CS_OK) return st;
+    CS_CUDA(S, cudaEventRecord(e1, S->stream));
+    CS_CUDA(S, cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CS_CUDA(S, cudaEventElapsedTime(&ms, e0, e1));
+    double total = 0.0;
+    CS_CUDA(S, cudaMemcpy(&total, out, sizeof(double), cudaMemcpyDeviceToHost));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (total != (double)n * S->grid * kBlock) { S->err = "barrier probe: wrong all-reduce result"; return CS_ECUDA; }
+    *us_per_barrier = 1e3 * ms / n;
     return CS_OK;
 }
 

@@ -4,10 +4,7 @@
 // are separated by grid-wide barriers, so that the scalars of the inner CG (alpha, beta, residual
 // norms) and its exit test never leave the device.  Citations P:<line> = /root/reference/PAPER.md.
 #pragma once
-#include <cooperative_groups.h>
 #include <cstdint>
-
-namespace cg = cooperative_groups;
 
 namespace csd {
 
@@ -67,7 +64,9 @@ struct Ctx {
     double *w, *r, *v, *wd, *D, *btil, *wsave;
     const double *b;
     double *partials;       // [2][kMaxRed][gridDim]
+    unsigned int *bar;      // grid-barrier word
     Scalars *sc;
+    double *partial_probe;  // scratch of cs_barrier_probe
     double mu, t, o_floor, cg_tol;
     int cg_max_iter;
     double norm_b, norm_c;
@@ -86,18 +85,44 @@ __device__ __forceinline__ double group_reduce(double v) {
     return v;
 }
 
+constexpr int kMaxGrid = 32 * 12;    // CTAs of a cooperative launch (148 SMs x 2 = 296 on B200)
+
+// Grid-wide barrier + deterministic all-reduce.
+//   barrier : one 32-bit word; every CTA adds 1 except CTA 0, which adds 2^31 - (grid-1), so the top
+//             bit flips exactly when the last CTA has arrived; each CTA's thread 0 spins on that bit.
+//             One atomic round trip plus the spin; the L2 atomic unit does the counting.
+//   reduce  : every CTA stores its NR partial sums before arriving; after the barrier NR warps of every
+//             CTA read all gridDim partials (<= 12 per lane, all loads in flight), add them in a fixed order
+//             and butterfly: every CTA gets the same bits without a second barrier.
+// Partials are double buffered (a fast CTA may already write the next reduction's partials while a slow
+// one still reads this one's; it cannot get two barriers ahead).
+// Measured on B200 (cs_barrier_probe): see profiles/r01_ncu_notes.md; a flag/mailbox barrier with a
+// collector CTA was 6.4 us per barrier and is not used.
 struct GridCtl {            // per-thread view of the grid barrier state (uniform over the grid)
-    cg::grid_group grid;
+    unsigned int *bar;
     int parity;
-    double *partials;
-    double *smem;           // [kMaxRed * kWarps]
+    double *partials;               // [2][kMaxRed][gridDim]
+    double *smem;                   // [kMaxRed * kWarps]
     unsigned long long t_last, ns[8];
-    __device__ GridCtl(double *partials_, double *smem_) : grid(cg::this_grid()), parity(0), partials(partials_), smem(smem_) {
+    __device__ GridCtl(double *partials_, double *smem_, unsigned int *bar_) : bar(bar_), parity(0), partials(partials_), smem(smem_) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) ns[i] = 0;
         t_last = now();
     }
-    __device__ void sync() { grid.sync(); }
+    __device__ void sync() {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned int inc = blockIdx.x == 0 ? 0x80000000u - (gridDim.x - 1) : 1u;
+            __threadfence();                                   // release the CTA's writes
+            const unsigned int old = atomicAdd(bar, inc);
+            unsigned int cur;
+            do {
+                asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(cur) : "l"(bar) : "memory");
+            } while (((old ^ cur) & 0x80000000u) == 0);
+            __threadfence();                                   // acquire everybody else's
+        }
+        __syncthreads();
+    }
     __device__ static unsigned long long now() {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -123,7 +148,7 @@ struct GridCtl {            // per-thread view of the grid barrier state (unifor
 // Every thread of every CTA returns the same bits.
 template <int NR, class Op = OpSum>
 __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
-    static_assert(NR <= kMaxRed, "too many scalars");
+    static_assert(NR <= kMaxRed && NR <= kWarps, "too many scalars");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
     for (int i = 0; i < NR; ++i) {
@@ -135,12 +160,19 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
     if (threadIdx.x < NR) {
         double acc = gc.smem[threadIdx.x * kWarps];
         for (int w = 1; w < kWarps; ++w) acc = Op::f(acc, gc.smem[threadIdx.x * kWarps + w]);
-        buf[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = acc;
+        __stcg(buf + (size_t)threadIdx.x * gridDim.x + blockIdx.x, acc);
     }
-    gc.grid.sync();
+    gc.sync();
     if (warp < NR) {
-        double acc = ident;
-        for (int b = lane; b < (int)gridDim.x; b += 32) acc = Op::f(acc, __ldcg(buf + (size_t)warp * gridDim.x + b));
+        double t[kMaxGrid / 32];
+#pragma unroll
+        for (int q = 0; q < kMaxGrid / 32; ++q) {
+            const int b = lane + 32 * q;
+            t[q] = b < (int)gridDim.x ? __ldcg(buf + (size_t)warp * gridDim.x + b) : ident;
+        }
+        double acc = t[0];
+#pragma unroll
+        for (int q = 1; q < kMaxGrid / 32; ++q) acc = Op::f(acc, t[q]);
         acc = group_reduce<32, Op>(acc);
         if (lane == 0) gc.smem[warp] = acc;
     }

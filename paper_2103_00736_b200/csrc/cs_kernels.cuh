@@ -166,7 +166,7 @@ struct EpiUpdate {  // steps 17-18: r = 2 A~'w - p ; s <- s/2 - r/2 + d = (s+p)/
 
 __global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_iter) {
     __shared__ double smem[kMaxRed * kWarps];
-    GridCtl gc(c.partials, smem);
+    GridCtl gc(c.partials, smem, c.bar);
     long long cg_total = 0;
     int cg_last = 0;
     bool any_max = false;

@@ -134,7 +134,7 @@ struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu
 // use_rule = 1: O from steps 5-11 applied to (xb, zb); 0: O already in c.O (cs_set_scaling)
 __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_rule) {
     __shared__ double smem[kMaxRed * kWarps];
-    GridCtl gc(c.partials, smem);
+    GridCtl gc(c.partials, smem, c.bar);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     if (use_rule) {
         double mm[2] = {-INFINITY, -INFINITY};
@@ -235,7 +235,7 @@ __device__ __forceinline__ double soc_dist2(double t, double nu2) {
 
 __global__ void __launch_bounds__(kBlock, CS_MINB) k_residuals(Ctx c) {
     __shared__ double smem[kMaxRed * kWarps];
-    GridCtl gc(c.partials, smem);
+    GridCtl gc(c.partials, smem, c.bar);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     TermCsrX t1{c.xb, c.O};
     EpiPres e1{c.btil, c.D, c.wd, c.w, c.mu, 0.0, 0.0};
@@ -276,6 +276,19 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_residuals(Ctx c) {
         o[7] = fmax(fmax(o[1], o[3]), fmax(o[5], o[6]));
         o[8] = cx; o[9] = by; o[10] = sqrt(c.sc->fp_res2);
     }
+}
+
+// n empty grid barriers (each with a 1-value all-reduce): measures the bare barrier latency.
+__global__ void __launch_bounds__(kBlock, CS_MINB) k_barrier_probe(Ctx c, int n, double *out) {
+    __shared__ double smem[kMaxRed * kWarps];
+    GridCtl gc(c.partials, smem, c.bar);
+    double acc = 0.0;
+    for (int i = 0; i < n; ++i) {
+        double v[1] = {1.0};
+        grid_reduce<1>(v, gc);
+        acc += v[0];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) *out = acc;
 }
 
 }  // namespace csd
