@@ -129,6 +129,32 @@ def whole_job_value(iters_per_rank: int, world: int, ms_max: float) -> float:
     return world * iters_per_rank / (ms_max * 1e-3)
 
 
+def solve_to_tolerance(a, p, S, torch):
+    """Time to kkt_rel <= tol with the paper's schedule L = {L_first, L_first + L_every, ...} (eq.(17),(18)),
+    one cs_residuals read-back every --check-every passes (B metric: "time to 1e-4 relative KKT residual")."""
+    L = set(p.schedule(a.max_iter))
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    l, hist, r = 0, [], None
+    while l < a.max_iter:
+        nxt = min(a.max_iter, (l // a.check_every + 1) * a.check_every)
+        S.run(nxt - l, L=[x for x in L if l < x <= nxt])
+        l = nxt
+        r = S.residuals()
+        hist.append((l, r["kkt_rel"], time.perf_counter() - t0, r["cg_steps_total"]))
+        if r["kkt_rel"] <= a.tol:
+            break
+    dt = time.perf_counter() - t0
+    print(json.dumps({"mode": "solve", "workload": p.name, "tol": a.tol, "reached": bool(r["kkt_rel"] <= a.tol),
+                      "time_to_tol_s": dt, "iterations": l, "cg_steps_total": r["cg_steps_total"],
+                      "n_conditionings": r["n_conditionings"], "kkt_rel": r["kkt_rel"], "pobj": r["pobj"],
+                      "opt_value": p.opt_value(), "iters_per_s": l / dt,
+                      "schedule": f"L={{{p.L_first},{p.L_first + p.L_every},...}}, t={p.t}, mu={p.mu}",
+                      "history": [(i, float(f"{k:.3e}"), round(t, 3), c) for i, k, t, c in hist[-12:]]}))
+    S.destroy()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -140,6 +166,11 @@ def main():
     ap.add_argument("--k", type=int, default=1, help="outer iterations per step (1 = continuous conditioning, P:313)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--solve", action="store_true",
+                    help="extra mode: run the paper's schedule (17)/(18) to --tol and report the time to tolerance")
+    ap.add_argument("--tol", type=float, default=1e-4)
+    ap.add_argument("--check-every", type=int, default=25)
+    ap.add_argument("--max-iter", type=int, default=3000)
     ap.add_argument("--cg-max-iter", type=int, default=0, help="profiling only: cap CG steps per solve (0 = library default)")
     a = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -175,6 +206,9 @@ def main():
     S = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     if a.cg_max_iter:
         S.set_params(cg_max_iter=a.cg_max_iter)
+
+    if a.solve:
+        return solve_to_tolerance(a, p, S, torch)
 
     def step():
         S.condition()

@@ -7,9 +7,11 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <chrono>
 #include <cstdlib>
 #include <new>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/cs.h"
@@ -266,6 +268,14 @@ int64_t cs_kernel_launches(const cs_solver *S) { return S ? S->launches : 0; }
 
 static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
                              const cs_cones *K) {
+    const bool verbose = getenv("CS_VERBOSE") != nullptr;      // stage timings of cs_create on stderr
+    auto t_prev = std::chrono::steady_clock::now();
+    auto lap = [&](const char *what) {
+        if (!verbose) return;
+        const auto t = std::chrono::steady_clock::now();
+        fprintf(stderr, "[cs_create] %-28s %8.1f ms\n", what, std::chrono::duration<double, std::milli>(t - t_prev).count());
+        t_prev = t;
+    };
     const int64_t m64 = A->m, n64 = A->n, nnz64 = A->nnz;
     if (m64 <= 0 || n64 <= 0 || nnz64 <= 0 || m64 >= INT32_MAX || n64 >= INT32_MAX || nnz64 >= INT32_MAX) {
         S->err = "sizes must be positive and below 2^31";
@@ -308,57 +318,48 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     double nb = 0.0, nc = 0.0;
     for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
     for (int j = 0; j < n; ++j) { if (!std::isfinite(hc[j])) { S->err = "non-finite c"; return CS_EINVAL; } nc += hc[j] * hc[j]; }
+    lap("fetch + validate");
     // ---- internal ordering: rows sorted by decreasing length, orthant columns likewise (Lorentz blocks
     //      keep their place so that cones stay contiguous).  perm[internal] = caller's index.
     std::vector<int> rlen((size_t)m), clen((size_t)n, 0);
     for (int i = 0; i < m; ++i) rlen[i] = rptr[i + 1] - rptr[i];
     for (int k = 0; k < nnz; ++k) clen[cidx[k]]++;
     const std::vector<int> perm_r = order_by_length(rlen, m);
-    std::vector<int> perm_c = order_by_length(clen, (int)K->n_lin);
-    {   // Within each length class, order the orthant columns lexicographically by the (internal, i.e.
-        // hottest-first) rows they touch.  Columns sharing the heavy rows of a power-law matrix become
-        // neighbours, so a heavy row's gathers from u run over a few contiguous stretches (coalesced
-        // L1 wavefronts) instead of one sector per entry.  Pure relabelling: results are unchanged.
-        std::vector<int> inv_r((size_t)m);
-        for (int i = 0; i < m; ++i) inv_r[perm_r[i]] = i;
-        std::vector<int> cp0((size_t)n + 1, 0), cr0((size_t)nnz);
-        for (int k = 0; k < nnz; ++k) cp0[(size_t)cidx[k] + 1]++;
-        for (int j = 0; j < n; ++j) cp0[(size_t)j + 1] += cp0[j];
-        std::vector<int> fill(cp0.begin(), cp0.end() - 1);
-        for (int i = 0; i < m; ++i) {           // internal row order => every column list comes out ascending
-            const int src = perm_r[i];
-            for (int k = rptr[src]; k < rptr[src + 1]; ++k) cr0[fill[cidx[k]]++] = i;
-        }
-        constexpr int kDepth = 4;
-        auto less = [&](int a, int b) {
-            const int la = clen[a], lb = clen[b];
-            if (la != lb) return la > lb;
-            const int d = std::min(la, kDepth);
-            for (int q = 0; q < d; ++q) {
-                const int ra = cr0[cp0[a] + q], rb = cr0[cp0[b] + q];
-                if (ra != rb) return ra < rb;
-            }
-            return a < b;
-        };
-        if (rlen[perm_r[0]] > kShortMax) std::sort(perm_c.begin(), perm_c.begin() + K->n_lin, less);
-    }
+    // (A lexicographic ordering of the columns by the heavy rows they touch was tried so that those rows'
+    //  gathers run over contiguous stretches; it cost 3.4 s at config 4 and changed nothing measurable.)
+    const std::vector<int> perm_c = order_by_length(clen, (int)K->n_lin);
     std::vector<int> inv_c((size_t)n);
     for (int j = 0; j < n; ++j) inv_c[perm_c[j]] = j;
+    lap("row/column ordering");
     // row-major copy in internal numbering (entries of a row sorted by internal column)
     std::vector<int> rp2((size_t)m + 1, 0), ci2((size_t)nnz);
     std::vector<double> va2((size_t)nnz);
+    for (int i = 0; i < m; ++i) rp2[(size_t)i + 1] = rp2[i] + rlen[perm_r[i]];
     {
-        std::vector<std::pair<int, double>> tmp;
-        for (int i = 0; i < m; ++i) {
-            const int src = perm_r[i], a0 = rptr[src], len = rlen[src];
-            tmp.resize(len);
-            for (int k = 0; k < len; ++k) tmp[k] = {inv_c[cidx[a0 + k]], val[a0 + k]};
-            std::sort(tmp.begin(), tmp.end(), [](const std::pair<int, double> &u, const std::pair<int, double> &v) { return u.first < v.first; });
-            const int dst = rp2[i];
-            rp2[(size_t)i + 1] = dst + len;
-            for (int k = 0; k < len; ++k) { ci2[dst + k] = tmp[k].first; va2[dst + k] = tmp[k].second; }
-        }
+        auto fill_rows = [&](int i0, int i1) {
+            std::vector<std::pair<int, double>> tmp;
+            for (int i = i0; i < i1; ++i) {
+                const int src = perm_r[i], a0 = rptr[src], len = rlen[src], dst = rp2[i];
+                if (len <= kShortMax) {     // order inside a short row is irrelevant
+                    for (int k = 0; k < len; ++k) { ci2[dst + k] = inv_c[cidx[a0 + k]]; va2[dst + k] = val[a0 + k]; }
+                    continue;
+                }
+                tmp.resize(len);            // long rows: ascending internal column, so their gathers stay as local as they were
+                for (int k = 0; k < len; ++k) tmp[k] = {inv_c[cidx[a0 + k]], val[a0 + k]};
+                std::sort(tmp.begin(), tmp.end(), [](const std::pair<int, double> &u, const std::pair<int, double> &v) { return u.first < v.first; });
+                for (int k = 0; k < len; ++k) { ci2[dst + k] = tmp[k].first; va2[dst + k] = tmp[k].second; }
+            }
+        };
+        const int nt = (int)std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
+        std::vector<std::thread> th;
+        // rows are sorted by decreasing length: deal them out round-robin in blocks so the long ones spread
+        std::vector<std::vector<std::pair<int, int>>> work(nt);
+        const int blk = 4096;
+        for (int i0 = 0, q = 0; i0 < m; i0 += blk, ++q) work[q % nt].push_back({i0, std::min(m, i0 + blk)});
+        for (int t = 0; t < nt; ++t) th.emplace_back([&, t] { for (auto &w : work[t]) fill_rows(w.first, w.second); });
+        for (auto &t : th) t.join();
     }
+    lap("row-major copy");
     // column-major copy (counting sort by internal column; rows come out sorted within a column)
     std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
     std::vector<double> cv2((size_t)nnz);
@@ -380,6 +381,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         for (int j = 0; j < n; ++j) t[j] = hc[perm_c[j]];
         std::copy(t.begin(), t.begin() + n, hc.begin());
     }
+    lap("column-major copy");
     // ---- device state
     Ctx &x = S->ctx;
     x.m = m; x.n = n; x.n_lin = (int)K->n_lin; x.n_soc = (int)K->n_soc;
@@ -388,8 +390,17 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_upload(S, &ip, cone_off.data(), cone_off.size())) != CS_OK) return st; x.cone_off = ip;
     if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
     if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
-    if ((st = upload_sparse(S, make_sparse(rp2, ci2, va2), &x.R)) != CS_OK) return st;
-    if ((st = upload_sparse(S, make_sparse(cp2, ri2, cv2), &x.C)) != CS_OK) return st;
+    {
+        HostSparse hr, hc2;
+        std::thread tr([&] { hr = make_sparse(rp2, ci2, va2); });
+        hc2 = make_sparse(cp2, ri2, cv2);
+        tr.join();
+        lap("slices (rows | columns)");
+        if ((st = upload_sparse(S, hr, &x.R)) != CS_OK) return st;
+        if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;
+        CS_CUDA(S, cudaStreamSynchronize(S->stream));
+        lap("upload");
+    }
     if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
     if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
     double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.d, &x.chat};
@@ -408,6 +419,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     }
     if ((st = dev_zeros(S, &x.sc, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partial_probe, 1)) != CS_OK) return st;
+    lap("vectors");
     // ---- cooperative grid: as many CTAs as can be co-resident
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
