@@ -139,6 +139,12 @@ cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, 
  * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6], [7] reserved.  One D2H copy + sync. */
 cs_status cs_phase_times(cs_solver *S, double out[8]);
 
+/* Diagnostic (no handle, current device, default stream, synchronous): time n_idx uniformly random 8-byte
+ * gathers from an n_vec-element vector with the launch shape of the solver's sparse passes (indices
+ * streamed, 8 gathers in flight per thread), and the same loop without the gathers.  The difference is the
+ * LSU/L1TEX gather ceiling that bounds the sparse passes on irregular matrices. */
+cs_status cs_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only);
+
 /* Diagnostic: run n empty grid barriers (each a 1-value all-reduce over all CTAs, result checked) in one
  * launch and report the mean latency in microseconds.  Synchronous. */
 cs_status cs_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier);

@@ -44,7 +44,7 @@ class cs_resid(C.Structure):
 
 
 EXPORTS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
-           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_phase_times", "cs_barrier_probe", "cs_kernel_launches", "cs_last_error",
+           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_phase_times", "cs_gather_probe", "cs_barrier_probe", "cs_kernel_launches", "cs_last_error",
            "cs_destroy")
 
 _lib = None
@@ -76,7 +76,8 @@ def lib():
         L.cs_destroy.restype = None
         L.cs_phase_times.argtypes = [vp, C.POINTER(C.c_double)]
         L.cs_barrier_probe.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
-        for name in EXPORTS[:11]:
+        L.cs_gather_probe.argtypes = [C.c_int64, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        for name in EXPORTS[:12]:
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -111,6 +112,15 @@ def _same_space(*tags):
     if tags and any(t != tags[0] for t in tags):
         raise ValueError("all arrays of one call must live in the same memory space")
     return tags[0] if tags else CS_HOST
+
+
+def gather_probe(n_vec, n_idx):
+    """(us with gathers, us without) of n_idx random 8-byte gathers from an n_vec vector (cs_gather_probe)."""
+    a, b = C.c_double(), C.c_double()
+    st = lib().cs_gather_probe(int(n_vec), int(n_idx), C.byref(a), C.byref(b))
+    if st != CS_OK:
+        raise CsError(st, "cs_gather_probe failed")
+    return a.value, b.value
 
 
 class Solver:

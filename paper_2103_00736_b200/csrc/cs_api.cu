@@ -544,6 +544,43 @@ cs_status cs_phase_times(cs_solver *S, double out[8]) {
     return CS_OK;
 }
 
+cs_status cs_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only) {
+    if (n_vec < 1 || n_idx < 1 || n_vec >= INT32_MAX || n_idx >= INT32_MAX || !us_gather || !us_stream_only) return CS_EINVAL;
+    int *idx = nullptr; double *x = nullptr, *out = nullptr;
+    int sms = 0, dev = 0;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cs_status st = CS_ECUDA;
+    do {
+        if (cudaGetDevice(&dev) != cudaSuccess) break;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) break;
+        const int grid = sms * 2;
+        if (cudaMalloc(&idx, sizeof(int) * n_idx) != cudaSuccess || cudaMalloc(&x, sizeof(double) * n_vec) != cudaSuccess ||
+            cudaMalloc(&out, sizeof(double) * (size_t)grid * kBlock) != cudaSuccess) { st = CS_ENOMEM; break; }
+        if (cudaMemset(x, 0, sizeof(double) * n_vec) != cudaSuccess) break;
+        k_probe_indices<<<sms * 8, 256>>>(idx, (int)n_idx, (int)n_vec);
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+        double us[2] = {0.0, 0.0};
+        bool ok = true;
+        for (int mode = 0; mode < 2 && ok; ++mode)
+            for (int rep = 0; rep < 3 && ok; ++rep) {           // keep the last of three
+                cudaEventRecord(e0);
+                k_gather_probe<<<grid, kBlock>>>(idx, x, out, (int)n_idx, 1 - mode);
+                cudaEventRecord(e1);
+                float ms = 0.f;
+                ok = cudaEventSynchronize(e1) == cudaSuccess && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess;
+                us[mode] = 1e3 * ms;
+            }
+        if (!ok) break;
+        *us_gather = us[0];
+        *us_stream_only = us[1];
+        st = CS_OK;
+    } while (false);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(idx); cudaFree(x); cudaFree(out);
+    return st;
+}
+
 cs_status cs_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier) {
     if (!S || n < 1 || !us_per_barrier) return CS_EINVAL;
     cudaEvent_t e0, e1;

@@ -291,4 +291,29 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_barrier_probe(Ctx c, int n,
     if (blockIdx.x == 0 && threadIdx.x == 0) *out = acc;
 }
 
+// Diagnostic: n_idx uniformly random 8-byte gathers from an n_vec-vector, 8 in flight per thread, indices
+// streamed; the launch shape of the solver's passes.  Measures the LSU/L1TEX gather ceiling of the GPU.
+__global__ void __launch_bounds__(kBlock, CS_MINB) k_gather_probe(const int *idx, const double *x, double *out, int n_idx, int gather) {
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    double acc = 0.0;
+    for (int i = tid; i + 7 * nth < n_idx; i += 8 * nth) {
+        int j[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) j[q] = __ldcs(idx + i + q * nth);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc += gather ? x[j[q]] : (double)j[q];
+    }
+    out[tid] = acc;
+}
+__global__ void k_probe_indices(int *idx, int n_idx, int n_vec) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int i = tid; i < n_idx; i += nth) {
+        unsigned long long z = (unsigned long long)i * 0x9E3779B97F4A7C15ull + 0x1234567ull;   // splitmix64
+        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+        z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+        z ^= z >> 31;
+        idx[i] = (int)(z % (unsigned long long)n_vec);
+    }
+}
+
 }  // namespace csd

@@ -226,3 +226,12 @@ def test_cg_max_is_reported_not_fatal():
         S.residuals(strict=True)
     assert ei.value.status == binding.CS_ECGMAX
     assert S.residuals(strict=True)["cg_hit_max"] == 0   # flag cleared by the previous readback
+
+
+def test_diagnostic_probes():
+    """cs_gather_probe / cs_barrier_probe run and give sane numbers (the barrier probe checks its all-reduce)."""
+    from paper_2103_00736_b200 import binding
+    us_g, us_s = binding.gather_probe(1_000_000, 8_000_000)
+    assert 0 < us_s < us_g < 5e4
+    S = binding.Solver.from_problem(W.config(1, 0.05), device="cuda:0")
+    assert 0.2 < S.barrier_probe(200) < 200.0
