@@ -78,7 +78,8 @@ typedef struct {
 } cs_params;
 
 /* Residuals of the KKT conditions (24) P:480-487 in ORIGINAL coordinates, for the current iterate
- * x = O(p+s)/2, z = O^{-1}(p-s)/(2mu) (steps 19-20) and y = D(w_d - w)/mu:
+ * x = O(p+s)/2, z = O^{-1}(p-s)/(2mu) (steps 19-20) and the derived multiplier y = D w/mu, where
+ * w is the solution of the pass's single solve (A~A~') w = b~ - A~(p - mu c^):
  *   pres_abs = ||Ax-b||_2 (16a)      pres_rel = pres_abs/(1+||b||_2)
  *   dres_abs = ||c-z-A'y||_2                dres_rel = dres_abs/(1+||c||_2)
  *   gap_abs  = |c'x-b'y|  (cf. 16b)  gap_rel  = gap_abs/(1+|c'x|+|b'y|)
@@ -88,7 +89,7 @@ typedef struct {
 typedef struct {
     int64_t iter;           /* passes of steps 16-18 done so far (l of Algorithm 2) */
     int64_t cg_steps_total; /* CG steps over all solves so far                       */
-    int64_t cg_steps_cond;  /* ... of which inside cs_condition's solve for d         */
+    int64_t cg_steps_cond;  /* ... of which inside cs_condition (0: d is folded into the pass) */
     int32_t cg_steps_last;  /* CG steps of the most recent solve                     */
     int32_t n_conditionings;
     int32_t cg_hit_max;     /* 1 if some solve hit cg_max_iter since the last cs_residuals */
@@ -118,7 +119,8 @@ cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem wh
 cs_status cs_iterate(cs_solver *S, int64_t k);
 
 /* Steps 5-14 from the current (x,z): o per cone, O = o^alpha, A_hat = D A O (D = row
- * equilibration, mathematically inert), c_hat = O c, d, and the recast s = O^{-1}x - mu O z.
+ * equilibration, mathematically inert), c_hat = O c, and the recast s = O^{-1}x - mu O z.  Step 13's vector d
+ * is folded into the pass (s+ = (s+p)/2 - mu c^ + A~'w), so a conditioning needs no linear solve.
  * The schedule L is the caller's: L = {300,400,...} is cs_iterate(299); cs_condition(); cs_iterate(100); ... */
 cs_status cs_condition(cs_solver *S);
 

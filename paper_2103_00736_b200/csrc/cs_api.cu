@@ -140,7 +140,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 const int len = ptr[seg + 1] - ptr[seg], t = lane % T;
                 for (int k = 0; k < width; ++k) {
                     const int e = k * T + t;
-                    h.idx[(size_t)off + 32u * k + lane] = idx[ptr[seg] + std::min(e, len - 1)];
+                    h.idx[(size_t)off + 32u * k + lane] = len > 0 ? idx[ptr[seg] + std::min(e, len - 1)] : 0;  // empty segment: any valid index
                     if (lane / T < cnt && e < len) h.val[(size_t)off + 32u * k + lane] = val[ptr[seg] + e];
                 }
             }
@@ -403,9 +403,9 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     }
     if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
     if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
-    double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.d, &x.chat};
+    double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.chat};
     for (double **q : nv) if ((st = dev_zeros(S, q, (size_t)n)) != CS_OK) return st;
-    double **mv[] = {&x.w, &x.r, &x.v, &x.wd, &x.btil, &x.wsave};
+    double **mv[] = {&x.w, &x.r, &x.v, &x.btil};
     for (double **q : mv) if ((st = dev_zeros(S, q, (size_t)m)) != CS_OK) return st;
     {   // O = 1, D = 1, x = z = e_K
         std::vector<double> ones((size_t)std::max(m, n), 1.0), ek((size_t)n, 0.0);

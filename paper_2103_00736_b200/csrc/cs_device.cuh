@@ -58,10 +58,10 @@ struct Ctx {
     const int *perm_r, *perm_c;  // internal index -> caller's index (rows / columns sorted by length)
     Sparse R, C;            // row-major (segments = rows) and column-major (segments = columns) copies of A
     // n-vectors
-    double *s, *p, *g, *e, *u, *d, *chat, *O, *xb, *zb;
+    double *s, *p, *g, *e, *u, *chat, *O, *xb, *zb;
     const double *c;
     // m-vectors
-    double *w, *r, *v, *wd, *D, *btil, *wsave;
+    double *w, *r, *v, *D, *btil;
     const double *b;
     double *partials;       // [2][kMaxRed][gridDim]
     unsigned int *bar;      // grid-barrier word

@@ -38,19 +38,28 @@ __device__ __forceinline__ void soc_abs_block(const double *s, int a, int b, int
     }
 }
 
-// step 16: p = abs_K(s) ; also e = p - g (the warm-start difference, g = A~' w of the previous pass)
+// step 16: p = abs_K(s) ; also the two vectors the rhs pass gathers:
+//   u := p - mu c^            (q = b~ - A~ u is the right-hand side of this pass's solve)
+//   e := p - mu c^ + g        (r0 = b~ - A~ e is its residual at the warm start w, g = A~'w kept from before)
 __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     for (int j = tid; j < c.n_lin; j += nth) {
         const double pj = fabs(c.s[j]);
+        const double uj = pj - c.mu * c.chat[j];
         c.p[j] = pj;
-        c.e[j] = pj - c.g[j];
+        c.u[j] = uj;
+        c.e[j] = uj + c.g[j];
     }
     if (c.n_soc) {
         const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
         constexpr int CPW = 32 / kConeLanes;
         const int gwarp = tid >> 5, nwarps = nth >> 5;
-        auto put = [&](int j, double, double pj) { c.p[j] = pj; c.e[j] = pj - c.g[j]; };
+        auto put = [&](int j, double, double pj) {
+            const double uj = pj - c.mu * c.chat[j];
+            c.p[j] = pj;
+            c.u[j] = uj;
+            c.e[j] = uj + c.g[j];
+        };
         for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
             const int ci = base + sub;
             const bool act = ci < c.n_soc;
@@ -61,6 +70,10 @@ __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// The ONE solve of a pass: with w_p = (A~A~')^{-1} A~ p and w_d = (A~A~')^{-1}(b~ + mu A~ c^),
+// s+ = (s+p)/2 - A~'w_p + d and d = A~'w_d - mu c^ give s+ = (s+p)/2 - mu c^ + A~'w with
+// (A~A~') w = b~ - A~(p - mu c^): neither d nor a solve at conditioning time is needed, and w = mu D^{-1} y
+// converges to the (scaling-independent) dual solution, which makes the warm start effective.
 // Inner solve: CG on (A~ A~') w = q, started from the current w with residual r already in c.r and
 // rho = ||r||^2, qq = ||q||^2 known.  Two sparse passes and two grid reductions per step:
 //   K1 (columns, CSC):  u = A~' r + beta u          sigma = ||u||^2       (u == A~' v by induction)
@@ -132,7 +145,7 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, d
 // ---------------------------------------------------------------------------------------------
 // k_iterate
 // ---------------------------------------------------------------------------------------------
-struct TermCsrPE {  // (A~ p, A~ (p - g))
+struct TermCsrPE {  // (A~ u, A~ e)
     const double *p, *e;
     typedef double2 G;
     __device__ __forceinline__ G fetch(int j) const { return make_double2(p[j], e[j]); }
@@ -141,23 +154,24 @@ struct TermCsrPE {  // (A~ p, A~ (p - g))
         acc[1] += a * g.y;
     }
 };
-struct EpiRhs {     // r = A~(p - g) = q - A~A~'w ;  qq = ||A~ p||^2 ; rho = ||r||^2
-    double *r; double qq, rho;
+struct EpiRhs {     // q = b~ - A~(p - mu c^) ; r = q - A~A~'w = b~ - A~ e ; qq = ||q||^2 ; rho = ||r||^2
+    double *r; const double *btil; double qq, rho;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[2], const Pre &) {
-        r[i] = a[1];
-        qq += a[0] * a[0];
-        rho += a[1] * a[1];
+        const double q = btil[i] - a[0], ri = btil[i] - a[1];
+        r[i] = ri;
+        qq += q * q;
+        rho += ri * ri;
     }
 };
-struct EpiUpdate {  // steps 17-18: r = 2 A~'w - p ; s <- s/2 - r/2 + d = (s+p)/2 - A~'w + d
-    double *s, *g; const double *p, *d; double fp2;
-    struct Pre { double s, p, d; };
-    __device__ __forceinline__ Pre pre(int j) const { return Pre{s[j], p[j], d[j]}; }
+struct EpiUpdate {  // steps 17-18 with d folded in: s <- (s+p)/2 - mu c^ + A~'w
+    double *s, *g; const double *p, *chat; double mu; double fp2;
+    struct Pre { double s, p, c; };
+    __device__ __forceinline__ Pre pre(int j) const { return Pre{s[j], p[j], chat[j]}; }
     __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &q) {
         const double sj = q.s;
-        const double sn = 0.5 * (sj + q.p) - a[0] + q.d;
+        const double sn = 0.5 * (sj + q.p) - mu * q.c + a[0];
         g[j] = a[0];
         s[j] = sn;
         fp2 += (sn - sj) * (sn - sj);
@@ -176,19 +190,19 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_
         phase_cone_reflect(c);                                   // step 16
         gc.sync();
         gc.lap(kPhCone);
-        TermCsrPE tq{c.p, c.e};
-        EpiRhs eq{c.r, 0.0, 0.0};
+        TermCsrPE tq{c.u, c.e};
+        EpiRhs eq{c.r, c.btil, 0.0, 0.0};
         seg_reduce<2, false>(c.R, tq, eq, gc);
         gc.lap(kPhRhs);
         double red[2] = {eq.qq, eq.rho};
         grid_reduce<2>(red, gc);
         gc.lap(kPhReduce);
         bool hm;
-        cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} A~ p
+        cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} (b~ - A~(p - mu c^)) = w_d - w_p
         any_max |= hm;
         cg_total += cg_last;
         TermDot tw{c.w};
-        EpiUpdate eu{c.s, c.g, c.p, c.d, 0.0};
+        EpiUpdate eu{c.s, c.g, c.p, c.chat, c.mu, 0.0};
         seg_reduce<1, false>(c.C, tw, eu, gc);                   // steps 17-18
         gc.lap(kPhUpdate);
         double rf[1] = {eu.fp2};

@@ -15,10 +15,10 @@ __global__ void k_materialize_xz(Ctx c) {
     }
 }
 
-// y = D (w_d - w) / mu  (derived multiplier; s+ = x~ - mu(c^ - A~'y'), y' = (w_d - w)/mu)
+// y = D w / mu  (derived multiplier: s+ = x~ - mu(c^ - A~'y'), y' = w/mu, w = w_d - w_p of cs_kernels.cuh)
 __global__ void k_dual_y(Ctx c, double *y) {   // written in the caller's (original) row order
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
-    for (int i = tid; i < c.m; i += nth) y[c.perm_r[i]] = c.D[i] * (c.wd[i] - c.w[i]) / c.mu;
+    for (int i = tid; i < c.m; i += nth) y[c.perm_r[i]] = c.D[i] * c.w[i] / c.mu;
 }
 
 // internal (sorted) order <-> caller's order: dst[i] = src[perm[i]]  /  dst[perm[i]] = src[i]
@@ -72,9 +72,9 @@ struct TermRowNorm {  // sum_j (A_ij O_j)^2   (traversed over the PRISTINE value
         acc[0] += x * x;
     }
 };
-struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b ; the multipliers follow the change of row scaling:
-                      // w_true = D w is what carries over, so w <- (D_old/D_new) w is the warm start (wsave), same for w_d (w)
-    double *D, *btil, *w, *wd, *wsave; const double *b;
+struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b ; the multiplier follows the change of row scaling:
+                      // D w = mu y is what carries over, so w <- (D_old/D_new) w is the warm start
+    double *D, *btil, *w; const double *b;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
@@ -82,8 +82,7 @@ struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b ; the multipliers foll
         const double ratio = D[i] / di;
         D[i] = di;
         btil[i] = di * b[i];
-        wsave[i] = ratio * w[i];
-        w[i] = ratio * wd[i];       // the solve for w_d below runs in c.w
+        w[i] = ratio * w[i];
     }
 };
 struct ScaleCsr {     // A~_ij = D_i A_ij O_j on the row-major copy (segment = row i, minor = column j)
@@ -94,40 +93,13 @@ struct ScaleCsc {     // same on the column-major copy (segment = column j, mino
     const double *O, *D;
     __device__ __forceinline__ double operator()(int j, double a0, int i) const { return a0 * O[j] * D[i]; }
 };
-struct EpiWarmE {     // e = mu c^ - A~'w_d(guess): the rhs pass below then gives the warm-start residual
-    double *e; const double *chat; double mu;
+struct EpiRecast {    // step 14: s = O^{-1}x - mu O z ; g = A~'w for the warm start of the next pass
+    double *s, *g; const double *xb, *zb, *O; double mu;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
-    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) { e[j] = mu * chat[j] - a[0]; }
-};
-struct TermTwo {      // (sum a x[j], sum a y[j])
-    const double *x, *y;
-    typedef double2 G;
-    __device__ __forceinline__ G fetch(int j) const { return make_double2(x[j], y[j]); }
-    __device__ __forceinline__ void fma(double a, G g, double (&acc)[2]) const {
-        acc[0] += a * g.x;
-        acc[1] += a * g.y;
-    }
-};
-struct EpiRhsD {      // q = b~ + mu A~ c^ ; r = q - A~A~'w_d(guess) = b~ + A~ e
-    double *r; const double *btil; double mu; double qq, rho;
-    typedef NoPre Pre;
-    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
-    __device__ __forceinline__ void operator()(int i, const double (&a)[2], const Pre &) {
-        const double q = btil[i] + mu * a[0], ri = btil[i] + a[1];
-        r[i] = ri;
-        qq += q * q;
-        rho += ri * ri;
-    }
-};
-struct EpiD {         // step 13: d = A~'w_d - mu c^ ; step 14: s = O^{-1}x - mu O z ; g = A~'w (warm start of the next pass)
-    double *d, *s, *g; const double *chat, *xb, *zb, *O; double mu;
-    typedef NoPre Pre;
-    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
-    __device__ __forceinline__ void operator()(int j, const double (&a)[2], const Pre &) {
-        d[j] = a[0] - mu * chat[j];
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) {
         s[j] = xb[j] / O[j] - mu * O[j] * zb[j];
-        g[j] = a[1];
+        g[j] = a[0];
     }
 };
 
@@ -148,7 +120,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     gc.sync();
     {   // row equilibration D
         TermRowNorm t{c.O};
-        EpiRowScale e{c.D, c.btil, c.w, c.wd, c.wsave, c.b};
+        EpiRowScale e{c.D, c.btil, c.w, c.b};
         seg_reduce<1, true>(c.R, t, e, gc);
     }
     gc.sync();
@@ -159,27 +131,13 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
         seg_rescale(c.C, f2);
     }
     gc.sync();
-    // d = A~^dagger b~ + (mu/2)(abs_{A~}(c^) - c^) = A~'w_d - mu c^  with (A~A~') w_d = b~ + mu A~ c^
-    // The solve is warm-started from the previous w_d carried over in true (unscaled) coordinates.
-    {
-        TermDot tg{c.w};
-        EpiWarmE ee{c.e, c.chat, c.mu};
-        seg_reduce<1, false>(c.C, tg, ee, gc);
-    }
-    gc.sync();
-    TermTwo tq{c.chat, c.e};
-    EpiRhsD eq{c.r, c.btil, c.mu, 0.0, 0.0};
-    seg_reduce<2, false>(c.R, tq, eq, gc);
-    double red[2] = {eq.qq, eq.rho};
-    grid_reduce<2>(red, gc);
-    bool hm;
-    const int steps = cg_solve(c, gc, red[1], red[0], hm);
-    for (int i = tid; i < c.m; i += nth) c.wd[i] = c.w[i];           // own elements only; w is gathered below
-    TermTwo tw{c.w, c.wsave};
-    EpiD ed{c.d, c.s, c.g, c.chat, c.xb, c.zb, c.O, c.mu};
-    seg_reduce<2, false>(c.C, tw, ed, gc);
-    gc.sync();
-    for (int i = tid; i < c.m; i += nth) c.w[i] = c.wsave[i];        // the iterate's multiplier, rescaled
+    // Step 13's d is never formed: it is folded into the pass (cs_kernels.cuh), so a conditioning needs no
+    // solve.  What remains is the recast of s (step 14) and g = A~'w in the new scaling.
+    TermDot tw{c.w};
+    EpiRecast er{c.s, c.g, c.xb, c.zb, c.O, c.mu};
+    seg_reduce<1, false>(c.C, tw, er, gc);
+    const int steps = 0;
+    const bool hm = false;
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         c.sc->n_cond += 1;
         c.sc->cg_steps_total += steps;
@@ -197,19 +155,19 @@ struct TermCsrX {     // A~ x^ with x^ = x/O
     __device__ __forceinline__ void fma(double a, G g, double (&acc)[1]) const { acc[0] += a * g; }
 };
 struct EpiPres {      // (Ax-b)_i = (A~x^ - b~)_i / D_i ; b'y = b~'y'
-    const double *btil, *D, *wd, *w; double mu; double pres2, by;
+    const double *btil, *D, *w; double mu; double pres2, by;
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
         const double e = (a[0] - btil[i]) / D[i];
         pres2 += e * e;
-        by += btil[i] * (wd[i] - w[i]) / mu;
+        by += btil[i] * w[i] / mu;
     }
 };
 struct TermCscY {     // A~' y'
-    const double *wd, *w; double mu;
+    const double *w; double mu;
     typedef double G;
-    __device__ __forceinline__ G fetch(int i) const { return (wd[i] - w[i]) / mu; }
+    __device__ __forceinline__ G fetch(int i) const { return w[i] / mu; }
     __device__ __forceinline__ void fma(double a, G g, double (&acc)[1]) const { acc[0] += a * g; }
 };
 struct EpiDres {      // (c - z - A'y)_j = c_j - z_j - (A~'y')_j / O_j
@@ -238,9 +196,9 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_residuals(Ctx c) {
     GridCtl gc(c.partials, smem, c.bar);
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     TermCsrX t1{c.xb, c.O};
-    EpiPres e1{c.btil, c.D, c.wd, c.w, c.mu, 0.0, 0.0};
+    EpiPres e1{c.btil, c.D, c.w, c.mu, 0.0, 0.0};
     seg_reduce<1, false>(c.R, t1, e1, gc);
-    TermCscY t2{c.wd, c.w, c.mu};
+    TermCscY t2{c.w, c.mu};
     EpiDres e2{c.c, c.xb, c.zb, c.O, 0.0, 0.0, 0.0, 0.0};
     seg_reduce<1, false>(c.C, t2, e2, gc);
     double vx = 0.0, vz = 0.0;

@@ -235,3 +235,37 @@ def test_diagnostic_probes():
     assert 0 < us_s < us_g < 5e4
     S = binding.Solver.from_problem(W.config(1, 0.05), device="cuda:0")
     assert 0.2 < S.barrier_probe(200) < 200.0
+
+
+def test_empty_columns_and_one_huge_cone():
+    """Degenerate structure: columns that appear in no constraint (empty column segments) and a single
+    Lorentz block far larger than the lanes that cooperate on it."""
+    import scipy.sparse as sp
+    import oracle
+    from paper_2103_00736_b200 import binding
+    rng = np.random.default_rng(3)
+    m, n_lin, big = 60, 90, 5000
+    n = n_lin + big + 7
+    A = sp.random(m, n, density=0.02, random_state=5, data_rvs=rng.standard_normal, format="lil")
+    for i in range(m):                       # no empty rows
+        A[i, rng.integers(0, n)] = rng.standard_normal()
+    A[:, [3, 17, n_lin + 11, n - 1]] = 0.0   # empty columns in the orthant part, inside the big cone, at the end
+    A = sp.csr_matrix(A)
+    A.eliminate_zeros()
+    A.sort_indices()
+    assert (np.diff(A.indptr) > 0).all() and (np.diff(A.tocsc().indptr) == 0).sum() >= 4
+    soc = np.array([big, 7], np.int32)
+    xf = rng.random(n)
+    xf[n_lin] = np.linalg.norm(xf[n_lin + 1:n_lin + big]) + 1.0
+    xf[n_lin + big] = np.linalg.norm(xf[n_lin + big + 1:]) + 1.0
+    p = W.Problem(name="degenerate", m=m, n=n, row_ptr=A.indptr.astype(np.int32), col_idx=A.indices.astype(np.int32),
+                  val=A.data.copy(), b=A @ xf, c=rng.random(n), n_lin=n_lin, soc_size=soc,
+                  x0=np.full(n, np.nan), y0=np.full(m, np.nan), s0=np.full(n, np.nan), t=1.7)
+    S, O = binding.Solver.from_problem(p, device="cuda:0"), oracle.Oracle.from_problem(p)
+    S.run(30, L=[10])
+    O.run(30, L=[10])
+    _check_iterates(S, O, keys=("x", "z", "y", "s", "O"), tol=1e-6)
+    S2, O2 = binding.Solver.from_problem(p), oracle.Oracle.from_problem(p)
+    S2.run(25)
+    O2.run(25)
+    _check_iterates(S2, O2)
