@@ -145,7 +145,7 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, d
 // ---------------------------------------------------------------------------------------------
 // k_iterate
 // ---------------------------------------------------------------------------------------------
-struct TermCsrPE {  // (A~ u, A~ e)
+struct TermPair {   // (sum a x[j], sum a y[j]): both gathers of the rhs pass
     const double *p, *e;
     typedef double2 G;
     __device__ __forceinline__ G fetch(int j) const { return make_double2(p[j], e[j]); }
@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_
         phase_cone_reflect(c);                                   // step 16
         gc.sync();
         gc.lap(kPhCone);
-        TermCsrPE tq{c.u, c.e};
+        TermPair tq{c.u, c.e};
         EpiRhs eq{c.r, c.btil, 0.0, 0.0};
         seg_reduce<2, false>(c.R, tq, eq, gc);
         gc.lap(kPhRhs);
