@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -91,40 +92,51 @@ struct HostSparse {
     int n_chunk = 0, n_slots = 0;
 };
 
+// Run f(block) for block = 0..n_blocks-1 on up to `nt` host threads (blocks are handed out dynamically).
+template <class F>
+void parallel_blocks(int n_blocks, int nt, F f) {
+    nt = std::max(1, std::min(nt, n_blocks));
+    if (nt == 1) { for (int b = 0; b < n_blocks; ++b) f(b); return; }
+    std::atomic<int> next{0};
+    std::vector<std::thread> th;
+    for (int t = 0; t < nt; ++t)
+        th.emplace_back([&] { for (int b = next.fetch_add(1); b < n_blocks; b = next.fetch_add(1)) f(b); });
+    for (auto &t : th) t.join();
+}
+
+int host_threads() { return (int)std::max(1u, std::min(16u, std::thread::hardware_concurrency())); }
+
 // ptr/idx/val: compressed segments in INTERNAL numbering (segment s = entries [ptr[s], ptr[s+1])).
-HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx, const std::vector<double> &val) {
+// Two phases: a serial plan (slice descriptors and offsets, O(#segments)), then a parallel fill.
+HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx, const std::vector<double> &val, int nt) {
     HostSparse h;
     const int nseg = (int)ptr.size() - 1;
     // several lanes per segment only pay when there are too few segments to fill the machine (measured:
     // T>1 is slower once every warp has >= 2 thread-per-segment slices)
     const bool split = nseg < 300000;
     auto lg_lanes = [split](int len) { return (!split || len <= 8) ? 0 : len <= 16 ? 1 : len <= 32 ? 2 : 3; };  // T = 1,2,4,8 lanes
-    auto new_slice = [&](int seg0, int meta, int width) {
-        const int off = (int)h.val.size();
-        h.slices.push_back(make_int4(off, seg0, meta, width));
-        h.val.resize((size_t)off + 32u * width, 0.0);
-        h.idx.resize((size_t)off + 32u * width, 0);
-        return off;
+    size_t total = 0;
+    std::vector<int> chunk_src;       // first source entry of every chunk slice
+    auto plan_slice = [&](int seg0, int meta, int width) {
+        h.slices.push_back(make_int4((int)total, seg0, meta, width));
+        total += 32u * (size_t)width;
     };
-    // pass 1: chunks of the long segments (T = 32: entry e of the chunk at lane e%32, row e/32)
+    // plan 1: chunks of the long segments (T = 32: entry e of the chunk at lane e%32, row e/32)
     for (int s = 0; s < nseg; ++s) {
         const int len = ptr[s + 1] - ptr[s];
         if (len <= kShortMax) continue;
         const int nch = (len + kChunk - 1) / kChunk;
         if (nch > 1) h.multi.push_back(make_int4(s, h.n_slots, nch, 0));
         for (int q = 0; q < nch; ++q) {
-            const int a = ptr[s] + q * kChunk, clen = std::min(kChunk, ptr[s + 1] - a), width = (clen + 31) / 32;
-            const int off = new_slice(s, 1 | (5 << 8), width);
-            for (int e = 0; e < 32 * width; ++e) {
-                h.idx[(size_t)off + e] = idx[a + std::min(e, clen - 1)];
-                if (e < clen) h.val[(size_t)off + e] = val[a + e];
-            }
+            const int a = ptr[s] + q * kChunk, clen = std::min(kChunk, ptr[s + 1] - a);
+            plan_slice(s, 1 | (5 << 8), (clen + 31) / 32);
+            chunk_src.push_back(a);
             h.chunk_slot.push_back(nch > 1 ? h.n_slots++ : -1);
         }
     }
     h.n_chunk = (int)h.slices.size();
-    // pass 2: runs of consecutive short segments -> slices of 32 lanes, T lanes per segment
-    auto flush_run = [&](int a, int b) {
+    // plan 2: runs of consecutive short segments -> slices of 32 lanes, T lanes per segment
+    auto plan_run = [&](int a, int b) {
         int s0 = a;
         while (s0 < b) {
             const int lgT = lg_lanes(ptr[s0 + 1] - ptr[s0]), T = 1 << lgT, cap = 32 / T;
@@ -133,27 +145,46 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 maxlen = std::max(maxlen, ptr[s0 + cnt + 1] - ptr[s0 + cnt]);
                 ++cnt;
             }
-            const int width = (maxlen + T - 1) / T;
-            const int off = new_slice(s0, cnt | (lgT << 8), width);
-            for (int lane = 0; lane < 32; ++lane) {
-                const int seg = s0 + std::min(lane / T, cnt - 1);   // padding lanes replicate a valid index
-                const int len = ptr[seg + 1] - ptr[seg], t = lane % T;
-                for (int k = 0; k < width; ++k) {
-                    const int e = k * T + t;
-                    h.idx[(size_t)off + 32u * k + lane] = len > 0 ? idx[ptr[seg] + std::min(e, len - 1)] : 0;  // empty segment: any valid index
-                    if (lane / T < cnt && e < len) h.val[(size_t)off + 32u * k + lane] = val[ptr[seg] + e];
-                }
-            }
+            plan_slice(s0, cnt | (lgT << 8), (maxlen + T - 1) / T);
             s0 += cnt;
         }
     };
     int run = 0;
     for (int s = 0; s < nseg; ++s) {
         if (ptr[s + 1] - ptr[s] <= kShortMax) continue;
-        flush_run(run, s);
+        plan_run(run, s);
         run = s + 1;
     }
-    flush_run(run, nseg);
+    plan_run(run, nseg);
+    // fill (padding: val = 0, a valid index replicated)
+    h.val.assign(total, 0.0);
+    h.idx.assign(total, 0);
+    const int n_slice = (int)h.slices.size(), blk = 512;
+    parallel_blocks((n_slice + blk - 1) / blk, nt, [&](int bi) {
+        for (int si = bi * blk; si < std::min(n_slice, (bi + 1) * blk); ++si) {
+            const int4 sl = h.slices[si];
+            const size_t off = (size_t)sl.x;
+            const int width = sl.w;
+            if (si < h.n_chunk) {
+                const int a = chunk_src[si], clen = std::min(kChunk, ptr[sl.y + 1] - a);
+                for (int e = 0; e < 32 * width; ++e) {
+                    h.idx[off + e] = idx[a + std::min(e, clen - 1)];
+                    if (e < clen) h.val[off + e] = val[a + e];
+                }
+                continue;
+            }
+            const int cnt = sl.z & 255, T = 1 << (sl.z >> 8), s0 = sl.y;
+            for (int lane = 0; lane < 32; ++lane) {
+                const int seg = s0 + std::min(lane / T, cnt - 1);   // padding lanes replicate a valid index
+                const int len = ptr[seg + 1] - ptr[seg], t = lane % T;
+                for (int k = 0; k < width; ++k) {
+                    const int e = k * T + t;
+                    h.idx[off + 32u * k + lane] = len > 0 ? idx[ptr[seg] + std::min(e, len - 1)] : 0;  // empty segment: any valid index
+                    if (lane / T < cnt && e < len) h.val[off + 32u * k + lane] = val[ptr[seg] + e];
+                }
+            }
+        }
+    });
     return h;
 }
 
@@ -165,7 +196,8 @@ cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     if ((st = dev_upload(S, &pi, h.chunk_slot.data(), h.chunk_slot.size())) != CS_OK) return st; out->chunk_slot = pi;
     if ((st = dev_upload(S, &pi, h.idx.data(), h.idx.size())) != CS_OK) return st; out->idx = pi;
     if ((st = dev_upload(S, &pd, h.val.data(), h.val.size())) != CS_OK) return st; out->val0 = pd;
-    if ((st = dev_upload(S, &out->val, h.val.data(), h.val.size())) != CS_OK) return st;
+    if ((st = dev_alloc(S, &out->val, h.val.size())) != CS_OK) return st;      // scaled copy starts as the pristine one
+    if (!h.val.empty()) CS_CUDA(S, cudaMemcpyAsync(out->val, pd, h.val.size() * sizeof(double), cudaMemcpyDeviceToDevice, S->stream));
     out->n_slice = (int)h.slices.size();
     out->n_chunk = h.n_chunk;
     out->n_multi = (int)h.multi.size();
@@ -307,13 +339,19 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     for (int i = 0; i < m; ++i) {
         if (rptr[i + 1] <= rptr[i]) { S->err = "row_ptr not increasing (empty rows are not allowed)"; return CS_EINVAL; }
         if (rptr[i + 1] > nnz) { S->err = "row_ptr out of range"; return CS_EINVAL; }
-        for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
-            if (cidx[k] < 0 || cidx[k] >= n || (k > rptr[i] && cidx[k] <= cidx[k - 1])) {
-                S->err = "col_idx out of range, unsorted or duplicated within a row";
-                return CS_EINVAL;
-            }
-            if (!std::isfinite(val[k])) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
-        }
+    }
+    {
+        std::atomic<int> bad{0};
+        const int blk = 16384;
+        parallel_blocks((m + blk - 1) / blk, host_threads(), [&](int bi) {
+            for (int i = bi * blk; i < std::min(m, (bi + 1) * blk); ++i)
+                for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
+                    if (cidx[k] < 0 || cidx[k] >= n || (k > rptr[i] && cidx[k] <= cidx[k - 1])) bad.store(1);
+                    else if (!std::isfinite(val[k])) bad.store(2);
+                }
+        });
+        if (bad.load() == 1) { S->err = "col_idx out of range, unsorted or duplicated within a row"; return CS_EINVAL; }
+        if (bad.load() == 2) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
     }
     double nb = 0.0, nc = 0.0;
     for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
@@ -350,30 +388,46 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
                 for (int k = 0; k < len; ++k) { ci2[dst + k] = tmp[k].first; va2[dst + k] = tmp[k].second; }
             }
         };
-        const int nt = (int)std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
-        std::vector<std::thread> th;
-        // rows are sorted by decreasing length: deal them out round-robin in blocks so the long ones spread
-        std::vector<std::vector<std::pair<int, int>>> work(nt);
-        const int blk = 4096;
-        for (int i0 = 0, q = 0; i0 < m; i0 += blk, ++q) work[q % nt].push_back({i0, std::min(m, i0 + blk)});
-        for (int t = 0; t < nt; ++t) th.emplace_back([&, t] { for (auto &w : work[t]) fill_rows(w.first, w.second); });
-        for (auto &t : th) t.join();
+        // blocks of rows with at most ~256k entries (the heavy rows come first and get blocks of their own)
+        std::vector<int> cut{0};
+        for (int i = 0, acc = 0; i < m; ++i) {
+            acc += rlen[perm_r[i]];
+            if (acc >= (1 << 18) || i + 1 == m) { cut.push_back(i + 1); acc = 0; }
+        }
+        parallel_blocks((int)cut.size() - 1, host_threads(), [&](int bi) { fill_rows(cut[bi], cut[bi + 1]); });
     }
     lap("row-major copy");
-    // column-major copy (counting sort by internal column; rows come out sorted within a column)
-    std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
-    std::vector<double> cv2((size_t)nnz);
-    for (int k = 0; k < nnz; ++k) cp2[(size_t)ci2[k] + 1]++;
-    for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] += cp2[j];
+    // column-major copy (counting sort by internal column; rows come out sorted within a column) and its
+    // slices on a second thread, while this thread builds the slices of the row-major copy
+    HostSparse hr, hc2;
     {
-        std::vector<int> fill(cp2.begin(), cp2.end() - 1);
-        for (int i = 0; i < m; ++i)
-            for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
-                const int q = fill[ci2[k]]++;
-                ri2[q] = i;
-                cv2[q] = va2[k];
-            }
+        const int nt = host_threads();
+        std::thread tc([&] {
+            std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
+            std::vector<double> cv2((size_t)nnz);
+            for (int k = 0; k < nnz; ++k) cp2[(size_t)ci2[k] + 1]++;
+            for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] += cp2[j];
+            std::vector<int> fill(cp2.begin(), cp2.end() - 1);
+            // every helper scans all entries in row order but places only those of its own column range:
+            // sequential reads, writes confined to the range, order within a column = row order (deterministic)
+            const int parts = std::max(1, nt / 2);
+            parallel_blocks(parts, parts, [&](int part) {
+                const int j0 = (int)((long long)n * part / parts), j1 = (int)((long long)n * (part + 1) / parts);
+                for (int i = 0; i < m; ++i)
+                    for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
+                        const int j = ci2[k];
+                        if (j < j0 || j >= j1) continue;
+                        const int q = fill[j]++;
+                        ri2[q] = i;
+                        cv2[q] = va2[k];
+                    }
+            });
+            hc2 = make_sparse(cp2, ri2, cv2, std::max(1, nt / 2));
+        });
+        hr = make_sparse(rp2, ci2, va2, std::max(1, nt / 2));
+        tc.join();
     }
+    lap("column-major copy + slices");
     {   // b, c in internal order
         std::vector<double> t((size_t)std::max(m, n));
         for (int i = 0; i < m; ++i) t[i] = hb[perm_r[i]];
@@ -381,7 +435,6 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         for (int j = 0; j < n; ++j) t[j] = hc[perm_c[j]];
         std::copy(t.begin(), t.begin() + n, hc.begin());
     }
-    lap("column-major copy");
     // ---- device state
     Ctx &x = S->ctx;
     x.m = m; x.n = n; x.n_lin = (int)K->n_lin; x.n_soc = (int)K->n_soc;
@@ -390,17 +443,10 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_upload(S, &ip, cone_off.data(), cone_off.size())) != CS_OK) return st; x.cone_off = ip;
     if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
     if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
-    {
-        HostSparse hr, hc2;
-        std::thread tr([&] { hr = make_sparse(rp2, ci2, va2); });
-        hc2 = make_sparse(cp2, ri2, cv2);
-        tr.join();
-        lap("slices (rows | columns)");
-        if ((st = upload_sparse(S, hr, &x.R)) != CS_OK) return st;
-        if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;
-        CS_CUDA(S, cudaStreamSynchronize(S->stream));
-        lap("upload");
-    }
+    if ((st = upload_sparse(S, hr, &x.R)) != CS_OK) return st;
+    if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    lap("upload");
     if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
     if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
     double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.chat};
