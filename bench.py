@@ -145,14 +145,15 @@ def solve_to_tolerance(a, p, S, torch):
         if r["kkt_rel"] <= a.tol:
             break
     dt = time.perf_counter() - t0
-    print(json.dumps({"mode": "solve", "workload": p.name, "tol": a.tol, "reached": bool(r["kkt_rel"] <= a.tol),
-                      "time_to_tol_s": dt, "iterations": l, "cg_steps_total": r["cg_steps_total"],
-                      "n_conditionings": r["n_conditionings"], "kkt_rel": r["kkt_rel"], "pobj": r["pobj"],
-                      "opt_value": p.opt_value(), "iters_per_s": l / dt,
-                      "schedule": f"L={{{p.L_first},{p.L_first + p.L_every},...}}, t={p.t}, mu={p.mu}",
-                      "history": [(i, float(f"{k:.3e}"), round(t, 3), c) for i, k, t, c in hist[-12:]]}))
+    out = {"mode": "solve", "workload": p.name, "tol": a.tol, "reached": bool(r["kkt_rel"] <= a.tol),
+           "time_to_tol_s": dt, "iterations": l, "cg_steps_total": r["cg_steps_total"],
+           "n_conditionings": r["n_conditionings"], "kkt_rel": r["kkt_rel"], "pobj": r["pobj"],
+           "cg_tol": S.get_params()["cg_tol"],
+           "opt_value": p.opt_value(), "iters_per_s": l / dt,
+           "schedule": f"L={{{p.L_first},{p.L_first + p.L_every},...}}, t={p.t}, mu={p.mu}",
+           "history": [(i, float(f"{k:.3e}"), round(t, 3), c) for i, k, t, c in hist[-12:]]}
     S.destroy()
-    return 0
+    return out
 
 
 def main():
@@ -170,6 +171,7 @@ def main():
     ap.add_argument("--solve", action="store_true",
                     help="extra mode: run the paper's schedule (17)/(18) to --tol and report the time to tolerance")
     ap.add_argument("--tol", type=float, default=1e-4)
+    ap.add_argument("--cg-tol", type=float, default=0.0, help="--solve only: inner CG tolerance (0 = library default 1e-15)")
     ap.add_argument("--check-every", type=int, default=25)
     ap.add_argument("--max-iter", type=int, default=3000)
     ap.add_argument("--cg-max-iter", type=int, default=0, help="profiling only: cap CG steps per solve (0 = library default)")
@@ -209,7 +211,10 @@ def main():
         S.set_params(cg_max_iter=a.cg_max_iter)
 
     if a.solve:
-        return solve_to_tolerance(a, p, S, torch)
+        if a.cg_tol > 0:
+            S.set_params(cg_tol=a.cg_tol)
+        print(json.dumps(solve_to_tolerance(a, p, S, torch)))
+        return 0
 
     def step():
         S.condition()
@@ -349,6 +354,20 @@ def finish(a, p, S, line, rank, world, dev, stream):
             line["secondary"] = {"cfg3_socp": secondary_workload(3, a, dev, stream, line["roofline"]["peak"])}
         except Exception as e:  # pragma: no cover
             line["secondary"] = {"error": str(e)}
+        # B's third metric, "time to 1e-4 relative KKT residual", on the headline workload with the paper's
+        # schedule (17).  With the parity setting cg_tol = 1e-15 the conditioned solves take 1e4 CG steps per pass
+        # (DESIGN.md 9), so this leg uses inexact projections, cg_tol = 1e-7 (a cs_set_params parameter; measured:
+        # 1e-6 stalls at kkt 1.3e-4, 1e-7 reaches 1e-4 in 51 s / 900 passes, 1e-8 in 128 s / 800 passes).
+        try:
+            import argparse as _ap
+            a2 = _ap.Namespace(**{**vars(a), "tol": 1e-4, "check_every": 50, "max_iter": 2000})
+            S3 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
+            S3.set_params(cg_tol=1e-7)
+            t2t = solve_to_tolerance(a2, p, S3, torch)
+            t2t.pop("history", None)
+            line["time_to_kkt_1e-4"] = t2t
+        except Exception as e:  # pragma: no cover
+            line["time_to_kkt_1e-4"] = {"error": str(e)}
 
     # ---- e2e: host buffers in, host buffers out, everything inside the timed region
     pin = lambda x: torch.from_numpy(np.ascontiguousarray(x)).pin_memory()

@@ -125,6 +125,25 @@ def test_cfg2_replica_illconditioned():
         assert rel(got[k], ref[k]) <= 1e-8, (k, rel(got[k], ref[k]))
 
 
+def test_inexact_projections_reach_the_same_optimum():
+    """cg_tol is a parameter: with 1e-8 the passes are inexact (no iterate parity is claimed) but the fixed
+    point is the same -- objective, unique dual solution and KKT residual at the end of the paper's
+    schedule agree with the oracle at convergence accuracy."""
+    p = W.config(1, 0.02)
+    S, O = _pair(p)
+    S.set_params(cg_tol=1e-8)
+    L = p.schedule(800)
+    S.run(800, L=L)
+    O.run(800, L=L)
+    r, q = S.residuals(), O.residuals()
+    assert r["kkt_rel"] <= 1e-4 and q["kkt_rel"] <= 1e-5
+    assert abs(r["pobj"] - q["pobj"]) <= 1e-4 * (1 + abs(q["pobj"]))
+    assert abs(r["pobj"] - p.opt_value()) <= 1e-4 * (1 + abs(p.opt_value()))
+    got = S.solution()
+    assert rel(got["z"], p.s0) <= 1e-3 and rel(got["y"], p.y0) <= 1e-3
+    assert r["cg_steps_total"] > 0
+
+
 def test_production_schedule_objective_and_kkt():
     """Protocol (iii): the paper's schedule L={300,400,...} (eq.(17)); objective and KKT terms to 1e-6."""
     p = W.config(1, 0.02)
