@@ -316,3 +316,26 @@ def test_cfg2_adaptive_versus_fixed_scaling_run():
         assert 0.3 < r["kkt_rel"] / q["kkt_rel"] < 3.0, (name, r["kkt_rel"], q["kkt_rel"])
         kkt[name] = (r["kkt_rel"], q["kkt_rel"])
     assert kkt["adaptive"][0] < kkt["fixed"][0] and kkt["adaptive"][1] < kkt["fixed"][1]
+
+
+@pytest.mark.parametrize("mu,t", [(0.5, 3.0), (4.0, 1.0)])
+def test_parameters_mu_and_t(mu, t):
+    """mu and t other than the paper's experiment values, with a conditioning from
+    identical inputs (protocol ii-a) so that the comparison stays at 1e-9."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = W.sparse_socp(91, 400, 1000, 30, 6, n_lin=250, lo=2, hi=60)
+    p.mu, p.t = mu, t
+    O0 = oracle.Oracle.from_problem(p)
+    O0.run(15)
+    start = O0.get()
+    S, O = binding.Solver.from_problem(p, device="cuda:0"), oracle.Oracle.from_problem(p)
+    assert S.get_params()["mu"] == mu and S.get_params()["t"] == t
+    S.set_point(start["x"], start["z"])
+    O.set_point(start["x"], start["z"])
+    S.iterate(25)      # implicit l=1 conditioning from the point
+    O.run(25)
+    got, ref = _check_iterates(S, O)
+    assert rel(got["O"], ref["O"]) <= 1e-12
+    assert np.log(got["O"].max() / got["O"].min()) <= t * (1 + 1e-12)
+    _check_resid(S, O)
