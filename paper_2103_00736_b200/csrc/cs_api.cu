@@ -477,6 +477,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     }
     if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
     S->grid = std::min(sms * occ_min, kMaxGrid);
+    if (nnz <= 8192) S->grid = 1;   // tiny problem (config 0): one CTA, barriers are __syncthreads (cs_device.cuh)
     if ((st = dev_zeros(S, &x.bar, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * kMaxGrid)) != CS_OK) return st;
     // ---- defaults (cs.h)

@@ -14,7 +14,7 @@ namespace csd {
 constexpr int kBlock = 512;          // threads per CTA (16 warps)
 constexpr int kWarps = kBlock / 32;
 constexpr int kMaxRed = 8;           // scalars per grid reduction
-constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (sub-warp groups)
+constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
 constexpr int kChunk = 1024;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
 constexpr int kRoundK = 8;           // slice rows loaded per batch (8 values + 8 indices + 8 gathers in flight per lane)
@@ -111,6 +111,7 @@ struct GridCtl {            // per-thread view of the grid barrier state (unifor
     }
     __device__ void sync() {
         __syncthreads();
+        if (gridDim.x == 1) return;                            // tiny problems run on one CTA: no global traffic
         if (threadIdx.x == 0) {
             const unsigned int inc = blockIdx.x == 0 ? 0x80000000u - (gridDim.x - 1) : 1u;
             __threadfence();                                   // release the CTA's writes
