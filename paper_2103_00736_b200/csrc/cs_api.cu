@@ -428,6 +428,10 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         tc.join();
     }
     lap("column-major copy + slices");
+    if (hr.val.size() >= (size_t)INT32_MAX || hc2.val.size() >= (size_t)INT32_MAX) {
+        S->err = "padded slice storage exceeds 2^31 entries";
+        return CS_EINVAL;
+    }
     {   // b, c in internal order
         std::vector<double> t((size_t)std::max(m, n));
         for (int i = 0; i < m; ++i) t[i] = hb[perm_r[i]];
