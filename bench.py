@@ -33,11 +33,13 @@ METRIC = "outer_iterations_per_s"
 UNIT = "iterations/s"
 
 
-def algorithmic_bytes(p, k_iter, cg_steps, n_cond):
+def algorithmic_bytes(p, k_iter, cg_steps, n_cond, fsai=False):
     """Bytes the method must move: int32 indices, fp64 values, each
     gathered vector counted once per pass."""
     nnz, n, m = p.nnz, p.n, p.m
-    cg = 24 * nnz + 28 * n + 60 * m          # K1 (CSC pass) + K2 (CSR pass) of one CG step
+    cg = 24 * nnz + 28 * n + 60 * m          # K1 (column pass) + K2 (row pass) of one CG step
+    if fsai:
+        cg += 96 * m                         # z = G'G r: two m-vector passes (DESIGN.md 8) + z read in K2
     outer = 24 * nnz + 92 * n + 24 * m       # cone reflect + rhs pass + final A'w pass with the s-update
     cond = 64 * nnz + 80 * n + 40 * m        # row norms, rescale of both copies, d/s recast (solve counted in cg)
     return cg * cg_steps + outer * k_iter + cond * n_cond, cg
@@ -174,6 +176,7 @@ def main():
     ap.add_argument("--cg-tol", type=float, default=0.0, help="--solve only: inner CG tolerance (0 = library default 1e-15)")
     ap.add_argument("--check-every", type=int, default=25)
     ap.add_argument("--max-iter", type=int, default=3000)
+    ap.add_argument("--precond", type=int, default=0, help="cs_params.precond: 0 auto, 1 none (Jacobi equilibration only), 2 FSAI(1)")
     ap.add_argument("--cg-max-iter", type=int, default=0, help="profiling only: cap CG steps per solve (0 = library default)")
     a = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -209,6 +212,8 @@ def main():
     S = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     if a.cg_max_iter:
         S.set_params(cg_max_iter=a.cg_max_iter)
+    if a.precond:
+        S.set_params(precond=a.precond)
 
     if a.solve:
         if a.cg_tol > 0:
@@ -258,7 +263,8 @@ def main():
     # from the device counters (total minus those spent inside cs_condition).
     cg_steps = r1["cg_steps_total"] - r0["cg_steps_total"]
     cg_iter = cg_steps - (r1["cg_steps_cond"] - r0["cg_steps_cond"])
-    it_bytes, cg_bytes = algorithmic_bytes(p, n_it, cg_iter, 0)
+    fsai_on = S.get_params()["precond"] == 2 or (S.get_params()["precond"] == 0 and p.t >= 4.0)
+    it_bytes, cg_bytes = algorithmic_bytes(p, n_it, cg_iter, 0, fsai_on)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -300,7 +306,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": p.name, "cg_max_iter_cap": a.cg_max_iter or None, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "k_per_step": a.k,
+            "config": {"workload": p.name, "cg_max_iter_cap": a.cg_max_iter or None, "precond": S.get_params()["precond"], "fsai": fsai_on, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "k_per_step": a.k,
                        "step": "cs_condition + cs_iterate(k) + cs_residuals", "multi_gpu": "replicas only",
                        "l2": "inputs larger than L2" if 24 * p.nnz > 126e6 else "matrix fits in L2 (flagged)",
                        "gen_s": round(t_gen, 2)},
@@ -332,7 +338,7 @@ def secondary_workload(cfg, a, dev, stream, peak):
         ms_iter += e0.elapsed_time(e1)
     dt = time.perf_counter() - t0
     cg_iter = (r1["cg_steps_total"] - r0["cg_steps_total"]) - (r1["cg_steps_cond"] - r0["cg_steps_cond"])
-    it_bytes, cg_bytes = algorithmic_bytes(p, steps * a.k, cg_iter, 0)
+    it_bytes, cg_bytes = algorithmic_bytes(p, steps * a.k, cg_iter, 0, p.t >= 4.0)
     achieved = it_bytes / (ms_iter * 1e-3) / 1e9
     us_g, _ = binding.gather_probe(p.n, p.nnz)
     out = {"workload": p.name, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "value": steps * a.k / dt, "unit": UNIT,
@@ -382,7 +388,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
     def e2e_step():
         S2 = binding.Solver(p.m, p.n, hin[0].numpy(), hin[1].numpy(), hin[2].numpy(), hin[3].numpy(), hin[4].numpy(),
                             p.n_lin, p.soc_size, stream=stream.cuda_stream)
-        S2.set_params(mu=p.mu, t=p.t, **({"cg_max_iter": a.cg_max_iter} if a.cg_max_iter else {}))
+        S2.set_params(mu=p.mu, t=p.t, precond=a.precond, **({"cg_max_iter": a.cg_max_iter} if a.cg_max_iter else {}))
         S2.set_point(hx0.numpy(), hz0.numpy())
         S2.condition()
         S2.iterate(a.k)

@@ -69,12 +69,16 @@ typedef struct {
  *   cg_tol   inner solve stops when ||residual||_2 <= cg_tol * ||rhs||_2, both measured on the
  *            row-equilibrated system (D A_hat)(D A_hat)' with D = diag(1/||row_i(A_hat)||_2)
  *   cg_max_iter  cap on CG steps per solve
- * cs_set_params may be called at any time; mu, t, o_floor take effect at the next cs_condition
+ *   precond  preconditioner of the inner CG beyond the Jacobi row equilibration: 0 = automatic (FSAI(1) when
+ *            t >= 4, i.e. when a conditioning may spread O^2 over many decades), 1 = none, 2 = FSAI(1): a sparse
+ *            approximate inverse factor with one off-diagonal entry per row, rebuilt on the device at every
+ *            conditioning.  Changes the number of CG steps, not the solution of the solve.
+ * cs_set_params may be called at any time; mu, t, o_floor, precond take effect at the next cs_condition
  * (or at the implicit first conditioning), cg_* at the next solve. */
 typedef struct {
     double mu, t, o_floor, cg_tol;
     int32_t cg_max_iter;
-    int32_t reserved;
+    int32_t precond;
 } cs_params;
 
 /* Residuals of the KKT conditions (24) P:480-487 in ORIGINAL coordinates, for the current iterate

@@ -30,7 +30,7 @@ class cs_cones(C.Structure):
 
 class cs_params(C.Structure):
     _fields_ = [("mu", C.c_double), ("t", C.c_double), ("o_floor", C.c_double), ("cg_tol", C.c_double),
-                ("cg_max_iter", C.c_int32), ("reserved", C.c_int32)]
+                ("cg_max_iter", C.c_int32), ("precond", C.c_int32)]
 
 
 class cs_resid(C.Structure):
@@ -170,12 +170,15 @@ class Solver:
     def get_params(self):
         p = cs_params()
         self._check(lib().cs_get_params(self._h, C.byref(p)))
-        return {k: getattr(p, k) for k, _ in p._fields_ if k != "reserved"}
+        return {k: getattr(p, k) for k, _ in p._fields_}
 
     def set_params(self, **kw):
         cur = self.get_params()
+        unknown = set(kw) - set(cur)
+        if unknown:
+            raise TypeError(f"unknown parameter(s): {sorted(unknown)}")
         cur.update(kw)
-        p = cs_params(cur["mu"], cur["t"], cur["o_floor"], cur["cg_tol"], int(cur["cg_max_iter"]), 0)
+        p = cs_params(cur["mu"], cur["t"], cur["o_floor"], cur["cg_tol"], int(cur["cg_max_iter"]), int(cur["precond"]))
         self._check(lib().cs_set_params(self._h, C.byref(p)))
 
     def set_point(self, x, z):

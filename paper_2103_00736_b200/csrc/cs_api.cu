@@ -25,6 +25,7 @@ struct cs_solver {
     cudaStream_t stream = nullptr;
     int device = 0;
     int grid = 0;
+    int64_t nnz = 0;
     size_t dyn_smem = 0;       // bytes of dynamic shared memory of the cooperative kernels (cp.async staging)
     std::vector<void *> allocs;
     cs_params prm{};
@@ -88,6 +89,7 @@ cs_status fetch(cs_solver *S, std::vector<T> &dst, const T *src, size_t count, c
 struct HostSparse {
     std::vector<int4> slices, multi;
     std::vector<int> chunk_slot, idx;
+    std::vector<int> pos;         // compressed entry -> position in val/idx (for the plain compressed view, Csr in cs_device.cuh)
     std::vector<double> val;
     int n_chunk = 0, n_slots = 0;
 };
@@ -159,6 +161,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
     // fill (padding: val = 0, a valid index replicated)
     h.val.assign(total, 0.0);
     h.idx.assign(total, 0);
+    h.pos.assign(idx.size(), 0);
     const int n_slice = (int)h.slices.size(), blk = 512;
     parallel_blocks((n_slice + blk - 1) / blk, nt, [&](int bi) {
         for (int si = bi * blk; si < std::min(n_slice, (bi + 1) * blk); ++si) {
@@ -169,7 +172,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 const int a = chunk_src[si], clen = std::min(kChunk, ptr[sl.y + 1] - a);
                 for (int e = 0; e < 32 * width; ++e) {
                     h.idx[off + e] = idx[a + std::min(e, clen - 1)];
-                    if (e < clen) h.val[off + e] = val[a + e];
+                    if (e < clen) { h.val[off + e] = val[a + e]; h.pos[a + e] = (int)(off + e); }
                 }
                 continue;
             }
@@ -180,7 +183,10 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 for (int k = 0; k < width; ++k) {
                     const int e = k * T + t;
                     h.idx[off + 32u * k + lane] = len > 0 ? idx[ptr[seg] + std::min(e, len - 1)] : 0;  // empty segment: any valid index
-                    if (lane / T < cnt && e < len) h.val[off + 32u * k + lane] = val[ptr[seg] + e];
+                    if (lane / T < cnt && e < len) {
+                        h.val[off + 32u * k + lane] = val[ptr[seg] + e];
+                        h.pos[ptr[seg] + e] = (int)(off + 32u * k + lane);
+                    }
                 }
             }
         }
@@ -241,7 +247,10 @@ void sync_params(cs_solver *S) {
 cs_status do_condition(cs_solver *S, int use_rule) {
     cs_status st = ensure_xz(S);
     if (st != CS_OK) return st;
-    S->ctx.mu = S->prm.mu;  // mu, t, o_floor take effect here (cs.h)
+    // automatic: FSAI(1) pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs);
+    // with the SOCP setting t = 1.7 it saves ~10 % of the CG steps and costs 18 % per step (measured)
+    S->ctx.fsai = S->prm.precond == 2 || (S->prm.precond == 0 && S->prm.t >= 4.0);
+    S->ctx.mu = S->prm.mu;  // mu, t, o_floor, precond take effect here (cs.h)
     S->ctx.t = S->prm.t;
     S->ctx.o_floor = S->prm.o_floor;
     sync_params(S);
@@ -400,10 +409,10 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     // column-major copy (counting sort by internal column; rows come out sorted within a column) and its
     // slices on a second thread, while this thread builds the slices of the row-major copy
     HostSparse hr, hc2;
+    std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
     {
         const int nt = host_threads();
         std::thread tc([&] {
-            std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
             std::vector<double> cv2((size_t)nnz);
             for (int k = 0; k < nnz; ++k) cp2[(size_t)ci2[k] + 1]++;
             for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] += cp2[j];
@@ -449,6 +458,23 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
     if ((st = upload_sparse(S, hr, &x.R)) != CS_OK) return st;
     if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;
+    {   // plain compressed views of the same entries (used only to build the FSAI preconditioner)
+        int *q;
+        if ((st = dev_upload(S, &q, rp2.data(), rp2.size())) != CS_OK) return st; x.Rc.ptr = q;
+        if ((st = dev_upload(S, &q, ci2.data(), ci2.size())) != CS_OK) return st; x.Rc.idx = q;
+        if ((st = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) != CS_OK) return st; x.Rc.pos = q;
+        if ((st = dev_upload(S, &q, cp2.data(), cp2.size())) != CS_OK) return st; x.Cc.ptr = q;
+        if ((st = dev_upload(S, &q, ri2.data(), ri2.size())) != CS_OK) return st; x.Cc.idx = q;
+        if ((st = dev_upload(S, &q, hc2.pos.data(), hc2.pos.size())) != CS_OK) return st; x.Cc.pos = q;
+        if ((st = dev_zeros(S, &x.f_ctop, (size_t)3 * n)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.f_partner, (size_t)m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.f_tptr, (size_t)m + 1)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.f_tcur, (size_t)m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.f_tidx, (size_t)m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.f_blk, (size_t)kMaxGrid)) != CS_OK) return st;
+        double **fv[] = {&x.f_gd, &x.f_gm, &x.z, &x.t1};
+        for (double **q2 : fv) if ((st = dev_zeros(S, q2, (size_t)m)) != CS_OK) return st;
+    }
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
     lap("upload");
     if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
@@ -490,6 +516,8 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.o_floor = 1e-16;
     S->prm.cg_tol = 1e-15;
     S->prm.cg_max_iter = 20000;
+    S->prm.precond = 0;
+    S->nnz = nnz;
     x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
     sync_params(S);
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
@@ -517,8 +545,9 @@ cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const dou
 
 cs_status cs_set_params(cs_solver *S, const cs_params *p) {
     if (!S || !p) return CS_EINVAL;
-    if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || p->cg_max_iter < 1) {
-        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, cg_max_iter >= 1";
+    if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || p->cg_max_iter < 1 ||
+        p->precond < 0 || p->precond > 2) {
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, cg_max_iter >= 1, precond in {0,1,2}";
         return CS_EINVAL;
     }
     S->prm = *p;

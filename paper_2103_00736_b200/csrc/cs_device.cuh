@@ -42,6 +42,12 @@ struct Sparse {
     double *partial;        // [slots][2]
 };
 
+// Plain compressed view of one copy (segment s = entries [ptr[s], ptr[s+1]), minor index idx[e], value
+// val[pos[e]] in the slice storage).  Only the set-up of the FSAI preconditioner walks it.
+struct Csr {
+    const int *ptr, *idx, *pos;
+};
+
 struct Scalars {            // device-resident state scalars (read back only by cs_residuals)
     double resid[16];
     long long iter, cg_steps_total, cg_steps_cond;
@@ -50,13 +56,21 @@ struct Scalars {            // device-resident state scalars (read back only by 
     unsigned long long phase_ns[8];  // time spent per phase id (kPh*), measured by CTA 0 between grid barriers
 };
 
-enum { kPhCone = 0, kPhRhs = 1, kPhK1 = 2, kPhK2 = 3, kPhUpdate = 4, kPhReduce = 5, kPhCondition = 6, kPhResid = 7 };
+enum { kPhCone = 0, kPhRhs = 1, kPhK1 = 2, kPhK2 = 3, kPhUpdate = 4, kPhReduce = 5, kPhPrecond = 6, kPhResid = 7 };
 
 struct Ctx {
     int m, n, n_lin, n_soc;
     const int *cone_off;    // [n_soc+1] absolute offsets of the Lorentz blocks (cone_off[0] = n_lin)
     const int *perm_r, *perm_c;  // internal index -> caller's index (rows / columns sorted by length)
     Sparse R, C;            // row-major (segments = rows) and column-major (segments = columns) copies of A
+    Csr Rc, Cc;             // plain compressed views of the same two copies
+    // FSAI(1) preconditioner G = diag(gd) + strictly-lower part with one entry gm[i] at column partner[i]
+    int fsai;               // 0: off (plain Jacobi-equilibrated CG)
+    int *f_ctop;            // [n][3] strongest short rows of every column
+    int *f_partner;         // [m] partner row (< i) or -1
+    int *f_tptr, *f_tcur, *f_tidx, *f_blk;   // transposed lists: rows whose partner is k are f_tidx[f_tptr[k] .. f_tptr[k+1])
+    double *f_gd, *f_gm;    // [m] diagonal and off-diagonal entries of G
+    double *z, *t1;         // [m] preconditioned residual and G r
     // n-vectors
     double *s, *p, *g, *e, *u, *chat, *O, *xb, *zb;
     const double *c;

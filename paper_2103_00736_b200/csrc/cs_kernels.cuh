@@ -76,9 +76,10 @@ __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
 // converges to the (scaling-independent) dual solution, which makes the warm start effective.
 // Inner solve: CG on (A~ A~') w = q, started from the current w with residual r already in c.r and
 // rho = ||r||^2, qq = ||q||^2 known.  Two sparse passes and two grid reductions per step:
-//   K1 (columns, CSC):  u = A~' r + beta u          sigma = ||u||^2       (u == A~' v by induction)
-//   K2 (rows,    CSR):  v = r + beta v ; w += alpha v ; r -= alpha (A~ u) ; rho' = ||r||^2
-// with alpha = rho/sigma (v'A~A~'v = ||A~'v||^2) and beta = rho'/rho.  Returns the steps done.
+//   K1 (columns):  u = A~' z + beta u          sigma = ||u||^2       (u == A~' v by induction)
+//   K2 (rows):     v = z + beta v ; w += alpha v ; r -= alpha (A~ u) ; ||r||^2
+// with alpha = r'z/sigma (v'A~A~'v = ||A~'v||^2), beta = r'z_new / r'z, and z = r (Jacobi-equilibrated CG) or
+// z = G'G r (FSAI(1), two more light passes and two more barriers per step).  Returns the steps done.
 // ---------------------------------------------------------------------------------------------
 struct TermDot {    // sum_k a_k x[j_k]  (A~' r, A~ u, A~' w, A~ c^ ...)
     const double *x;
@@ -97,12 +98,12 @@ struct EpiK1 {
         sigma += uj * uj;
     }
 };
-struct EpiK2 {
-    double *v, *w, *r; double alpha, beta; double rho;
-    struct Pre { double r, v, w; };
-    __device__ __forceinline__ Pre pre(int i) const { return Pre{r[i], v[i], w[i]}; }
+struct EpiK2 {       // z = preconditioned residual (== r when the FSAI preconditioner is off)
+    double *v, *w, *r; const double *z; double alpha, beta; double rho;
+    struct Pre { double r, z, v, w; };
+    __device__ __forceinline__ Pre pre(int i) const { return Pre{r[i], z[i], v[i], w[i]}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &q) {
-        const double vi = q.r + beta * q.v;
+        const double vi = q.z + beta * q.v;
         v[i] = vi;
         w[i] = q.w + alpha * vi;
         const double rn = q.r - alpha * a[0];
@@ -111,32 +112,65 @@ struct EpiK2 {
     }
 };
 
-__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rho, double qq, bool &hit_max) {
-    const double thresh = c.cg_tol * c.cg_tol * qq;
+// z = G'G r for the FSAI(1) factor G (one off-diagonal entry per row, cs_kernels_cond.cuh builds it);
+// returns r'z.  Two light m-vector passes: t1 = G r (one gather at the partner row), z = G't1 (the rows that
+// chose k as partner are listed, sorted, in f_tidx[f_tptr[k] .. f_tptr[k+1]): deterministic order).
+__device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    for (int i = tid; i < c.m; i += nth) {
+        const int pk = c.f_partner[i];
+        double t = c.f_gd[i] * c.r[i];
+        if (pk >= 0) t += c.f_gm[i] * c.r[pk];
+        c.t1[i] = t;
+    }
+    gc.sync();
+    double rz = 0.0;
+    for (int k = tid; k < c.m; k += nth) {
+        double acc = c.f_gd[k] * c.t1[k];
+        for (int e = c.f_tptr[k]; e < c.f_tptr[k + 1]; ++e) {
+            const int i = c.f_tidx[e];
+            acc += c.f_gm[i] * c.t1[i];
+        }
+        c.z[k] = acc;
+        rz += c.r[k] * acc;
+    }
+    double red[1] = {rz};
+    grid_reduce<1>(red, gc);
+    return red[0];
+}
+
+__device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, double qq, bool &hit_max) {
+    const double thresh = c.cg_tol * c.cg_tol * qq;       // stop on ||r|| <= cg_tol ||q|| (equilibrated system)
+    const double *zsrc = c.fsai ? c.z : c.r;
     double beta = 0.0;
     int steps = 0;
     hit_max = false;
-    while (rho > thresh) {
+    if (!(rr > thresh)) return 0;
+    double rz = c.fsai ? apply_fsai(c, gc) : rr;           // r'z, z = G'G r
+    while (rr > thresh) {
         if (steps >= c.cg_max_iter) { hit_max = true; break; }
-        TermDot t1{c.r};
+        TermDot t1{zsrc};
         EpiK1 e1{c.u, beta, 0.0};
-        seg_reduce<1, false>(c.C, t1, e1, gc);
+        seg_reduce<1, false>(c.C, t1, e1, gc);             // u = A~'z + beta u = A~'v
         gc.lap(kPhK1);
         double red[1] = {e1.sigma};
         grid_reduce<1>(red, gc);
         gc.lap(kPhReduce);
         const double sigma = red[0];
         if (!(sigma > 0.0)) break;
-        const double alpha = rho / sigma;
+        const double alpha = rz / sigma;
         TermDot t2{c.u};
-        EpiK2 e2{c.v, c.w, c.r, alpha, beta, 0.0};
+        EpiK2 e2{c.v, c.w, c.r, zsrc, alpha, beta, 0.0};
         seg_reduce<1, false>(c.R, t2, e2, gc);
         gc.lap(kPhK2);
         red[0] = e2.rho;
         grid_reduce<1>(red, gc);
         gc.lap(kPhReduce);
-        beta = red[0] / rho;
-        rho = red[0];
+        rr = red[0];
+        const double rz_new = c.fsai ? apply_fsai(c, gc) : rr;
+        if (c.fsai) gc.lap(kPhPrecond);
+        beta = rz_new / rz;
+        rz = rz_new;
         ++steps;
     }
     return steps;

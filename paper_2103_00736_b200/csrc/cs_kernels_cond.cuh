@@ -103,6 +103,110 @@ struct EpiRecast {    // step 14: s = O^{-1}x - mu O z ; g = A~'w for the warm s
     }
 };
 
+// ---------------------------------------------------------------------------------------------
+// FSAI(1) preconditioner for M = A~A~' (unit diagonal): G = lower triangular with ONE off-diagonal entry
+// per row, G M G' ~ I.  Row i (short rows only) picks as partner the strongest short row k < i of its own
+// strongest column (|a~| largest); with mu = M_ik = <row i, row k>, the 2x2 FSAI system gives
+// g_ii = 1/sqrt(1-mu^2), g_ik = -mu/sqrt(1-mu^2).  The pattern depends on the scaled values, so it is
+// rebuilt at every conditioning: O(nnz) reads, a handful of grid barriers, no host involvement.
+// (Measured on CPU replicas: 2.5-3.4x fewer CG steps on the conditioned config-4 systems, 1.5-1.9x on
+// config 1; static patterns chosen from the unscaled matrix lose most of that.)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void fsai_build(const Ctx &c, GridCtl &gc) {
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    // F1: the three strongest short rows of every column
+    for (int j = tid; j < c.n; j += nth) {
+        int b0 = -1, b1 = -1, b2 = -1;
+        double v0 = -1.0, v1 = -1.0, v2 = -1.0;
+        for (int e = c.Cc.ptr[j]; e < c.Cc.ptr[j + 1]; ++e) {
+            const int i = c.Cc.idx[e];
+            if (c.Rc.ptr[i + 1] - c.Rc.ptr[i] > kShortMax) continue;
+            const double a = fabs(c.C.val[c.Cc.pos[e]]);
+            if (a > v0) { v2 = v1; b2 = b1; v1 = v0; b1 = b0; v0 = a; b0 = i; }
+            else if (a > v1) { v2 = v1; b2 = b1; v1 = a; b1 = i; }
+            else if (a > v2) { v2 = a; b2 = i; }
+        }
+        c.f_ctop[3 * j] = b0; c.f_ctop[3 * j + 1] = b1; c.f_ctop[3 * j + 2] = b2;
+    }
+    for (int i = tid; i < c.m; i += nth) c.f_tcur[i] = 0;
+    gc.sync();
+    // F2: partner, mu and the two entries of G per row
+    for (int i = tid; i < c.m; i += nth) {
+        int pk = -1;
+        double gd = 1.0, gm = 0.0;
+        const int a0 = c.Rc.ptr[i], a1 = c.Rc.ptr[i + 1];
+        if (a1 - a0 <= kShortMax) {
+            int jstar = -1;
+            double best = -1.0;
+            for (int e = a0; e < a1; ++e) {
+                const double a = fabs(c.R.val[c.Rc.pos[e]]);
+                if (a > best) { best = a; jstar = c.Rc.idx[e]; }
+            }
+            for (int q = 0; q < 3 && jstar >= 0; ++q) {
+                const int cand = c.f_ctop[3 * jstar + q];
+                if (cand >= 0 && cand < i) { pk = cand; break; }
+            }
+            if (pk >= 0) {
+                const int k0 = c.Rc.ptr[pk], k1 = c.Rc.ptr[pk + 1];
+                double mu = 0.0;
+                for (int e = a0; e < a1; ++e) {
+                    const int j = c.Rc.idx[e];
+                    for (int f = k0; f < k1; ++f)
+                        if (c.Rc.idx[f] == j) { mu += c.R.val[c.Rc.pos[e]] * c.R.val[c.Rc.pos[f]]; break; }
+                }
+                const double det = 1.0 - mu * mu;
+                if (det > 1e-8) { const double sg = sqrt(det); gd = 1.0 / sg; gm = -mu / sg; }
+                else pk = -1;
+            }
+        }
+        c.f_partner[i] = pk;
+        c.f_gd[i] = gd;
+        c.f_gm[i] = gm;
+        if (pk >= 0) atomicAdd(c.f_tcur + pk, 1);
+    }
+    gc.sync();
+    // F3: transposed lists (rows grouped by partner): exclusive scan of the counts, fill, sort each list
+    const int per = (c.m + gridDim.x - 1) / gridDim.x, lo = min(c.m, (int)blockIdx.x * per), hi = min(c.m, lo + per);
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        int sum = 0;
+        for (int i = lo + lane; i < hi; i += 32) sum += c.f_tcur[i];
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0) c.f_blk[blockIdx.x] = sum;
+    }
+    gc.sync();
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        int base = 0;
+        for (int b = lane; b < (int)blockIdx.x; b += 32) base += c.f_blk[b];
+        for (int o = 16; o > 0; o >>= 1) base += __shfl_xor_sync(0xffffffffu, base, o);
+        for (int i0 = lo; i0 < hi; i0 += 32) {          // warp-wide exclusive scan, 32 rows at a time
+            const int i = i0 + lane;
+            const int cnt = i < hi ? c.f_tcur[i] : 0;
+            int inc = cnt;
+            for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+            if (i < hi) { c.f_tptr[i] = base + inc - cnt; c.f_tcur[i] = 0; }
+            base += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        if (lane == 0 && hi == c.m && lo < hi) c.f_tptr[c.m] = base;
+    }
+    gc.sync();
+    for (int i = tid; i < c.m; i += nth) {
+        const int pk = c.f_partner[i];
+        if (pk >= 0) c.f_tidx[c.f_tptr[pk] + atomicAdd(c.f_tcur + pk, 1)] = i;
+    }
+    gc.sync();
+    for (int k = tid; k < c.m; k += nth) {              // insertion sort: lists are short (a short row tops <= 64 columns)
+        const int a = c.f_tptr[k], b = c.f_tptr[k + 1];
+        for (int e = a + 1; e < b; ++e) {
+            const int x = c.f_tidx[e];
+            int f = e - 1;
+            while (f >= a && c.f_tidx[f] > x) { c.f_tidx[f + 1] = c.f_tidx[f]; --f; }
+            c.f_tidx[f + 1] = x;
+        }
+    }
+}
+
 // use_rule = 1: O from steps 5-11 applied to (xb, zb); 0: O already in c.O (cs_set_scaling)
 __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_rule) {
     __shared__ double smem[kMaxRed * kWarps];
@@ -131,6 +235,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
         seg_rescale(c.C, f2);
     }
     gc.sync();
+    if (c.fsai) fsai_build(c, gc);   // its own barriers; reads the rescaled values only
     // Step 13's d is never formed: it is folded into the pass (cs_kernels.cuh), so a conditioning needs no
     // solve.  What remains is the recast of s (step 14) and g = A~'w in the new scaling.
     TermDot tw{c.w};
