@@ -339,3 +339,35 @@ def test_parameters_mu_and_t(mu, t):
     assert rel(got["O"], ref["O"]) <= 1e-12
     assert np.log(got["O"].max() / got["O"].min()) <= t * (1 + 1e-12)
     _check_resid(S, O)
+
+
+@pytest.mark.parametrize("name", ["cfg1_x0.3_pcg", "cfg4_x0.02_zipf_pcg", "mixed_cones"])
+def test_preconditioner_changes_the_steps_not_the_iterates(name):
+    """cs_params.precond: 1 = Jacobi equilibration only, 2 = FSAI(1).  Same passes (incl. a conditioning from
+    identical inputs) to 1e-9 against each other and against the oracle; fewer CG steps with FSAI on the LPs."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    make, k, okw = CASES[name]
+    p = make()
+    O0 = oracle.Oracle.from_problem(p)
+    O0.run(10)
+    start = O0.get()
+    O = oracle.Oracle.from_problem(p)
+    O.set_point(start["x"], start["z"])
+    O.run(8)
+    ref, sols, steps = O.get(), {}, {}
+    for pc in (1, 2):
+        S = binding.Solver.from_problem(p, device="cuda:0")
+        S.set_params(precond=pc)
+        assert S.get_params()["precond"] == pc
+        S.set_point(start["x"], start["z"])
+        S.iterate(8)
+        sols[pc], steps[pc] = S.solution(), S.residuals()["cg_steps_total"]
+        for key in ("x", "z", "y", "s"):
+            assert rel(sols[pc][key], ref[key]) <= TOL_ITER, (pc, key, rel(sols[pc][key], ref[key]))
+    for key in ("x", "z", "y", "s"):
+        assert rel(sols[2][key], sols[1][key]) <= TOL_ITER
+    if p.n_soc == 0:
+        assert steps[2] < 0.8 * steps[1], steps
+    with pytest.raises(binding.CsError):
+        S.set_params(precond=3)
