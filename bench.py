@@ -285,18 +285,19 @@ def main():
     except Exception as e:  # pragma: no cover
         gather = {"error": str(e)}
     ph1 = S.phase_times()
-    ph = {k: (ph1[k] - ph0[k]) * 1e-6 for k in ph1 if k not in ("r6", "r7")}   # ms, device globaltimer
+    ph = {k: (ph1[k] - ph0[k]) * 1e-6 for k in ph1 if k != "r7"}   # ms, device globaltimer
     k1_b, k2_b = 12 * p.nnz + 8 * p.m + 16 * p.n, 12 * p.nnz + 8 * p.n + 52 * p.m
     phases = {"ms": {k: round(v, 3) for k, v in ph.items()},
               "K1_GBs": k1_b * cg_iter / max(ph["K1"], 1e-9) / 1e6, "K2_GBs": k2_b * cg_iter / max(ph["K2"], 1e-9) / 1e6,
               "K1_us": 1e3 * ph["K1"] / max(1, cg_iter), "K2_us": 1e3 * ph["K2"] / max(1, cg_iter),
-              "reduce_us_per_cg": 1e3 * ph["reduce"] / max(1, cg_iter)}
+              "reduce_us_per_cg": 1e3 * ph["reduce"] / max(1, cg_iter),
+              "precond_us_per_cg": 1e3 * ph["precond"] / max(1, cg_iter)}
     # DRAM bytes of k_iterate from the ncu --set full captures in profiles/r01_ncu_notes.md, as a ratio to
     # the algorithmic bytes of the captured launch (dram__bytes_read.sum + dram__bytes_write.sum) / bytes
-    ncu_ratio = {3: 0.826, 4: 0.912}.get(a.config if a.scale == 1.0 else -1)
+    ncu_ratio = {3: 0.826, 4: 0.923 if fsai_on else 0.912}.get(a.config if a.scale == 1.0 else -1)
     roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "traffic": ncu_ratio * it_bytes / a.steps if ncu_ratio else None,
-            "traffic_source": "profiles/r01_ncu_notes.md (v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
+            "traffic_source": "profiles/r01_ncu_notes.md (v5/v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
                               "launch, applied to this launch)" if ncu_ratio else None,
             "peak_source": peak_src,
             "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,

@@ -142,7 +142,7 @@ cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, 
 
 /* Device time per phase of k_iterate so far, in ns, measured on the device between grid barriers:
  * out[0] cone reflect, [1] rhs pass, [2] CG pass K1 (A~'r, columns), [3] CG pass K2 (A~u, rows),
- * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6], [7] reserved.  One D2H copy + sync. */
+ * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6] preconditioner application z = G'G r, [7] reserved.  One D2H copy + sync. */
 cs_status cs_phase_times(cs_solver *S, double out[8]);
 
 /* Diagnostic (no handle, current device, default stream, synchronous): time n_idx uniformly random 8-byte

@@ -212,10 +212,10 @@ class Solver:
         return out
 
     def phase_times(self):
-        """Device time per phase of k_iterate so far (ns): cone, rhs, K1, K2, update, reduce."""
+        """Device time per phase of k_iterate so far (ns): cone, rhs, K1, K2, update, reduce, precond."""
         a = (C.c_double * 8)()
         self._check(lib().cs_phase_times(self._h, a))
-        names = ("cone", "rhs", "K1", "K2", "update", "reduce", "r6", "r7")
+        names = ("cone", "rhs", "K1", "K2", "update", "reduce", "precond", "r7")
         return dict(zip(names, [float(x) for x in a]))
 
     def barrier_probe(self, n=1000):
