@@ -39,7 +39,7 @@ def algorithmic_bytes(p, k_iter, cg_steps, n_cond, fsai=False):
     nnz, n, m = p.nnz, p.n, p.m
     cg = 24 * nnz + 28 * n + 60 * m          # K1 (column pass) + K2 (row pass) of one CG step
     if fsai:
-        cg += 96 * m                         # z = G'G r: two m-vector passes + z read in K2
+        cg += 60 * m                         # z = G'G r: one m-vector pass (r, z, dd, ee, partner, lists) + z read in K2
     outer = 24 * nnz + 92 * n + 24 * m       # cone reflect + rhs pass + final A'w pass with the s-update
     cond = 64 * nnz + 80 * n + 40 * m        # row norms, rescale of both copies, d/s recast (solve counted in cg)
     return cg * cg_steps + outer * k_iter + cond * n_cond, cg

@@ -472,7 +472,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         if ((st = dev_zeros(S, &x.f_tcur, (size_t)m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_tidx, (size_t)m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_blk, (size_t)kMaxGrid)) != CS_OK) return st;
-        double **fv[] = {&x.f_gd, &x.f_gm, &x.z, &x.t1};
+        double **fv[] = {&x.f_gd, &x.f_gm, &x.f_tc, &x.z, &x.t1};
         for (double **q2 : fv) if ((st = dev_zeros(S, q2, (size_t)m)) != CS_OK) return st;
     }
     CS_CUDA(S, cudaStreamSynchronize(S->stream));

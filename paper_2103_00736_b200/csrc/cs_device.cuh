@@ -69,8 +69,9 @@ struct Ctx {
     int *f_ctop;            // [n][3] strongest short rows of every column
     int *f_partner;         // [m] partner row (< i) or -1
     int *f_tptr, *f_tcur, *f_tidx, *f_blk;   // transposed lists: rows whose partner is k are f_tidx[f_tptr[k] .. f_tptr[k+1])
-    double *f_gd, *f_gm;    // [m] diagonal and off-diagonal entries of G
-    double *z, *t1;         // [m] preconditioned residual and G r
+    double *f_gd, *f_gm;    // [m] during the build: g_ii and g_{i,partner}; afterwards the diagonal dd and the partner entry ee of G'G
+    double *f_tc;           // [m] coefficients of the transposed-list entries of G'G
+    double *z, *t1;         // [m] preconditioned residual; build scratch
     // n-vectors
     double *s, *p, *g, *e, *u, *chat, *O, *xb, *zb;
     const double *c;

@@ -79,7 +79,7 @@ __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
 //   K1 (columns):  u = A~' z + beta u          sigma = ||u||^2       (u == A~' v by induction)
 //   K2 (rows):     v = z + beta v ; w += alpha v ; r -= alpha (A~ u) ; ||r||^2
 // with alpha = r'z/sigma (v'A~A~'v = ||A~'v||^2), beta = r'z_new / r'z, and z = r (Jacobi-equilibrated CG) or
-// z = G'G r (FSAI(1), two more light passes and two more barriers per step).  Returns the steps done.
+// z = G'G r (FSAI(1), one more light pass and one more barrier per step).  Returns the steps done.
 // ---------------------------------------------------------------------------------------------
 struct TermDot {    // sum_k a_k x[j_k]  (A~' r, A~ u, A~' w, A~ c^ ...)
     const double *x;
@@ -112,27 +112,22 @@ struct EpiK2 {       // z = preconditioned residual (== r when the FSAI precondi
     }
 };
 
-// z = G'G r for the FSAI(1) factor G (one off-diagonal entry per row, cs_kernels_cond.cuh builds it);
-// returns r'z.  Two light m-vector passes: t1 = G r (one gather at the partner row), z = G't1 (the rows that
-// chose k as partner are listed, sorted, in f_tidx[f_tptr[k] .. f_tptr[k+1]): deterministic order).
+// z = G'G r for the FSAI(1) factor G (one off-diagonal entry per row, cs_kernels_cond.cuh builds it); returns
+// r'z.  G'G is applied as ONE sparse symmetric operator assembled at build time:
+//   z_k = dd_k r_k + ee_k r_{partner(k)} + sum_{e in list(k)} cc_e r_{tidx[e]}
+// with dd_k = gd_k^2 + sum_{i in list(k)} gm_i^2, ee_k = gd_k gm_k, cc_e = gd_i gm_i (i = tidx[e]); list(k) = the
+// rows whose partner is k, sorted, so the sum has a fixed order.  One light m-vector pass and one barrier.
 __device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
-    for (int i = tid; i < c.m; i += nth) {
-        const int pk = c.f_partner[i];
-        double t = c.f_gd[i] * c.r[i];
-        if (pk >= 0) t += c.f_gm[i] * c.r[pk];
-        c.t1[i] = t;
-    }
-    gc.sync();
     double rz = 0.0;
     for (int k = tid; k < c.m; k += nth) {
-        double acc = c.f_gd[k] * c.t1[k];
-        for (int e = c.f_tptr[k]; e < c.f_tptr[k + 1]; ++e) {
-            const int i = c.f_tidx[e];
-            acc += c.f_gm[i] * c.t1[i];
-        }
+        const int pk = c.f_partner[k];
+        const double rk = c.r[k];
+        double acc = c.f_gd[k] * rk;                         // f_gd holds dd after the build
+        if (pk >= 0) acc += c.f_gm[k] * c.r[pk];             // f_gm holds ee
+        for (int e = c.f_tptr[k]; e < c.f_tptr[k + 1]; ++e) acc += c.f_tc[e] * c.r[c.f_tidx[e]];
         c.z[k] = acc;
-        rz += c.r[k] * acc;
+        rz += rk * acc;
     }
     double red[1] = {rz};
     grid_reduce<1>(red, gc);

@@ -205,6 +205,21 @@ __device__ __forceinline__ void fsai_build(const Ctx &c, GridCtl &gc) {
             c.f_tidx[f + 1] = x;
         }
     }
+    gc.sync();
+    // F4: assemble G'G row by row (cs_kernels.cuh apply_fsai): t1 <- dd, z <- ee, f_tc <- cc, then move dd/ee
+    // into f_gd/f_gm (gd, gm of OTHER rows are still read here, hence the staging in t1/z and a barrier)
+    for (int k = tid; k < c.m; k += nth) {
+        double dd = c.f_gd[k] * c.f_gd[k];
+        for (int e = c.f_tptr[k]; e < c.f_tptr[k + 1]; ++e) {
+            const int i = c.f_tidx[e];
+            dd += c.f_gm[i] * c.f_gm[i];
+            c.f_tc[e] = c.f_gd[i] * c.f_gm[i];
+        }
+        c.t1[k] = dd;
+        c.z[k] = c.f_gd[k] * c.f_gm[k];
+    }
+    gc.sync();
+    for (int k = tid; k < c.m; k += nth) { c.f_gd[k] = c.t1[k]; c.f_gm[k] = c.z[k]; }
 }
 
 // use_rule = 1: O from steps 5-11 applied to (xb, zb); 0: O already in c.O (cs_set_scaling)

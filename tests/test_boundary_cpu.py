@@ -121,6 +121,6 @@ def test_bench_byte_accounting():
     p = W.config(1, 0.05)
     total, per_cg = bench.algorithmic_bytes(p, k_iter=2, cg_steps=10, n_cond=0)
     assert per_cg == 24 * p.nnz + 28 * p.n + 60 * p.m
-    assert bench.algorithmic_bytes(p, 2, 10, 0, fsai=True)[1] == per_cg + 96 * p.m
+    assert bench.algorithmic_bytes(p, 2, 10, 0, fsai=True)[1] == per_cg + 60 * p.m
     assert total == 10 * per_cg + 2 * (24 * p.nnz + 92 * p.n + 24 * p.m)
     assert bench.max_over_ranks(3.5) == 3.5                  # no process group: identity
