@@ -521,6 +521,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
     sync_params(S);
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    lap("grid + parameters");
     return CS_OK;
 }
 
