@@ -294,10 +294,10 @@ def main():
               "precond_us_per_cg": 1e3 * ph["precond"] / max(1, cg_iter)}
     # DRAM bytes of k_iterate from the ncu --set full captures in profiles/r01_ncu_notes.md, as a ratio to
     # the algorithmic bytes of the captured launch (dram__bytes_read.sum + dram__bytes_write.sum) / bytes
-    ncu_ratio = {3: 0.826, 4: 0.923 if fsai_on else 0.912}.get(a.config if a.scale == 1.0 else -1)
+    ncu_ratio = {3: 0.826, 4: 0.956 if fsai_on else 0.912}.get(a.config if a.scale == 1.0 else -1)
     roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "traffic": ncu_ratio * it_bytes / a.steps if ncu_ratio else None,
-            "traffic_source": "profiles/r01_ncu_notes.md (v5/v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
+            "traffic_source": "profiles/r01_ncu_notes.md (v6/v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
                               "launch, applied to this launch)" if ncu_ratio else None,
             "peak_source": peak_src,
             "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
