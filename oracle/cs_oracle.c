@@ -336,6 +336,81 @@ int orc_run(orc_solver *S, int64_t k_iter, const int64_t *L, int64_t nL) {
     return 0;
 }
 
+/* Step 4 with a "user-defined criteria" instead of a set L [P:295]: the paper leaves the criterion
+ * open; the reading taken here (reading (y)) is a stall test on the fixed-point residual
+ * f_l = ||s_l - s_{l-1}||_2 of pass l:
+ *     condition at the start of iteration l > 1  iff  (l-1) is a multiple of `window`
+ *                                               and  f_{l-1} > ratio * f_{l-1-lag}
+ * with 1 <= lag < window, so that both residuals were measured after the previous conditioning (which
+ * can only have happened at the start of iteration l-window or earlier) and therefore in the same
+ * scaled space.  Iteration 1 always conditions (L u {1}).  f_hist[l] must hold max(l)+1 doubles
+ * (f_hist[0] unused); cond_iters receives the iterations that conditioned (at most cap of them).
+ * Returns the number of conditionings of this call, or -1 on a solve error. */
+int64_t orc_run_stall(orc_solver *S, int64_t k_iter, int64_t window, int64_t lag, double ratio,
+                      double *f_hist, int64_t *cond_iters, int64_t cap) {
+    int64_t n_c = 0;
+    if (window < 2 || lag < 1 || lag >= window) return -1;
+    for (int64_t it = 0; it < k_iter; ++it) {
+        S->l += 1;                                             /* step 3 */
+        const int64_t l = S->l;
+        int cond = (l == 1);
+        if (l > 1 && (l - 1) % window == 0 && f_hist[l - 1] > ratio * f_hist[l - 1 - lag]) cond = 1;
+        if (cond) {                                            /* step 4 */
+            conditioning_rule(S);                              /* steps 5-11 */
+            if (apply_scaling(S)) return -1;                   /* steps 12-14 */
+            if (n_c < cap) cond_iters[n_c] = l;
+            n_c += 1;
+        }
+        one_pass(S);                                           /* steps 16-20 */
+        f_hist[l] = S->fp_res;
+    }
+    return n_c;
+}
+
+/* Fixed equilibration, the practice the paper argues against [P:130-132: "matrix equilibration
+ * heuristics such as Sinkhorn-Knopp and Ruiz methods ... equalizing l_p norm for each row through
+ * diagonal choices of D and E"; P:148-152 uses the l_2 norms].  The paper gives no listing; this is
+ * Ruiz's simultaneous square-root iteration in the l_2 norm (reading (z)):
+ *     B = D A E ;  r_i = ||row_i(B)||_2 ;  c_j = ||col_j(B)||_2
+ *     D_i <- D_i / sqrt(r_i) ;  E_j <- E_j / sqrt(c_j / tau) ,  tau = sqrt(m/n)
+ * (rows are driven to norm 1 and columns to norm tau: sum r_i^2 = sum c_j^2 forces m = n tau^2).
+ * E has to commute with the cone [P:122-126 E^{-1}K = K], i.e. be constant on a Lorentz block: c_j^2
+ * is replaced by its mean over the block.  Empty rows / columns keep their factor.  D is returned
+ * for the pins only: abs_{A_hat} does not depend on a row scaling (D^AC = I). */
+void orc_ruiz(const orc_solver *S, int64_t n_iter, double *D, double *E) {
+    const int64_t m = S->m, n = S->n;
+    const double tau = sqrt((double)m / (double)n);
+    double *r2 = (double *)malloc(sizeof(double) * (size_t)(m > 0 ? m : 1));
+    double *c2 = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    for (int64_t i = 0; i < m; ++i) D[i] = 1.0;
+    for (int64_t j = 0; j < n; ++j) E[j] = 1.0;
+    for (int64_t it = 0; it < n_iter; ++it) {
+        for (int64_t j = 0; j < n; ++j) c2[j] = 0.0;
+        for (int64_t i = 0; i < m; ++i) {
+            double acc = 0.0;
+            for (int64_t q = S->row_ptr[i]; q < S->row_ptr[i + 1]; ++q) {
+                const int64_t j = S->col_idx[q];
+                const double bij = D[i] * S->val[q] * E[j];
+                acc += bij * bij;
+                c2[j] += bij * bij;
+            }
+            r2[i] = acc;
+        }
+        int64_t a = S->n_lin;                                  /* block means over the Lorentz cones */
+        for (int64_t k = 0; k < S->n_soc; ++k) {
+            const int64_t sz = S->soc_size[k];
+            double mean = 0.0;
+            for (int64_t j = a; j < a + sz; ++j) mean += c2[j];
+            mean /= (double)sz;
+            for (int64_t j = a; j < a + sz; ++j) c2[j] = mean;
+            a += sz;
+        }
+        for (int64_t i = 0; i < m; ++i) if (r2[i] > 0.0) D[i] /= sqrt(sqrt(r2[i]));
+        for (int64_t j = 0; j < n; ++j) if (c2[j] > 0.0) E[j] /= sqrt(sqrt(c2[j]) / tau);
+    }
+    free(r2); free(c2);
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* handle management and accessors (plumbing)                                                  */
 /* ------------------------------------------------------------------------------------------ */

@@ -252,3 +252,118 @@ def test_constructed_socp_reaches_known_value():
     assert r["kkt_rel"] < 1e-7
     assert np.isclose(r["pobj"], p.opt_value(), rtol=1e-6, atol=1e-6)
     assert np.isclose(r["dobj"], p.opt_value(), rtol=1e-6, atol=1e-6)
+
+
+# ------------------------------------------------------------------ criterion-driven conditioning
+def _start_ones(p):
+    o = oracle.Oracle.from_problem(p)
+    ones = np.ones(p.n)
+    o.set_point(ones, ones)
+    return o
+
+
+def test_stall_criterion_limits_reduce_to_a_set_L():
+    """ratio = 0: every residual is a stall => conditions at every multiple of the window, i.e. the set
+    L = {W+1, 2W+1, ...}; ratio = huge: never => L = {} (both bit for bit)."""
+    p = W.gaussian_dense_lp(100)
+    a = _start_ones(p)
+    conds = a.run_stall(330, 50, 20, 0.0)
+    assert conds == [1, 51, 101, 151, 201, 251, 301]
+    b = _start_ones(p)
+    b.run(330, L=(51, 101, 151, 201, 251, 301))
+    assert np.array_equal(a.get()["x"], b.get()["x"]) and np.array_equal(a.get()["O"], b.get()["O"])
+    a = _start_ones(p)
+    assert a.run_stall(330, 50, 20, 1e300) == [1]
+    b = _start_ones(p)
+    b.run(330, L=())
+    assert np.array_equal(a.get()["s"], b.get()["s"])
+
+
+def test_stall_criterion_replayed_pass_by_pass():
+    """The decisions of orc_run_stall re-taken outside it: one pass at a time through orc_run, the
+    fixed-point residual read back through orc_residuals, the rule applied here (reading (y))."""
+    p = W.gaussian_dense_lp(101)
+    window, lag, ratio = 40, 15, 0.85
+    a = _start_ones(p)
+    conds = a.run_stall(200, window, lag, ratio) + a.run_stall(221, window, lag, ratio)   # resumable
+    b = _start_ones(p)
+    f, mine = {}, []
+    for l in range(1, 422):
+        cond = l == 1 or ((l - 1) % window == 0 and f[l - 1] > ratio * f[l - 1 - lag])
+        if cond:
+            mine.append(l)
+        b.run(1, L=(l,) if cond else ())
+        f[l] = b.residuals()["fp_res"]
+    assert mine == conds and 3 <= len(conds) < 11
+    assert np.array_equal(a.get()["x"], b.get()["x"])
+    # no decision was a near tie (so a device run in a different rounding order takes the same ones)
+    for l in range(window + 1, 422, window):
+        assert abs(f[l - 1] / (ratio * f[l - 1 - lag]) - 1.0) > 1e-3
+
+
+def test_stall_criterion_beats_no_conditioning():
+    """conditioning when the residual stalls does what L = {300} does in Fig. 2."""
+    for seed in range(3):
+        p = W.gaussian_dense_lp(100 + seed)
+        a = _start_ones(p)
+        a.run(1500, L=())
+        b = _start_ones(p)
+        conds = b.run_stall(1500, 50, 25, 0.5)
+        assert len(conds) > 2
+        assert b.residuals()["pres_abs"] < 1e-2 * a.residuals()["pres_abs"]
+
+
+# ------------------------------------------------------------------ fixed equilibration (P:130-132, P:148-152)
+def test_ruiz_diagonal_matrix_closed_form():
+    """A = diag(a): B = DAE is diagonal, one sweep gives D_i = E_i = |a_i|^{-1/2} and B_ii = sign(a_i)."""
+    a = np.array([4.0, -9.0, 0.25, 100.0])
+    n = a.size
+    o = oracle.Oracle(n, n, np.arange(n + 1), np.arange(n), a, np.ones(n), np.ones(n), n, [])
+    for sweeps in (1, 2, 7):
+        D, E = o.ruiz(sweeps)
+        assert np.allclose(D, np.abs(a) ** -0.5, rtol=1e-14) and np.allclose(E, D, rtol=1e-14)
+
+
+def test_ruiz_equilibrates_rows_and_columns():
+    """Fixed point: every row of DAE has l2 norm 1 and every column sqrt(m/n) (sparse LP pattern)."""
+    p = W.sparse_lp(5, 40, 100, 16, row_log10=2, col_log10=1)   # dense enough for an exact equilibration to exist
+    o = oracle.Oracle.from_problem(p)
+    D, E = o.ruiz(400)
+    B = sp.diags(D) @ p.csr() @ sp.diags(E)
+    rn = np.sqrt(np.asarray(B.multiply(B).sum(axis=1)).ravel())
+    cn = np.sqrt(np.asarray(B.multiply(B).sum(axis=0)).ravel())
+    assert np.allclose(rn, 1.0, atol=1e-8) and np.allclose(cn, np.sqrt(40 / 100), atol=1e-8)
+    assert (D > 0).all() and (E > 0).all()
+
+
+def test_ruiz_undoes_a_diagonal_scaling_of_a_sign_matrix():
+    """A = D0 S E0 with |S_ij| = 1: the only equilibrated scaling of the pattern is |B_ij| = 1/sqrt(n)."""
+    rng = np.random.default_rng(3)
+    m, n = 6, 9
+    S = rng.choice([-1.0, 1.0], size=(m, n))
+    A = sp.csr_matrix(np.diag(10 ** rng.uniform(-3, 3, m)) @ S @ np.diag(10 ** rng.uniform(-2, 2, n)))
+    o = oracle.Oracle(m, n, A.indptr, A.indices, A.data, np.ones(m), np.ones(n), n, [])
+    D, E = o.ruiz(60)
+    B = np.diag(D) @ A.toarray() @ np.diag(E)
+    assert np.allclose(np.abs(B), 1 / np.sqrt(n), rtol=1e-10)
+
+
+def test_ruiz_is_constant_on_lorentz_blocks():
+    """E commutes with K: one factor per block; the block MEAN of the squared column norms
+    is what reaches m/n."""
+    p = W.sparse_socp(11, 30, 90, 8, 4, n_lin=10, lo=3, hi=12)
+    o = oracle.Oracle.from_problem(p)
+    D, E = o.ruiz(300)
+    B = sp.diags(D) @ p.csr() @ sp.diags(E)
+    c2 = np.asarray(B.multiply(B).sum(axis=0)).ravel()
+    a = p.n_lin
+    assert np.allclose(c2[:a], 30 / 90, atol=1e-8)
+    for sz in p.soc_size:
+        assert np.ptp(E[a:a + sz]) == 0.0
+        assert np.isclose(c2[a:a + sz].mean(), 30 / 90, atol=1e-8)
+        a += sz
+    # and the run on the equilibrated data reaches the same optimum (Algorithm 1 on scaled data, P:118-128)
+    o.set_scaling(E)
+    o.run_fixed(4000)
+    r = o.residuals()
+    assert r["kkt_rel"] < 1e-6 and np.isclose(r["pobj"], p.opt_value(), rtol=1e-5, atol=1e-6)
