@@ -132,6 +132,43 @@ cs_status cs_condition(cs_solver *S);
  * eq.(4)-(5)), then steps 12-14.  Block-constant O is the caller's responsibility. */
 cs_status cs_set_scaling(cs_solver *S, const double *O, cs_mem where);
 
+/* Fixed equilibration: n_sweeps of Ruiz's simultaneous square-root iteration in the l2 norm on the pristine A
+ * (the practice of P:130-132, "equalizing l_p norm for each row through diagonal choices of D and E"; l2 as
+ * in P:148-152), entirely on the device:  B = D A E;  D_i <- D_i / sqrt(||row_i(B)||_2);
+ * E_j <- E_j / sqrt(||col_j(B)||_2 / sqrt(m/n)), the squared column norms averaged over a Lorentz block so
+ * that E commutes with K.  Then O := E is installed exactly as cs_set_scaling does (steps
+ * 12-14).  This is the "fixed-scaling run" comparator of Algorithm 2; D is inert for the method.
+ * n_sweeps >= 0 (0 installs O = I).  One kernel launch + the conditioning launch, no host synchronisation. */
+cs_status cs_equilibrate(cs_solver *S, int32_t n_sweeps);
+
+/* Step 4 of Algorithm 2 as a whole-run driver ("Adaptive conditioning can be done based
+ * on a user-defined criteria or in the simplest case, at a set of user-defined iterations L").
+ *   rule CS_RULE_SET   : L = {first, first+every, first+2*every, ...}  (eq.(17): 300,100; eq.(18): 200,100;
+ *                        first <= 0: L empty; every <= 0: L = {first}).
+ *   rule CS_RULE_STALL : with f_l = ||s_l - s_{l-1}||_2 the fixed-point residual of pass l, condition at the
+ *                        start of iteration l > 1 iff (l-1) is a multiple of `window` and
+ *                        f_{l-1} > ratio * f_{l-1-lag}  and  f_{l-1} > f_floor   (1 <= lag < window; both
+ *                        residuals belong to the current scaling; f_floor keeps a converged run from
+ *                        conditioning on rounding noise).  Costs two 8-byte read-backs per window.
+ * Iteration 1 always conditions (L u {1}).  l is the handle's pass counter (cs_resid.iter), so calls
+ * can be chained; the stall rule's lagged residual does not carry over from one call to the next (the first
+ * window of a call that starts off a window boundary takes no decision).
+ * Stops after max_iter passes, or earlier at the first multiple of check_every (> 0) where kkt_rel <= tol
+ * (tol <= 0: never).  *out gets the residuals of the final iterate.  cond_iters (may be NULL) receives the
+ * iterations that conditioned, at most cond_cap of them; *n_cond (may be NULL) their number.
+ * Synchronous.  Returns CS_ECGMAX like cs_residuals. */
+enum { CS_RULE_SET = 0, CS_RULE_STALL = 1 };
+typedef struct {
+    int64_t max_iter, check_every;
+    double tol;
+    int32_t rule, reserved;
+    int64_t first, every;      /* CS_RULE_SET   */
+    int64_t window, lag;       /* CS_RULE_STALL */
+    double ratio, f_floor;
+} cs_schedule;
+cs_status cs_solve(cs_solver *S, const cs_schedule *sch, cs_resid *out, int64_t *cond_iters, int64_t cond_cap,
+                   int64_t *n_cond);
+
 /* Residual norms of the current iterate; ONE device->host copy and a stream synchronisation.
  * Returns CS_ECGMAX (with *out filled) if a solve hit cg_max_iter since the previous call. */
 cs_status cs_residuals(cs_solver *S, cs_resid *out);

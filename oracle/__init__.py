@@ -49,7 +49,7 @@ def _load():
         lib.orc_run.argtypes = [C.c_void_p, i64, C.POINTER(i64), i64]
         lib.orc_run.restype = C.c_int
         lib.orc_run_fixed.argtypes = [C.c_void_p, i64]
-        lib.orc_run_stall.argtypes = [C.c_void_p, i64, i64, i64, C.c_double, dp, C.POINTER(i64), i64]
+        lib.orc_run_stall.argtypes = [C.c_void_p, i64, i64, i64, C.c_double, C.c_double, dp, C.POINTER(i64), i64]
         lib.orc_run_stall.restype = i64
         lib.orc_ruiz.argtypes = [C.c_void_p, i64, dp, dp]
         lib.orc_get.argtypes = [C.c_void_p] + [dp] * 7
@@ -142,7 +142,7 @@ class Oracle:
     def run_fixed(self, k):
         _load().orc_run_fixed(self._h, int(k))
 
-    def run_stall(self, k, window, lag, ratio):
+    def run_stall(self, k, window, lag, ratio, f_floor=0.0):
         """orc_run_stall: k more passes of Algorithm 2 with the stall criterion in place of a set L.
         Returns the list of iterations that conditioned during this call."""
         l0 = self.counters()["l"]
@@ -151,7 +151,7 @@ class Oracle:
             f = np.concatenate([f, np.zeros(l0 + int(k) + 1 - f.size)])
         self._f_hist = f
         out = np.zeros(int(k) + 1, np.int64)
-        nc = _load().orc_run_stall(self._h, int(k), int(window), int(lag), float(ratio), _d(f),
+        nc = _load().orc_run_stall(self._h, int(k), int(window), int(lag), float(ratio), float(f_floor), _d(f),
                                    out.ctypes.data_as(C.POINTER(C.c_int64)), out.size)
         if nc < 0:
             raise RuntimeError("oracle stall-criterion run failed (bad arguments or solve error)")

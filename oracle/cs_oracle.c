@@ -341,12 +341,14 @@ int orc_run(orc_solver *S, int64_t k_iter, const int64_t *L, int64_t nL) {
  * f_l = ||s_l - s_{l-1}||_2 of pass l:
  *     condition at the start of iteration l > 1  iff  (l-1) is a multiple of `window`
  *                                               and  f_{l-1} > ratio * f_{l-1-lag}
+ *                                               and  f_{l-1} > f_floor
  * with 1 <= lag < window, so that both residuals were measured after the previous conditioning (which
  * can only have happened at the start of iteration l-window or earlier) and therefore in the same
- * scaled space.  Iteration 1 always conditions (L u {1}).  f_hist[l] must hold max(l)+1 doubles
+ * scaled space; f_floor keeps a run that has converged to rounding noise from conditioning on noise.
+ * Iteration 1 always conditions (L u {1}).  f_hist[l] must hold max(l)+1 doubles
  * (f_hist[0] unused); cond_iters receives the iterations that conditioned (at most cap of them).
  * Returns the number of conditionings of this call, or -1 on a solve error. */
-int64_t orc_run_stall(orc_solver *S, int64_t k_iter, int64_t window, int64_t lag, double ratio,
+int64_t orc_run_stall(orc_solver *S, int64_t k_iter, int64_t window, int64_t lag, double ratio, double f_floor,
                       double *f_hist, int64_t *cond_iters, int64_t cap) {
     int64_t n_c = 0;
     if (window < 2 || lag < 1 || lag >= window) return -1;
@@ -354,7 +356,8 @@ int64_t orc_run_stall(orc_solver *S, int64_t k_iter, int64_t window, int64_t lag
         S->l += 1;                                             /* step 3 */
         const int64_t l = S->l;
         int cond = (l == 1);
-        if (l > 1 && (l - 1) % window == 0 && f_hist[l - 1] > ratio * f_hist[l - 1 - lag]) cond = 1;
+        if (l > 1 && (l - 1) % window == 0 && f_hist[l - 1] > ratio * f_hist[l - 1 - lag] &&
+            f_hist[l - 1] > f_floor) cond = 1;
         if (cond) {                                            /* step 4 */
             conditioning_rule(S);                              /* steps 5-11 */
             if (apply_scaling(S)) return -1;                   /* steps 12-14 */

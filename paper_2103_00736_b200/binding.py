@@ -43,9 +43,18 @@ class cs_resid(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
 
 
-EXPORTS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
-           "cs_set_scaling", "cs_residuals", "cs_solution", "cs_phase_times", "cs_gather_probe", "cs_barrier_probe", "cs_kernel_launches", "cs_last_error",
-           "cs_destroy")
+class cs_schedule(C.Structure):
+    _fields_ = [("max_iter", C.c_int64), ("check_every", C.c_int64), ("tol", C.c_double), ("rule", C.c_int32),
+                ("reserved", C.c_int32), ("first", C.c_int64), ("every", C.c_int64), ("window", C.c_int64),
+                ("lag", C.c_int64), ("ratio", C.c_double), ("f_floor", C.c_double)]
+
+
+CS_RULE_SET, CS_RULE_STALL = 0, 1
+
+_INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
+               "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_phase_times",
+               "cs_gather_probe", "cs_barrier_probe")
+EXPORTS = _INT_STATUS + ("cs_kernel_launches", "cs_last_error", "cs_destroy")
 
 _lib = None
 
@@ -77,7 +86,10 @@ def lib():
         L.cs_phase_times.argtypes = [vp, C.POINTER(C.c_double)]
         L.cs_barrier_probe.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
         L.cs_gather_probe.argtypes = [C.c_int64, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-        for name in EXPORTS[:12]:
+        L.cs_equilibrate.argtypes = [vp, C.c_int32]
+        L.cs_solve.argtypes = [vp, C.POINTER(cs_schedule), C.POINTER(cs_resid), C.POINTER(C.c_int64), C.c_int64,
+                               C.POINTER(C.c_int64)]
+        for name in _INT_STATUS:
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -194,6 +206,26 @@ class Solver:
     def set_scaling(self, O):
         op = _ptr(O, np.float64)
         self._check(lib().cs_set_scaling(self._h, op[0], op[1]))
+
+    def equilibrate(self, n_sweeps):
+        """cs_equilibrate: fixed l2 Ruiz equilibration E installed as O."""
+        self._check(lib().cs_equilibrate(self._h, int(n_sweeps)))
+
+    def solve(self, max_iter, tol=0.0, check_every=0, first=0, every=0, stall=None, strict=False):
+        """cs_solve: Algorithm 2 with L = {first, first+every, ...} or, with stall=(window, lag, ratio[, f_floor]), the stall
+        rule.  Returns (residual dict, list of the iterations that conditioned)."""
+        sch = cs_schedule(max_iter=int(max_iter), check_every=int(check_every), tol=float(tol),
+                          rule=CS_RULE_STALL if stall else CS_RULE_SET, reserved=0, first=int(first),
+                          every=int(every), window=int(stall[0]) if stall else 0, lag=int(stall[1]) if stall else 0,
+                          ratio=float(stall[2]) if stall else 0.0,
+                          f_floor=float(stall[3]) if stall and len(stall) > 3 else 0.0)
+        cap = 4096
+        conds = (C.c_int64 * cap)()
+        nc = C.c_int64(0)
+        r = cs_resid()
+        self._check(lib().cs_solve(self._h, C.byref(sch), C.byref(r), conds, cap, C.byref(nc)),
+                    ok=(CS_OK,) if strict else (CS_OK, CS_ECGMAX))
+        return r.as_dict(), [int(conds[i]) for i in range(min(cap, nc.value))]
 
     def residuals(self, strict=False):
         r = cs_resid()

@@ -33,6 +33,9 @@ struct cs_solver {
     bool xz_stale = false;     // xb, zb older than (p, s)
     bool started = false;      // some pass or conditioning has run (cs_set_point no longer allowed)
     int64_t launches = 0;
+    int64_t iter = 0;          // passes done (Algorithm 2's l), mirrors Scalars::iter
+    double stall_f = 0.0;      // cs_solve, stall rule: fixed-point residual sampled after pass stall_at (-1: none)
+    int64_t stall_at = -1;
     std::string err;
 };
 
@@ -259,6 +262,7 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     if (st != CS_OK) return st;
     S->conditioned = true;
     S->started = true;
+    S->stall_at = -1;          // residuals of the old scaling do not compare with the new one's
     return CS_OK;
 }
 
@@ -594,6 +598,7 @@ cs_status cs_iterate(cs_solver *S, int64_t k) {
     if ((st = launch_coop(S, (const void *)k_iterate, args, S->dyn_smem)) != CS_OK) return st;
     S->xz_stale = true;
     S->started = true;
+    S->iter += k;
     return CS_OK;
 }
 
@@ -614,6 +619,95 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     out->gap_abs = h.resid[4]; out->gap_rel = h.resid[5]; out->cone_viol_rel = h.resid[6]; out->kkt_rel = h.resid[7];
     out->pobj = h.resid[8]; out->dobj = h.resid[9]; out->fp_res = h.resid[10];
     return h.cg_hit_max ? CS_ECGMAX : CS_OK;
+}
+
+cs_status cs_equilibrate(cs_solver *S, int32_t n_sweeps) {
+    if (!S || n_sweeps < 0) return CS_EINVAL;
+    cs_status st = ensure_xz(S);  // x,z of the OLD scaling, before O is overwritten
+    if (st != CS_OK) return st;
+    int ns = n_sweeps;
+    void *args[] = {&S->ctx, &ns};
+    if ((st = launch_coop(S, (const void *)k_equilibrate, args, S->dyn_smem)) != CS_OK) return st;
+    return do_condition(S, 0);
+}
+
+namespace {
+cs_status fetch_fp_res(cs_solver *S, double *f) {
+    double f2 = 0.0;
+    CS_CUDA(S, cudaMemcpyAsync(&f2, &S->ctx.sc->fp_res2, sizeof(double), cudaMemcpyDeviceToHost, S->stream));
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    *f = std::sqrt(f2);
+    return CS_OK;
+}
+int64_t next_multiple(int64_t l, int64_t q) { return (l / q + 1) * q; }   // smallest multiple of q above l
+}  // namespace
+
+cs_status cs_solve(cs_solver *S, const cs_schedule *sch, cs_resid *out, int64_t *cond_iters, int64_t cond_cap,
+                   int64_t *n_cond) {
+    if (!S || !sch || !out || sch->max_iter < 0 || sch->check_every < 0 || cond_cap < 0) return CS_EINVAL;
+    const bool stall = sch->rule == CS_RULE_STALL;
+    if (sch->rule != CS_RULE_SET && !stall) { S->err = "cs_solve: unknown rule"; return CS_EINVAL; }
+    if (stall && (sch->window < 2 || sch->lag < 1 || sch->lag >= sch->window || !(sch->ratio >= 0.0))) {
+        S->err = "cs_solve: the stall rule needs window >= 2, 1 <= lag < window, ratio >= 0";
+        return CS_EINVAL;
+    }
+    const int64_t kInf = INT64_MAX / 2;
+    const int64_t start = S->iter, end = start + sch->max_iter;
+    int64_t nc = 0;
+    auto note = [&](int64_t l) { if (cond_iters && nc < cond_cap) cond_iters[nc] = l; ++nc; };
+    auto in_L = [&](int64_t l) {   // CS_RULE_SET membership
+        if (sch->first <= 0 || l < sch->first) return false;
+        return l == sch->first || (sch->every > 0 && (l - sch->first) % sch->every == 0);
+    };
+    cs_status st, sticky = CS_OK;
+    bool have_resid = false;
+    if (!S->conditioned && S->iter == 0 && sch->max_iter > 0) note(1);   // cs_iterate runs the l = 1 conditioning
+    while (true) {
+        const int64_t l = S->iter;   // passes done; the next iteration is l + 1
+        have_resid = false;
+        if (sch->check_every > 0 && l > start && l % sch->check_every == 0 && sch->tol > 0.0) {
+            st = cs_residuals(S, out);
+            if (st == CS_ECGMAX) sticky = st; else if (st != CS_OK) return st;
+            have_resid = true;
+            if (out->kkt_rel <= sch->tol) break;
+        }
+        if (l >= end) break;
+        if (stall && l > 0) {
+            if ((l + sch->lag) % sch->window == 0) {
+                if ((st = fetch_fp_res(S, &S->stall_f)) != CS_OK) return st;
+                S->stall_at = l;
+            }
+            if (l % sch->window == 0 && S->stall_at == l - sch->lag) {
+                double f_now;
+                if ((st = fetch_fp_res(S, &f_now)) != CS_OK) return st;
+                if (f_now > sch->ratio * S->stall_f && f_now > sch->f_floor) {
+                    if ((st = do_condition(S, 1)) != CS_OK) return st;
+                    note(l + 1);
+                }
+            }
+        } else if (!stall && l > 0 && in_L(l + 1)) {
+            if ((st = do_condition(S, 1)) != CS_OK) return st;
+            note(l + 1);
+        }
+        int64_t nxt = end;
+        if (sch->check_every > 0 && sch->tol > 0.0) nxt = std::min(nxt, next_multiple(l, sch->check_every));
+        if (stall) {
+            nxt = std::min(nxt, next_multiple(l, sch->window));
+            nxt = std::min(nxt, next_multiple(l + sch->lag, sch->window) - sch->lag);
+        } else if (sch->first > 0) {
+            int64_t c = kInf;   // smallest member of L above l + 1
+            if (l + 1 < sch->first) c = sch->first;
+            else if (sch->every > 0) c = sch->first + ((l + 1 - sch->first) / sch->every + 1) * sch->every;
+            nxt = std::min(nxt, c - 1);
+        }
+        if ((st = cs_iterate(S, nxt - l)) != CS_OK) return st;
+    }
+    if (!have_resid) {
+        st = cs_residuals(S, out);
+        if (st == CS_ECGMAX) sticky = st; else if (st != CS_OK) return st;
+    }
+    if (n_cond) *n_cond = nc;
+    return sticky;
 }
 
 cs_status cs_phase_times(cs_solver *S, double out[8]) {

@@ -276,6 +276,74 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     }
 }
 
+// ---- fixed equilibration (cs_equilibrate): Ruiz's simultaneous square-root iteration in the l2 norm ---------
+// P:130-132 (row/column norm equalisation by diagonal D, E), l2 as in P:148-152.  E lives in c.O (the caller has
+// materialised x,z first), D ping-pongs between c.z and c.t1, the squared column norms go through c.u.
+struct EpiRuizRow {   // D_i <- D_i / sqrt(r_i),  r_i^2 = D_i^2 sum_j (A_ij E_j)^2   (empty row: unchanged)
+    const double *Dold; double *Dnew;
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
+        const double d = Dold[i], r2 = d * d * a[0];
+        Dnew[i] = r2 > 0.0 ? d / sqrt(sqrt(r2)) : d;
+    }
+};
+struct EpiRuizCol {   // c_j^2 = E_j^2 sum_i (A_ij D_i)^2
+    const double *E; double *c2;
+    typedef NoPre Pre;
+    __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
+    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &) {
+        const double e = E[j];
+        c2[j] = e * e * a[0];
+    }
+};
+
+__global__ void __launch_bounds__(kBlock, CS_MINB) k_equilibrate(Ctx c, int n_sweeps) {
+    __shared__ double smem[kMaxRed * kWarps];
+    GridCtl gc(c.partials, smem, c.bar);
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    double *E = c.O, *Dold = c.z, *Dnew = c.t1, *c2 = c.u;
+    const double tau = sqrt((double)c.m / (double)c.n);
+    for (int j = tid; j < c.n; j += nth) E[j] = 1.0;
+    for (int i = tid; i < c.m; i += nth) Dold[i] = 1.0;
+    gc.sync();
+    for (int it = 0; it < n_sweeps; ++it) {
+        {   // both norms from the same B = D A E (simultaneous update)
+            TermRowNorm tr{E};
+            EpiRuizRow er{Dold, Dnew};
+            seg_reduce<1, true>(c.R, tr, er, gc);
+            TermRowNorm tc{Dold};
+            EpiRuizCol ec{E, c2};
+            seg_reduce<1, true>(c.C, tc, ec, gc);
+        }
+        gc.sync();
+        for (int j = tid; j < c.n_lin; j += nth) {
+            const double v = c2[j];
+            if (v > 0.0) E[j] = E[j] / sqrt(sqrt(v) / tau);
+        }
+        if (c.n_soc) {   // one factor per Lorentz block: the block mean of c_j^2 (E must commute with K)
+            const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
+            constexpr int CPW = 32 / kConeLanes;
+            const int gwarp = tid >> 5, nwarps = nth >> 5;
+            for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
+                const int ci = base + sub;
+                const bool act = ci < c.n_soc;
+                const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
+                double sum = 0.0;
+                for (int j = a + sl; j < b; j += kConeLanes) sum += c2[j];
+                sum = group_reduce<kConeLanes>(sum);
+                const double mean = act ? sum / (double)(b - a) : 0.0;
+                if (mean > 0.0) {
+                    const double f = sqrt(sqrt(mean) / tau);
+                    for (int j = a + sl; j < b; j += kConeLanes) E[j] = E[j] / f;
+                }
+            }
+        }
+        double *t = Dold; Dold = Dnew; Dnew = t;
+        gc.sync();
+    }
+}
+
 // ---- residuals (original coordinates; xb, zb must be current) --------------------------------
 struct TermCsrX {     // A~ x^ with x^ = x/O
     const double *xb, *O;

@@ -371,3 +371,118 @@ def test_preconditioner_changes_the_steps_not_the_iterates(name):
         assert steps[2] < 0.8 * steps[1], steps
     with pytest.raises(binding.CsError):
         S.set_params(precond=3)
+
+
+# ------------------------------------------------------------------ S 8(f) rows 2, 3: schedules, fixed equilibration
+@pytest.mark.parametrize("name", ["lp_scaled", "mixed_cones", "cfg4_zipf"])
+def test_equilibrate_matches_oracle_ruiz(name):
+    """cs_equilibrate (l2 Ruiz on the device) against orc_ruiz, then the fixed-scaling run."""
+    p = {"lp_scaled": lambda: W.sparse_lp(5, 700, 1800, 6, row_log10=3, col_log10=2),
+         "mixed_cones": lambda: W.sparse_socp(77, 500, 1300, 30, 6, n_lin=333, lo=1, hi=70),
+         "cfg4_zipf": lambda: W.config(4, 0.004)}[name]()
+    S, O = _pair(p)
+    S.equilibrate(12)
+    _, E = O.ruiz(12)
+    got = S.solution()
+    assert np.max(np.abs(got["O"] / E - 1.0)) <= 1e-12
+    O.set_scaling(E)
+    assert rel(got["s"], O.get()["s"]) <= 1e-12
+    S.iterate(40)
+    O.run_fixed(40)
+    _check_iterates(S, O)
+    _check_resid(S, O)
+    r = S.residuals()
+    assert r["n_conditionings"] == 1 and r["iter"] == 40
+    S.destroy()
+
+
+def test_equilibrate_zero_sweeps_is_the_identity_scaling():
+    from paper_2103_00736_b200 import binding
+    p = W.config(1, 0.02)
+    a, b = binding.Solver.from_problem(p), binding.Solver.from_problem(p)
+    a.equilibrate(0)
+    a.iterate(20)
+    b.iterate(20)          # x = z = e_K start: the l = 1 conditioning is the identity
+    ga, gb = a.solution(), b.solution()
+    assert np.array_equal(ga["O"], np.ones(p.n)) and np.array_equal(ga["x"], gb["x"])
+    with pytest.raises(binding.CsError):
+        a.equilibrate(-1)
+
+
+def test_solve_set_rule_is_the_manual_schedule():
+    """cs_solve(CS_RULE_SET) = the cs_iterate / cs_condition sequence of the same L, bit for bit."""
+    from paper_2103_00736_b200 import binding
+    p = W.config(1, 0.02)
+    a, b = binding.Solver.from_problem(p), binding.Solver.from_problem(p)
+    r, conds = a.solve(137, first=30, every=25)
+    assert conds == [1, 30, 55, 80, 105, 130] and r["iter"] == 137 and r["n_conditionings"] == 6
+    r2, conds2 = a.solve(40, first=30, every=25)          # chained: l continues at 138
+    assert conds2 == [155] and r2["iter"] == 177
+    b.run(177, L=[30, 55, 80, 105, 130, 155])
+    ga, gb = a.solution(), b.solution()
+    for k in ga:
+        assert np.array_equal(ga[k], gb[k]), k
+    c = binding.Solver.from_problem(p)
+    r3, conds3 = c.solve(60, first=20, every=0)           # L = {20}
+    assert conds3 == [1, 20] and r3["n_conditionings"] == 2
+    c2 = binding.Solver.from_problem(p)
+    assert c2.solve(60)[1] == [1]                         # L = {}
+
+
+def test_solve_stops_at_the_tolerance():
+    from paper_2103_00736_b200 import binding
+    p = W.config(1, 0.02)
+    S = binding.Solver.from_problem(p)
+    r, conds = S.solve(3000, tol=1e-4, check_every=25, first=p.L_first, every=p.L_every)
+    assert r["kkt_rel"] <= 1e-4 and r["iter"] % 25 == 0 and r["iter"] < 3000
+    assert conds == [1] + [l for l in p.schedule(3000) if l <= r["iter"]]
+    before = S.kernel_launches()
+    S.iterate(25)
+    assert S.residuals()["kkt_rel"] < r["kkt_rel"] * 1.5 and S.kernel_launches() > before
+
+
+def test_solve_stall_rule_matches_the_oracle():
+    """P:295 "user-defined criteria" (reading (y)): same decisions as orc_run_stall on section IV-A's
+    80 x 100 LP (the oracle pin checks that none of them is a near tie), iterates to protocol (ii-b)."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = W.gaussian_dense_lp(100)
+    window, lag, ratio, floor = 20, 8, 0.7, 1e-8
+    ones = np.ones(p.n)
+    S, O = binding.Solver.from_problem(p), oracle.Oracle.from_problem(p)
+    S.set_point(ones, ones)
+    O.set_point(ones, ones)
+    ref = O.run_stall(200, window, lag, ratio, floor) + O.run_stall(221, window, lag, ratio, floor)
+    r1, c1 = S.solve(200, stall=(window, lag, ratio, floor))
+    r2, c2 = S.solve(221, stall=(window, lag, ratio, floor))     # 200 = 10 windows: nothing is lost at the seam
+    assert len(ref) >= 5
+    assert c1 + c2 == ref and r2["iter"] == 421 and r2["n_conditionings"] == len(ref)
+    _check_iterates(S, O, keys=("x", "z", "s"), tol=1e-6)
+    q = O.residuals()
+    assert abs(r2["pobj"] - q["pobj"]) <= TOL_RES * (1 + abs(q["pobj"]))
+    with pytest.raises(binding.CsError):
+        S.solve(10, stall=(10, 10, 0.5))                  # lag must be < window
+
+
+@pytest.mark.parametrize("seed", [100, 102])
+def test_section4a_three_schedules_on_the_device(seed):
+    """P:302-322 (Fig. 2): L = {}, {300}, {1..50} on the paper's 80 x 100 Gaussian LPs, device vs oracle."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = W.gaussian_dense_lp(seed)
+    ones = np.ones(p.n)
+    pres = {}
+    for name, L, k in (("none", (), 600), ("one", (300,), 600), ("cont", tuple(range(1, 51)), 300)):
+        S, O = binding.Solver.from_problem(p), oracle.Oracle.from_problem(p)
+        S.set_point(ones, ones)
+        O.set_point(ones, ones)
+        S.run(k, L=L)
+        O.run(k, L=L)
+        r, q = S.residuals(), O.residuals()
+        assert abs(r["pobj"] - q["pobj"]) <= TOL_RES * (1 + abs(q["pobj"])), name
+        assert abs(r["pres_abs"] - q["pres_abs"]) <= 1e-5 * q["pres_abs"] + 1e-9, name
+        if not L:       # with in-run conditionings of a run still in flight only protocol (iii) applies (DESIGN.md 7)
+            _check_iterates(S, O, keys=("x", "z"))
+        pres[name] = r["pres_abs"]
+        S.destroy()
+    assert pres["one"] < pres["none"] and pres["cont"] < 1e-2 * pres["none"]

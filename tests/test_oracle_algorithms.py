@@ -282,23 +282,29 @@ def test_stall_criterion_limits_reduce_to_a_set_L():
 def test_stall_criterion_replayed_pass_by_pass():
     """The decisions of orc_run_stall re-taken outside it: one pass at a time through orc_run, the
     fixed-point residual read back through orc_residuals, the rule applied here (reading (y))."""
-    p = W.gaussian_dense_lp(101)
-    window, lag, ratio = 40, 15, 0.85
+    p = W.gaussian_dense_lp(100)
+    window, lag, ratio, floor = 20, 8, 0.7, 1e-8
     a = _start_ones(p)
-    conds = a.run_stall(200, window, lag, ratio) + a.run_stall(221, window, lag, ratio)   # resumable
+    conds = a.run_stall(200, window, lag, ratio, floor) + a.run_stall(221, window, lag, ratio, floor)   # resumable
     b = _start_ones(p)
     f, mine = {}, []
     for l in range(1, 422):
-        cond = l == 1 or ((l - 1) % window == 0 and f[l - 1] > ratio * f[l - 1 - lag])
+        cond = l == 1 or ((l - 1) % window == 0 and f[l - 1] > ratio * f[l - 1 - lag] and f[l - 1] > floor)
         if cond:
             mine.append(l)
         b.run(1, L=(l,) if cond else ())
         f[l] = b.residuals()["fp_res"]
-    assert mine == conds and 3 <= len(conds) < 11
+    assert mine == conds and 5 <= len(conds) < 12
     assert np.array_equal(a.get()["x"], b.get()["x"])
-    # no decision was a near tie (so a device run in a different rounding order takes the same ones)
+    # no decision was a near tie (so a device run in a different rounding order takes the same ones), and the
+    # floor is what ends the conditionings once the run has converged
     for l in range(window + 1, 422, window):
-        assert abs(f[l - 1] / (ratio * f[l - 1 - lag]) - 1.0) > 1e-3
+        assert abs(f[l - 1] / floor - 1.0) > 1e-3
+        if f[l - 1] > floor:
+            assert abs(f[l - 1] / (ratio * f[l - 1 - lag]) - 1.0) > 1e-3
+    assert f[420] < floor and max(conds) < 300
+    c = _start_ones(p)
+    assert len(c.run_stall(421, window, lag, ratio, 0.0)) > len(conds)     # without it: decisions on noise
 
 
 def test_stall_criterion_beats_no_conditioning():
