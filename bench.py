@@ -170,6 +170,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 (SOCP) block")
+    ap.add_argument("--no-time-to-tol", action="store_true", help="skip the time-to-1e-4-KKT leg of the default run")
     ap.add_argument("--solve", action="store_true",
                     help="extra mode: run the paper's schedule (17)/(18) to --tol and report the time to tolerance")
     ap.add_argument("--tol", type=float, default=1e-4)
@@ -370,6 +371,8 @@ def finish(a, p, S, line, rank, world, dev, stream):
         # (DESIGN.md 9), so this leg uses inexact projections, cg_tol = 1e-7 (a cs_set_params parameter; measured:
         # 1e-6 stalls at kkt 1.3e-4, 1e-7 reaches 1e-4 in 51 s / 900 passes, 1e-8 in 128 s / 800 passes).
         try:
+            if a.no_time_to_tol:
+                raise RuntimeError("skipped (--no-time-to-tol)")
             import argparse as _ap
             a2 = _ap.Namespace(**{**vars(a), "tol": 1e-4, "check_every": 50, "max_iter": 2000})
             S3 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)

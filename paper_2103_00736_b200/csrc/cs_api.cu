@@ -26,7 +26,7 @@ struct cs_solver {
     int device = 0;
     int grid = 0;
     int64_t nnz = 0;
-    size_t dyn_smem = 0;       // bytes of dynamic shared memory of the cooperative kernels (cp.async staging)
+    size_t dyn_smem = 0;       // bytes of dynamic shared memory of the cooperative kernels (per-warp TMA staging rings)
     std::vector<void *> allocs;
     cs_params prm{};
     bool conditioned = false;  // the l=1 conditioning of step 4 has run
@@ -227,8 +227,8 @@ std::vector<int> order_by_length(const std::vector<int> &len, int n_sort) {
     return perm;
 }
 
-cs_status launch_coop(cs_solver *S, const void *fn, void **args, size_t smem = 0) {
-    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, smem, S->stream));
+cs_status launch_coop(cs_solver *S, const void *fn, void **args) {   // every cooperative kernel carries the staging ring
+    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, S->dyn_smem, S->stream));
     S->launches += 1;
     return CS_OK;
 }
@@ -258,7 +258,7 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     S->ctx.o_floor = S->prm.o_floor;
     sync_params(S);
     void *args[] = {&S->ctx, &use_rule};
-    st = launch_coop(S, (const void *)k_condition, args, S->dyn_smem);
+    st = launch_coop(S, (const void *)k_condition, args);
     if (st != CS_OK) return st;
     S->conditioned = true;
     S->started = true;
@@ -503,14 +503,19 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     // ---- cooperative grid: as many CTAs as can be co-resident
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
-    const void *kernels[] = {(const void *)k_iterate, (const void *)k_condition, (const void *)k_residuals};
-    S->dyn_smem = 0;
+    const void *kernels[] = {(const void *)k_iterate, (const void *)k_condition, (const void *)k_residuals,
+                             (const void *)k_equilibrate, (const void *)k_barrier_probe};
+    S->dyn_smem = kDynSmem;
     for (const void *k : kernels) {
+        if (S->dyn_smem) CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S->dyn_smem));
+        if (const char *cv = getenv("CS_CARVEOUT"))   // experiment switch: shared-memory carve-out in percent (L1 gets the rest)
+            CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(cv)));
         CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, S->dyn_smem));
         occ_min = std::min(occ_min, occ);
     }
     if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
     S->grid = std::min(sms * occ_min, kMaxGrid);
+    if (verbose) fprintf(stderr, "cs_create: %d SMs x %d CTAs of %d threads, %zu B dynamic shared memory\n", sms, occ_min, kBlock, S->dyn_smem);
     if (nnz <= 8192) S->grid = 1;   // tiny problem (config 0): one CTA, barriers are __syncthreads (cs_device.cuh)
     if ((st = dev_zeros(S, &x.bar, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * kMaxGrid)) != CS_OK) return st;
@@ -595,7 +600,7 @@ cs_status cs_iterate(cs_solver *S, int64_t k) {
     sync_params(S);
     long long kk = k;
     void *args[] = {&S->ctx, &kk};
-    if ((st = launch_coop(S, (const void *)k_iterate, args, S->dyn_smem)) != CS_OK) return st;
+    if ((st = launch_coop(S, (const void *)k_iterate, args)) != CS_OK) return st;
     S->xz_stale = true;
     S->started = true;
     S->iter += k;
@@ -608,7 +613,7 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     if (!S->conditioned && (st = do_condition(S, 1)) != CS_OK) return st;
     if ((st = ensure_xz(S)) != CS_OK) return st;
     void *args[] = {&S->ctx};
-    if ((st = launch_coop(S, (const void *)k_residuals, args, S->dyn_smem)) != CS_OK) return st;
+    if ((st = launch_coop(S, (const void *)k_residuals, args)) != CS_OK) return st;
     Scalars h;
     CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
     CS_CUDA(S, cudaMemsetAsync(&S->ctx.sc->cg_hit_max, 0, sizeof(int), S->stream));
@@ -627,7 +632,7 @@ cs_status cs_equilibrate(cs_solver *S, int32_t n_sweeps) {
     if (st != CS_OK) return st;
     int ns = n_sweeps;
     void *args[] = {&S->ctx, &ns};
-    if ((st = launch_coop(S, (const void *)k_equilibrate, args, S->dyn_smem)) != CS_OK) return st;
+    if ((st = launch_coop(S, (const void *)k_equilibrate, args)) != CS_OK) return st;
     return do_condition(S, 0);
 }
 

@@ -5,6 +5,7 @@
 // norms) and its exit test never leave the device.  Citations P:<line> = /root/reference/PAPER.md.
 #pragma once
 #include <cstdint>
+#include <type_traits>
 
 namespace csd {
 
@@ -17,7 +18,25 @@ constexpr int kMaxRed = 8;           // scalars per grid reduction
 constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
 constexpr int kChunk = 1024;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
-constexpr int kRoundK = 8;           // slice rows loaded per batch (8 values + 8 indices + 8 gathers in flight per lane)
+// Build-time alternative, measured and NOT the default (profiles/r01_ncu_notes.md, "TMA-staged stream"): with
+// CS_TMA=1 the matrix stream of every traversal is staged through per-warp shared-memory rings by bulk async
+// copies (cp.async.bulk + mbarrier) instead of ld.global.cs.  Parity-identical; config 4 307 vs 295 us per CG
+// step: the rings take L1 capacity away from the gathers, and below ~90 KB of L1 per SM the gathers collapse
+// (which is why that build uses batches of 4 rows and 2 stages: 48 KB per CTA).
+#ifndef CS_TMA
+#define CS_TMA 0
+#endif
+#ifndef CS_ROUNDK
+#define CS_ROUNDK (CS_TMA ? 4 : 8)
+#endif
+#ifndef CS_STAGES
+#define CS_STAGES 2
+#endif
+constexpr int kRoundK = CS_ROUNDK;   // slice rows per batch (8 values + 8 indices + 8 gathers in flight per lane)
+constexpr int kStages = CS_STAGES;   // per-warp ring of staged batches
+constexpr int kStageVal = kRoundK * 32 * 8, kStageIdx = kRoundK * 32 * 4, kStageBytes = kStageVal + kStageIdx;
+// dynamic shared memory of every cooperative kernel: [warp][stage]{values, indices} then [warp][stage] mbarriers
+constexpr int kDynSmem = CS_TMA ? kWarps * kStages * (kStageBytes + 8) : 0;
 
 // One sparse format (rows of the row-major copy or columns of the column-major copy): a list of SLICES.
 // A slice is 32 lanes x width entries stored [k][lane] (entry k of lane l at off + 32k + l), so that a
@@ -100,6 +119,38 @@ __device__ __forceinline__ double group_reduce(double v) {
     return v;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Bulk asynchronous copies (TMA, cp.async.bulk) global -> shared with mbarrier completion, used by the
+// CS_TMA=1 build only: the matrix stream (values + minor indices of a batch of slice rows) then never enters
+// the LSU/L1TEX pipeline that bounds the gathers, needs no registers while in flight, and one
+// lane issues a whole batch.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ unsigned long long policy_evict_first() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tma_load(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar, unsigned long long pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+// generic-proxy writes to global memory that a later bulk copy will read (the rescaled matrix values)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
 constexpr int kMaxGrid = 32 * 12;    // CTAs of a cooperative launch (148 SMs x 2 = 296 on B200)
 
 // Grid-wide barrier + deterministic all-reduce.
@@ -118,11 +169,25 @@ struct GridCtl {            // per-thread view of the grid barrier state (unifor
     int parity;
     double *partials;               // [2][kMaxRed][gridDim]
     double *smem;                   // [kMaxRed * kWarps]
-    unsigned long long t_last, ns[8];
+    uint32_t ring, mbar, units;     // this warp's staging ring and mbarriers (shared-window addresses); batches consumed so far
+    // phase clock of CTA 0 / thread 0: [0..7] ns per phase, [8] time of the previous lap (shared memory: no registers)
+    __device__ static unsigned long long *clock() { __shared__ unsigned long long ns[9]; return ns; }
     __device__ GridCtl(double *partials_, double *smem_, unsigned int *bar_) : bar(bar_), parity(0), partials(partials_), smem(smem_) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) ns[i] = 0;
-        t_last = now();
+        if (threadIdx.x == 0) for (int i = 0; i < 8; ++i) clock()[i] = 0;
+#if CS_TMA
+        extern __shared__ __align__(128) unsigned char dyn_smem[];
+        const int warp = threadIdx.x >> 5;
+        ring = smem_u32(dyn_smem) + warp * kStages * kStageBytes;
+        mbar = smem_u32(dyn_smem) + kWarps * kStages * kStageBytes + warp * kStages * 8;
+        units = 0;
+        if ((threadIdx.x & 31) == 0) {
+            for (int i = 0; i < kStages; ++i) mbar_init(mbar + 8 * i, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            fence_proxy_async();
+        }
+        __syncthreads();
+#endif
+        if (threadIdx.x == 0) clock()[8] = now();
     }
     __device__ void sync() {
         __syncthreads();
@@ -148,14 +213,14 @@ struct GridCtl {            // per-thread view of the grid barrier state (unifor
     __device__ void lap(int id) {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             const unsigned long long t = now();
-            ns[id] += t - t_last;
-            t_last = t;
+            clock()[id] += t - clock()[8];
+            clock()[8] = t;
         }
     }
     __device__ void flush(Scalars *sc) {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) sc->phase_ns[i] += ns[i];
+            for (int i = 0; i < 8; ++i) sc->phase_ns[i] += clock()[i];
         }
     }
 };
@@ -216,24 +281,83 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
 template <int NV, bool PRISTINE, class Term, class Epi>
 __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
     const int lane = threadIdx.x & 31;
-    const int gwarp = (blockIdx.x * kBlock + threadIdx.x) >> 5;
+    // slice s goes to CTA s mod grid (then round-robin over its warps): every CTA -- hence every SM -- gets the
+    // same number of slices (+-1) of every width class, also in the last, partial round
+    const int gwarp = blockIdx.x + gridDim.x * (threadIdx.x >> 5);
     const int nwarps = (gridDim.x * kBlock) >> 5;
     const double *gval = PRISTINE ? S.val0 : S.val;
     constexpr int UN = NV == 1 ? kRoundK : kRoundK / 2;   // two-operand gathers: half the batch, same registers
     int s = gwarp;
     int4 sl = s < S.n_slice ? __ldg(S.slices + s) : make_int4(0, 0, 0, 0);
-    while (s < S.n_slice) {
+#if CS_TMA
+    // Producer side of this warp's ring: the batches (<= kRoundK rows of one slice) are issued in the order
+    // the loop below consumes them, kStages ahead; lane 0 issues, every lane keeps the (uniform) iterator.
+    int is = s, ioff = sl.x, irem = sl.w;                    // slice, next entry offset, rows left in it
+    while (is < S.n_slice && irem == 0) {
+        is += nwarps;
+        if (is < S.n_slice) { const int4 d = __ldg(S.slices + is); ioff = d.x; irem = d.w; }
+    }
+    auto issue = [&](uint32_t slot) {
+        if (is >= S.n_slice) return;
+        const int rows = min(kRoundK, irem);
+        if (lane == 0) {
+            const uint32_t dst = gc.ring + slot * kStageBytes, mb = gc.mbar + slot * 8;
+            const unsigned long long pol = policy_evict_first();
+            mbar_expect_tx(mb, (uint32_t)rows * 32u * 12u);
+            tma_load(dst, gval + ioff, (uint32_t)rows * 256u, mb, pol);
+            tma_load(dst + kStageVal, S.idx + ioff, (uint32_t)rows * 128u, mb, pol);
+        }
+        ioff += 32 * kRoundK;
+        irem -= kRoundK;
+        while (is < S.n_slice && irem <= 0) {
+            is += nwarps;
+            if (is < S.n_slice) { const int4 d = __ldg(S.slices + is); ioff = d.x; irem = d.w; }
+        }
+    };
+    uint32_t units = gc.units;
+#pragma unroll
+    for (int i = 0; i < kStages; ++i) issue((units + i) % kStages);
+    extern __shared__ __align__(128) unsigned char dyn_smem[];
+    const unsigned char *my_ring = dyn_smem + (threadIdx.x >> 5) * kStages * kStageBytes;
+#endif
+    // The walk is instantiated twice: chunk slices (T = 32, one segment, partial-sum slot) and short-segment slices.
+    auto walk = [&](auto chunk_tag, const int s_end) {
+    constexpr bool CH = decltype(chunk_tag)::value;
+    while (s < s_end) {
         const int sn = s + nwarps;
         const int4 nxt = sn < S.n_slice ? __ldg(S.slices + sn) : make_int4(0, 0, 0, 0);
-        const double *vp = gval + sl.x + lane;
-        const int *ip = S.idx + sl.x + lane;
-        const int lgT = sl.z >> 8, T = 1 << lgT;              // lanes per segment in this slice
+        const int lgT = CH ? 5 : sl.z >> 8, T = 1 << lgT;     // lanes per segment in this slice
         const int seg = sl.y + (lane >> lgT);
         const bool head = (lane >> lgT) < (sl.z & 255) && (lane & (T - 1)) == 0;
+        const int cslot = CH ? __ldg(S.chunk_slot + s) : -1;  // fetched early, like `pre` (warp-uniform address)
         typename Epi::Pre pre = epi.pre(head ? seg : sl.y);
         double acc[NV];
 #pragma unroll
         for (int i = 0; i < NV; ++i) acc[i] = 0.0;
+#if CS_TMA
+        for (int k = 0; k < sl.w; k += kRoundK) {
+            const uint32_t slot = units % kStages;
+            mbar_wait(gc.mbar + slot * 8, (units / kStages) & 1);
+            const double *sv = reinterpret_cast<const double *>(my_ring + slot * kStageBytes) + lane;
+            const int *si = reinterpret_cast<const int *>(my_ring + slot * kStageBytes + kStageVal) + lane;
+#pragma unroll
+            for (int q0 = 0; q0 < kRoundK; q0 += UN) {
+                int j[UN];
+#pragma unroll
+                for (int q = 0; q < UN; ++q) j[q] = k + q0 + q < sl.w ? si[32 * (q0 + q)] : -1;
+                typename Term::G g[UN];
+#pragma unroll
+                for (int q = 0; q < UN; ++q) g[q] = term.fetch(j[q] >= 0 ? j[q] : 0);   // index 0: one broadcast wavefront
+#pragma unroll
+                for (int q = 0; q < UN; ++q) if (j[q] >= 0) term.fma(sv[32 * (q0 + q)], g[q], acc);
+            }
+            __syncwarp();                                    // every lane has consumed the stage
+            issue(slot);
+            ++units;
+        }
+#else
+        const double *vp = gval + sl.x + lane;
+        const int *ip = S.idx + sl.x + lane;
         for (int k = 0; k < sl.w; k += UN) {
             double a[UN]; int j[UN];
 #pragma unroll
@@ -248,21 +372,32 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
 #pragma unroll
             for (int q = 0; q < UN; ++q) if (j[q] >= 0) term.fma(a[q], g[q], acc);
         }
-        for (int o = T >> 1; o > 0; o >>= 1) {
+#endif
+        if (CH) {
 #pragma unroll
-            for (int i = 0; i < NV; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
+            for (int i = 0; i < NV; ++i) acc[i] = group_reduce<32>(acc[i]);
+        } else {
+            for (int o = T >> 1; o > 0; o >>= 1) {
+#pragma unroll
+                for (int i = 0; i < NV; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
+            }
         }
         if (head) {
-            const int slot = s < S.n_chunk ? __ldg(S.chunk_slot + s) : -1;
-            if (slot < 0) epi(seg, acc, pre);
+            if (cslot < 0) epi(seg, acc, pre);
             else {
 #pragma unroll
-                for (int i = 0; i < NV; ++i) S.partial[(size_t)slot * 2 + i] = acc[i];
+                for (int i = 0; i < NV; ++i) S.partial[(size_t)cslot * 2 + i] = acc[i];
             }
         }
         s = sn;
         sl = nxt;
     }
+    };
+    walk(std::true_type{}, S.n_chunk);
+    walk(std::false_type{}, S.n_slice);
+#if CS_TMA
+    gc.units = units;
+#endif
     if (S.n_multi) {
         gc.sync();
         for (int r = gwarp; r < S.n_multi; r += nwarps) {
@@ -302,6 +437,9 @@ __device__ __forceinline__ void seg_rescale(const Sparse &S, F &f) {
             for (int k = 0; k < sl.w; ++k) S.val[base + 32 * k] = f(seg, S.val0[base + 32 * k], __ldg(S.idx + base + 32 * k));
         }
     }
+#if CS_TMA
+    fence_proxy_async();   // the next reader of S.val is a bulk async copy (after a grid barrier)
+#endif
 }
 
 }  // namespace csd
