@@ -298,7 +298,7 @@ def main():
     ncu_ratio = {3: 0.826, 4: 0.956 if fsai_on else 0.912}.get(a.config if a.scale == 1.0 else -1)
     roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "traffic": ncu_ratio * it_bytes / a.steps if ncu_ratio else None,
-            "traffic_source": "profiles/r01_ncu_notes.md (v6/v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
+            "traffic_source": "profiles/r01_ncu_notes.md (v7/v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
                               "launch, applied to this launch)" if ncu_ratio else None,
             "peak_source": peak_src,
             "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
