@@ -191,7 +191,10 @@ def main():
         line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": a.gpus,
                 "steps": a.steps, "warmup": a.warmup, "ms_per_step": 1e3 * dt / max(1, a.steps),
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": f"cfg{a.config}"}, "cpu_baseline": base,
+                "config": {"workload": {0: "cfg0_tiny_lp", 1: "cfg1_sparse_lp", 2: "cfg2_illcond_lp", 3: "cfg3_sparse_socp",
+                                        4: "cfg4_zipf_lp"}[a.config] + (f"_x{a.scale:g}" if a.config else ""),
+                           "k_per_step": a.k, "step": "cs_condition + cs_iterate(k) + cs_residuals",
+                           "sample": base["sample"]}, "cpu_baseline": base,
                 "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
         print(json.dumps(line))
         return 0

@@ -12,7 +12,10 @@ namespace csd {
 #ifndef CS_MINB
 #define CS_MINB 2
 #endif
-constexpr int kBlock = 512;          // threads per CTA (16 warps)
+#ifndef CS_BLOCK
+#define CS_BLOCK 512
+#endif
+constexpr int kBlock = CS_BLOCK;          // threads per CTA (16 warps)
 constexpr int kWarps = kBlock / 32;
 constexpr int kMaxRed = 8;           // scalars per grid reduction
 constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
