@@ -73,12 +73,20 @@ typedef struct {
  *            t >= 4, i.e. when a conditioning may spread O^2 over many decades), 1 = none, 2 = FSAI(1): a sparse
  *            approximate inverse factor with one off-diagonal entry per row, rebuilt on the device at every
  *            conditioning.  Changes the number of CG steps, not the solution of the solve.
- * cs_set_params may be called at any time; mu, t, o_floor, precond take effect at the next cs_condition
- * (or at the implicit first conditioning), cg_* at the next solve. */
+ *   dense_m_threshold  dense factor-apply instead of CG where A is small enough that the solve truly is a dense
+ *            contraction (B north_star; S 8(a) a3): when the problem runs on one CTA (nnz <= 8192) and
+ *            m <= dense_m_threshold (<= 256), every conditioning forms A~A~' (m x m, fp64), factors it by
+ *            Cholesky on the device, and every pass applies the factor (two triangular solves + one step of
+ *            iterative refinement) -- no CG steps are counted.  0 = never; default 128.  A non-positive pivot
+ *            (rank-deficient A) falls back to CG for that scaling.
+ * cs_set_params may be called at any time; mu, t, o_floor, precond, dense_m_threshold take effect at the next
+ * cs_condition (or at the implicit first conditioning), cg_* at the next solve. */
 typedef struct {
     double mu, t, o_floor, cg_tol;
     int32_t cg_max_iter;
     int32_t precond;
+    int32_t dense_m_threshold;
+    int32_t reserved;
 } cs_params;
 
 /* Residuals of the KKT conditions (24) P:480-487 in ORIGINAL coordinates, for the current iterate

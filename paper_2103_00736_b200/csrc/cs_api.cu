@@ -252,7 +252,8 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     if (st != CS_OK) return st;
     // automatic: FSAI(1) pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs);
     // with the SOCP setting t = 1.7 it saves ~10 % of the CG steps and costs 18 % per step (measured)
-    S->ctx.fsai = S->prm.precond == 2 || (S->prm.precond == 0 && S->prm.t >= 4.0);
+    S->ctx.dense = S->grid == 1 && S->ctx.dM && S->ctx.m <= S->prm.dense_m_threshold;
+    S->ctx.fsai = !S->ctx.dense && (S->prm.precond == 2 || (S->prm.precond == 0 && S->prm.t >= 4.0));
     S->ctx.mu = S->prm.mu;  // mu, t, o_floor, precond take effect here (cs.h)
     S->ctx.t = S->prm.t;
     S->ctx.o_floor = S->prm.o_floor;
@@ -517,6 +518,11 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->grid = std::min(sms * occ_min, kMaxGrid);
     if (verbose) fprintf(stderr, "cs_create: %d SMs x %d CTAs of %d threads, %zu B dynamic shared memory\n", sms, occ_min, kBlock, S->dyn_smem);
     if (nnz <= 8192) S->grid = 1;   // tiny problem (config 0): one CTA, barriers are __syncthreads (cs_device.cuh)
+    if (S->grid == 1 && m <= kDenseMax) {   // scratch of the dense factor-apply path (cs_params.dense_m_threshold)
+        if ((st = dev_zeros(S, &x.dM, (size_t)m * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.dMd, (size_t)m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.dv, (size_t)2 * m)) != CS_OK) return st;
+    }
     if ((st = dev_zeros(S, &x.bar, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * kMaxGrid)) != CS_OK) return st;
     // ---- defaults (cs.h)
@@ -526,6 +532,8 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.cg_tol = 1e-15;
     S->prm.cg_max_iter = 20000;
     S->prm.precond = 0;
+    S->prm.dense_m_threshold = 128;
+    S->prm.reserved = 0;
     S->nnz = nnz;
     x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
     sync_params(S);
@@ -556,8 +564,8 @@ cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const dou
 cs_status cs_set_params(cs_solver *S, const cs_params *p) {
     if (!S || !p) return CS_EINVAL;
     if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || p->cg_max_iter < 1 ||
-        p->precond < 0 || p->precond > 2) {
-        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, cg_max_iter >= 1, precond in {0,1,2}";
+        p->precond < 0 || p->precond > 2 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseMax) {
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, cg_max_iter >= 1, precond in {0,1,2}, dense_m_threshold in [0,256]";
         return CS_EINVAL;
     }
     S->prm = *p;

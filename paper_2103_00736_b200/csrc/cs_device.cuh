@@ -21,6 +21,7 @@ constexpr int kMaxRed = 8;           // scalars per grid reduction
 constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
 constexpr int kChunk = 1024;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
+constexpr int kDenseMax = 256;       // largest m of the dense factor-apply path (cs_params.dense_m_threshold)
 // Build-time alternative, measured and NOT the default (profiles/r01_ncu_notes.md, "TMA-staged stream"): with
 // CS_TMA=1 the matrix stream of every traversal is staged through per-warp shared-memory rings by bulk async
 // copies (cp.async.bulk + mbarrier) instead of ld.global.cs.  Parity-identical; config 4 307 vs 295 us per CG
@@ -73,7 +74,7 @@ struct Csr {
 struct Scalars {            // device-resident state scalars (read back only by cs_residuals)
     double resid[16];
     long long iter, cg_steps_total, cg_steps_cond;
-    int cg_steps_last, n_cond, cg_hit_max, pad;
+    int cg_steps_last, n_cond, cg_hit_max, dense_ok;   // dense_ok: the Cholesky factor of the current scaling is usable
     double fp_res2;         // ||s_new - s||^2 of the last pass
     unsigned long long phase_ns[8];  // time spent per phase id (kPh*), measured by CTA 0 between grid barriers
 };
@@ -94,6 +95,11 @@ struct Ctx {
     double *f_gd, *f_gm;    // [m] during the build: g_ii and g_{i,partner}; afterwards the diagonal dd and the partner entry ee of G'G
     double *f_tc;           // [m] coefficients of the transposed-list entries of G'G
     double *z, *t1;         // [m] preconditioned residual; build scratch
+    // dense factor-apply path (one-CTA problems with m <= dense_m_threshold, cs.h)
+    int dense;              // 0: off
+    double *dM;             // [m][m] row-major: lower triangle incl. diagonal = Cholesky factor L, strict upper = A~A~'
+    double *dMd;            // [m] diagonal of A~A~'
+    double *dv;             // [2m] scratch of the triangular solves
     // n-vectors
     double *s, *p, *g, *e, *u, *chat, *O, *xb, *zb;
     const double *c;

@@ -134,6 +134,85 @@ __device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
     return red[0];
 }
 
+// ---------------------------------------------------------------------------------------------
+// Dense factor-apply path (cs_params.dense_m_threshold): one CTA, M = A~A~' in c.dM.
+// dense_factor: M from the two compressed views (thread i owns row i: fixed summation order), then an in-place
+// right-looking Cholesky on the lower triangle; the strict upper triangle and c.dMd keep M for the refinement.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void dense_factor(const Ctx &c) {
+    const int m = c.m;
+    double *M = c.dM;
+    for (int i = threadIdx.x; i < m; i += kBlock) {
+        double *row = M + (size_t)i * m;
+        for (int j = 0; j < m; ++j) row[j] = 0.0;
+        for (int e = c.Rc.ptr[i]; e < c.Rc.ptr[i + 1]; ++e) {
+            const int k = c.Rc.idx[e];
+            const double a = c.R.val[c.Rc.pos[e]];
+            for (int f = c.Cc.ptr[k]; f < c.Cc.ptr[k + 1]; ++f) row[c.Cc.idx[f]] += a * c.C.val[c.Cc.pos[f]];
+        }
+        c.dMd[i] = row[i];
+    }
+    bool ok = true;
+    for (int k = 0; k < m; ++k) {
+        __syncthreads();
+        const double piv = M[(size_t)k * m + k];
+        if (!(piv > 0.0)) { ok = false; break; }              // uniform: every thread reads the same pivot
+        const double d = sqrt(piv);
+        __syncthreads();
+        if (threadIdx.x == 0) M[(size_t)k * m + k] = d;
+        for (int i = k + 1 + threadIdx.x; i < m; i += kBlock) M[(size_t)i * m + k] /= d;
+        __syncthreads();
+        const int t = m - k - 1;                              // trailing (i, j), k < j <= i < m
+        for (int q = threadIdx.x; q < t * t; q += kBlock) {
+            const int i = k + 1 + q / t, j = k + 1 + q % t;
+            if (j <= i) M[(size_t)i * m + j] -= M[(size_t)i * m + k] * M[(size_t)j * m + k];
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) c.sc->dense_ok = ok ? 1 : 0;
+}
+
+// x <- L^-T L^-1 x on one warp (x in global scratch, m <= 256; every lane computes the same pivots)
+__device__ __forceinline__ void dense_llt_solve(const double *M, int m, double *x, int lane) {
+    for (int k = 0; k < m; ++k) {                             // forward: L y = x
+        __syncwarp();
+        const double yk = x[k] / M[(size_t)k * m + k];
+        __syncwarp();
+        if (lane == 0) x[k] = yk;
+        for (int i = k + 1 + lane; i < m; i += 32) x[i] -= M[(size_t)i * m + k] * yk;
+    }
+    for (int k = m - 1; k >= 0; --k) {                        // backward: L' w = y (row k of L = column k of L')
+        __syncwarp();
+        const double wk = x[k] / M[(size_t)k * m + k];
+        __syncwarp();
+        if (lane == 0) x[k] = wk;
+        for (int i = lane; i < k; i += 32) x[i] -= M[(size_t)k * m + i] * wk;
+    }
+    __syncwarp();
+}
+
+// w += M^-1 r with one step of iterative refinement against the stored M (r = residual of the warm start w)
+__device__ __forceinline__ void dense_solve(const Ctx &c) {
+    const int m = c.m, lane = threadIdx.x & 31;
+    double *d1 = c.dv, *d2 = c.dv + m;
+    if (threadIdx.x < 32) {
+        for (int i = lane; i < m; i += 32) d1[i] = c.r[i];
+        dense_llt_solve(c.dM, m, d1, lane);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < m; i += kBlock) {           // r2 = r - M d1
+        double a = c.dMd[i] * d1[i];
+        for (int j = 0; j < i; ++j) a += c.dM[(size_t)j * m + i] * d1[j];
+        for (int j = i + 1; j < m; ++j) a += c.dM[(size_t)i * m + j] * d1[j];
+        d2[i] = c.r[i] - a;
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) dense_llt_solve(c.dM, m, d2, lane);
+    __syncthreads();
+    for (int i = threadIdx.x; i < m; i += kBlock) c.w[i] += d1[i] + d2[i];
+    __syncthreads();
+}
+
 __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, double qq, bool &hit_max) {
     const double thresh = c.cg_tol * c.cg_tol * qq;       // stop on ||r|| <= cg_tol ||q|| (equilibrated system)
     const double *zsrc = c.fsai ? c.z : c.r;
@@ -227,7 +306,8 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_iterate(Ctx c, long long k_
         grid_reduce<2>(red, gc);
         gc.lap(kPhReduce);
         bool hm;
-        cg_last = cg_solve(c, gc, red[1], red[0], hm);           // w = (A~A~')^{-1} (b~ - A~(p - mu c^)) = w_d - w_p
+        if (c.dense && c.sc->dense_ok) { dense_solve(c); cg_last = 0; hm = false; }   // dense factor-apply (one CTA)
+        else cg_last = cg_solve(c, gc, red[1], red[0], hm);      // w = (A~A~')^{-1} (b~ - A~(p - mu c^)) = w_d - w_p
         any_max |= hm;
         cg_total += cg_last;
         TermDot tw{c.w};

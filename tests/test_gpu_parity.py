@@ -373,6 +373,47 @@ def test_preconditioner_changes_the_steps_not_the_iterates(name):
         S.set_params(precond=3)
 
 
+@pytest.mark.parametrize("name", ["cfg0", "tiny_socp", "sec4a_gaussian"])
+def test_dense_factor_apply_matches_cg_and_oracle(name):
+    """cs_params.dense_m_threshold (S 8(a) a3, B north_star "dense factor-apply kernel only where A is small enough"):
+    one-CTA problems solve with a device-side Cholesky factor of A~A~' instead of CG.  Same passes incl. two
+    conditionings: dense path (no CG steps counted) and CG path both within 1e-9 of the oracle (whose small-m
+    solve is a dense Cholesky too) and of each other."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = {"cfg0": lambda: W.config(0),
+         "tiny_socp": lambda: W.sparse_socp(5, 40, 110, 12, 5, n_lin=30, lo=2, hi=12),
+         "sec4a_gaussian": lambda: W.gaussian_dense_lp(3)}[name]()
+    assert p.nnz <= 8192 and p.m <= 128
+    L = [20]
+    O = oracle.Oracle.from_problem(p)
+    O.run(60, L=L)
+    ref, sols = O.get(), {}
+    for thr in (128, 0):
+        S = binding.Solver.from_problem(p, device="cuda:0")
+        S.set_params(dense_m_threshold=thr)
+        assert S.get_params()["dense_m_threshold"] == thr
+        S.run(60, L=L)
+        sols[thr], r = S.solution(), S.residuals()
+        assert (r["cg_steps_total"] == 0) == (thr > 0), (thr, r["cg_steps_total"])
+        for key in ("x", "z", "y"):
+            assert rel(sols[thr][key], ref[key]) <= 1e-6, (thr, key, rel(sols[thr][key], ref[key]))   # protocol (ii-b)
+        q = O.residuals()
+        for k in ("kkt_rel", "pres_abs", "dres_abs"):
+            assert abs(r[k] - q[k]) <= TOL_RES * abs(q[k]) + 1e-11, (thr, k, r[k], q[k])
+        S.destroy()
+    # no conditioning inside the run: protocol (i), 1e-9 against the oracle
+    O = oracle.Oracle.from_problem(p)
+    O.run(80)
+    S = binding.Solver.from_problem(p, device="cuda:0")
+    S.iterate(80)
+    assert S.residuals()["cg_steps_total"] == 0
+    _check_iterates(S, O)
+    _check_resid(S, O)
+    with pytest.raises(binding.CsError):
+        S.set_params(dense_m_threshold=257)
+
+
 # ------------------------------------------------------------------ S 8(f) rows 2, 3: schedules, fixed equilibration
 @pytest.mark.parametrize("name", ["lp_scaled", "mixed_cones", "cfg4_zipf"])
 def test_equilibrate_matches_oracle_ruiz(name):
