@@ -504,7 +504,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     // ---- cooperative grid: as many CTAs as can be co-resident
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
-    const void *kernels[] = {(const void *)k_iterate, (const void *)k_condition, (const void *)k_residuals,
+    const void *kernels[] = {(const void *)k_iterate, (const void *)k_iterate_dense, (const void *)k_condition, (const void *)k_residuals,
                              (const void *)k_equilibrate, (const void *)k_barrier_probe};
     S->dyn_smem = kDynSmem;
     for (const void *k : kernels) {
@@ -608,7 +608,7 @@ cs_status cs_iterate(cs_solver *S, int64_t k) {
     sync_params(S);
     long long kk = k;
     void *args[] = {&S->ctx, &kk};
-    if ((st = launch_coop(S, (const void *)k_iterate, args)) != CS_OK) return st;
+    if ((st = launch_coop(S, S->ctx.dense ? (const void *)k_iterate_dense : (const void *)k_iterate, args)) != CS_OK) return st;
     S->xz_stale = true;
     S->started = true;
     S->iter += k;

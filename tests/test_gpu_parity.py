@@ -521,7 +521,10 @@ def test_section4a_three_schedules_on_the_device(seed):
         O.run(k, L=L)
         r, q = S.residuals(), O.residuals()
         assert abs(r["pobj"] - q["pobj"]) <= TOL_RES * (1 + abs(q["pobj"])), name
-        assert abs(r["pres_abs"] - q["pres_abs"]) <= 1e-5 * q["pres_abs"] + 1e-9, name
+        # A converged run sits on the rounding floor of its affine projection, eps * cond(A^ A^') * ||b|| (O^2 spans up
+        # to e^(2t) = 1e8 here); below 1e-10 (1 + ||b||) the two solves (device: dense factor + refinement; oracle:
+        # dense Cholesky) have no common digits to compare.
+        assert abs(r["pres_abs"] - q["pres_abs"]) <= 1e-5 * q["pres_abs"] + 1e-10 * (1 + np.linalg.norm(p.b)), name
         if not L:       # with in-run conditionings of a run still in flight only protocol (iii) applies
             _check_iterates(S, O, keys=("x", "z"))
         pres[name] = r["pres_abs"]
