@@ -68,6 +68,11 @@ typedef struct {
  *   o_floor  absolute floor of numerator and denominator of o_i in step 7 (paper silent on 0/0)
  *   cg_tol   inner solve stops when ||residual||_2 <= cg_tol * ||rhs||_2, both measured on the
  *            row-equilibrated system (D A_hat)(D A_hat)' with D = diag(1/||row_i(A_hat)||_2)
+ *   cg_reduce    inexact projections (0 = off, the default): the solve of a pass also stops once the residual of
+ *            the WARM START has been reduced by this factor, ||residual||_2 <= max(cg_tol ||rhs||_2,
+ *            cg_reduce ||residual at the warm start||_2).  The warm-start residual shrinks as the outer iteration
+ *            converges (w converges to mu D^{-1} y), so the projection error shrinks with it -- an adaptive
+ *            tolerance with the fixed point unchanged; 0 < cg_reduce < 1.
  *   cg_max_iter  cap on CG steps per solve
  *   precond  preconditioner of the inner CG beyond the Jacobi row equilibration: 0 = automatic (FSAI(1) when
  *            t >= 4, i.e. when a conditioning may spread O^2 over many decades), 1 = none, 2 = FSAI(1): a sparse
@@ -82,7 +87,7 @@ typedef struct {
  * cs_set_params may be called at any time; mu, t, o_floor, precond, dense_m_threshold take effect at the next
  * cs_condition (or at the implicit first conditioning), cg_* at the next solve. */
 typedef struct {
-    double mu, t, o_floor, cg_tol;
+    double mu, t, o_floor, cg_tol, cg_reduce;
     int32_t cg_max_iter;
     int32_t precond;
     int32_t dense_m_threshold;

@@ -30,7 +30,7 @@ class cs_cones(C.Structure):
 
 class cs_params(C.Structure):
     _fields_ = [("mu", C.c_double), ("t", C.c_double), ("o_floor", C.c_double), ("cg_tol", C.c_double),
-                ("cg_max_iter", C.c_int32), ("precond", C.c_int32),
+                ("cg_reduce", C.c_double), ("cg_max_iter", C.c_int32), ("precond", C.c_int32),
                 ("dense_m_threshold", C.c_int32), ("reserved", C.c_int32)]
 
 
@@ -191,7 +191,8 @@ class Solver:
         if unknown:
             raise TypeError(f"unknown parameter(s): {sorted(unknown)}")
         cur.update(kw)
-        p = cs_params(cur["mu"], cur["t"], cur["o_floor"], cur["cg_tol"], int(cur["cg_max_iter"]), int(cur["precond"]),
+        p = cs_params(cur["mu"], cur["t"], cur["o_floor"], cur["cg_tol"], cur["cg_reduce"], int(cur["cg_max_iter"]),
+                      int(cur["precond"]),
                       int(cur["dense_m_threshold"]), 0)
         self._check(lib().cs_set_params(self._h, C.byref(p)))
 

@@ -244,6 +244,7 @@ cs_status ensure_xz(cs_solver *S) {
 
 void sync_params(cs_solver *S) {
     S->ctx.cg_tol = S->prm.cg_tol;
+    S->ctx.cg_reduce = S->prm.cg_reduce;
     S->ctx.cg_max_iter = S->prm.cg_max_iter;
 }
 
@@ -530,6 +531,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
     S->prm.o_floor = 1e-16;
     S->prm.cg_tol = 1e-15;
+    S->prm.cg_reduce = 0.0;
     S->prm.cg_max_iter = 20000;
     S->prm.precond = 0;
     S->prm.dense_m_threshold = 128;
@@ -563,9 +565,9 @@ cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const dou
 
 cs_status cs_set_params(cs_solver *S, const cs_params *p) {
     if (!S || !p) return CS_EINVAL;
-    if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || p->cg_max_iter < 1 ||
+    if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || !(p->cg_reduce >= 0.0 && p->cg_reduce < 1.0) || p->cg_max_iter < 1 ||
         p->precond < 0 || p->precond > 2 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseMax) {
-        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, cg_max_iter >= 1, precond in {0,1,2}, dense_m_threshold in [0,256]";
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2}, dense_m_threshold in [0,256]";
         return CS_EINVAL;
     }
     S->prm = *p;

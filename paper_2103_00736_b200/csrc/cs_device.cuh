@@ -110,7 +110,7 @@ struct Ctx {
     unsigned int *bar;      // grid-barrier word
     Scalars *sc;
     double *partial_probe;  // scratch of cs_barrier_probe
-    double mu, t, o_floor, cg_tol;
+    double mu, t, o_floor, cg_tol, cg_reduce;
     int cg_max_iter;
     double norm_b, norm_c;
 };

@@ -214,7 +214,8 @@ __device__ __forceinline__ void dense_solve(const Ctx &c) {
 }
 
 __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, double qq, bool &hit_max) {
-    const double thresh = c.cg_tol * c.cg_tol * qq;       // stop on ||r|| <= cg_tol ||q|| (equilibrated system)
+    // stop on ||r|| <= max(cg_tol ||q||, cg_reduce ||r at the warm start||) (equilibrated system; cs.h)
+    const double thresh = fmax(c.cg_tol * c.cg_tol * qq, c.cg_reduce * c.cg_reduce * rr);
     const double *zsrc = c.fsai ? c.z : c.r;
     double beta = 0.0;
     int steps = 0;

@@ -24,7 +24,7 @@ def test_library_exports_every_declared_symbol():
         assert getattr(lib, name) is not None, name
     assert declared == set(binding.EXPORTS)
     # struct layouts agree with the header (sizes the C side would compute)
-    assert ctypes.sizeof(binding.cs_params) == 48
+    assert ctypes.sizeof(binding.cs_params) == 56
     assert ctypes.sizeof(binding.cs_resid) == 3 * 8 + 4 * 4 + 11 * 8
     assert ctypes.sizeof(binding.cs_csr) == 56 and ctypes.sizeof(binding.cs_cones) == 24
 

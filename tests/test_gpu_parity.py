@@ -144,6 +144,42 @@ def test_inexact_projections_reach_the_same_optimum():
     assert r["cg_steps_total"] > 0
 
 
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_adaptive_inexact_projections_cg_reduce(cfg):
+    """cs_params.cg_reduce: the solve of a pass stops once the warm-start residual has dropped by that factor.  Same
+    fixed point as the exact run for a fraction of the CG steps: objective (against the exact device run, the
+    constructed optimum and, on the LP, the oracle), unique dual solution, comparable KKT residual; invalid values
+    are rejected."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = W.config(cfg, 0.05)
+    k = 1500
+    L = p.schedule(k)
+    S = binding.Solver.from_problem(p, device="cuda:0")
+    S.run(k, L=L)
+    exact = S.residuals()
+    S.destroy()
+    S = binding.Solver.from_problem(p, device="cuda:0")
+    S.set_params(cg_reduce=0.2, cg_tol=1e-12)
+    assert S.get_params()["cg_reduce"] == 0.2
+    S.run(k, L=L)
+    r, got = S.residuals(), S.solution()
+    assert exact["kkt_rel"] <= 1e-3 and r["kkt_rel"] <= 2 * exact["kkt_rel"] + 1e-5, (r["kkt_rel"], exact["kkt_rel"])
+    refs = [exact["pobj"], p.opt_value()]
+    if cfg == 1:
+        O = oracle.Oracle.from_problem(p)
+        O.run(k, L=L)
+        refs.append(O.residuals()["pobj"])
+        assert r["kkt_rel"] <= 1e-4
+    for ref in refs:
+        assert abs(r["pobj"] - ref) <= 10 * r["kkt_rel"] * (1 + abs(ref)), (r["pobj"], ref)
+    assert rel(got["z"], p.s0) <= 100 * r["kkt_rel"] and rel(got["y"], p.y0) <= 100 * r["kkt_rel"]
+    assert r["cg_steps_total"] < 0.5 * exact["cg_steps_total"], (r["cg_steps_total"], exact["cg_steps_total"])
+    for bad in (1.0, -0.1):
+        with pytest.raises(binding.CsError):
+            S.set_params(cg_reduce=bad)
+
+
 def test_production_schedule_objective_and_kkt():
     """Protocol (iii): the paper's schedule L={300,400,...} (eq.(17)); objective and KKT terms to 1e-6."""
     p = W.config(1, 0.02)
