@@ -116,9 +116,9 @@ typedef struct {
 
 /* Build a solver for (A,b,c,K): validates the input, copies it to the device, builds the CSC copy of A
  * and the work partitions.  b[m], c[n] live in `vec_where`.  Parameters start at mu=1, t=9.2 (n_soc=0)
- * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-15, cg_max_iter=20000; the starting point is x=z=e_K
- * (1 on each cone's first coordinate), which makes the mandatory first conditioning (l=1) the
- * identity and s=0.  Synchronous.  On failure *out is NULL. */
+ * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-15, cg_reduce=0, cg_max_iter=20000, precond=0,
+ * dense_m_threshold=128; the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
+ * mandatory first conditioning (l=1) the identity and s=0.  Synchronous.  On failure *out is NULL. */
 cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
                     const cs_cones *K, void *cuda_stream);
 
