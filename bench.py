@@ -349,12 +349,16 @@ def secondary_workload(cfg, a, dev, stream, peak):
     it_bytes, cg_bytes = algorithmic_bytes(p, steps * a.k, cg_iter, 0, p.t >= 4.0)
     achieved = it_bytes / (ms_iter * 1e-3) / 1e9
     us_g, _ = binding.gather_probe(p.n, p.nnz)
+    ph = S.phase_times()       # device time per phase over the whole life of the handle (warm-up included), ns
+    cg_all = max(1, r1["cg_steps_total"] - r1["cg_steps_cond"])
+    phases = {k + "_us_per_cg": ph[k] / cg_all / 1e3 for k in ("K1", "K2", "reduce", "precond")}
     out = {"workload": p.name, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "value": steps * a.k / dt, "unit": UNIT,
            "steps": steps, "k_per_step": a.k, "cg_steps_per_iter": cg_iter / (steps * a.k),
            "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "bytes_per_cg_step": cg_bytes,
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                         "note": "the 96 MB of matrix copies partly stay in the 126 MB L2"},
-           "gather_ceiling_frac": (2 * p.nnz * cg_iter / (ms_iter * 1e-3)) / (p.nnz / (us_g * 1e-6)), "kkt_rel": r1["kkt_rel"]}
+           "gather_ceiling_frac": (2 * p.nnz * cg_iter / (ms_iter * 1e-3)) / (p.nnz / (us_g * 1e-6)), "phases": phases,
+           "kkt_rel": r1["kkt_rel"]}
     S.destroy()
     return out
 
