@@ -457,7 +457,20 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
             hc2 = make_sparse(cp2, ri2, cv2, std::max(1, nt / 2));
         });
         hr = make_sparse(rp2, ci2, va2, std::max(1, nt / 2));
+        // the row-major copy goes to the device while the other thread is still building the column-major one
+        cs_status su = CS_OK;
+        if (hr.val.size() < (size_t)INT32_MAX) {
+            int *q;
+            if ((su = upload_sparse(S, hr, &S->ctx.R)) == CS_OK && (su = dev_upload(S, &q, rp2.data(), rp2.size())) == CS_OK) {
+                S->ctx.Rc.ptr = q;
+                if ((su = dev_upload(S, &q, ci2.data(), ci2.size())) == CS_OK) {
+                    S->ctx.Rc.idx = q;
+                    if ((su = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) == CS_OK) S->ctx.Rc.pos = q;
+                }
+            }
+        }
         tc.join();
+        if (su != CS_OK) return su;
     }
     lap("column-major copy + slices");
     if (hr.val.size() >= (size_t)INT32_MAX || hc2.val.size() >= (size_t)INT32_MAX) {
@@ -479,13 +492,9 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_upload(S, &ip, cone_off.data(), cone_off.size())) != CS_OK) return st; x.cone_off = ip;
     if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
     if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
-    if ((st = upload_sparse(S, hr, &x.R)) != CS_OK) return st;
-    if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;
-    {   // plain compressed views of the same entries (used only to build the FSAI preconditioner)
+    if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;      // x.R and x.Rc went up above
+    {   // plain compressed views of the same entries (the FSAI build and the dense factor path walk them)
         int *q;
-        if ((st = dev_upload(S, &q, rp2.data(), rp2.size())) != CS_OK) return st; x.Rc.ptr = q;
-        if ((st = dev_upload(S, &q, ci2.data(), ci2.size())) != CS_OK) return st; x.Rc.idx = q;
-        if ((st = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) != CS_OK) return st; x.Rc.pos = q;
         if ((st = dev_upload(S, &q, cp2.data(), cp2.size())) != CS_OK) return st; x.Cc.ptr = q;
         if ((st = dev_upload(S, &q, ri2.data(), ri2.size())) != CS_OK) return st; x.Cc.idx = q;
         if ((st = dev_upload(S, &q, hc2.pos.data(), hc2.pos.size())) != CS_OK) return st; x.Cc.pos = q;
