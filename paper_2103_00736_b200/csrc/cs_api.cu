@@ -10,9 +10,11 @@
 #include <cstring>
 #include <chrono>
 #include <cstdlib>
+#include <memory>
 #include <new>
 #include <string>
 #include <thread>
+#include <utility>
 #include <vector>
 
 #include "../../include/cs.h"
@@ -87,13 +89,27 @@ cs_status fetch(cs_solver *S, std::vector<T> &dst, const T *src, size_t count, c
     return CS_OK;
 }
 
+// std::vector without value-initialisation: the big host arrays (hundreds of MB each) are written once, in parallel,
+// by the code that fills them -- a serial zero-fill (and its page faults) would cost more than the fill itself.
+template <class T>
+struct NoInit : std::allocator<T> {
+    template <class U> struct rebind { using other = NoInit<U>; };
+    template <class U, class... Args>
+    void construct(U *p, Args &&...args) {
+        if constexpr (sizeof...(Args) == 0) ::new ((void *)p) U;
+        else ::new ((void *)p) U(std::forward<Args>(args)...);
+    }
+};
+template <class T> using uvec = std::vector<T, NoInit<T>>;
+
 // Host image of one Sparse (cs_device.cuh): chunk slices of the long segments first, then the slices of
 // the short ones, all in one pair of arrays.
 struct HostSparse {
     std::vector<int4> slices, multi;
-    std::vector<int> chunk_slot, idx;
-    std::vector<int> pos;         // compressed entry -> position in val/idx (for the plain compressed view, Csr in cs_device.cuh)
-    std::vector<double> val;
+    std::vector<int> chunk_slot;
+    uvec<int> idx;
+    uvec<int> pos;                // compressed entry -> position in val/idx (for the plain compressed view, Csr in cs_device.cuh)
+    uvec<double> val;
     int n_chunk = 0, n_slots = 0;
 };
 
@@ -113,7 +129,7 @@ int host_threads() { return (int)std::max(1u, std::min(16u, std::thread::hardwar
 
 // ptr/idx/val: compressed segments in INTERNAL numbering (segment s = entries [ptr[s], ptr[s+1])).
 // Two phases: a serial plan (slice descriptors and offsets, O(#segments)), then a parallel fill.
-HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx, const std::vector<double> &val, int nt) {
+HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const uvec<double> &val, int nt) {
     HostSparse h;
     const int nseg = (int)ptr.size() - 1;
     // several lanes per segment only pay when there are too few segments to fill the machine (measured:
@@ -162,9 +178,9 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
     }
     plan_run(run, nseg);
     // fill (padding: val = 0, a valid index replicated)
-    h.val.assign(total, 0.0);
-    h.idx.assign(total, 0);
-    h.pos.assign(idx.size(), 0);
+    h.val.resize(total);          // no zero-fill: the fill below writes every slot (padding values = 0)
+    h.idx.resize(total);
+    h.pos.resize(idx.size());
     const int n_slice = (int)h.slices.size(), blk = 512;
     parallel_blocks((n_slice + blk - 1) / blk, nt, [&](int bi) {
         for (int si = bi * blk; si < std::min(n_slice, (bi + 1) * blk); ++si) {
@@ -175,7 +191,8 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 const int a = chunk_src[si], clen = std::min(kChunk, ptr[sl.y + 1] - a);
                 for (int e = 0; e < 32 * width; ++e) {
                     h.idx[off + e] = idx[a + std::min(e, clen - 1)];
-                    if (e < clen) { h.val[off + e] = val[a + e]; h.pos[a + e] = (int)(off + e); }
+                    h.val[off + e] = e < clen ? val[a + e] : 0.0;
+                    if (e < clen) h.pos[a + e] = (int)(off + e);
                 }
                 continue;
             }
@@ -186,10 +203,9 @@ HostSparse make_sparse(const std::vector<int> &ptr, const std::vector<int> &idx,
                 for (int k = 0; k < width; ++k) {
                     const int e = k * T + t;
                     h.idx[off + 32u * k + lane] = len > 0 ? idx[ptr[seg] + std::min(e, len - 1)] : 0;  // empty segment: any valid index
-                    if (lane / T < cnt && e < len) {
-                        h.val[off + 32u * k + lane] = val[ptr[seg] + e];
-                        h.pos[ptr[seg] + e] = (int)(off + 32u * k + lane);
-                    }
+                    const bool valid = lane / T < cnt && e < len;
+                    h.val[off + 32u * k + lane] = valid ? val[ptr[seg] + e] : 0.0;
+                    if (valid) h.pos[ptr[seg] + e] = (int)(off + 32u * k + lane);
                 }
             }
         }
@@ -395,8 +411,9 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     for (int j = 0; j < n; ++j) inv_c[perm_c[j]] = j;
     lap("row/column ordering");
     // row-major copy in internal numbering (entries of a row sorted by internal column)
-    std::vector<int> rp2((size_t)m + 1, 0), ci2((size_t)nnz);
-    std::vector<double> va2((size_t)nnz);
+    std::vector<int> rp2((size_t)m + 1, 0);
+    uvec<int> ci2((size_t)nnz);
+    uvec<double> va2((size_t)nnz);
     for (int i = 0; i < m; ++i) rp2[(size_t)i + 1] = rp2[i] + rlen[perm_r[i]];
     {
         auto fill_rows = [&](int i0, int i1) {
@@ -433,11 +450,12 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     // column-major copy (counting sort by internal column; rows come out sorted within a column) and its
     // slices on a second thread, while this thread builds the slices of the row-major copy
     HostSparse hr, hc2;
-    std::vector<int> cp2((size_t)n + 1, 0), ri2((size_t)nnz);
+    std::vector<int> cp2((size_t)n + 1, 0);
+    uvec<int> ri2((size_t)nnz);
     {
         const int nt = host_threads();
         std::thread tc([&] {
-            std::vector<double> cv2((size_t)nnz);
+            uvec<double> cv2((size_t)nnz);
             for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] = cp2[j] + clen[perm_c[j]];   // internal column j = caller's perm_c[j]
             std::vector<int> fill(cp2.begin(), cp2.end() - 1);
             // every helper scans all entries in row order but places only those of its own column range:
