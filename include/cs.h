@@ -82,8 +82,8 @@ typedef struct {
  *            contraction (B north_star; S 8(a) a3): when the problem runs on one CTA (nnz <= 8192) and
  *            m <= dense_m_threshold (<= 256), every conditioning forms A~A~' (m x m, fp64), factors it by
  *            Cholesky on the device, and every pass applies the factor (two triangular solves + one step of
- *            iterative refinement) -- no CG steps are counted.  0 = never; default 128.  A non-positive pivot
- *            (rank-deficient A) falls back to CG for that scaling.
+ *            iterative refinement) -- no CG steps are counted.  0 = never; default 128.  A pivot below 1e-12 (the
+ *            diagonal of A~A~' is 1: numerically rank-deficient A) falls back to CG for that scaling.
  * cs_set_params may be called at any time; mu, t, o_floor, precond, dense_m_threshold take effect at the next
  * cs_condition (or at the implicit first conditioning), cg_* at the next solve. */
 typedef struct {

@@ -156,7 +156,7 @@ __device__ __forceinline__ void dense_factor(const Ctx &c) {
     for (int k = 0; k < m; ++k) {
         __syncthreads();
         const double piv = M[(size_t)k * m + k];
-        if (!(piv > 0.0)) { ok = false; break; }              // uniform: every thread reads the same pivot
+        if (!(piv > 1e-12)) { ok = false; break; }            // diag(A~A~') = 1: a relative test; uniform over the CTA (same pivot)
         const double d = sqrt(piv);
         __syncthreads();
         if (threadIdx.x == 0) M[(size_t)k * m + k] = d;

@@ -450,6 +450,26 @@ def test_dense_factor_apply_matches_cg_and_oracle(name):
         S.set_params(dense_m_threshold=257)
 
 
+def test_dense_path_falls_back_to_cg_on_a_rank_deficient_matrix():
+    """A duplicated row makes A~A~' singular: the Cholesky pivot test fails and the pass's solve goes through CG (which
+    handles the consistent singular system, DESIGN.md 3 reading (r)); the run still converges to the same optimum."""
+    import scipy.sparse as sp
+    from paper_2103_00736_b200 import binding
+    p = W.config(0)
+    A = sp.csr_matrix((p.val, p.col_idx, p.row_ptr), shape=(p.m, p.n))
+    A2 = sp.vstack([A, A[7]]).tocsr()
+    A2.sort_indices()
+    b2 = np.concatenate([p.b, p.b[7:8]])
+    S = binding.Solver(p.m + 1, p.n, A2.indptr.astype(np.int32), A2.indices.astype(np.int32), A2.data.copy(), b2, p.c,
+                       p.n_lin, p.soc_size)
+    S.run(400, L=[100, 200, 300])
+    r = S.residuals()
+    assert r["cg_steps_total"] > 0                      # the factor was refused, CG did the solves
+    assert r["kkt_rel"] <= 1e-5
+    assert abs(r["pobj"] - p.opt_value()) <= 1e-4 * (1 + abs(p.opt_value()))
+    S.destroy()
+
+
 # ------------------------------------------------------------------ S 8(f) rows 2, 3: schedules, fixed equilibration
 @pytest.mark.parametrize("name", ["lp_scaled", "mixed_cones", "cfg4_zipf"])
 def test_equilibrate_matches_oracle_ruiz(name):
