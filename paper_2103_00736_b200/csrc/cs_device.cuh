@@ -18,8 +18,14 @@ namespace csd {
 constexpr int kBlock = CS_BLOCK;          // threads per CTA (16 warps)
 constexpr int kWarps = kBlock / 32;
 constexpr int kMaxRed = 8;           // scalars per grid reduction
-constexpr int kShortMax = 64;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
-constexpr int kChunk = 1024;         // long segments are cut into warp-sized chunks of this many non-zeros
+#ifndef CS_SHORTMAX
+#define CS_SHORTMAX 64
+#endif
+#ifndef CS_CHUNK
+#define CS_CHUNK 1024
+#endif
+constexpr int kShortMax = CS_SHORTMAX;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
+constexpr int kChunk = CS_CHUNK;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
 constexpr int kDenseMax = 256;       // largest m of the dense factor-apply path (cs_params.dense_m_threshold)
 // Build-time alternative, measured and NOT the default (profiles/r01_ncu_notes.md, "TMA-staged stream"): with
