@@ -373,3 +373,147 @@ def test_ruiz_is_constant_on_lorentz_blocks():
     o.run_fixed(4000)
     r = o.residuals()
     assert r["kkt_rel"] < 1e-6 and np.isclose(r["pobj"], p.opt_value(), rtol=1e-5, atol=1e-6)
+
+
+# ------------------------------------------------------------------ hand-computed 1 x 2 LP (tests/golden/hand_1x2_lp.txt)
+def _hand_lp(mu=1.0, t=9.2):
+    A = np.array([[1.0, 1.0]])
+    return _problem_from_dense(A, np.array([2.0]), np.array([1.0, 3.0]), 2, [], mu=mu, t=t)
+
+
+def test_residuals_hand_example_every_term():
+    """orc_residuals term by term ((16a) P:332, (16b) P:335, (34) P:566-572) on a NON-optimal iterate whose x, z, y
+    and every norm are rational numbers worked out by hand in the golden file: mu = 2 (a dropped 1/mu in y or z
+    shows), ||b|| = 2 != ||c|| = sqrt(10) (a swapped normaliser shows), all four relative terms distinct and the
+    maximum attained by the gap (a max over the wrong terms shows)."""
+    g = _golden("hand_1x2_lp.txt")
+    o = oracle.Oracle.from_problem(_hand_lp(mu=2.0))
+    o.run(1)
+    sol, r = o.get(), o.residuals()
+    assert np.allclose(sol["x"], [g["mu2_x1"], g["mu2_x2"]], rtol=0, atol=1e-15)
+    assert np.allclose(sol["z"], [g["mu2_z1"], g["mu2_z2"]], rtol=0, atol=1e-15)
+    assert np.allclose(sol["y"], [g["mu2_y"]], rtol=0, atol=1e-15)
+    for k in oracle.RESID_FIELDS:
+        assert abs(r[k] - g["mu2_" + k]) <= 1e-15 * (1 + abs(g["mu2_" + k])), (k, r[k], g["mu2_" + k])
+    terms = sorted(r[k] for k in ("pres_rel", "dres_rel", "gap_rel", "cone_viol_rel"))
+    assert all(b - a > 1e-3 for a, b in zip(terms, terms[1:]))      # the pin can tell the four apart
+
+
+def test_residuals_term_by_term_on_a_mixed_cone_iterate():
+    """The same terms on a mid-run (non-optimal) iterate of a mixed orthant + Lorentz problem, evaluated with scipy
+    sparse products and with the cone distance taken from Definition 1 as a constrained minimisation
+    (SLSQP), not from the closed form the oracle uses."""
+    p = W.sparse_socp(21, 30, 80, 8, 4, n_lin=20, lo=2, hi=12)
+    p.mu = 1.7
+    o = oracle.Oracle.from_problem(p)
+    o.run(7, L=[4])
+    s, r = o.get(), o.residuals()
+    A, x, z, y = p.csr(), s["x"], s["z"], s["y"]
+
+    def dist_K(v):
+        tot, off = float(np.sum(np.minimum(v[:p.n_lin], 0.0) ** 2)), p.n_lin
+        for sz in p.soc_size.tolist():
+            blk = v[off:off + sz]
+            if sz == 1:
+                tot += min(blk[0], 0.0) ** 2
+            else:
+                cons = {"type": "ineq", "fun": lambda u: u[0] ** 2 - np.sum(u[1:] ** 2)}
+                best = min((so.minimize(lambda u: np.sum((u - blk) ** 2), u0, constraints=[cons], bounds=[(0, None)] + [(None, None)] * (sz - 1),
+                                        method="SLSQP", options={"ftol": 1e-15, "maxiter": 500}).fun
+                            for u0 in (np.r_[np.linalg.norm(blk) + 1.0, blk[1:]], np.r_[1.0, np.zeros(sz - 1)])))
+                tot += max(best, 0.0)
+            off += sz
+        return np.sqrt(tot)
+
+    pres, dres = np.linalg.norm(A @ x - p.b), np.linalg.norm(p.c - z - A.T @ y)
+    cx, by = float(p.c @ x), float(p.b @ y)
+    exp = {"pres_abs": pres, "pres_rel": pres / (1 + np.linalg.norm(p.b)), "dres_abs": dres,
+           "dres_rel": dres / (1 + np.linalg.norm(p.c)), "gap_abs": abs(cx - by),
+           "gap_rel": abs(cx - by) / (1 + abs(cx) + abs(by)), "pobj": cx, "dobj": by}
+    for k, v in exp.items():
+        assert abs(r[k] - v) <= 1e-11 * (1 + abs(v)), (k, r[k], v)
+    cv = (dist_K(x) + dist_K(z)) / (1 + np.linalg.norm(x) + np.linalg.norm(z))
+    assert cv > 1e-3 and abs(r["cone_viol_rel"] - cv) <= 1e-6 * cv, (r["cone_viol_rel"], cv)   # SLSQP accuracy
+    assert r["kkt_rel"] == max(r["pres_rel"], r["dres_rel"], r["gap_rel"], r["cone_viol_rel"])
+    assert min(r["pres_rel"], r["dres_rel"], r["gap_rel"], r["cone_viol_rel"]) > 1e-6     # nothing is at its zero
+
+
+def test_o_floor_branch_hand_example():
+    """Step 7 with exact zeros, reading (g): numerator AND denominator are floored at o_floor, separately.
+    K = R^3_+ x K_3 x K_2, o_floor = 1e-3:
+        x = (0, 2, 5 | 5, 3, 4 | 0, 0),  z = (4, 0, 5 | 2, ., . | 0, .)
+        o = (1e-3/4, 2/1e-3, 5/5 | |5 - 5| -> 1e-3, /2 | 1e-3/1e-3) = (2.5e-4, 2000, 1, 5e-4, 1)
+    (flooring the ratio instead would give 1e-3, inf, 1, 1e-3, nan).  t = 50: alpha = 1 and O = o; t = ln 100:
+    alpha = ln 100 / ln(2000/2.5e-4)."""
+    rng = np.random.default_rng(4)
+    x = np.array([0.0, 2.0, 5.0, 5.0, 3.0, 4.0, 0.0, 0.0])
+    z = np.array([4.0, 0.0, 5.0, 2.0, 0.7, -0.2, 0.0, 0.3])
+    o_exp = np.array([2.5e-4, 2000.0, 1.0, 5e-4, 5e-4, 5e-4, 1.0, 1.0])
+    A = rng.standard_normal((2, 8))
+    for t, alpha in ((50.0, 1.0), (np.log(100.0), np.log(100.0) / np.log(2000.0 / 2.5e-4))):
+        p = _problem_from_dense(A, A @ np.abs(x), rng.standard_normal(8), 3, [3, 2], t=t)
+        o = oracle.Oracle.from_problem(p, o_floor=1e-3)
+        o.set_point(x, z)
+        o.run(1)
+        O = o.get()["O"]
+        assert np.all(np.isfinite(O)) and np.allclose(O, o_exp ** alpha, rtol=1e-13), (t, O)
+    # the default floor (1e-16) only guards exact zeros; the cap of step 11 then keeps O moderate
+    o_def = np.array([1e-16 / 4, 2 / 1e-16, 1.0, 5e-17, 5e-17, 5e-17, 1.0, 1.0])
+    alpha = np.log(100.0) / np.log(o_def.max() / o_def.min())
+    p = _problem_from_dense(A, A @ np.abs(x), rng.standard_normal(8), 3, [3, 2], t=np.log(100.0))
+    o = oracle.Oracle.from_problem(p)
+    o.set_point(x, z)
+    o.run(1)
+    assert np.allclose(o.get()["O"], o_def ** alpha, rtol=1e-13)
+
+
+def test_L_membership_timing_hand_example():
+    """Step 4: l in L conditions at the START of iteration l, from the (x, z) left by iteration l-1.
+    Hand-computed in the golden file: with L = {3} the rule sees (x2, z2) = ((5/2,-1/2), (-1/2,1/2)) => O = (5, 1)
+    and iteration 3 ends at x = (240/26, -19/26), z = (6/26, 45/26); one iteration late it would see
+    (x3, z3) = ((3,-1/2), (0, 3/2)) => o = (3/o_floor, 1/3)."""
+    g = _golden("hand_1x2_lp.txt")
+    o = oracle.Oracle.from_problem(_hand_lp())
+    o.run(2, L=[3])
+    assert np.array_equal(o.get()["O"], [1.0, 1.0])                 # not yet
+    assert np.allclose(o.get()["x"], [2.5, -0.5], atol=1e-15) and np.allclose(o.get()["z"], [-0.5, 0.5], atol=1e-15)
+    o.run(1, L=[3])
+    s = o.get()
+    assert np.allclose(s["O"], [g["L3_O1"], g["L3_O2"]], rtol=1e-14)
+    assert np.allclose(s["x"], [g["L3_x1"], g["L3_x2"]], rtol=1e-13) and np.allclose(s["z"], [g["L3_z1"], g["L3_z2"]], rtol=1e-13)
+    assert np.allclose(s["s"], [g["L3_s1"], g["L3_s2"]], rtol=1e-13)
+    assert o.counters()["n_cond"] == 2
+    o2 = oracle.Oracle.from_problem(_hand_lp())
+    o2.run(3)                                                       # L = {}: a different third iterate
+    s2 = o2.get()
+    assert np.allclose(s2["x"], [g["noL_x1"], g["noL_x2"]], atol=1e-14) and np.allclose(s2["z"], [g["noL_z1"], g["noL_z2"]], atol=1e-14)
+    o3 = oracle.Oracle.from_problem(_hand_lp())
+    o3.run(4, L=[4])                                                # L = {4}: the rule sees (x3, z3); z3_1 = 0 hits the floor
+    O3 = o3.get()["O"]
+    assert O3[0] / O3[1] > 1e3 and not np.allclose(O3, [5.0, 1.0])
+
+
+def test_exact_solve_resolves_the_projection_on_an_ill_conditioned_system():
+    """Reading (s): the solve inside A^dagger is exact.  On the config-2 recipe (rows 10^U(-3,3), columns 10^U(-2,2))
+    both solve modes must give A^dagger rhs to ~1e-13 of a reference obtained by iterative refinement with
+    EXTENDED-precision residuals (numpy longdouble, dense): the dense Cholesky with its two refinement steps, and the
+    Jacobi-PCG at its tight tolerance."""
+    import scipy.linalg as sl
+    p = W.config(2, 0.004)
+    A = p.csr().toarray()
+    Al = A.astype(np.longdouble)
+    G = A @ A.T
+    e = 1.0 / np.sqrt(np.diag(G))
+    Lc = np.linalg.cholesky(G * np.outer(e, e))
+    apply = lambda r: e * sl.solve_triangular(Lc.T, sl.solve_triangular(Lc, e * r, lower=True), lower=False)
+    rhs = A @ np.random.default_rng(0).standard_normal(p.n)
+    w = apply(rhs).astype(np.longdouble)
+    for _ in range(8):
+        w = w + apply(np.asarray(rhs - Al @ (Al.T @ w), dtype=np.float64)).astype(np.longdouble)
+    ref = np.asarray(Al.T @ w, dtype=np.float64)
+    assert np.linalg.cond(G) > 1e10
+    for mode, tol, bound in ((1, 1e-14, 2e-14), (2, 1e-15, 5e-13)):
+        o = oracle.Oracle.from_problem(p, solve_mode=mode, pcg_tol=tol, pcg_max=100000)
+        o.run(1)                                                    # l = 1: O = I
+        err = np.linalg.norm(o.pinv_apply(rhs) - ref) / np.linalg.norm(ref)
+        assert err <= bound, (mode, err)
