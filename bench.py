@@ -286,7 +286,7 @@ def main():
         us_g, us_s = binding.gather_probe(p.n, min(p.nnz, 2**31 - 2))
         gather = {"unit": "Ggather/s", "achieved": 2 * p.nnz * cg_iter / (ms_iter * 1e-3) / 1e9, "peak": p.nnz / (us_g * 1e-6) / 1e9,
                   "probe_us": us_g, "probe_us_without_gathers": us_s,
-                  "note": "2 gathers per stored entry per CG step; peak = cs_gather_probe (uniformly random indices, "
+                  "note": "2 gathers per stored entry per CG step; peak = cs_diag_gather_probe (uniformly random indices, "
                           "no coalescing); >1 is possible where a workload's gathers coalesce (config 4's heavy rows)"}
         gather["frac"] = gather["achieved"] / gather["peak"]
     except Exception as e:  # pragma: no cover

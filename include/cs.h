@@ -67,7 +67,10 @@ typedef struct {
  *   t        cap on ln(max O / min O) in step 11; 9.2 for LP, 1.7 for SOCP
  *   o_floor  absolute floor of numerator and denominator of o_i in step 7 (paper silent on 0/0)
  *   cg_tol   inner solve stops when ||residual||_2 <= cg_tol * ||rhs||_2, both measured on the
- *            row-equilibrated system (D A_hat)(D A_hat)' with D = diag(1/||row_i(A_hat)||_2)
+ *            row-equilibrated system (D A_hat)(D A_hat)' with D = diag(1/||row_i(A_hat)||_2).  The residual is
+ *            the recurrence residual of CG, which keeps shrinking below the rounding level of the true one; the
+ *            default 1e-16 takes the solve to that floor ("exact" projections, the parity setting: an in-run
+ *            conditioning amplifies what is left of the solve error by 1e3-1e4)
  *   cg_reduce    inexact projections (0 = off, the default): the solve of a pass also stops once the residual of
  *            the WARM START has been reduced by this factor, ||residual||_2 <= max(cg_tol ||rhs||_2,
  *            cg_reduce ||residual at the warm start||_2).  The warm-start residual shrinks as the outer iteration
@@ -116,7 +119,7 @@ typedef struct {
 
 /* Build a solver for (A,b,c,K): validates the input, copies it to the device, builds the CSC copy of A
  * and the work partitions.  b[m], c[n] live in `vec_where`.  Parameters start at mu=1, t=9.2 (n_soc=0)
- * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-15, cg_reduce=0, cg_max_iter=20000, precond=0,
+ * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-16, cg_reduce=0, cg_max_iter=20000, precond=0,
  * dense_m_threshold=128; the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
  * mandatory first conditioning (l=1) the identity and s=0.  Synchronous.  On failure *out is NULL. */
 cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
@@ -189,21 +192,6 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out);
 /* Copy out the current x[n], z[n], y[m], s[n], O[n] (original coordinates for x,z,y; scaled for s).
  * Any pointer may be NULL.  Synchronous when where == CS_HOST. */
 cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where);
-
-/* Device time per phase of k_iterate so far, in ns, measured on the device between grid barriers:
- * out[0] cone reflect, [1] rhs pass, [2] CG pass K1 (A~'r, columns), [3] CG pass K2 (A~u, rows),
- * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6] preconditioner application z = G'G r, [7] reserved.  One D2H copy + sync. */
-cs_status cs_phase_times(cs_solver *S, double out[8]);
-
-/* Diagnostic (no handle, current device, default stream, synchronous): time n_idx uniformly random 8-byte
- * gathers from an n_vec-element vector with the launch shape of the solver's sparse passes (indices
- * streamed, 8 gathers in flight per thread), and the same loop without the gathers.  The difference is the
- * LSU/L1TEX gather ceiling that bounds the sparse passes on irregular matrices. */
-cs_status cs_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only);
-
-/* Diagnostic: run n empty grid barriers (each a 1-value all-reduce over all CTAs, result checked) in one
- * launch and report the mean latency in microseconds.  Synchronous. */
-cs_status cs_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier);
 
 /* Number of kernels the library has launched on this handle so far (for bench accounting). */
 int64_t cs_kernel_launches(const cs_solver *S);

@@ -1,0 +1,33 @@
+/*
+ * cs_diag.h -- DIAGNOSTICS of libcs.so, not part of the product ABI of cs.h: instrumentation that
+ * bench.py and profiles/ use to explain the numbers (per-phase device time of k_iterate, the gather ceiling of the
+ * SM's load path, the latency of the grid barrier).  Nothing on the hot path depends on these calls.
+ */
+#ifndef CS_DIAG_H_
+#define CS_DIAG_H_
+
+#include "cs.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Device time per phase of k_iterate so far, in ns, measured on the device between grid barriers:
+ * out[0] cone reflect, [1] rhs pass, [2] CG pass K1 (A~'r, columns), [3] CG pass K2 (A~u, rows),
+ * [4] A~'w + s-update pass, [5] grid reductions/barriers, [6] preconditioner application z = G'G r, [7] reserved.  One D2H copy + sync. */
+cs_status cs_diag_phase_times(cs_solver *S, double out[8]);
+
+/* Diagnostic (no handle, current device, default stream, synchronous): time n_idx uniformly random 8-byte
+ * gathers from an n_vec-element vector with the launch shape of the solver's sparse passes (indices
+ * streamed, 8 gathers in flight per thread), and the same loop without the gathers.  The difference is the
+ * LSU/L1TEX gather ceiling that bounds the sparse passes on irregular matrices. */
+cs_status cs_diag_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only);
+
+/* Diagnostic: run n empty grid barriers (each a 1-value all-reduce over all CTAs, result checked) in one
+ * launch and report the mean latency in microseconds.  Synchronous. */
+cs_status cs_diag_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CS_DIAG_H_ */

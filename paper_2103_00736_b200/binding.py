@@ -1,4 +1,4 @@
-"""ctypes binding of libcs.so (include/cs.h): same names, argument marshalling only.
+"""ctypes binding of libcs.so (include/cs.h, diagnostics in include/cs_diag.h): same names, argument marshalling only.
 
 Arrays may be numpy arrays (host memory) or torch tensors (host or CUDA memory); the binding passes
 their raw pointers with the matching ``cs_mem`` tag.  There is NO fallback: if ``libcs.so`` is missing
@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("CS_LIB") or os.path.join(_HERE, "libcs.so")  # CS_LIB: alternative build (tuning only)
+LIB_PATH = os.path.join(_HERE, "libcs.so")
 
 CS_OK, CS_EINVAL, CS_ENOMEM, CS_ECUDA, CS_ESTATE, CS_ECGMAX = range(6)
 CS_HOST, CS_DEVICE = 0, 1
@@ -53,8 +53,8 @@ class cs_schedule(C.Structure):
 CS_RULE_SET, CS_RULE_STALL = 0, 1
 
 _INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
-               "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_phase_times",
-               "cs_gather_probe", "cs_barrier_probe")
+               "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_diag_phase_times",
+               "cs_diag_gather_probe", "cs_diag_barrier_probe")
 EXPORTS = _INT_STATUS + ("cs_kernel_launches", "cs_last_error", "cs_destroy")
 
 _lib = None
@@ -84,9 +84,9 @@ def lib():
         L.cs_last_error.restype = C.c_char_p
         L.cs_destroy.argtypes = [vp]
         L.cs_destroy.restype = None
-        L.cs_phase_times.argtypes = [vp, C.POINTER(C.c_double)]
-        L.cs_barrier_probe.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
-        L.cs_gather_probe.argtypes = [C.c_int64, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.cs_diag_phase_times.argtypes = [vp, C.POINTER(C.c_double)]
+        L.cs_diag_barrier_probe.argtypes = [vp, C.c_int32, C.POINTER(C.c_double)]
+        L.cs_diag_gather_probe.argtypes = [C.c_int64, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cs_equilibrate.argtypes = [vp, C.c_int32]
         L.cs_solve.argtypes = [vp, C.POINTER(cs_schedule), C.POINTER(cs_resid), C.POINTER(C.c_int64), C.c_int64,
                                C.POINTER(C.c_int64)]
@@ -128,11 +128,11 @@ def _same_space(*tags):
 
 
 def gather_probe(n_vec, n_idx):
-    """(us with gathers, us without) of n_idx random 8-byte gathers from an n_vec vector (cs_gather_probe)."""
+    """(us with gathers, us without) of n_idx random 8-byte gathers from an n_vec vector (cs_diag_gather_probe)."""
     a, b = C.c_double(), C.c_double()
-    st = lib().cs_gather_probe(int(n_vec), int(n_idx), C.byref(a), C.byref(b))
+    st = lib().cs_diag_gather_probe(int(n_vec), int(n_idx), C.byref(a), C.byref(b))
     if st != CS_OK:
-        raise CsError(st, "cs_gather_probe failed")
+        raise CsError(st, "cs_diag_gather_probe failed")
     return a.value, b.value
 
 
@@ -249,13 +249,13 @@ class Solver:
     def phase_times(self):
         """Device time per phase of k_iterate so far (ns): cone, rhs, K1, K2, update, reduce, precond."""
         a = (C.c_double * 8)()
-        self._check(lib().cs_phase_times(self._h, a))
+        self._check(lib().cs_diag_phase_times(self._h, a))
         names = ("cone", "rhs", "K1", "K2", "update", "reduce", "precond", "r7")
         return dict(zip(names, [float(x) for x in a]))
 
     def barrier_probe(self, n=1000):
         us = C.c_double()
-        self._check(lib().cs_barrier_probe(self._h, int(n), C.byref(us)))
+        self._check(lib().cs_diag_barrier_probe(self._h, int(n), C.byref(us)))
         return us.value
 
     def kernel_launches(self):

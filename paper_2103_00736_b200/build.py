@@ -13,8 +13,8 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 
 def sources():
     d = os.path.join(HERE, "csrc")
-    inc = os.path.join(os.path.dirname(HERE), "include", "cs.h")
-    return [os.path.join(d, f) for f in sorted(os.listdir(d))] + [inc]
+    inc = os.path.join(os.path.dirname(HERE), "include")
+    return [os.path.join(d, f) for f in sorted(os.listdir(d))] + [os.path.join(inc, f) for f in sorted(os.listdir(inc))]
 
 
 def needs_build() -> bool:

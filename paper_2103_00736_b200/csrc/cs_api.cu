@@ -17,8 +17,12 @@
 #include <utility>
 #include <vector>
 
-#include "../../include/cs.h"
+#include "../../include/cs_diag.h"
 #include "cs_kernels_cond.cuh"
+
+#ifndef CS_FUSE_CARVEOUT
+#define CS_FUSE_CARVEOUT 43
+#endif
 
 using namespace csd;
 
@@ -28,7 +32,7 @@ struct cs_solver {
     int device = 0;
     int grid = 0;
     int64_t nnz = 0;
-    size_t dyn_smem = 0;       // bytes of dynamic shared memory of the cooperative kernels (per-warp TMA staging rings)
+    size_t dyn_smem = 0;       // bytes of dynamic shared memory of k_iterate (accumulators of the heavy-row fusion)
     std::vector<void *> allocs;
     cs_params prm{};
     bool conditioned = false;  // the l=1 conditioning of step 4 has run
@@ -44,6 +48,8 @@ struct cs_solver {
 namespace {
 
 thread_local std::string g_create_err;
+constexpr int kFuseCarveoutPct = CS_FUSE_CARVEOUT;   // percent of the SM's 228 KB of shared memory asked for when k_iterate fuses rows
+constexpr int kOneCtaNnz = 8192;   // problems up to this many non-zeros run on ONE CTA
 
 #define CS_CUDA(S, call)                                                                         \
     do {                                                                                         \
@@ -105,55 +111,98 @@ template <class T> using uvec = std::vector<T, NoInit<T>>;
 // Host image of one Sparse (cs_device.cuh): chunk slices of the long segments first, then the slices of
 // the short ones, all in one pair of arrays.
 struct HostSparse {
-    std::vector<int4> slices, multi;
+    std::vector<int4> slices, multi, multi_k2;
     std::vector<int> chunk_slot;
     uvec<int> idx;
     uvec<int> pos;                // compressed entry -> position in val/idx (for the plain compressed view, Csr in cs_device.cuh)
     uvec<double> val;
-    int n_chunk = 0, n_slots = 0;
+    std::vector<unsigned> fmask;  // column-major copy with fused rows: [short slice][kFuseK] lane masks of the fused entries
+    int n_chunk = 0, n_chunk_k2 = 0, n_slots = 0;
+    bool too_big = false;         // padded storage would exceed 2^31 entries: nothing was filled
 };
 
 // Run f(block) for block = 0..n_blocks-1 on up to `nt` host threads (blocks are handed out dynamically).
+// Nothing may throw across a thread boundary: an exception in a worker is recorded and rethrown by the caller's
+// thread as std::bad_alloc (cs_create turns that into CS_ENOMEM).
 template <class F>
 void parallel_blocks(int n_blocks, int nt, F f) {
     nt = std::max(1, std::min(nt, n_blocks));
     if (nt == 1) { for (int b = 0; b < n_blocks; ++b) f(b); return; }
     std::atomic<int> next{0};
+    std::atomic<bool> failed{false};
     std::vector<std::thread> th;
-    for (int t = 0; t < nt; ++t)
-        th.emplace_back([&] { for (int b = next.fetch_add(1); b < n_blocks; b = next.fetch_add(1)) f(b); });
+    auto body = [&] {
+        try { for (int b = next.fetch_add(1); b < n_blocks && !failed.load(); b = next.fetch_add(1)) f(b); }
+        catch (...) { failed.store(true); }
+    };
+    try { for (int t = 0; t < nt; ++t) th.emplace_back(body); }
+    catch (...) { failed.store(true); }
     for (auto &t : th) t.join();
+    if (failed.load()) throw std::bad_alloc();
 }
 
 int host_threads() { return (int)std::max(1u, std::min(16u, std::thread::hardware_concurrency())); }
 
+// Heavy-row fusion plan (cs_device.cuh): internal rows [0, n_fa) are class A, [n_fa, n_fa + n_fb) class B.
+struct FusePlan { int n_fa = 0, n_fb = 0; int rows() const { return n_fa + n_fb; } };
+
 // ptr/idx/val: compressed segments in INTERNAL numbering (segment s = entries [ptr[s], ptr[s+1])).
 // Two phases: a serial plan (slice descriptors and offsets, O(#segments)), then a parallel fill.
-HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const uvec<double> &val, int nt) {
+//   Column-major copy (fuse != nullptr, fused_out != nullptr): an entry of a one-thread-per-column slice whose row is a
+//     fused row gets its lane's bit in the slice's masks (HostSparse::fmask) and fused_out[compressed position] = 1 --
+//     class A always, class B only for the lowest lane of its slice that holds that row (the accumulators of class B
+//     are per warp); only the first kFuseK entries of a column qualify.
+//   Row-major copy (split != nullptr): the first split[s] entries of fused row s stay with the row pass of a CG step
+//     (K2 view), the rest have been taken over by the column pass; each part gets its own chunk slices.
+HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const uvec<double> &val, int nt,
+                       const FusePlan *fuse = nullptr, uvec<unsigned char> *fused_out = nullptr,
+                       const std::vector<int> *split = nullptr) {
     HostSparse h;
     const int nseg = (int)ptr.size() - 1;
     // several lanes per segment only pay when there are too few segments to fill the machine (measured:
     // T>1 is slower once every warp has >= 2 thread-per-segment slices)
-    const bool split = nseg < 300000;
-    auto lg_lanes = [split](int len) { return (!split || len <= 8) ? 0 : len <= 16 ? 1 : len <= 32 ? 2 : 3; };  // T = 1,2,4,8 lanes
+    const bool split_lanes = nseg < 300000;
+    auto lg_lanes = [split_lanes](int len) { return (!split_lanes || len <= 8) ? 0 : len <= 16 ? 1 : len <= 32 ? 2 : 3; };  // T = 1,2,4,8 lanes
     size_t total = 0;
-    std::vector<int> chunk_src;       // first source entry of every chunk slice
+    std::vector<int> chunk_src, chunk_len;       // first source entry and length of every chunk slice
     auto plan_slice = [&](int seg0, int meta, int width) {
-        h.slices.push_back(make_int4((int)total, seg0, meta, width));
+        h.slices.push_back(make_int4((int)std::min<size_t>(total, INT32_MAX), seg0, meta, width));
         total += 32u * (size_t)width;
     };
-    // plan 1: chunks of the long segments (T = 32: entry e of the chunk at lane e%32, row e/32)
+    // plan 1: chunks of the long segments (T = 32: entry e of the chunk at lane e%32, row e/32).  Pass 0 plans the part
+    // every traversal walks (the K2 view), pass 1 the fused tails of the fused rows; slots are numbered per segment,
+    // K2 part first, so that a chunk has the same slot in both views.
+    const int n_split = split ? (int)split->size() : 0;
+    std::vector<int> first_slot((size_t)nseg, -1);
     for (int s = 0; s < nseg; ++s) {
         const int len = ptr[s + 1] - ptr[s];
         if (len <= kShortMax) continue;
-        const int nch = (len + kChunk - 1) / kChunk;
-        if (nch > 1) h.multi.push_back(make_int4(s, h.n_slots, nch, 0));
-        for (int q = 0; q < nch; ++q) {
-            const int a = ptr[s] + q * kChunk, clen = std::min(kChunk, ptr[s + 1] - a);
-            plan_slice(s, 1 | (5 << 8), (clen + 31) / 32);
-            chunk_src.push_back(a);
-            h.chunk_slot.push_back(nch > 1 ? h.n_slots++ : -1);
+        const int nu = s < n_split ? (*split)[s] : len, nf = len - nu;
+        const int nch_u = (nu + kChunk - 1) / kChunk, nch_f = (nf + kChunk - 1) / kChunk;
+        if (nch_u + nch_f > 1 || nf > 0) { first_slot[s] = h.n_slots; h.n_slots += nch_u + nch_f; }
+        if (nch_u + nch_f > 1) h.multi.push_back(make_int4(s, first_slot[s], nch_u + nch_f, 0));
+        if (nf > 0) h.multi_k2.push_back(make_int4(s, first_slot[s], nch_u, s + 1));
+        else if (nch_u > 1) h.multi_k2.push_back(make_int4(s, first_slot[s], nch_u, 0));
+    }
+    for (int pass = 0; pass < 2; ++pass) {
+        for (int s = 0; s < nseg; ++s) {
+            const int len = ptr[s + 1] - ptr[s];
+            if (len <= kShortMax) continue;
+            const int nu = s < n_split ? (*split)[s] : len, nf = len - nu;
+            const int nch_u = (nu + kChunk - 1) / kChunk;
+            const int beg = pass ? ptr[s] + nu : ptr[s], cnt = pass ? nf : nu, nch = (cnt + kChunk - 1) / kChunk;
+            const bool direct = nf == 0 && nch_u == 1;      // a single chunk that completes its segment
+            for (int q = 0; q < nch; ++q) {
+                const int a = beg + q * kChunk, clen = std::min(kChunk, beg + cnt - a);
+                plan_slice(s, 1 | (5 << 8), (clen + 31) / 32);
+                chunk_src.push_back(a);
+                chunk_len.push_back(clen);
+                int slot = direct ? -1 : first_slot[s] + (pass ? nch_u : 0) + q;
+                if (pass && nu == 0 && nch == 1) slot = -1;  // all entries fused, one chunk: the full view completes it directly
+                h.chunk_slot.push_back(slot);
+            }
         }
+        if (pass == 0) h.n_chunk_k2 = (int)h.slices.size();
     }
     h.n_chunk = (int)h.slices.size();
     // plan 2: runs of consecutive short segments -> slices of 32 lanes, T lanes per segment
@@ -177,18 +226,21 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
         run = s + 1;
     }
     plan_run(run, nseg);
+    if (total >= (size_t)INT32_MAX) { h.too_big = true; return h; }   // offsets are int32: refuse before anything is filled
     // fill (padding: val = 0, a valid index replicated)
     h.val.resize(total);          // no zero-fill: the fill below writes every slot (padding values = 0)
     h.idx.resize(total);
     h.pos.resize(idx.size());
+    const int n_fuse = fuse ? fuse->rows() : 0, n_fa = fuse ? fuse->n_fa : 0;
     const int n_slice = (int)h.slices.size(), blk = 512;
+    if (n_fuse) h.fmask.assign((size_t)(n_slice - h.n_chunk) * kFuseK, 0u);
     parallel_blocks((n_slice + blk - 1) / blk, nt, [&](int bi) {
         for (int si = bi * blk; si < std::min(n_slice, (bi + 1) * blk); ++si) {
             const int4 sl = h.slices[si];
             const size_t off = (size_t)sl.x;
             const int width = sl.w;
             if (si < h.n_chunk) {
-                const int a = chunk_src[si], clen = std::min(kChunk, ptr[sl.y + 1] - a);
+                const int a = chunk_src[si], clen = chunk_len[si];
                 for (int e = 0; e < 32 * width; ++e) {
                     h.idx[off + e] = idx[a + std::min(e, clen - 1)];
                     h.val[off + e] = e < clen ? val[a + e] : 0.0;
@@ -196,7 +248,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
                 }
                 continue;
             }
-            const int cnt = sl.z & 255, T = 1 << (sl.z >> 8), s0 = sl.y;
+            const int cnt = sl.z & 255, lgT = sl.z >> 8, T = 1 << lgT, s0 = sl.y;
             for (int lane = 0; lane < 32; ++lane) {
                 const int seg = s0 + std::min(lane / T, cnt - 1);   // padding lanes replicate a valid index
                 const int len = ptr[seg + 1] - ptr[seg], t = lane % T;
@@ -208,6 +260,27 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
                     if (valid) h.pos[ptr[seg] + e] = (int)(off + 32u * k + lane);
                 }
             }
+            if (n_fuse && lgT == 0) {   // one thread per column: mark the entries the column pass takes over
+                bool any_fused = false;
+                int seen[kFuseB + 1], n_seen = 0;                    // class-B rows already fused in this slice (by a lower lane)
+                for (int lane = 0; lane < cnt; ++lane) {
+                    const int seg = s0 + lane, len = ptr[seg + 1] - ptr[seg];
+                    for (int k = 0; k < std::min(len, kFuseK); ++k) {
+                        const int i = idx[ptr[seg] + k];
+                        if (i >= n_fuse) break;                      // rows ascend within a column
+                        if (i >= n_fa) {                             // class B: one lane per row and slice
+                            bool dup = false;
+                            for (int q = 0; q < n_seen; ++q) dup |= seen[q] == i;
+                            if (dup) continue;
+                            seen[n_seen++] = i;
+                        }
+                        h.fmask[(size_t)(si - h.n_chunk) * kFuseK + k] |= 1u << lane;
+                        (*fused_out)[ptr[seg] + k] = 1;
+                        any_fused = true;
+                    }
+                }
+                if (any_fused) h.slices[si].z |= 1 << 16;
+            }
         }
     });
     return h;
@@ -218,6 +291,9 @@ cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     int4 *p4; int *pi; double *pd;
     if ((st = dev_upload(S, &p4, h.slices.data(), h.slices.size())) != CS_OK) return st; out->slices = p4;
     if ((st = dev_upload(S, &p4, h.multi.data(), h.multi.size())) != CS_OK) return st; out->multi = p4;
+    if ((st = dev_upload(S, &p4, h.multi_k2.data(), h.multi_k2.size())) != CS_OK) return st; out->multi_k2 = p4;
+    unsigned *pu;
+    if ((st = dev_upload(S, &pu, h.fmask.data(), h.fmask.size())) != CS_OK) return st; out->fmask = pu;
     if ((st = dev_upload(S, &pi, h.chunk_slot.data(), h.chunk_slot.size())) != CS_OK) return st; out->chunk_slot = pi;
     if ((st = dev_upload(S, &pi, h.idx.data(), h.idx.size())) != CS_OK) return st; out->idx = pi;
     if ((st = dev_upload(S, &pd, h.val.data(), h.val.size())) != CS_OK) return st; out->val0 = pd;
@@ -225,7 +301,9 @@ cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     if (!h.val.empty()) CS_CUDA(S, cudaMemcpyAsync(out->val, pd, h.val.size() * sizeof(double), cudaMemcpyDeviceToDevice, S->stream));
     out->n_slice = (int)h.slices.size();
     out->n_chunk = h.n_chunk;
+    out->n_chunk_k2 = h.n_chunk_k2;
     out->n_multi = (int)h.multi.size();
+    out->n_multi_k2 = (int)h.multi_k2.size();
     return dev_zeros(S, &out->partial, (size_t)h.n_slots * 2);
 }
 
@@ -243,8 +321,9 @@ std::vector<int> order_by_length(const std::vector<int> &len, int n_sort) {
     return perm;
 }
 
-cs_status launch_coop(cs_solver *S, const void *fn, void **args) {   // every cooperative kernel carries the staging ring
-    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, S->dyn_smem, S->stream));
+cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
+    const size_t dyn = fn == (const void *)k_iterate ? S->dyn_smem : 0;
+    CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, dyn, S->stream));
     S->launches += 1;
     return CS_OK;
 }
@@ -447,53 +526,85 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         parallel_blocks((int)cut.size() - 1, host_threads(), [&](int bi) { fill_rows(cut[bi], cut[bi + 1]); });
     }
     lap("row-major copy");
-    // column-major copy (counting sort by internal column; rows come out sorted within a column) and its
-    // slices on a second thread, while this thread builds the slices of the row-major copy
+    // column-major copy (counting sort by internal column; rows come out sorted within a column)
     HostSparse hr, hc2;
     std::vector<int> cp2((size_t)n + 1, 0);
     uvec<int> ri2((size_t)nnz);
+    const int nt = host_threads();
     {
-        const int nt = host_threads();
-        std::thread tc([&] {
-            uvec<double> cv2((size_t)nnz);
-            for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] = cp2[j] + clen[perm_c[j]];   // internal column j = caller's perm_c[j]
-            std::vector<int> fill(cp2.begin(), cp2.end() - 1);
-            // every helper scans all entries in row order but places only those of its own column range:
-            // sequential reads, writes confined to the range, order within a column = row order (deterministic)
-            const int parts = std::max(1, nt / 2);
-            parallel_blocks(parts, parts, [&](int part) {
-                const int j0 = (int)((long long)n * part / parts), j1 = (int)((long long)n * (part + 1) / parts);
-                for (int i = 0; i < m; ++i)
-                    for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
-                        const int j = ci2[k];
-                        if (j < j0 || j >= j1) continue;
-                        const int q = fill[j]++;
-                        ri2[q] = i;
-                        cv2[q] = va2[k];
-                    }
-            });
-            hc2 = make_sparse(cp2, ri2, cv2, std::max(1, nt / 2));
-        });
-        hr = make_sparse(rp2, ci2, va2, std::max(1, nt / 2));
-        // the row-major copy goes to the device while the other thread is still building the column-major one
-        cs_status su = CS_OK;
-        if (hr.val.size() < (size_t)INT32_MAX) {
-            int *q;
-            if ((su = upload_sparse(S, hr, &S->ctx.R)) == CS_OK && (su = dev_upload(S, &q, rp2.data(), rp2.size())) == CS_OK) {
-                S->ctx.Rc.ptr = q;
-                if ((su = dev_upload(S, &q, ci2.data(), ci2.size())) == CS_OK) {
-                    S->ctx.Rc.idx = q;
-                    if ((su = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) == CS_OK) S->ctx.Rc.pos = q;
+        uvec<double> cv2((size_t)nnz);
+        for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] = cp2[j] + clen[perm_c[j]];   // internal column j = caller's perm_c[j]
+        std::vector<int> fill(cp2.begin(), cp2.end() - 1);
+        // every helper scans all entries in row order but places only those of its own column range:
+        // sequential reads, writes confined to the range, order within a column = row order (deterministic)
+        const int parts = std::max(1, nt);
+        parallel_blocks(parts, parts, [&](int part) {
+            const int j0 = (int)((long long)n * part / parts), j1 = (int)((long long)n * (part + 1) / parts);
+            for (int i = 0; i < m; ++i)
+                for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
+                    const int j = ci2[k];
+                    if (j < j0 || j >= j1) continue;
+                    const int q = fill[j]++;
+                    ri2[q] = i;
+                    cv2[q] = va2[k];
                 }
-            }
+        });
+        lap("column-major copy");
+        // Heavy-row fusion plan: the longest rows (internal rows come sorted by decreasing length), if they are long
+        // enough to be worth it and the problem runs on more than one CTA.
+        FusePlan fuse;
+        if (nnz > kOneCtaNnz)
+            for (int i = 0; i < std::min(m, kFuseA + kFuseB) && rp2[(size_t)i + 1] - rp2[i] >= kFuseMinLen; ++i)
+                (i < kFuseA ? fuse.n_fa : fuse.n_fb) += 1;
+        uvec<unsigned char> fused;
+        if (fuse.rows()) {
+            fused.resize((size_t)nnz);
+            std::memset(fused.data(), 0, (size_t)nnz);
         }
-        tc.join();
-        if (su != CS_OK) return su;
+        hc2 = make_sparse(cp2, ri2, cv2, nt, fuse.rows() ? &fuse : nullptr, fuse.rows() ? &fused : nullptr);
+        lap("column-major slices");
+        // fused rows: entries that stay with the row pass first, the fused ones after them (each part keeps its
+        // ascending column order); split[s] = size of the first part
+        std::vector<int> split((size_t)fuse.rows());
+        if (fuse.rows() && !hc2.too_big) {
+            for (int sfr = 0; sfr < fuse.rows(); ++sfr) {
+                const int a0 = rp2[sfr], len = rp2[(size_t)sfr + 1] - a0;
+                uvec<int> tj((size_t)len);
+                uvec<double> tv((size_t)len);
+                uvec<unsigned char> tf((size_t)len);
+                const int blk = 1 << 16;
+                parallel_blocks((len + blk - 1) / blk, nt, [&](int bi) {
+                    for (int k = bi * blk; k < std::min(len, (bi + 1) * blk); ++k) {
+                        const int j = ci2[a0 + k];
+                        const int *lo = ri2.data() + cp2[j], *hi = ri2.data() + cp2[(size_t)j + 1];
+                        const int *q = std::lower_bound(lo, hi, sfr);      // rows are ascending within a column
+                        tf[k] = fused[(size_t)(q - ri2.data())];
+                        tj[k] = j;
+                        tv[k] = va2[a0 + k];
+                    }
+                });
+                int w0 = a0;
+                for (int k = 0; k < len; ++k) if (!tf[k]) { ci2[w0] = tj[k]; va2[w0] = tv[k]; ++w0; }
+                split[sfr] = w0 - a0;
+                for (int k = 0; k < len; ++k) if (tf[k]) { ci2[w0] = tj[k]; va2[w0] = tv[k]; ++w0; }
+            }
+            S->ctx.n_fa = fuse.n_fa;
+            S->ctx.n_fb = fuse.n_fb;
+            lap("fused rows: partition");
+        }
+        hr = make_sparse(rp2, ci2, va2, nt, nullptr, nullptr, fuse.rows() ? &split : nullptr);
     }
-    lap("column-major copy + slices");
-    if (hr.val.size() >= (size_t)INT32_MAX || hc2.val.size() >= (size_t)INT32_MAX) {
+    lap("row-major slices");
+    if (hr.too_big || hc2.too_big) {
         S->err = "padded slice storage exceeds 2^31 entries";
         return CS_EINVAL;
+    }
+    {
+        int *q;
+        if ((st = upload_sparse(S, hr, &S->ctx.R)) != CS_OK) return st;
+        if ((st = dev_upload(S, &q, rp2.data(), rp2.size())) != CS_OK) return st; S->ctx.Rc.ptr = q;
+        if ((st = dev_upload(S, &q, ci2.data(), ci2.size())) != CS_OK) return st; S->ctx.Rc.idx = q;
+        if ((st = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) != CS_OK) return st; S->ctx.Rc.pos = q;
     }
     {   // b, c in internal order
         std::vector<double> t((size_t)std::max(m, n));
@@ -511,6 +622,8 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
     if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
     if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;      // x.R and x.Rc went up above
+    if ((st = dev_zeros(S, &x.fpart, (size_t)(x.n_fa + x.n_fb) * kMaxGrid)) != CS_OK) return st;
+    x.R.fpart = x.fpart;
     {   // plain compressed views of the same entries (the FSAI build and the dense factor path walk them)
         int *q;
         if ((st = dev_upload(S, &q, cp2.data(), cp2.size())) != CS_OK) return st; x.Cc.ptr = q;
@@ -546,23 +659,29 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     if ((st = dev_zeros(S, &x.sc, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partial_probe, 1)) != CS_OK) return st;
     lap("vectors");
-    // ---- cooperative grid: as many CTAs as can be co-resident
+    // ---- cooperative grid: as many CTAs as can be co-resident (k_iterate carries the fusion accumulators in dynamic
+    //      shared memory when some rows are fused)
     int sms = 0, occ = 0, occ_min = 1 << 30;
     CS_CUDA(S, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, S->device));
     const void *kernels[] = {(const void *)k_iterate, (const void *)k_iterate_dense, (const void *)k_condition, (const void *)k_residuals,
                              (const void *)k_equilibrate, (const void *)k_barrier_probe};
-    S->dyn_smem = kDynSmem;
+    S->dyn_smem = x.n_fa + x.n_fb > 0 ? (size_t)kFuseSmem : 0;
     for (const void *k : kernels) {
-        if (S->dyn_smem) CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S->dyn_smem));
-        if (const char *cv = getenv("CS_CARVEOUT"))   // experiment switch: shared-memory carve-out in percent (L1 gets the rest)
-            CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(cv)));
-        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, S->dyn_smem));
+        const size_t dyn = k == (const void *)k_iterate ? S->dyn_smem : 0;
+        if (dyn) {
+            CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+            // < 96 KB: ask for the 100 KB carve-out, so that the gathers keep ~128 KB of L1 (they collapse below ~90 KB,
+            // DESIGN.md 8); left to itself the driver picked 132 KB for 2 x 49 KB in an earlier build
+            CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, kFuseCarveoutPct));
+        }
+        CS_CUDA(S, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, kBlock, dyn));
         occ_min = std::min(occ_min, occ);
     }
     if (occ_min < 1) { S->err = "kernel does not fit on an SM"; return CS_ECUDA; }
     S->grid = std::min(sms * occ_min, kMaxGrid);
-    if (verbose) fprintf(stderr, "cs_create: %d SMs x %d CTAs of %d threads, %zu B dynamic shared memory\n", sms, occ_min, kBlock, S->dyn_smem);
-    if (nnz <= 8192) S->grid = 1;   // tiny problem (config 0): one CTA, barriers are __syncthreads (cs_device.cuh)
+    if (verbose) fprintf(stderr, "cs_create: %d SMs x %d CTAs of %d threads, %zu B dynamic shared memory in k_iterate, fused rows %d + %d\n",
+                         sms, occ_min, kBlock, S->dyn_smem, x.n_fa, x.n_fb);
+    if (nnz <= kOneCtaNnz) S->grid = 1;   // tiny problem (config 0): one CTA, barriers are __syncthreads (cs_device.cuh)
     if (S->grid == 1 && m <= kDenseMax) {   // scratch of the dense factor-apply path (cs_params.dense_m_threshold)
         if ((st = dev_zeros(S, &x.dM, (size_t)m * m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.dMd, (size_t)m)) != CS_OK) return st;
@@ -574,7 +693,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.mu = 1.0;
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
     S->prm.o_floor = 1e-16;
-    S->prm.cg_tol = 1e-15;
+    S->prm.cg_tol = 1e-16;
     S->prm.cg_reduce = 0.0;
     S->prm.cg_max_iter = 20000;
     S->prm.precond = 0;
@@ -769,7 +888,7 @@ cs_status cs_solve(cs_solver *S, const cs_schedule *sch, cs_resid *out, int64_t 
     return sticky;
 }
 
-cs_status cs_phase_times(cs_solver *S, double out[8]) {
+cs_status cs_diag_phase_times(cs_solver *S, double out[8]) {
     if (!S || !out) return CS_EINVAL;
     Scalars h;
     CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
@@ -778,7 +897,7 @@ cs_status cs_phase_times(cs_solver *S, double out[8]) {
     return CS_OK;
 }
 
-cs_status cs_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only) {
+cs_status cs_diag_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only) {
     if (n_vec < 1 || n_idx < 1 || n_vec >= INT32_MAX || n_idx >= INT32_MAX || !us_gather || !us_stream_only) return CS_EINVAL;
     int *idx = nullptr; double *x = nullptr, *out = nullptr;
     int sms = 0, dev = 0;
@@ -815,7 +934,7 @@ cs_status cs_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, doubl
     return st;
 }
 
-cs_status cs_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier) {
+cs_status cs_diag_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier) {
     if (!S || n < 1 || !us_per_barrier) return CS_EINVAL;
     cudaEvent_t e0, e1;
     CS_CUDA(S, cudaEventCreate(&e0));

@@ -9,13 +9,16 @@
 
 namespace csd {
 
+// One CTA of 768 threads per SM: 80 registers per thread.  At 64 (2 x 512 threads) ptxas serialises the row pass's batch
+// -- index load, gather, FMA one after the other -- to fit its live values; at 80 it keeps the 8 index loads and the
+// gathers of a batch in flight together (config 4: row pass 138 -> 125 us; profiles/r02_ncu_notes.md).
 #ifndef CS_MINB
-#define CS_MINB 2
+#define CS_MINB 1
 #endif
 #ifndef CS_BLOCK
-#define CS_BLOCK 512
+#define CS_BLOCK 768
 #endif
-constexpr int kBlock = CS_BLOCK;          // threads per CTA (16 warps)
+constexpr int kBlock = CS_BLOCK;          // threads per CTA (24 warps)
 constexpr int kWarps = kBlock / 32;
 constexpr int kMaxRed = 8;           // scalars per grid reduction
 #ifndef CS_SHORTMAX
@@ -28,25 +31,39 @@ constexpr int kShortMax = CS_SHORTMAX;        // segments up to this many non-ze
 constexpr int kChunk = CS_CHUNK;         // long segments are cut into warp-sized chunks of this many non-zeros
 constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
 constexpr int kDenseMax = 256;       // largest m of the dense factor-apply path (cs_params.dense_m_threshold)
-// Build-time alternative, measured and NOT the default (profiles/r01_ncu_notes.md, "TMA-staged stream"): with
-// CS_TMA=1 the matrix stream of every traversal is staged through per-warp shared-memory rings by bulk async
-// copies (cp.async.bulk + mbarrier) instead of ld.global.cs.  Parity-identical; config 4 307 vs 295 us per CG
-// step: the rings take L1 capacity away from the gathers, and below ~90 KB of L1 per SM the gathers collapse
-// (which is why that build uses batches of 4 rows and 2 stages: 48 KB per CTA).
-#ifndef CS_TMA
-#define CS_TMA 0
-#endif
 #ifndef CS_ROUNDK
-#define CS_ROUNDK (CS_TMA ? 4 : 8)
-#endif
-#ifndef CS_STAGES
-#define CS_STAGES 2
+#define CS_ROUNDK 8
 #endif
 constexpr int kRoundK = CS_ROUNDK;   // slice rows per batch (8 values + 8 indices + 8 gathers in flight per lane)
-constexpr int kStages = CS_STAGES;   // per-warp ring of staged batches
-constexpr int kStageVal = kRoundK * 32 * 8, kStageIdx = kRoundK * 32 * 4, kStageBytes = kStageVal + kStageIdx;
-// dynamic shared memory of every cooperative kernel: [warp][stage]{values, indices} then [warp][stage] mbarriers
-constexpr int kDynSmem = CS_TMA ? kWarps * kStages * (kStageBytes + 8) : 0;
+// (A TMA-staged matrix stream -- per-warp shared-memory rings filled by cp.async.bulk + mbarrier -- was built and
+//  measured in round 1: parity-identical, 307 vs 295 us per CG step at config 4, because the rings take L1 capacity
+//  away from the gathers; profiles/r01_ncu_notes.md.  It is not in the tree any more.)
+
+// Heavy-row fusion: the column pass K1 of a CG step holds a_ij and the fresh u_j of every entry in
+// registers, so it can accumulate sum_j a_ij u_j for the few heaviest rows itself; those entries then leave the row
+// pass K2, which would otherwise stream them a second time and gather u through L2.  The accumulators live in shared
+// memory and are private, so that the sums have a fixed order (no atomics):
+//   class A: the kFuseA longest rows -- one accumulator per THREAD and row (any number of lanes may hit the same
+//            row in one instruction);
+//   class B: the next kFuseB rows    -- one accumulator per WARP and row; cs_create marks an entry as fused only if
+//            no lower lane of the same slice (32 columns) holds the same row, the others stay with K2.
+// Which entries are fused is a bit mask per slice row of the column-major copy (Sparse::fmask).
+// Sizes: kFuseA * 6 KB + kFuseB * 192 B (one CTA of 768 threads per SM) must stay below ~96 KB, or the shared-memory
+// carve-out moves from 100 KB to 132 KB per SM and the gathers lose the L1 capacity they need.
+#ifndef CS_FUSE_A
+#define CS_FUSE_A 4
+#endif
+#ifndef CS_FUSE_B
+#define CS_FUSE_B 320
+#endif
+#ifndef CS_FUSE_MINLEN
+#define CS_FUSE_MINLEN 4096
+#endif
+constexpr int kFuseA = CS_FUSE_A, kFuseB = CS_FUSE_B;
+constexpr int kFuseMinLen = CS_FUSE_MINLEN;     // rows shorter than this are never fused
+constexpr int kFuseSmem = (kFuseA * kBlock + kWarps * kFuseB) * 8;   // dynamic shared memory of k_iterate when rows are fused
+constexpr int kFuseK = CS_ROUNDK;          // only the first kFuseK entries of a column can be fused (the heavy rows come first)
+static_assert(kRoundK % 4 == 0 && kFuseA <= kMaxRed, "scatter works in groups of 4; fuse_flush borrows the reduction scratch");
 
 // One sparse format (rows of the row-major copy or columns of the column-major copy): a list of SLICES.
 // A slice is 32 lanes x width entries stored [k][lane] (entry k of lane l at off + 32k + l), so that a
@@ -56,6 +73,7 @@ constexpr int kDynSmem = CS_TMA ? kWarps * kStages * (kStageBytes + 8) : 0;
 //              fill the machine with one thread per segment
 //   T = 32     one CHUNK (<= kChunk entries) of a long segment; these slices come first, and chunk c
 //              either completes its segment (chunk_slot[c] < 0) or writes a partial sum to a slot.
+// Slice descriptor: {offset, first segment id, segments | log2(T) << 8 | (has fused entries) << 16, width}.
 // Padding entries have val = 0 and a valid index.  Rows (and orthant columns) are physically sorted by
 // length at cs_create, so padding is negligible.
 struct Sparse {
@@ -69,6 +87,15 @@ struct Sparse {
     int n_multi;
     const int4 *multi;      // long segments spanning several chunks: {segment id, first slot, number of slots, 0}
     double *partial;        // [slots][2]
+    // K2 view of the row-major copy (heavy-row fusion): the chunk slices [0, n_chunk_k2) hold the entries the row pass
+    // of a CG step still has to do; [n_chunk_k2, n_chunk) hold the fused entries (done by the column pass).  Fused
+    // rows are always finished through multi_k2 = {segment id, first slot, number of slots, fused index + 1 or 0},
+    // which adds the column pass's partial sums fpart[fused index][CTA] in CTA order.
+    int n_chunk_k2, n_multi_k2;
+    const int4 *multi_k2;
+    const double *fpart;
+    // column-major copy only: fmask[(s - n_chunk) * kFuseK + k] = lanes of short slice s whose k-th entry is fused
+    const unsigned *fmask;
 };
 
 // Plain compressed view of one copy (segment s = entries [ptr[s], ptr[s+1]), minor index idx[e], value
@@ -92,6 +119,8 @@ struct Ctx {
     const int *cone_off;    // [n_soc+1] absolute offsets of the Lorentz blocks (cone_off[0] = n_lin)
     const int *perm_r, *perm_c;  // internal index -> caller's index (rows / columns sorted by length)
     Sparse R, C;            // row-major (segments = rows) and column-major (segments = columns) copies of A
+    int n_fa, n_fb;         // heavy-row fusion: internal rows [0, n_fa) are class A, [n_fa, n_fa + n_fb) class B (0, 0: off)
+    double *fpart;          // [n_fa + n_fb][gridDim]: the column pass's partial sums of the fused rows, per CTA
     Csr Rc, Cc;             // plain compressed views of the same two copies
     // FSAI(1) preconditioner G = diag(gd) + strictly-lower part with one entry gm[i] at column partner[i]
     int fsai;               // 0: off (plain Jacobi-equilibrated CG)
@@ -115,7 +144,7 @@ struct Ctx {
     double *partials;       // [2][kMaxRed][gridDim]
     unsigned int *bar;      // grid-barrier word
     Scalars *sc;
-    double *partial_probe;  // scratch of cs_barrier_probe
+    double *partial_probe;  // scratch of cs_diag_barrier_probe
     double mu, t, o_floor, cg_tol, cg_reduce;
     int cg_max_iter;
     double norm_b, norm_c;
@@ -134,74 +163,28 @@ __device__ __forceinline__ double group_reduce(double v) {
     return v;
 }
 
-// ---------------------------------------------------------------------------------------------
-// Bulk asynchronous copies (TMA, cp.async.bulk) global -> shared with mbarrier completion, used by the
-// CS_TMA=1 build only: the matrix stream (values + minor indices of a batch of slice rows) then never enters
-// the LSU/L1TEX pipeline that bounds the gathers, needs no registers while in flight, and one
-// lane issues a whole batch.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ unsigned long long policy_evict_first() {
-    unsigned long long pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ void tma_load(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar, unsigned long long pol) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
-}
-// generic-proxy writes to global memory that a later bulk copy will read (the rescaled matrix values)
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
-
-constexpr int kMaxGrid = 32 * 12;    // CTAs of a cooperative launch (148 SMs x 2 = 296 on B200)
+constexpr int kMaxGrid = 32 * 6;     // CTAs of a cooperative launch (148 SMs x 1 on B200)
 
 // Grid-wide barrier + deterministic all-reduce.
 //   barrier : one 32-bit word; every CTA adds 1 except CTA 0, which adds 2^31 - (grid-1), so the top
 //             bit flips exactly when the last CTA has arrived; each CTA's thread 0 spins on that bit.
 //             One atomic round trip plus the spin; the L2 atomic unit does the counting.
 //   reduce  : every CTA stores its NR partial sums before arriving; after the barrier NR warps of every
-//             CTA read all gridDim partials (<= 12 per lane, all loads in flight), add them in a fixed order
+//             CTA read all gridDim partials (<= 6 per lane, all loads in flight), add them in a fixed order
 //             and butterfly: every CTA gets the same bits without a second barrier.
 // Partials are double buffered (a fast CTA may already write the next reduction's partials while a slow
 // one still reads this one's; it cannot get two barriers ahead).
-// Measured on B200 (cs_barrier_probe): see profiles/r01_ncu_notes.md; a flag/mailbox barrier with a
+// Measured on B200 (cs_diag_barrier_probe): see profiles/r01_ncu_notes.md; a flag/mailbox barrier with a
 // collector CTA was 6.4 us per barrier and is not used.
 struct GridCtl {            // per-thread view of the grid barrier state (uniform over the grid)
     unsigned int *bar;
     int parity;
     double *partials;               // [2][kMaxRed][gridDim]
     double *smem;                   // [kMaxRed * kWarps]
-    uint32_t ring, mbar, units;     // this warp's staging ring and mbarriers (shared-window addresses); batches consumed so far
     // phase clock of CTA 0 / thread 0: [0..7] ns per phase, [8] time of the previous lap (shared memory: no registers)
     __device__ static unsigned long long *clock() { __shared__ unsigned long long ns[9]; return ns; }
     __device__ GridCtl(double *partials_, double *smem_, unsigned int *bar_) : bar(bar_), parity(0), partials(partials_), smem(smem_) {
         if (threadIdx.x == 0) for (int i = 0; i < 8; ++i) clock()[i] = 0;
-#if CS_TMA
-        extern __shared__ __align__(128) unsigned char dyn_smem[];
-        const int warp = threadIdx.x >> 5;
-        ring = smem_u32(dyn_smem) + warp * kStages * kStageBytes;
-        mbar = smem_u32(dyn_smem) + kWarps * kStages * kStageBytes + warp * kStages * 8;
-        units = 0;
-        if ((threadIdx.x & 31) == 0) {
-            for (int i = 0; i < kStages; ++i) mbar_init(mbar + 8 * i, 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            fence_proxy_async();
-        }
-        __syncthreads();
-#endif
         if (threadIdx.x == 0) clock()[8] = now();
     }
     __device__ void sync() {
@@ -285,63 +268,88 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
 // `epi(seg, sums, pre)` is called once per segment with the complete sums, where
 // `pre = epi.pre(seg)` holds whatever the epilogue reads from memory (fetched early).
 //
-// Every warp walks its slices (s = gwarp, gwarp + nwarps, ...).  Per slice, rows are consumed 8 at a
-// time: 8 value + 8 index loads (ld.global.cs: streamed, evict-first, so that the gathered vectors stay
-// in L2), then 8 gathers, then the FMAs -- all loads of a batch are in flight before the first use.
-// The epilogue operands and the next slice descriptor are fetched before the batch loop.
-// (A cp.async-staged variant of this loop was measured SLOWER on B200 -- the LDGSTS instructions add
-// to the L1TEX load that already bounds the gathers; see profiles/r01_ncu_notes.md.)
+// Slice s of the walked range goes to CTA s mod grid (then round-robin over its warps): every CTA -- hence every
+// SM -- gets the same number of slices (+-1) of every width class, also in the last, partial round.  Per slice,
+// rows are consumed 8 at a time: 8 value + 8 index loads (ld.global.cs: streamed, evict-first, so that the
+// gathered vectors stay in L2), then 8 gathers, then the FMAs -- all loads of a batch are in flight before the
+// first use.  The epilogue operands and the next slice descriptor are fetched before the batch loop.
+// (cp.async- and TMA-staged variants of this loop were measured SLOWER on B200, profiles/r01_ncu_notes.md; so was a
+//  software prefetch of the warp's next slice into L2, profiles/r02_ncu_notes.md: the passes are bound by the SM's
+//  L1TEX request path, not by DRAM latency.)
 // Long segments (chunks) leave partial sums; they are finished after a grid barrier in fixed order.
+//
+// VIEW = 1 walks the K2 view of the copy (Sparse::n_chunk_k2, multi_k2): the entries the heavy-row fusion left.
+// FUSE : the traversal is the column pass of a CG step and accumulates a_ij * (value returned by the epilogue of
+//        column j) for every fused entry (Sparse::fmask) into the private shared-memory accumulators.
 // ---------------------------------------------------------------------------------------------
-template <int NV, bool PRISTINE, class Term, class Epi>
-__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc) {
+struct NoFuse {
+    static constexpr bool on = false;
+    template <int N> __device__ __forceinline__ void flags(const unsigned *, int, int, bool (&)[N]) const {}
+    template <int N> __device__ __forceinline__ void scatter(const double (&)[N], const int (&)[N], const bool (&)[N], double) const {}
+};
+// Shared-memory accumulators of the heavy-row fusion (see kFuseA / kFuseB above), in the dynamic shared memory of
+// k_iterate:  A [kFuseA][kBlock]      class A, per thread
+//             B [kWarps][kFuseB]      class B, per warp
+constexpr int kFuseOffB = kFuseA * kBlock;
+struct FuseAcc {
+    static constexpr bool on = true;
+    int n_fa;               // rows [0, n_fa) are class A, [n_fa, n_fa + n_fb) class B
+    __device__ static double *smem() { extern __shared__ __align__(16) double fuse_smem[]; return fuse_smem; }
+    // which of the first kFuseK entries of this lane's column are fused: one warp-uniform 32-byte load of the slice's masks
+    template <int N>
+    __device__ __forceinline__ void flags(const unsigned *fmask, int short_slice, int lane, bool (&f)[N]) const {
+        static_assert(N == kFuseK && N == 8, "the masks of a slice are two 16-byte loads");
+        const uint4 *mp = reinterpret_cast<const uint4 *>(fmask) + 2 * (size_t)short_slice;
+        const uint4 m0 = __ldg(mp), m1 = __ldg(mp + 1);
+        const unsigned m[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+#pragma unroll
+        for (int q = 0; q < N; ++q) f[q] = (m[q] >> lane) & 1u;
+    }
+    // acc[row j[q]] += a[q] * uj for the fused entries (f[q]) among N entries of one column.  The read-modify-writes
+    // are predicated, not branched around, and issued four at a time (loads, adds, stores), so that they overlap: the
+    // rows of a column are distinct, and cs_create fuses a class-B row in at most one lane per slice, so no two of a
+    // warp's read-modify-writes between two __syncwarp()s touch the same accumulator.
+    template <int N>
+    __device__ __forceinline__ void scatter(const double (&a)[N], const int (&j)[N], const bool (&f)[N], double uj) const {
+        double *sm = smem();
+        const int my_a = threadIdx.x, my_b = kFuseOffB + (threadIdx.x >> 5) * kFuseB - n_fa;
+#pragma unroll
+        for (int h = 0; h < N; h += 4) {
+            int q[4];
+            double v[4];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) q[t] = j[h + t] < n_fa ? my_a + j[h + t] * kBlock : my_b + j[h + t];
+#pragma unroll
+            for (int t = 0; t < 4; ++t) v[t] = f[h + t] ? sm[q[t]] : 0.0;
+#pragma unroll
+            for (int t = 0; t < 4; ++t) if (f[h + t]) sm[q[t]] = v[t] + a[h + t] * uj;
+        }
+    }
+};
+
+// the epilogue of a fused column pass returns the value its column's fused entries are multiplied with
+template <bool FUSED, class Epi, class Acc, class Pre>
+__device__ __forceinline__ double call_epi(Epi &epi, int seg, const Acc &acc, const Pre &pre) {
+    if constexpr (FUSED) return epi(seg, acc, pre);
+    else { epi(seg, acc, pre); return 0.0; }
+}
+
+template <int NV, bool PRISTINE, int VIEW = 0, class Term, class Epi, class Fuse = NoFuse>
+__device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi, GridCtl &gc, Fuse fuse = Fuse{}) {
     const int lane = threadIdx.x & 31;
-    // slice s goes to CTA s mod grid (then round-robin over its warps): every CTA -- hence every SM -- gets the
-    // same number of slices (+-1) of every width class, also in the last, partial round
     const int gwarp = blockIdx.x + gridDim.x * (threadIdx.x >> 5);
     const int nwarps = (gridDim.x * kBlock) >> 5;
     const double *gval = PRISTINE ? S.val0 : S.val;
     constexpr int UN = NV == 1 ? kRoundK : kRoundK / 2;   // two-operand gathers: half the batch, same registers
-    int s = gwarp;
-    int4 sl = s < S.n_slice ? __ldg(S.slices + s) : make_int4(0, 0, 0, 0);
-#if CS_TMA
-    // Producer side of this warp's ring: the batches (<= kRoundK rows of one slice) are issued in the order
-    // the loop below consumes them, kStages ahead; lane 0 issues, every lane keeps the (uniform) iterator.
-    int is = s, ioff = sl.x, irem = sl.w;                    // slice, next entry offset, rows left in it
-    while (is < S.n_slice && irem == 0) {
-        is += nwarps;
-        if (is < S.n_slice) { const int4 d = __ldg(S.slices + is); ioff = d.x; irem = d.w; }
-    }
-    auto issue = [&](uint32_t slot) {
-        if (is >= S.n_slice) return;
-        const int rows = min(kRoundK, irem);
-        if (lane == 0) {
-            const uint32_t dst = gc.ring + slot * kStageBytes, mb = gc.mbar + slot * 8;
-            const unsigned long long pol = policy_evict_first();
-            mbar_expect_tx(mb, (uint32_t)rows * 32u * 12u);
-            tma_load(dst, gval + ioff, (uint32_t)rows * 256u, mb, pol);
-            tma_load(dst + kStageVal, S.idx + ioff, (uint32_t)rows * 128u, mb, pol);
-        }
-        ioff += 32 * kRoundK;
-        irem -= kRoundK;
-        while (is < S.n_slice && irem <= 0) {
-            is += nwarps;
-            if (is < S.n_slice) { const int4 d = __ldg(S.slices + is); ioff = d.x; irem = d.w; }
-        }
-    };
-    uint32_t units = gc.units;
-#pragma unroll
-    for (int i = 0; i < kStages; ++i) issue((units + i) % kStages);
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
-    const unsigned char *my_ring = dyn_smem + (threadIdx.x >> 5) * kStages * kStageBytes;
-#endif
+    const int chunk_end = VIEW ? S.n_chunk_k2 : S.n_chunk;
     // The walk is instantiated twice: chunk slices (T = 32, one segment, partial-sum slot) and short-segment slices.
-    auto walk = [&](auto chunk_tag, const int s_end) {
+    auto walk = [&](auto chunk_tag, int s, const int s_end) {
     constexpr bool CH = decltype(chunk_tag)::value;
+    int4 sl = s < s_end ? __ldg(S.slices + s) : make_int4(0, 0, 0, 0);
     while (s < s_end) {
         const int sn = s + nwarps;
-        const int4 nxt = sn < S.n_slice ? __ldg(S.slices + sn) : make_int4(0, 0, 0, 0);
-        const int lgT = CH ? 5 : sl.z >> 8, T = 1 << lgT;     // lanes per segment in this slice
+        const int4 nxt = sn < s_end ? __ldg(S.slices + sn) : make_int4(0, 0, 0, 0);
+        const int lgT = CH ? 5 : (sl.z >> 8) & 7, T = 1 << lgT;     // lanes per segment in this slice
         const int seg = sl.y + (lane >> lgT);
         const bool head = (lane >> lgT) < (sl.z & 255) && (lane & (T - 1)) == 0;
         const int cslot = CH ? __ldg(S.chunk_slot + s) : -1;  // fetched early, like `pre` (warp-uniform address)
@@ -349,34 +357,12 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
         double acc[NV];
 #pragma unroll
         for (int i = 0; i < NV; ++i) acc[i] = 0.0;
-#if CS_TMA
-        for (int k = 0; k < sl.w; k += kRoundK) {
-            const uint32_t slot = units % kStages;
-            mbar_wait(gc.mbar + slot * 8, (units / kStages) & 1);
-            const double *sv = reinterpret_cast<const double *>(my_ring + slot * kStageBytes) + lane;
-            const int *si = reinterpret_cast<const int *>(my_ring + slot * kStageBytes + kStageVal) + lane;
-#pragma unroll
-            for (int q0 = 0; q0 < kRoundK; q0 += UN) {
-                int j[UN];
-#pragma unroll
-                for (int q = 0; q < UN; ++q) j[q] = k + q0 + q < sl.w ? si[32 * (q0 + q)] : -1;
-                typename Term::G g[UN];
-#pragma unroll
-                for (int q = 0; q < UN; ++q) g[q] = term.fetch(j[q] >= 0 ? j[q] : 0);   // index 0: one broadcast wavefront
-#pragma unroll
-                for (int q = 0; q < UN; ++q) if (j[q] >= 0) term.fma(sv[32 * (q0 + q)], g[q], acc);
-            }
-            __syncwarp();                                    // every lane has consumed the stage
-            issue(slot);
-            ++units;
-        }
-#else
         const double *vp = gval + sl.x + lane;
         const int *ip = S.idx + sl.x + lane;
-        for (int k = 0; k < sl.w; k += UN) {
-            double a[UN]; int j[UN];
+        // one batch: UN slice rows from row k on -- all value and index loads, then the gathers, then the FMAs
+        auto batch = [&](int k, double (&a)[UN], int (&j)[UN]) {
 #pragma unroll
-            for (int q = 0; q < UN; ++q) {                   // predicated: no traffic for rows past the end
+            for (int q = 0; q < UN; ++q) {                   // predicated (warp-uniform): no traffic for rows past the end
                 const bool ok = k + q < sl.w;
                 a[q] = ok ? __ldcs(vp + 32 * (k + q)) : 0.0;
                 j[q] = ok ? __ldcs(ip + 32 * (k + q)) : -1;
@@ -386,8 +372,31 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
             for (int q = 0; q < UN; ++q) g[q] = term.fetch(j[q] >= 0 ? j[q] : 0);   // index 0: one broadcast wavefront
 #pragma unroll
             for (int q = 0; q < UN; ++q) if (j[q] >= 0) term.fma(a[q], g[q], acc);
+        };
+        if constexpr (Fuse::on && !CH) {
+            // Column pass of a CG step with heavy-row fusion.  Columns of at most UN entries (the bulk) are one batch
+            // whose values and indices are still in registers when the epilogue has produced u_j.
+            if (sl.w <= UN) {
+                double a[UN]; int j[UN];
+                batch(0, a, j);
+                for (int o = T >> 1; o > 0; o >>= 1) acc[0] += __shfl_xor_sync(0xffffffffu, acc[0], o);
+                double uj = 0.0;
+                if (head) uj = call_epi<Fuse::on>(epi, seg, acc, pre);   // T = 1 whenever the slice has fused entries (cs_create)
+                if (sl.z >> 16) {                            // warp-uniform: some entry of this slice is fused
+                    bool f[UN];
+                    fuse.flags(S.fmask, s - S.n_chunk, lane, f);
+                    fuse.scatter(a, j, f, uj);
+                    __syncwarp();                            // the warp's next slice may hit the same class-B accumulators from other lanes
+                }
+                s = sn;
+                sl = nxt;
+                continue;
+            }
         }
-#endif
+        for (int k = 0; k < sl.w; k += UN) {
+            double a[UN]; int j[UN];
+            batch(k, a, j);
+        }
         if (CH) {
 #pragma unroll
             for (int i = 0; i < NV; ++i) acc[i] = group_reduce<32>(acc[i]);
@@ -397,7 +406,20 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
                 for (int i = 0; i < NV; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], o);
             }
         }
-        if (head) {
+        if constexpr (Fuse::on && !CH) {
+            double uj = 0.0;
+            if (head) uj = call_epi<Fuse::on>(epi, seg, acc, pre);
+            if (sl.z >> 16) {                                // longer columns: their first entries come back from L1 / L2
+                double a[UN]; int j[UN]; bool f[UN];
+                fuse.flags(S.fmask, s - S.n_chunk, lane, f);
+#pragma unroll
+                for (int q = 0; q < UN; ++q) j[q] = f[q] ? __ldg(ip + 32 * q) : 0;
+#pragma unroll
+                for (int q = 0; q < UN; ++q) a[q] = f[q] ? __ldg(vp + 32 * q) : 0.0;
+                fuse.scatter(a, j, f, uj);
+                __syncwarp();
+            }
+        } else if (head) {
             if (cslot < 0) epi(seg, acc, pre);
             else {
 #pragma unroll
@@ -407,16 +429,18 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
         s = sn;
         sl = nxt;
     }
+    return s;
     };
-    walk(std::true_type{}, S.n_chunk);
-    walk(std::false_type{}, S.n_slice);
-#if CS_TMA
-    gc.units = units;
-#endif
-    if (S.n_multi) {
+    // the short-segment slices continue the deal where the chunk slices of this view left off: the chunk walk ends on
+    // the warp's first slice number >= chunk_end, which is congruent to gwarp - chunk_end modulo nwarps past it
+    const int s_short = walk(std::true_type{}, gwarp, chunk_end) - chunk_end + S.n_chunk;
+    walk(std::false_type{}, s_short, S.n_slice);
+    const int n_multi = VIEW ? S.n_multi_k2 : S.n_multi;
+    if (n_multi) {
+        const int4 *multi = VIEW ? S.multi_k2 : S.multi;
         gc.sync();
-        for (int r = gwarp; r < S.n_multi; r += nwarps) {
-            const int4 mr = __ldg(S.multi + r);
+        for (int r = gwarp; r < n_multi; r += nwarps) {
+            const int4 mr = __ldg(multi + r);
             double tot[NV];
 #pragma unroll
             for (int i = 0; i < NV; ++i) {
@@ -431,6 +455,14 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
                     for (int q = 0; q < 8; ++q) a += t[q];
                 }
                 for (; k < mr.z; k += 32) a += __ldcg(pp + (size_t)k * 2);
+                if (VIEW && i == 0 && mr.w) {            // the column pass's share of a fused row, in CTA order
+                    const double *fp = S.fpart + (size_t)(mr.w - 1) * gridDim.x;
+                    double t[kMaxGrid / 32];
+#pragma unroll
+                    for (int q = 0; q < kMaxGrid / 32; ++q) t[q] = lane + 32 * q < (int)gridDim.x ? __ldcg(fp + lane + 32 * q) : 0.0;
+#pragma unroll
+                    for (int q = 0; q < kMaxGrid / 32; ++q) a += t[q];
+                }
                 tot[i] = group_reduce<32>(a);
             }
             if (lane == 0) epi(mr.x, tot, epi.pre(mr.x));
@@ -446,15 +478,12 @@ __device__ __forceinline__ void seg_rescale(const Sparse &S, F &f) {
     const int nwarps = (gridDim.x * kBlock) >> 5;
     for (int s = gwarp; s < S.n_slice; s += nwarps) {
         const int4 sl = __ldg(S.slices + s);
-        const int lgT = sl.z >> 8;
+        const int lgT = (sl.z >> 8) & 7;
         if ((lane >> lgT) < (sl.z & 255)) {
             const int base = sl.x + lane, seg = sl.y + (lane >> lgT);
             for (int k = 0; k < sl.w; ++k) S.val[base + 32 * k] = f(seg, S.val0[base + 32 * k], __ldg(S.idx + base + 32 * k));
         }
     }
-#if CS_TMA
-    fence_proxy_async();   // the next reader of S.val is a bulk async copy (after a grid barrier)
-#endif
 }
 
 }  // namespace csd

@@ -1,7 +1,7 @@
 // cs_kernels.cuh -- the persistent cooperative kernels of libcs.so.
 //
 //   k_iterate   : k passes of Algorithm 2 steps 16-18 incl. the inner CG on (A~ A~')
-//   k_condition : Algorithm 2 steps 5-14 incl. the solve for d
+//   k_condition : Algorithm 2 steps 5-14; step 13's d is folded into the pass, so no solve here
 //   k_residuals : KKT residual norms of the current iterate
 //
 // A~ = D A O is the row-equilibrated, column-conditioned matrix; D = diag(1/||row_i(A O)||_2) is
@@ -92,10 +92,11 @@ struct EpiK1 {
     double *u; double beta; double sigma;
     struct Pre { double u; };
     __device__ __forceinline__ Pre pre(int j) const { return Pre{u[j]}; }
-    __device__ __forceinline__ void operator()(int j, const double (&a)[1], const Pre &q) {
+    __device__ __forceinline__ double operator()(int j, const double (&a)[1], const Pre &q) {
         const double uj = a[0] + beta * q.u;
         u[j] = uj;
         sigma += uj * uj;
+        return uj;           // the fused column pass multiplies the column's heavy-row entries with it
     }
 };
 struct EpiK2 {       // z = preconditioned residual (== r when the FSAI preconditioner is off)
@@ -117,17 +118,50 @@ struct EpiK2 {       // z = preconditioned residual (== r when the FSAI precondi
 //   z_k = dd_k r_k + ee_k r_{partner(k)} + sum_{e in list(k)} cc_e r_{tidx[e]}
 // with dd_k = gd_k^2 + sum_{i in list(k)} gm_i^2, ee_k = gd_k gm_k, cc_e = gd_i gm_i (i = tidx[e]); list(k) = the
 // rows whose partner is k, sorted, so the sum has a fixed order.  One light m-vector pass and one barrier.
+#ifndef CS_FSAI_NB
+#define CS_FSAI_NB 2
+#endif
+// CS_FSAI_NB rows per thread at a time: the loads of a row form a dependent chain (partner / list bounds -> list
+// entry -> r), so the rows of a batch are interleaved by hand to keep several chains in flight (latency-bound).
 __device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
+    constexpr int NB = CS_FSAI_NB;
     double rz = 0.0;
-    for (int k = tid; k < c.m; k += nth) {
-        const int pk = c.f_partner[k];
-        const double rk = c.r[k];
-        double acc = c.f_gd[k] * rk;                         // f_gd holds dd after the build
-        if (pk >= 0) acc += c.f_gm[k] * c.r[pk];             // f_gm holds ee
-        for (int e = c.f_tptr[k]; e < c.f_tptr[k + 1]; ++e) acc += c.f_tc[e] * c.r[c.f_tidx[e]];
-        c.z[k] = acc;
-        rz += rk * acc;
+    for (int k0 = tid; k0 < c.m; k0 += NB * nth) {
+        int pk[NB], e0[NB], e1[NB];
+        double rk[NB], acc[NB], rp[NB], ee[NB];
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const int k = k0 + q * nth;
+            const bool ok = k < c.m;
+            pk[q] = ok ? c.f_partner[k] : -1;
+            e0[q] = ok ? c.f_tptr[k] : 0;
+            e1[q] = ok ? e0[q] + c.f_tcur[k] : 0;          // f_tcur: list length after the build (capped, cs_kernels_cond.cuh)
+            rk[q] = ok ? c.r[k] : 0.0;
+            acc[q] = ok ? c.f_gd[k] : 0.0;                 // f_gd holds dd after the build
+            ee[q] = ok ? c.f_gm[k] : 0.0;                  // f_gm holds ee
+        }
+#pragma unroll
+        for (int q = 0; q < NB; ++q) rp[q] = pk[q] >= 0 ? c.r[pk[q]] : 0.0;
+        int i0[NB];
+        double c0[NB];
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {                     // first list entry of each row (most lists hold 0-2 rows)
+            const bool has = e0[q] < e1[q];
+            i0[q] = has ? c.f_tidx[e0[q]] : -1;
+            c0[q] = has ? c.f_tc[e0[q]] : 0.0;
+        }
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            acc[q] = acc[q] * rk[q] + ee[q] * rp[q];
+            if (i0[q] >= 0) acc[q] += c0[q] * c.r[i0[q]];
+        }
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            for (int e = e0[q] + 1; e < e1[q]; ++e) acc[q] += c.f_tc[e] * c.r[c.f_tidx[e]];
+            const int k = k0 + q * nth;
+            if (k < c.m) { c.z[k] = acc[q]; rz += rk[q] * acc[q]; }
+        }
     }
     double red[1] = {rz};
     grid_reduce<1>(red, gc);
@@ -213,10 +247,42 @@ __device__ __forceinline__ void dense_solve(const Ctx &c) {
     __syncthreads();
 }
 
+// Heavy-row fusion (cs_device.cuh): shared-memory accumulators of the column pass.  fuse_zero before the pass;
+// fuse_flush after it: the CTA's sums per fused row in a fixed order (class A: lanes by butterfly, then warps in
+// order; class B: warps in order) -> c.fpart[row][CTA], which K2's finishing step adds up in CTA order.
+__device__ __forceinline__ void fuse_zero(const Ctx &c) {
+    double *A = FuseAcc::smem(), *B = A + kFuseOffB;
+    for (int i = threadIdx.x; i < c.n_fa * kBlock; i += kBlock) A[i] = 0.0;
+    for (int i = threadIdx.x; i < kWarps * kFuseB; i += kBlock) B[i] = 0.0;
+    __syncthreads();
+}
+__device__ __forceinline__ void fuse_flush(const Ctx &c, double *scratch /* [kFuseA * kWarps] */) {
+    const double *A = FuseAcc::smem(), *B = A + kFuseOffB;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    for (int i = 0; i < c.n_fa; ++i) {
+        const double v = group_reduce<32>(A[i * kBlock + threadIdx.x]);
+        if (lane == 0) scratch[i * kWarps + warp] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < c.n_fa) {
+        double acc = scratch[threadIdx.x * kWarps];
+        for (int w = 1; w < kWarps; ++w) acc += scratch[threadIdx.x * kWarps + w];
+        __stcg(c.fpart + (size_t)threadIdx.x * gridDim.x + blockIdx.x, acc);
+    }
+    for (int i = threadIdx.x; i < c.n_fb; i += kBlock) {
+        double acc = B[i];
+        for (int w = 1; w < kWarps; ++w) acc += B[w * kFuseB + i];
+        __stcg(c.fpart + (size_t)(c.n_fa + i) * gridDim.x + blockIdx.x, acc);
+    }
+    __syncthreads();
+}
+
 __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, double qq, bool &hit_max) {
     // stop on ||r|| <= max(cg_tol ||q||, cg_reduce ||r at the warm start||) (equilibrated system; cs.h)
     const double thresh = fmax(c.cg_tol * c.cg_tol * qq, c.cg_reduce * c.cg_reduce * rr);
     const double *zsrc = c.fsai ? c.z : c.r;
+    const bool fused = c.n_fa + c.n_fb > 0;                  // uniform over the grid
     double beta = 0.0;
     int steps = 0;
     hit_max = false;
@@ -226,7 +292,13 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, do
         if (steps >= c.cg_max_iter) { hit_max = true; break; }
         TermDot t1{zsrc};
         EpiK1 e1{c.u, beta, 0.0};
-        seg_reduce<1, false>(c.C, t1, e1, gc);             // u = A~'z + beta u = A~'v
+        if (fused) {                                       // u = A~'z + beta u = A~'v, and the heavy rows' share of A~u
+            fuse_zero(c);
+            seg_reduce<1, false, 0, TermDot, EpiK1, FuseAcc>(c.C, t1, e1, gc, FuseAcc{c.n_fa});
+            fuse_flush(c, gc.smem);
+        } else {
+            seg_reduce<1, false>(c.C, t1, e1, gc);
+        }
         gc.lap(kPhK1);
         double red[1] = {e1.sigma};
         grid_reduce<1>(red, gc);
@@ -236,7 +308,7 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, do
         const double alpha = rz / sigma;
         TermDot t2{c.u};
         EpiK2 e2{c.v, c.w, c.r, zsrc, alpha, beta, 0.0};
-        seg_reduce<1, false>(c.R, t2, e2, gc);
+        seg_reduce<1, false, 1>(c.R, t2, e2, gc);          // K2 view: without the entries the column pass has done
         gc.lap(kPhK2);
         red[0] = e2.rho;
         grid_reduce<1>(red, gc);

@@ -78,7 +78,7 @@ struct EpiRowScale {  // D_i = 1/||row_i(A O)||, b~ = D b ; the multiplier follo
     typedef NoPre Pre;
     __device__ __forceinline__ Pre pre(int) const { return Pre{}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &) {
-        const double di = 1.0 / sqrt(a[0]);
+        const double di = a[0] > 0.0 && a[0] < INFINITY ? 1.0 / sqrt(a[0]) : D[i];   // a row whose scaled entries underflow keeps its D
         const double ratio = D[i] / di;
         D[i] = di;
         btil[i] = di * b[i];
@@ -113,6 +113,11 @@ struct EpiRecast {    // step 14: s = O^{-1}x - mu O z ; g = A~'w for the warm s
 // config 1; static patterns chosen from the unscaled matrix lose most of that.)
 // ---------------------------------------------------------------------------------------------
 constexpr int kFsaiTop = 3;   // strongest rows kept per column
+// Bounds on the serial work of one thread (every other CTA waits in a grid barrier meanwhile): columns longer than
+// kFsaiColMax propose no partners (one thread walks a column), and a row keeps at most kFsaiListMax of the rows that
+// chose it -- the ones with the smallest indices, so that the choice does not depend on the order of arrival; the
+// others go without a partner.  (A dense column would otherwise make one row the partner of O(m) rows.)
+constexpr int kFsaiColMax = 64, kFsaiListMax = 32;
 
 __device__ __forceinline__ void fsai_build(const Ctx &c, GridCtl &gc) {
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
@@ -120,7 +125,8 @@ __device__ __forceinline__ void fsai_build(const Ctx &c, GridCtl &gc) {
     for (int j = tid; j < c.n; j += nth) {
         int b0 = -1, b1 = -1, b2 = -1;
         double v0 = -1.0, v1 = -1.0, v2 = -1.0;
-        for (int e = c.Cc.ptr[j]; e < c.Cc.ptr[j + 1]; ++e) {
+        const int ce = c.Cc.ptr[j + 1] - c.Cc.ptr[j] <= kFsaiColMax ? c.Cc.ptr[j + 1] : c.Cc.ptr[j];
+        for (int e = c.Cc.ptr[j]; e < ce; ++e) {
             const int i = c.Cc.idx[e];
             if (c.Rc.ptr[i + 1] - c.Rc.ptr[i] > kShortMax) continue;
             const double a = fabs(c.C.val[c.Cc.pos[e]]);
@@ -205,21 +211,26 @@ __device__ __forceinline__ void fsai_build(const Ctx &c, GridCtl &gc) {
         if (pk >= 0) c.f_tidx[c.f_tptr[pk] + atomicAdd(c.f_tcur + pk, 1)] = i;
     }
     gc.sync();
-    for (int k = tid; k < c.m; k += nth) {              // insertion sort: lists are short (a short row tops <= 64 columns)
-        const int a = c.f_tptr[k], b = c.f_tptr[k + 1];
-        for (int e = a + 1; e < b; ++e) {
-            const int x = c.f_tidx[e];
-            int f = e - 1;
-            while (f >= a && c.f_tidx[f] > x) { c.f_tidx[f + 1] = c.f_tidx[f]; --f; }
-            c.f_tidx[f + 1] = x;
+    for (int k = tid; k < c.m; k += nth) {              // selection sort of the kFsaiListMax smallest; the rest lose their partner
+        const int a = c.f_tptr[k], b = c.f_tptr[k + 1], keep = min(b - a, kFsaiListMax);
+        for (int e = a; e < a + keep; ++e) {
+            int best = e, x = c.f_tidx[e];
+            for (int f = e + 1; f < b; ++f) { const int y = c.f_tidx[f]; if (y < x) { x = y; best = f; } }
+            c.f_tidx[best] = c.f_tidx[e];
+            c.f_tidx[e] = x;
         }
+        for (int e = a + keep; e < b; ++e) {
+            const int i = c.f_tidx[e];
+            c.f_partner[i] = -1; c.f_gd[i] = 1.0; c.f_gm[i] = 0.0;
+        }
+        c.f_tcur[k] = keep;                               // list length from here on (apply_fsai)
     }
     gc.sync();
     // F4: assemble G'G row by row (cs_kernels.cuh apply_fsai): t1 <- dd, z <- ee, f_tc <- cc, then move dd/ee
     // into f_gd/f_gm (gd, gm of OTHER rows are still read here, hence the staging in t1/z and a barrier)
     for (int k = tid; k < c.m; k += nth) {
         double dd = c.f_gd[k] * c.f_gd[k];
-        for (int e = c.f_tptr[k]; e < c.f_tptr[k + 1]; ++e) {
+        for (int e = c.f_tptr[k]; e < c.f_tptr[k] + c.f_tcur[k]; ++e) {
             const int i = c.f_tidx[e];
             dd += c.f_gm[i] * c.f_gm[i];
             c.f_tc[e] = c.f_gd[i] * c.f_gm[i];
@@ -266,15 +277,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     TermDot tw{c.w};
     EpiRecast er{c.s, c.g, c.xb, c.zb, c.O, c.mu};
     seg_reduce<1, false>(c.C, tw, er, gc);
-    const int steps = 0;
-    const bool hm = false;
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        c.sc->n_cond += 1;
-        c.sc->cg_steps_total += steps;
-        c.sc->cg_steps_cond += steps;
-        c.sc->cg_steps_last = steps;
-        if (hm) c.sc->cg_hit_max = 1;
-    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) c.sc->n_cond += 1;
 }
 
 // ---- fixed equilibration (cs_equilibrate): Ruiz's simultaneous square-root iteration in the l2 norm ---------

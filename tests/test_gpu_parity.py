@@ -284,7 +284,7 @@ def test_cg_max_is_reported_not_fatal():
 
 
 def test_diagnostic_probes():
-    """cs_gather_probe / cs_barrier_probe run and give sane numbers (the barrier probe checks its all-reduce)."""
+    """cs_diag_gather_probe / cs_diag_barrier_probe run and give sane numbers (the barrier probe checks its all-reduce)."""
     from paper_2103_00736_b200 import binding
     us_g, us_s = binding.gather_probe(1_000_000, 8_000_000)
     assert 0 < us_s < us_g < 5e4

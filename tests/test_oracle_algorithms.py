@@ -517,3 +517,23 @@ def test_exact_solve_resolves_the_projection_on_an_ill_conditioned_system():
         o.run(1)                                                    # l = 1: O = I
         err = np.linalg.norm(o.pinv_apply(rhs) - ref) / np.linalg.norm(ref)
         assert err <= bound, (mode, err)
+
+
+def test_singleton_rows_make_the_zipf_draw_rank_deficient():
+    """Reading (r)/(x): the proofs use A A^dagger = I, i.e. full row rank.  The steep Zipf draw of the GPU shape
+    sweep with rows topped up to ONE entry only has singleton rows that share a column -- two parallel rows, so A is
+    rank-deficient whatever the values -- and the oracle's Cholesky refuses such a matrix; topped up to two entries
+    the draw has no such pair (and thousands of 2-3-entry rows), which is the case the GPU sweep keeps."""
+    def parallel_singletons(p):
+        single = np.flatnonzero(np.diff(p.row_ptr) == 1)
+        cols = p.col_idx[p.row_ptr[single]]
+        return single.size, single.size - np.unique(cols).size
+    bad = W.sparse_lp(15, 4000, 12000, 4, zipf=1.6, min_row_nnz=1)
+    n_single, n_shared = parallel_singletons(bad)
+    assert n_single > 1000 and n_shared > 10
+    small = W.sparse_lp(15, 600, 1800, 4, zipf=1.6, min_row_nnz=1)
+    assert parallel_singletons(small)[1] > 0
+    with pytest.raises(RuntimeError):
+        oracle.Oracle.from_problem(small, solve_mode=1).run(1)
+    ok = W.sparse_lp(15, 4000, 12000, 4, zipf=1.6, min_row_nnz=2)
+    assert parallel_singletons(ok) == (0, 0) and (np.diff(ok.row_ptr) < 4).sum() > 1000
