@@ -98,31 +98,88 @@ def test_conditioning_from_identical_point(name):
 
 @pytest.mark.parametrize("name", COND_CASES)
 def test_iterates_one_early_conditioning(name):
-    """Protocol (ii-b): conditioning at l=20 inside a run.  The rule o = |x|/|z| amplifies the 1e-13
-    differences of the iterates (the oracle's own Cholesky and PCG modes
-    differ by up to 4e-9 here), so x,z,y are compared to 1e-6 and the objective to 1e-6."""
+    """Protocol (ii-b), S 8(c): conditioning at l=20 INSIDE a run, each side from its own iterate.  The rule
+    o = |x|/|z| amplifies what the two sides' iterates differ by before it (1e-14 with the solves taken to their
+    floor) by 1e3-1e4: x, z, y to 1e-9 (B north_star), s and O -- which the protocol holds to 1e-6 -- to 1e-8.
+    Measured (profiles/r02_parity_gaps.md): worst case cfg1 x 1.5e-10, O 3.5e-10; the oracle's own two solve modes
+    differ by x 3.9e-10, O 9.7e-10 there."""
     make, k, okw = CASES[name]
     p = make()
     S, O = _pair(p, solve_mode=1 if p.m <= 4000 else 0)
     S.run(40, L=[20])
     O.run(40, L=[20])
-    got, ref = _check_iterates(S, O, keys=("x", "z", "y", "s", "O"), tol=1e-6)
+    _check_iterates(S, O, keys=("x", "z", "y"), tol=TOL_ITER)
+    _check_iterates(S, O, keys=("s", "O"), tol=1e-8)
     r = _check_resid(S, O)
     assert r["n_conditionings"] == 2  # l=1 and l=20
 
 
+def _oracle_mode_gap(p, run, keys):
+    """What the oracle itself can resolve on this instance: the distance between its two 'exact' solve modes (dense
+    Cholesky with refinement / Jacobi-PCG at 1e-15) after the same run.  Returns (gap per key, mode-1 iterate)."""
+    import oracle
+    outs = []
+    for mode in (1, 2):
+        O = oracle.Oracle.from_problem(p, solve_mode=mode, pcg_tol=1e-15, pcg_max=400000)
+        run(O)
+        outs.append(O.get())
+    return {k: rel(outs[1][k], outs[0][k]) for k in keys}, outs[0]
+
+
 def test_cfg2_replica_illconditioned():
-    """Config 2 recipe (row 10^U(-3,3), column 10^U(-2,2)) at 1/100 scale; the inner systems have
-    cond(AA') ~ 1e13+.  The oracle's own Cholesky and PCG(1e-15) modes differ by 3e-9 on this instance
-    after 30 passes (measured, profiles/r01_parity_notes.md), which bounds what a comparison can resolve:
-    tolerance 1e-8."""
+    """Config 2 recipe (row 10^U(-3,3), column 10^U(-2,2)) at 1/100 scale, 30 passes, L = {}.  ||c|| is 2e4 x ||s||
+    on this instance, so step 18's d = A^dagger b + ... cancels 5 digits and fp64 resolves the iterate to ~1e-9
+    only: against an extended-precision rerun the oracle's Cholesky mode is 6e-10 off, its PCG mode 2e-9
+    (profiles/r02_parity_gaps.md).  Tolerance: 1e-9, or 3x the distance between the oracle's own two modes where
+    that is larger (measured in the test; 2.0e-9 on x, z, s here)."""
     p = W.config(2, 0.01)
-    S, O = _pair(p, solve_mode=1)
+    gap, ref = _oracle_mode_gap(p, lambda O: O.run(30), ("x", "z", "s"))
+    from paper_2103_00736_b200 import binding
+    S = binding.Solver.from_problem(p, device="cuda:0")
     S.run(30)
-    O.run(30)
-    got, ref = S.solution(), O.get()
+    got = S.solution()
     for k in ("x", "z", "s"):
-        assert rel(got[k], ref[k]) <= 1e-8, (k, rel(got[k], ref[k]))
+        tol = max(TOL_ITER, 3.0 * gap[k])
+        assert tol <= 1e-8 and rel(got[k], ref[k]) <= tol, (k, rel(got[k], ref[k]), gap[k])
+
+
+@pytest.mark.parametrize("cfg,scale", [(4, 0.02), (2, 0.02)])
+def test_conditioned_passes_on_midsize_replicas(cfg, scale):
+    """The regime bench.py times (passes AFTER a conditioning, FSAI on) at a size the oracle still finishes: steps
+    5-14 from identical (x, z) bits (the oracle's iterate after 10 passes), then 3 passes.
+    Config 4 (Zipf rows, heavy-row fusion active): x, z, y, s to 1e-9, O to 1e-12.
+    Config 2: after a conditioning with t = 9.2 the scaled cost vector is ~1e7 x ||s||, and fp64 resolves a pass to
+    ~3e-7 only -- both oracle modes are 3e-7 from an extended-precision rerun and from each other
+    (profiles/r02_parity_gaps.md) -- so the tolerance there is 3x the oracle's own mode-to-mode distance."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = W.config(cfg, scale)
+    O0 = oracle.Oracle.from_problem(p)
+    O0.run(10)
+    start = O0.get()
+
+    def run(O):
+        O.set_point(start["x"], start["z"])
+        O.run(3, L=[1])
+
+    keys = ("x", "z", "y", "s")
+    if cfg == 2:
+        gap, ref = _oracle_mode_gap(p, run, keys)
+        tol = {k: max(TOL_ITER, 3.0 * gap[k]) for k in keys}
+        assert max(tol.values()) <= 1e-5, gap
+    else:
+        O = oracle.Oracle.from_problem(p, pcg_tol=1e-15, pcg_max=400000)
+        run(O)
+        ref, tol = O.get(), {k: TOL_ITER for k in keys}
+    S = binding.Solver.from_problem(p, device="cuda:0")
+    S.set_point(start["x"], start["z"])
+    S.run(3, L=[1])
+    got, r = S.solution(), S.residuals()
+    assert rel(got["O"], ref["O"]) <= 1e-12
+    assert got["O"].max() / got["O"].min() > 100.0
+    for k in keys:
+        assert rel(got[k], ref[k]) <= tol[k], (k, rel(got[k], ref[k]), tol[k])
+    assert r["cg_steps_total"] > 300 and r["cg_hit_max"] == 0
 
 
 def test_inexact_projections_reach_the_same_optimum():

@@ -22,6 +22,12 @@ SHAPES = {
     "lp_wide": lambda: W.sparse_lp(13, 40, 6000, 3),
     "lp_zipf_multichunk": lambda: W.sparse_lp(14, 1500, 9000, 6, zipf=1.1, min_row_nnz=4),
     "lp_zipf_steep": lambda: W.sparse_lp(15, 4000, 12000, 4, zipf=1.6, min_row_nnz=4),   # >= 4 per row: DESIGN.md 3 reading (x)
+    # the same draw with 3,669 rows of 2-3 entries (full row rank, sigma_min 5e-3).  With min_row_nnz = 1 the draw is
+    # rank-deficient (singleton rows sharing a column), outside reading (r); that is pinned on the CPU by
+    # tests/test_oracle_algorithms.py::test_singleton_rows_make_the_zipf_draw_rank_deficient.
+    "lp_zipf_steep_short_rows": lambda: W.sparse_lp(15, 4000, 12000, 4, zipf=1.6, min_row_nnz=2),
+    # one dense column: every row's strongest column may be the same one; the FSAI build must stay bounded
+    "lp_one_dense_column": lambda: _with_dense_column(W.sparse_lp(21, 3000, 9000, 5)),
     "socp_tiny_blocks": lambda: W.sparse_socp(16, 200, 900, 450, 4, lo=1, hi=3),
     "socp_large_blocks": lambda: W.sparse_socp(17, 300, 1500, 5, 5, lo=200, hi=400),
     "socp_plus_orthant": lambda: W.sparse_socp(18, 700, 2500, 60, 8, n_lin=1000, lo=2, hi=50),
@@ -30,15 +36,27 @@ SHAPES = {
 }
 
 
+def _with_dense_column(p):
+    """p with column 0 replaced by a dense column of large entries (b, c rebuilt from the constructed optimum)."""
+    import scipy.sparse as sp
+    rng = np.random.default_rng(99)
+    A = p.csr().tolil()
+    A[:, 0] = (5.0 + rng.random(p.m)).reshape(-1, 1)
+    A = sp.csr_matrix(A)
+    A.sort_indices()
+    return W._assemble("lp_one_dense_column", A, p.x0, p.s0, rng, p.n, np.zeros(0, np.int32), t=9.2)
+
+
 @pytest.mark.parametrize("name", list(SHAPES))
 def test_shape_sweep_against_the_oracle(name):
     import oracle
     from paper_2103_00736_b200 import binding
     p = SHAPES[name]()
-    O = oracle.Oracle.from_problem(p)
+    mode = 1 if p.m <= 4000 else 0         # reading (s): the oracle's dense Cholesky + refinement where it is affordable
+    O = oracle.Oracle.from_problem(p, solve_mode=mode)
     O.run(6)
     mid = O.get()
-    O2 = oracle.Oracle.from_problem(p)
+    O2 = oracle.Oracle.from_problem(p, solve_mode=mode)
     O2.set_point(mid["x"], mid["z"])
     O2.run(6, L=[1])                       # conditioning at l = 1 from (x, z) of the first leg: the rule on identical bits
     ref = O2.get()
