@@ -193,6 +193,20 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out);
  * Any pointer may be NULL.  Synchronous when where == CS_HOST. */
 cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where);
 
+/* The ONE entry point that allocates nothing -- no handle, no cudaMalloc/cudaFree, no allocating library routine --
+ * for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid it): the cone
+ * part of the residual norms (a6; P:566-572 x in K, z in K) of a caller-held iterate,
+ *     out[0] = ||x - proj_K x||_2   out[1] = ||z - proj_K z||_2   out[2] = ||x||_2   out[3] = ||z||_2
+ *     out[4] = cone_viol_rel = (out[0] + out[1]) / (1 + out[2] + out[3])          (cs_resid.cone_viol_rel)
+ * x_dev, z_dev: DEVICE arrays [n] in the caller's order (orthant coordinates first, then the Lorentz blocks of K);
+ * out: 5 doubles in `out_where` (CS_HOST: synchronous; CS_DEVICE: asynchronous on `cuda_stream`).
+ * Its scratch (cone offsets, per-CTA partial sums) is a file-scope device array of 145 KB that every GPU loading the
+ * library holds until exit; hence the LIMIT K->n_soc <= 32768 Lorentz cones (any n_lin, n < 2^31), beyond which the
+ * call returns CS_EINVAL with the limit in cs_last_error(NULL).  All calls share that array: calls that overlap on
+ * the GPU (other streams, other host threads) race -- serialise them.  Runs on the current device. */
+cs_status cs_cone_violation_static(const double *x_dev, const double *z_dev, int64_t n, const cs_cones *K, double *out,
+                                   cs_mem out_where, void *cuda_stream);
+
 /* Number of kernels the library has launched on this handle so far (for bench accounting). */
 int64_t cs_kernel_launches(const cs_solver *S);
 

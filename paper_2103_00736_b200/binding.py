@@ -54,7 +54,7 @@ CS_RULE_SET, CS_RULE_STALL = 0, 1
 
 _INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
                "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_diag_phase_times",
-               "cs_diag_gather_probe", "cs_diag_barrier_probe")
+               "cs_diag_gather_probe", "cs_diag_barrier_probe", "cs_cone_violation_static")
 EXPORTS = _INT_STATUS + ("cs_kernel_launches", "cs_last_error", "cs_destroy")
 
 _lib = None
@@ -90,6 +90,7 @@ def lib():
         L.cs_equilibrate.argtypes = [vp, C.c_int32]
         L.cs_solve.argtypes = [vp, C.POINTER(cs_schedule), C.POINTER(cs_resid), C.POINTER(C.c_int64), C.c_int64,
                                C.POINTER(C.c_int64)]
+        L.cs_cone_violation_static.argtypes = [vp, vp, C.c_int64, C.POINTER(cs_cones), vp, C.c_int, vp]
         for name in _INT_STATUS:
             getattr(L, name).restype = C.c_int
         _lib = L
@@ -134,6 +135,22 @@ def gather_probe(n_vec, n_idx):
     if st != CS_OK:
         raise CsError(st, "cs_diag_gather_probe failed")
     return a.value, b.value
+
+
+def cone_violation_static(x, z, n_lin, soc_size=None, out=None, stream=None):
+    """cs_cone_violation_static: x, z = CUDA tensors [n]; returns the 5 doubles (numpy) or fills the CUDA tensor `out`."""
+    xp, zp = _ptr(x, np.float64), _ptr(z, np.float64)
+    if xp[1] != CS_DEVICE or zp[1] != CS_DEVICE:
+        raise ValueError("x and z must live in device memory")
+    soc = np.ascontiguousarray(soc_size if soc_size is not None else [], dtype=np.int32)
+    K = cs_cones(int(n_lin), int(soc.shape[0]), soc.ctypes.data if soc.size else None)
+    res = np.empty(5) if out is None else out
+    op = _ptr(res, np.float64)
+    st = lib().cs_cone_violation_static(xp[0], zp[0], int(x.shape[0]), C.byref(K), op[0], op[1],
+                                        C.c_void_p(int(stream)) if stream else None)
+    if st != CS_OK:
+        raise CsError(st, lib().cs_last_error(None).decode())
+    return res
 
 
 class Solver:

@@ -11,6 +11,7 @@
 #include <chrono>
 #include <cstdlib>
 #include <memory>
+#include <mutex>
 #include <new>
 #include <string>
 #include <thread>
@@ -20,6 +21,9 @@
 #include "../../include/cs_diag.h"
 #include "cs_kernels_cond.cuh"
 
+#ifndef CS_STATIC_MAX_SOC
+#define CS_STATIC_MAX_SOC 32768
+#endif
 #ifndef CS_FUSE_CARVEOUT
 #define CS_FUSE_CARVEOUT 43
 #endif
@@ -981,3 +985,160 @@ cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, 
 }
 
 }  // extern "C"
+
+// =================================================================================================
+// cs_cone_violation_static -- the ONE entry point of the library that allocates nothing (cs.h): for callers that
+// cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it).  It is the cone
+// part of k_residuals (distance of x and z to K, their norms) as a handle-free kernel whose scratch -- the cone
+// offsets, the per-CTA partial sums, the arrival ticket and the result -- lives in a file-scope device array of
+// fixed size.  Every GPU that loads libcs.so holds these kStaticBytes until the process exits.
+// In host code `g_static_scratch` is only a stand-in for the symbol; the device address comes from
+// cudaGetSymbolAddress, once per device, with that device current (static_scratch_address).
+// All calls share the array: calls that overlap on the GPU (different streams, different host threads) RACE.
+// =================================================================================================
+namespace {
+constexpr int kStaticMaxSoc = CS_STATIC_MAX_SOC;     // largest n_soc the entry point accepts
+constexpr int kStaticMaxGrid = 512;                  // CTAs of its launch (<= 2 per SM)
+constexpr int kStaticThreads = 256;
+constexpr size_t kStaticOffPartials = ((size_t)(kStaticMaxSoc + 1) * sizeof(int) + 255) / 256 * 256;
+constexpr size_t kStaticOffTicket = kStaticOffPartials + (size_t)4 * kStaticMaxGrid * sizeof(double);
+constexpr size_t kStaticOffOut = kStaticOffTicket + 256;
+constexpr size_t kStaticBytes = kStaticOffOut + 256;   // 128 KB of offsets + 16 KB of partials + ticket + result
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+namespace {
+// x, z [n] in the caller's order (orthant coordinates first, then the Lorentz blocks at off[0..n_soc]); out[5] =
+// {||x - proj_K x||, ||z - proj_K z||, ||x||, ||z||, cone_viol_rel}.  One launch: every CTA leaves its four partial
+// sums in the scratch, the last one to arrive (ticket) adds them in CTA order -- deterministic.
+__global__ void __launch_bounds__(kStaticThreads) k_cone_violation_static(const double *x, const double *z, int n_lin, int n_soc,
+                                                                          unsigned char *scratch, double *out) {
+    const int *off = reinterpret_cast<const int *>(scratch);
+    double *partials = reinterpret_cast<double *>(scratch + kStaticOffPartials);     // [4][gridDim]
+    unsigned int *ticket = reinterpret_cast<unsigned int *>(scratch + kStaticOffTicket);
+    __shared__ double sm[4][kStaticThreads / 32];
+    __shared__ bool last;
+    const int tid = blockIdx.x * kStaticThreads + threadIdx.x, nth = gridDim.x * kStaticThreads;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double v[4] = {0.0, 0.0, 0.0, 0.0};                      // dist2(x), dist2(z), ||x||^2, ||z||^2
+    for (int j = tid; j < n_lin; j += nth) {
+        const double a = x[j], b = z[j], am = fmin(a, 0.0), bm = fmin(b, 0.0);
+        v[0] += am * am; v[1] += bm * bm; v[2] += a * a; v[3] += b * b;
+    }
+    {   // Lorentz blocks: kConeLanes lanes per block, as in k_residuals
+        const int sub = lane / kConeLanes, sl = lane % kConeLanes;
+        constexpr int CPW = 32 / kConeLanes;
+        const int gwarp = tid >> 5, nwarps = nth >> 5;
+        for (int base = gwarp * CPW; base < n_soc; base += nwarps * CPW) {
+            const int ci = base + sub;
+            const bool act = ci < n_soc;
+            const int a = act ? off[ci] : 0, b = act ? off[ci + 1] : 0;
+            double nx = 0.0, nz = 0.0;
+            for (int j = a + 1 + sl; j < b; j += kConeLanes) { nx += x[j] * x[j]; nz += z[j] * z[j]; }
+            nx = group_reduce<kConeLanes>(nx);
+            nz = group_reduce<kConeLanes>(nz);
+            if (act && sl == 0) {
+                v[0] += soc_dist2(x[a], nx); v[1] += soc_dist2(z[a], nz);
+                v[2] += x[a] * x[a] + nx;    v[3] += z[a] * z[a] + nz;
+            }
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const double r = group_reduce<32>(v[q]);
+        if (lane == 0) sm[q][warp] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double acc = sm[threadIdx.x][0];
+        for (int w = 1; w < kStaticThreads / 32; ++w) acc += sm[threadIdx.x][w];
+        __stcg(partials + (size_t)threadIdx.x * gridDim.x + blockIdx.x, acc);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    if (warp < 4) {                                          // warp q adds the partials of sum q in CTA order
+        double acc = 0.0;
+        for (int b = lane; b < (int)gridDim.x; b += 32) acc += __ldcg(partials + (size_t)warp * gridDim.x + b);
+        acc = group_reduce<32>(acc);
+        if (lane == 0) sm[warp][0] = sqrt(acc);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        out[0] = sm[0][0]; out[1] = sm[1][0]; out[2] = sm[2][0]; out[3] = sm[3][0];
+        out[4] = (sm[0][0] + sm[1][0]) / (1.0 + sm[2][0] + sm[3][0]);
+        *ticket = 0u;                                        // leave the ticket at zero for the next call
+    }
+}
+
+// device address of g_static_scratch on the CURRENT device, resolved once per device (cudaGetSymbolAddress)
+cs_status static_scratch_address(unsigned char **out, std::string *err) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static unsigned char *addr[kMaxDev] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) { *err = "no CUDA device"; return CS_ECUDA; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        unsigned char *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void **)&p, g_static_scratch);
+        if (e != cudaSuccess || !p) { *err = std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e); return CS_ECUDA; }
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return CS_OK;
+}
+}  // namespace
+
+extern "C" cs_status cs_cone_violation_static(const double *x_dev, const double *z_dev, int64_t n, const cs_cones *K,
+                                              double *out, cs_mem out_where, void *cuda_stream) {
+    std::string &err = g_create_err;                         // no handle: the text goes where cs_create's goes (cs_last_error(NULL))
+    if (!x_dev || !z_dev || !K || !out || n <= 0 || n >= INT32_MAX || K->n_lin < 0 || K->n_soc < 0 || (K->n_soc > 0 && !K->soc_size)) {
+        err = "cs_cone_violation_static: NULL argument or bad sizes";
+        return CS_EINVAL;
+    }
+    if (K->n_soc > kStaticMaxSoc) {
+        err = "cs_cone_violation_static: n_soc = " + std::to_string(K->n_soc) + " exceeds the static scratch (at most " +
+              std::to_string(kStaticMaxSoc) + " Lorentz cones); use cs_create + cs_residuals";
+        return CS_EINVAL;
+    }
+    static thread_local int h_off[kStaticMaxSoc + 1];        // host staging of the offsets: no heap either
+    int64_t off = K->n_lin;
+    for (int64_t i = 0; i < K->n_soc; ++i) {
+        if (K->soc_size[i] < 1) { err = "cs_cone_violation_static: soc_size entries must be >= 1"; return CS_EINVAL; }
+        h_off[i] = (int)off;
+        off += K->soc_size[i];
+        if (off > n) break;
+    }
+    if (off != n) { err = "cs_cone_violation_static: n_lin + sum(soc_size) != n"; return CS_EINVAL; }
+    h_off[K->n_soc] = (int)n;
+    unsigned char *scratch = nullptr;
+    cs_status st = static_scratch_address(&scratch, &err);
+    if (st != CS_OK) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // the array keeps the previous call's contents: the offsets are overwritten, the ticket must start at zero
+    if (e == cudaSuccess) e = cudaMemcpyAsync(scratch, h_off, sizeof(int) * (size_t)(K->n_soc + 1), cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(scratch + kStaticOffTicket, 0, sizeof(unsigned int), stream);
+    if (e == cudaSuccess) {
+        const int64_t want = (n + kStaticThreads - 1) / kStaticThreads;
+        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(want, std::min(2 * sms, kStaticMaxGrid)));
+        double *out_dev = out_where == CS_DEVICE ? out : reinterpret_cast<double *>(scratch + kStaticOffOut);
+        k_cone_violation_static<<<grid, kStaticThreads, 0, stream>>>(x_dev, z_dev, (int)K->n_lin, (int)K->n_soc, scratch, out_dev);
+        e = cudaGetLastError();
+        if (e == cudaSuccess && out_where == CS_HOST) {
+            e = cudaMemcpyAsync(out, out_dev, 5 * sizeof(double), cudaMemcpyDeviceToHost, stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        }
+    }
+    // h_off is reused by the next call of this thread: the H2D copy from pageable memory has been staged when
+    // cudaMemcpyAsync returns (CUDA runtime semantics for pageable host memory)
+    if (e != cudaSuccess) { err = std::string("cs_cone_violation_static: ") + cudaGetErrorString(e); return CS_ECUDA; }
+    return CS_OK;
+}
