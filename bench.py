@@ -45,6 +45,34 @@ def algorithmic_bytes(p, k_iter, cg_steps, n_cond, fsai=False):
     return cg * cg_steps + outer * k_iter + cond * n_cond, cg
 
 
+def survey_bytes(p, k_iter, cg_steps):
+    """SURVEY.md 8(d) as written: one CG step = 24 nnz + 20 n + 100 m; one outer iteration = (n_cg + 1) CG-step
+    equivalents + 40 n.  Preconditioner traffic is NOT counted as algorithmic here."""
+    cg = 24 * p.nnz + 20 * p.n + 100 * p.m
+    return cg * (cg_steps + k_iter) + 40 * p.n * k_iter, cg
+
+
+def ncu_capture(cfg):
+    """DRAM / L2 bytes, duration and registers of ONE k_iterate launch from the committed `ncu --set full` capture
+    (profiles/r02_ncu_k_iterate_cfg<N>.csv: metric,value,unit rows exported with --page raw; the .md beside it names
+    the command).  The captured launch is capped at 30 CG steps per pass, so the bytes are scaled per CG step."""
+    path = os.path.join(ROOT, "profiles", f"r02_ncu_k_iterate_cfg{cfg}.csv")
+    if not os.path.exists(path):
+        return None
+    unit_scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12,
+                  "ns": 1e-9, "us": 1e-6, "ms": 1e-3, "s": 1.0, "usecond": 1e-6, "msecond": 1e-3, "nsecond": 1e-9, "second": 1.0}
+    out = {}
+    for line in open(path):
+        parts = [x.strip() for x in line.rstrip("\n").split(",")]
+        if len(parts) < 2 or parts[0].startswith("#") or parts[0] == "metric":
+            continue
+        try:
+            out[parts[0]] = float(parts[1]) * unit_scale.get(parts[2] if len(parts) > 2 else "", 1.0)
+        except ValueError:
+            out[parts[0]] = parts[1]
+    return out
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -107,7 +135,8 @@ def oracle_sample(cfg, scale, steps, warmup, k):
             "sample": f"{p.name}: m={p.m} n={p.n} nnz={p.nnz}, {steps} steps of (conditioning + {k} passes) in {dt:.2f}s = "
                       f"{its:.4f} it/s on the replica, scaled by nnz ratio {ratio:.4g} to the full config (CG-step growth "
                       f"with size ignored)",
-            "pcg_steps_per_pass": (O.counters()["pcg_steps_total"] - c0) / (steps * k)}, dt
+            "pcg_steps_per_pass": (O.counters()["pcg_steps_total"] - c0) / (steps * k),
+            "pcg_steps_per_s_full_size": (O.counters()["pcg_steps_total"] - c0) / dt * ratio, "steps": steps, "warmup": warmup}, dt
 
 
 ORACLE_SCALE = {0: 1.0, 1: 0.25, 2: 0.02, 3: 0.1, 4: 0.01}
@@ -138,7 +167,8 @@ def solve_to_tolerance(a, p, S, torch):
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     l, hist, r = 0, [], None
-    while l < a.max_iter:
+    cap_s = getattr(a, "time_cap_s", None)
+    while l < a.max_iter and not (cap_s and time.perf_counter() - t0 > cap_s):
         nxt = min(a.max_iter, (l // a.check_every + 1) * a.check_every)
         S.run(nxt - l, L=[x for x in L if l < x <= nxt])
         l = nxt
@@ -148,7 +178,7 @@ def solve_to_tolerance(a, p, S, torch):
             break
     dt = time.perf_counter() - t0
     out = {"mode": "solve", "workload": p.name, "tol": a.tol, "reached": bool(r["kkt_rel"] <= a.tol),
-           "time_to_tol_s": dt, "iterations": l, "cg_steps_total": r["cg_steps_total"],
+           "time_to_tol_s": dt, "time_cap_s": cap_s, "iterations": l, "cg_steps_total": r["cg_steps_total"],
            "n_conditionings": r["n_conditionings"], "kkt_rel": r["kkt_rel"], "pobj": r["pobj"],
            "cg_tol": S.get_params()["cg_tol"], "cg_reduce": S.get_params()["cg_reduce"],
            "opt_value": p.opt_value(), "iters_per_s": l / dt,
@@ -167,7 +197,7 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--k", type=int, default=1, help="outer iterations per step (1 = continuous conditioning, P:313)")
-    ap.add_argument("--e2e-steps", type=int, default=1)
+    ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 (SOCP) block")
     ap.add_argument("--no-time-to-tol", action="store_true", help="skip the time-to-1e-4-KKT leg of the default run")
@@ -299,17 +329,32 @@ def main():
               "K1_us": 1e3 * ph["K1"] / max(1, cg_iter), "K2_us": 1e3 * ph["K2"] / max(1, cg_iter),
               "reduce_us_per_cg": 1e3 * ph["reduce"] / max(1, cg_iter),
               "precond_us_per_cg": 1e3 * ph["precond"] / max(1, cg_iter)}
-    # DRAM bytes of k_iterate from the ncu --set full captures in profiles/r01_ncu_notes.md, as a ratio to
-    # the algorithmic bytes of the captured launch (dram__bytes_read.sum + dram__bytes_write.sum) / bytes
-    ncu_ratio = {3: 0.826, 4: 0.956 if fsai_on else 0.912}.get(a.config if a.scale == 1.0 else -1)
-    roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": ncu_ratio * it_bytes / a.steps if ncu_ratio else None,
-            "traffic_source": "profiles/r01_ncu_notes.md (v7/v4/v3 captures: DRAM bytes / algorithmic bytes of the captured "
-                              "launch, applied to this launch)" if ncu_ratio else None,
+    # `achieved` follows SURVEY.md 8(d)'s per-unit bytes (24 nnz + 20 n + 100 m per CG step; no preconditioner traffic);
+    # the figure with DESIGN.md's own per-kernel accounting (incl. the FSAI pass) is reported beside it.
+    sv_bytes, sv_cg = survey_bytes(p, n_it, cg_iter)
+    achieved_sv = sv_bytes / (ms_iter * 1e-3) / 1e9
+    # DRAM traffic of k_iterate: from the committed `ncu --set full` capture of the same kernel (one launch capped at
+    # 30 CG steps per pass), per CG step, applied to this launch's CG steps
+    cap = ncu_capture(a.config) if a.scale == 1.0 else None
+    traffic = traffic_src = None
+    if cap and cap.get("cg_steps_in_launch"):
+        per_cg = (cap["dram__bytes_read.sum"] + cap["dram__bytes_write.sum"]) / (cap["cg_steps_in_launch"] + 1)
+        traffic = per_cg * (cg_iter + n_it) / a.steps
+        traffic_src = (f"profiles/r02_ncu_k_iterate_cfg{a.config}.csv: (dram__bytes_read.sum + dram__bytes_write.sum) of the captured launch "
+                       f"/ its {int(cap['cg_steps_in_launch'])} + 1 CG-step equivalents = {per_cg / 1e9:.4f} GB per CG step "
+                       f"({per_cg / sv_cg:.3f} x the algorithmic bytes), times this launch's CG steps")
+    roof = {"bound": "hbm", "kernel": "k_iterate", "achieved": achieved_sv, "peak": peak, "unit": "GB/s",
+            "frac": achieved_sv / peak, "traffic": traffic, "traffic_source": traffic_src,
+            "bytes_source": "SURVEY.md 8(d): (24 nnz + 20 n + 100 m) per CG step, (n_cg + 1) CG-step equivalents + 40 n per pass",
             "peak_source": peak_src,
-            "bytes_per_launch": it_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
-            "cg_steps_per_launch": cg_iter / a.steps, "bytes_per_cg_step": cg_bytes,
-            "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "frac_of_8TBs": achieved / 8000.0,
+            "bytes_per_launch": sv_bytes / a.steps, "ms_per_launch": ms_iter / a.steps,
+            "cg_steps_per_launch": cg_iter / a.steps, "bytes_per_cg_step": sv_cg,
+            "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "cg_steps_per_s": cg_iter / (ms_iter * 1e-3),
+            "frac_of_8TBs": achieved_sv / 8000.0,
+            "design_bytes": {"achieved": achieved, "frac": achieved / peak, "bytes_per_cg_step": cg_bytes,
+                             "note": "DESIGN.md 8 per-kernel accounting: 24 nnz + 28 n + 60 m, + 60 m for the FSAI pass"},
+            "ncu_capture": {k: cap[k] for k in ("gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum", "lts__t_bytes.sum",
+                                                "launch__registers_per_thread", "cg_steps_in_launch") if k in cap} if cap else None,
             "kernel_share_of_step": ms_iter / ms_total, "phases": phases, "gather_ceiling": gather}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms_max / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -319,11 +364,15 @@ def main():
                        "l2": "inputs larger than L2" if 24 * p.nnz > 126e6 else "matrix fits in L2 (flagged)",
                        "gen_s": round(t_gen, 2)},
             "clocks": clk, "gpu_launches": int(launches), "kkt_rel": r1["kkt_rel"], "iter_total": r1["iter"],
-            "cg_steps_timed": int(cg_steps), "cg_steps_per_iter": cg_iter / n_it, "roofline": roof}
+            "cg_steps_timed": int(cg_steps), "cg_steps_per_iter": cg_iter / n_it,
+            "value_note": "CG steps per pass depend on where the timed steps fall in the run (they grow while continuous "
+                          "conditioning proceeds), so `value` depends on --steps/--warmup; roofline.cg_steps_per_s and "
+                          "us_per_cg_step do not",
+            "roofline": roof}
     return finish(a, p, S, line, rank, world, dev, stream)
 
 
-def secondary_workload(cfg, a, dev, stream, peak):
+def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
     """The same step on another config, reported inside the one JSON line (north_star names the largest LP
     AND the SOCP): value, us per CG step and the roofline fraction, no e2e / CPU legs."""
     import torch
@@ -347,20 +396,67 @@ def secondary_workload(cfg, a, dev, stream, peak):
     dt = time.perf_counter() - t0
     cg_iter = (r1["cg_steps_total"] - r0["cg_steps_total"]) - (r1["cg_steps_cond"] - r0["cg_steps_cond"])
     it_bytes, cg_bytes = algorithmic_bytes(p, steps * a.k, cg_iter, 0, p.t >= 4.0)
-    achieved = it_bytes / (ms_iter * 1e-3) / 1e9
+    sv_bytes, sv_cg = survey_bytes(p, steps * a.k, cg_iter)
+    achieved = sv_bytes / (ms_iter * 1e-3) / 1e9
     us_g, _ = binding.gather_probe(p.n, p.nnz)
     ph = S.phase_times()       # device time per phase over the whole life of the handle (warm-up included), ns
     cg_all = max(1, r1["cg_steps_total"] - r1["cg_steps_cond"])
     phases = {k + "_us_per_cg": ph[k] / cg_all / 1e3 for k in ("K1", "K2", "reduce", "precond")}
+    # L2 roofline (configs 1-3 are L2-resident, "report L2 throughput for them"): achieved = bytes the
+    # kernel pulls through L2 per CG step (lts__t_bytes of the committed ncu capture) / time, against an L2-resident copy
+    # measured live (l2_copy_peak)
+    cap = ncu_capture(cfg)
+    l2 = None
+    if cap and cap.get("cg_steps_in_launch") and l2_peak:
+        lts_per_cg = cap["lts__t_bytes.sum"] / (cap["cg_steps_in_launch"] + 1)
+        ach = lts_per_cg * (cg_iter + steps * a.k) / (ms_iter * 1e-3) / 1e9
+        l2 = {"bound": "l2", "achieved": ach, "peak": l2_peak["gbs"], "unit": "GB/s", "frac": ach / l2_peak["gbs"],
+              "lts_bytes_per_cg_step": lts_per_cg, "peak_source": l2_peak["how"],
+              "source": f"profiles/r02_ncu_k_iterate_cfg{cfg}.csv lts__t_bytes.sum per CG step x this run's CG steps"}
     out = {"workload": p.name, "m": p.m, "n": p.n, "nnz": p.nnz, "n_soc": p.n_soc, "value": steps * a.k / dt, "unit": UNIT,
            "steps": steps, "k_per_step": a.k, "cg_steps_per_iter": cg_iter / (steps * a.k),
-           "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "bytes_per_cg_step": cg_bytes,
+           "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "cg_steps_per_s": cg_iter / (ms_iter * 1e-3), "bytes_per_cg_step": sv_cg,
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                        "note": "the 96 MB of matrix copies partly stay in the 126 MB L2"},
+                        "note": "matrix copies of %d MB: (partly) resident in the 126 MB L2, so the HBM fraction is not the yardstick "
+                                "here; see roofline_l2" % (24 * p.nnz // 10**6)},
+           "roofline_l2": l2,
            "gather_ceiling_frac": (2 * p.nnz * cg_iter / (ms_iter * 1e-3)) / (p.nnz / (us_g * 1e-6)), "phases": phases,
            "kkt_rel": r1["kkt_rel"]}
     S.destroy()
+    # B's third metric on this workload: paper schedule, exact projections (the parity setting) and cg_reduce = 0.3
+    import argparse as _ap
+    for tag, prm in (("time_to_kkt_1e-4_exact", {}), ("time_to_kkt_1e-4", {"cg_tol": 1e-12, "cg_reduce": 0.3})):
+        try:
+            a2 = _ap.Namespace(**{**vars(a), "tol": 1e-4, "check_every": 25, "max_iter": 3000, "time_cap_s": 60.0})
+            S2 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
+            if prm:
+                S2.set_params(**prm)
+            t2t = solve_to_tolerance(a2, p, S2, torch)
+            t2t.pop("history", None)
+            out[tag] = t2t
+        except Exception as e:  # pragma: no cover
+            out[tag] = {"error": str(e)}
     return out
+
+
+def l2_copy_peak(torch, dev):
+    """L2-resident copy bandwidth (read + write bytes / s): torch b.copy_(a) over 2 x 24 MB buffers that stay in the
+    126 MB L2, best of 20 back-to-back batches of 20 copies (CUDA events)."""
+    nbytes = 24 * 2**20
+    a_ = torch.empty(nbytes // 8, dtype=torch.float64, device=dev).normal_()
+    b_ = torch.empty_like(a_)
+    for _ in range(5):
+        b_.copy_(a_)
+    best = 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(20):
+        e0.record()
+        for _ in range(20):
+            b_.copy_(a_)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, 20 * 2 * nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return {"gbs": best, "how": "torch b.copy_(a), 2 x 24 MB fp64 buffers (L2-resident), read + write bytes, best of 20 batches of 20 copies"}
 
 
 def finish(a, p, S, line, rank, world, dev, stream):
@@ -373,7 +469,10 @@ def finish(a, p, S, line, rank, world, dev, stream):
     S.destroy()
     if a.config == 4 and a.scale == 1.0 and world == 1 and not a.cg_max_iter and not a.no_secondary:
         try:
-            line["secondary"] = {"cfg3_socp": secondary_workload(3, a, dev, stream, line["roofline"]["peak"])}
+            l2p = l2_copy_peak(torch, dev)
+            line["secondary"] = {"l2_copy_peak": l2p,
+                                 "cfg3_socp": secondary_workload(3, a, dev, stream, line["roofline"]["peak"], l2p),
+                                 "cfg1_lp": secondary_workload(1, a, dev, stream, line["roofline"]["peak"], l2p)}
         except Exception as e:  # pragma: no cover
             line["secondary"] = {"error": str(e)}
         # B's third metric, "time to 1e-4 relative KKT residual", on the headline workload with the paper's
@@ -392,6 +491,12 @@ def finish(a, p, S, line, rank, world, dev, stream):
             t2t.pop("history", None)
             t2t["inexact_projections"] = "cg_reduce=0.2: a pass's solve stops when the warm-start residual has dropped 5x (cs.h)"
             line["time_to_kkt_1e-4"] = t2t
+            # exact projections (the parity setting, cg_tol 1e-16): 719 s in round 1, so a 60 s cap and what it reached
+            a3 = _ap.Namespace(**{**vars(a), "tol": 1e-4, "check_every": 25, "max_iter": 3000, "time_cap_s": 60.0})
+            S5 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
+            t2e = solve_to_tolerance(a3, p, S5, torch)
+            t2e.pop("history", None)
+            line["time_to_kkt_1e-4_exact"] = t2e
             # the same with a criteria-driven schedule ("user-defined criteria"): cs_solve's stall rule
             S4 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
             S4.set_params(cg_tol=1e-12, cg_reduce=0.3)
@@ -438,7 +543,12 @@ def finish(a, p, S, line, rank, world, dev, stream):
                            "cs_residuals + cs_solution(host x,z)"}
     if rank == 0:
         if not a.no_cpu_baseline and world == 1:
-            base, _ = oracle_sample(a.config, ORACLE_SCALE[a.config] * a.scale, 2, 1, a.k)
+            # the same protocol as the --impl reference arm (oracle_sample with this line's steps / warm-up), bounded to
+            # 5 + 3 steps so that the default run stays within its ~30 s of CPU work; the cap is stated in `sample`
+            bs, bw = min(a.steps, 5), min(a.warmup, 3)
+            base, _ = oracle_sample(a.config, ORACLE_SCALE[a.config] * a.scale, bs, bw, a.k)
+            if (bs, bw) != (a.steps, a.warmup):
+                base["sample"] += f"; bounded to {bs} steps after {bw} warm-up steps (the GPU line ran {a.steps} after {a.warmup})"
             line["cpu_baseline"] = base
         else:
             line["cpu_baseline"] = None
