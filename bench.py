@@ -404,7 +404,7 @@ def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
     phases = {k + "_us_per_cg": ph[k] / cg_all / 1e3 for k in ("K1", "K2", "reduce", "precond")}
     # L2 roofline (configs 1-3 are L2-resident, "report L2 throughput for them"): achieved = bytes the
     # kernel pulls through L2 per CG step (lts__t_bytes of the committed ncu capture) / time, against an L2-resident copy
-    # measured live (l2_copy_peak)
+    # measured live (l2_read_peak)
     cap = ncu_capture(cfg)
     l2 = None
     if cap and cap.get("cg_steps_in_launch") and l2_peak:
@@ -439,24 +439,12 @@ def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
     return out
 
 
-def l2_copy_peak(torch, dev):
-    """L2-resident copy bandwidth (read + write bytes / s): torch b.copy_(a) over 2 x 24 MB buffers that stay in the
-    126 MB L2, best of 20 back-to-back batches of 20 copies (CUDA events)."""
-    nbytes = 24 * 2**20
-    a_ = torch.empty(nbytes // 8, dtype=torch.float64, device=dev).normal_()
-    b_ = torch.empty_like(a_)
-    for _ in range(5):
-        b_.copy_(a_)
-    best = 0.0
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for _ in range(20):
-        e0.record()
-        for _ in range(20):
-            b_.copy_(a_)
-        e1.record()
-        torch.cuda.synchronize()
-        best = max(best, 20 * 2 * nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9)
-    return {"gbs": best, "how": "torch b.copy_(a), 2 x 24 MB fp64 buffers (L2-resident), read + write bytes, best of 20 batches of 20 copies"}
+def l2_read_peak():
+    """L2 -> SM read bandwidth measured live with the library's probe (cs_diag_l2_probe: 16-byte loads over a 32 MB
+    buffer, 50 passes, best of 4)."""
+    from paper_2103_00736_b200 import binding
+    return {"gbs": binding.l2_probe(32 * 2**20, 50),
+            "how": "cs_diag_l2_probe: 16-byte ld.global.cg over a 32 MB L2-resident buffer, 50 passes, best of 4 launches"}
 
 
 def finish(a, p, S, line, rank, world, dev, stream):
@@ -469,8 +457,8 @@ def finish(a, p, S, line, rank, world, dev, stream):
     S.destroy()
     if a.config == 4 and a.scale == 1.0 and world == 1 and not a.cg_max_iter and not a.no_secondary:
         try:
-            l2p = l2_copy_peak(torch, dev)
-            line["secondary"] = {"l2_copy_peak": l2p,
+            l2p = l2_read_peak()
+            line["secondary"] = {"l2_read_peak": l2p,
                                  "cfg3_socp": secondary_workload(3, a, dev, stream, line["roofline"]["peak"], l2p),
                                  "cfg1_lp": secondary_workload(1, a, dev, stream, line["roofline"]["peak"], l2p)}
         except Exception as e:  # pragma: no cover

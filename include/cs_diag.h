@@ -23,6 +23,10 @@ cs_status cs_diag_phase_times(cs_solver *S, double out[8]);
  * LSU/L1TEX gather ceiling that bounds the sparse passes on irregular matrices. */
 cs_status cs_diag_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only);
 
+/* Diagnostic (no handle, current device, default stream, synchronous): L2 -> SM read bandwidth in GB/s -- `reps` passes
+ * of 16-byte loads over a `bytes`-sized buffer that stays in L2 (choose bytes well below the 126 MB of L2), best of 4. */
+cs_status cs_diag_l2_probe(int64_t bytes, int32_t reps, double *gbs);
+
 /* Diagnostic: run n empty grid barriers (each a 1-value all-reduce over all CTAs, result checked) in one
  * launch and report the mean latency in microseconds.  Synchronous. */
 cs_status cs_diag_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier);

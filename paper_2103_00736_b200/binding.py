@@ -54,7 +54,7 @@ CS_RULE_SET, CS_RULE_STALL = 0, 1
 
 _INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
                "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_diag_phase_times",
-               "cs_diag_gather_probe", "cs_diag_barrier_probe", "cs_cone_violation_static")
+               "cs_diag_gather_probe", "cs_diag_barrier_probe", "cs_diag_l2_probe", "cs_cone_violation_static")
 EXPORTS = _INT_STATUS + ("cs_kernel_launches", "cs_last_error", "cs_destroy")
 
 _lib = None
@@ -90,6 +90,7 @@ def lib():
         L.cs_equilibrate.argtypes = [vp, C.c_int32]
         L.cs_solve.argtypes = [vp, C.POINTER(cs_schedule), C.POINTER(cs_resid), C.POINTER(C.c_int64), C.c_int64,
                                C.POINTER(C.c_int64)]
+        L.cs_diag_l2_probe.argtypes = [C.c_int64, C.c_int32, C.POINTER(C.c_double)]
         L.cs_cone_violation_static.argtypes = [vp, vp, C.c_int64, C.POINTER(cs_cones), vp, C.c_int, vp]
         for name in _INT_STATUS:
             getattr(L, name).restype = C.c_int
@@ -135,6 +136,15 @@ def gather_probe(n_vec, n_idx):
     if st != CS_OK:
         raise CsError(st, "cs_diag_gather_probe failed")
     return a.value, b.value
+
+
+def l2_probe(nbytes=32 * 2**20, reps=50):
+    """L2 -> SM read bandwidth in GB/s (cs_diag_l2_probe)."""
+    g = C.c_double()
+    st = lib().cs_diag_l2_probe(int(nbytes), int(reps), C.byref(g))
+    if st != CS_OK:
+        raise CsError(st, "cs_diag_l2_probe failed")
+    return g.value
 
 
 def cone_violation_static(x, z, n_lin, soc_size=None, out=None, stream=None):

@@ -568,30 +568,34 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         hc2 = make_sparse(cp2, ri2, cv2, nt, fuse.rows() ? &fuse : nullptr, fuse.rows() ? &fused : nullptr);
         lap("column-major slices");
         // fused rows: entries that stay with the row pass first, the fused ones after them (each part keeps its
-        // ascending column order); split[s] = size of the first part
+        // ascending column order); split[s] = size of the first part.  The rows are rebuilt from the column-major copy
+        // by two sequential scans over the columns (count, then place): the fused rows are the first entries of a
+        // column (rows ascend), so a column is left as soon as a row >= fuse.rows() shows up -- no searching.
         std::vector<int> split((size_t)fuse.rows());
         if (fuse.rows() && !hc2.too_big) {
-            for (int sfr = 0; sfr < fuse.rows(); ++sfr) {
-                const int a0 = rp2[sfr], len = rp2[(size_t)sfr + 1] - a0;
-                uvec<int> tj((size_t)len);
-                uvec<double> tv((size_t)len);
-                uvec<unsigned char> tf((size_t)len);
-                const int blk = 1 << 16;
-                parallel_blocks((len + blk - 1) / blk, nt, [&](int bi) {
-                    for (int k = bi * blk; k < std::min(len, (bi + 1) * blk); ++k) {
-                        const int j = ci2[a0 + k];
-                        const int *lo = ri2.data() + cp2[j], *hi = ri2.data() + cp2[(size_t)j + 1];
-                        const int *q = std::lower_bound(lo, hi, sfr);      // rows are ascending within a column
-                        tf[k] = fused[(size_t)(q - ri2.data())];
-                        tj[k] = j;
-                        tv[k] = va2[a0 + k];
-                    }
-                });
-                int w0 = a0;
-                for (int k = 0; k < len; ++k) if (!tf[k]) { ci2[w0] = tj[k]; va2[w0] = tv[k]; ++w0; }
-                split[sfr] = w0 - a0;
-                for (int k = 0; k < len; ++k) if (tf[k]) { ci2[w0] = tj[k]; va2[w0] = tv[k]; ++w0; }
+            const int nf = fuse.rows(), cblk = 1 << 16, nblk = (n + cblk - 1) / cblk;
+            std::vector<int> cnt((size_t)nblk * nf * 2, 0);      // [block][row][unfused, fused]
+            parallel_blocks(nblk, nt, [&](int bi) {
+                int *c = cnt.data() + (size_t)bi * nf * 2;
+                for (int j = bi * cblk; j < std::min(n, (bi + 1) * cblk); ++j)
+                    for (int e = cp2[j]; e < cp2[(size_t)j + 1] && ri2[e] < nf; ++e) c[2 * ri2[e] + fused[e]] += 1;
+            });
+            std::vector<int> off((size_t)nblk * nf * 2);
+            for (int r = 0; r < nf; ++r) {
+                int u = rp2[r];
+                for (int bi = 0; bi < nblk; ++bi) { off[((size_t)bi * nf + r) * 2] = u; u += cnt[((size_t)bi * nf + r) * 2]; }
+                split[r] = u - rp2[r];
+                for (int bi = 0; bi < nblk; ++bi) { off[((size_t)bi * nf + r) * 2 + 1] = u; u += cnt[((size_t)bi * nf + r) * 2 + 1]; }
             }
+            parallel_blocks(nblk, nt, [&](int bi) {
+                int *o = off.data() + (size_t)bi * nf * 2;
+                for (int j = bi * cblk; j < std::min(n, (bi + 1) * cblk); ++j)
+                    for (int e = cp2[j]; e < cp2[(size_t)j + 1] && ri2[e] < nf; ++e) {
+                        const int q = o[2 * ri2[e] + fused[e]]++;
+                        ci2[q] = j;
+                        va2[q] = cv2[e];
+                    }
+            });
             S->ctx.n_fa = fuse.n_fa;
             S->ctx.n_fb = fuse.n_fb;
             lap("fused rows: partition");
@@ -935,6 +939,38 @@ cs_status cs_diag_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, 
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
     cudaFree(idx); cudaFree(x); cudaFree(out);
+    return st;
+}
+
+cs_status cs_diag_l2_probe(int64_t bytes, int32_t reps, double *gbs) {
+    if (bytes < 4096 || bytes > ((int64_t)1 << 32) || reps < 1 || !gbs) return CS_EINVAL;
+    double2 *buf = nullptr; double *out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cs_status st = CS_ECUDA;
+    int sms = 0, dev = 0;
+    do {
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) break;
+        const long long n16 = bytes / 16;
+        if (cudaMalloc(&buf, (size_t)n16 * 16) != cudaSuccess || cudaMalloc(&out, 8) != cudaSuccess) { st = CS_ENOMEM; break; }
+        if (cudaMemset(buf, 0, (size_t)n16 * 16) != cudaSuccess) break;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+        double best = 0.0;
+        bool ok = true;
+        for (int rep = 0; rep < 4 && ok; ++rep) {                // the first launch also warms L2; keep the best
+            cudaEventRecord(e0);
+            k_l2_probe<<<sms * 4, 512>>>(buf, n16, reps, out);
+            cudaEventRecord(e1);
+            float ms = 0.f;
+            ok = cudaEventSynchronize(e1) == cudaSuccess && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess;
+            if (ok && ms > 0.f) best = std::max(best, (double)n16 * 16.0 * reps / (ms * 1e-3) / 1e9);
+        }
+        if (!ok) break;
+        *gbs = best;
+        st = CS_OK;
+    } while (false);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf); cudaFree(out);
     return st;
 }
 

@@ -464,6 +464,24 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_gather_probe(const int *idx
     }
     out[tid] = acc;
 }
+// Diagnostic: every thread streams 16-byte loads over a buffer small enough to stay in L2, `reps` times: the L2 -> SM
+// read bandwidth of the chip (the roofline of the L2-resident configs 1-3).
+__global__ void __launch_bounds__(512) k_l2_probe(const double2 *buf, long long n16, int reps, double *out) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nth = (long long)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    for (int r = 0; r < reps; ++r) {
+        long long i = tid;
+        for (; i + 3 * nth < n16; i += 4 * nth) {
+            double2 v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) v[q] = __ldcg(buf + i + q * nth);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc += v[q].x + v[q].y;
+        }
+        for (; i < n16; i += nth) { const double2 v = __ldcg(buf + i); acc += v.x + v.y; }
+    }
+    if (acc == 12345.6789) out[0] = acc;      // keeps the loads alive
+}
 __global__ void k_probe_indices(int *idx, int n_idx, int n_vec) {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
     for (int i = tid; i < n_idx; i += nth) {

@@ -19,7 +19,7 @@ def test_library_exports_every_declared_symbol():
     inc = os.path.join(ROOT, "include")
     header = "".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b(cs_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(cs_[a-z0-9_]+)\s*\(", header))
     assert {"cs_create", "cs_set_params", "cs_iterate", "cs_condition", "cs_residuals", "cs_solution"} <= declared
     for name in declared:
         assert getattr(lib, name) is not None, name
