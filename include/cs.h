@@ -82,11 +82,16 @@ typedef struct {
  *            approximate inverse factor with one off-diagonal entry per row, rebuilt on the device at every
  *            conditioning.  Changes the number of CG steps, not the solution of the solve.
  *   dense_m_threshold  dense factor-apply instead of CG where A is small enough that the solve truly is a dense
- *            contraction (B north_star; S 8(a) a3): when the problem runs on one CTA (nnz <= 8192) and
- *            m <= dense_m_threshold (<= 256), every conditioning forms A~A~' (m x m, fp64), factors it by
- *            Cholesky on the device, and every pass applies the factor (two triangular solves + one step of
- *            iterative refinement) -- no CG steps are counted.  0 = never; default 128.  A pivot below 1e-12 (the
- *            diagonal of A~A~' is 1: numerically rank-deficient A) falls back to CG for that scaling.
+ *            contraction (B north_star; S 8(a) a3, S 8(f).3), for m <= dense_m_threshold (<= 4096; 0 = never):
+ *            - problems that run on one CTA (nnz <= 8192) with m <= 256: every conditioning forms A~A~' (m x m, fp64) and
+ *              factors it by Cholesky in that CTA; every pass applies the factor (two triangular solves + one step of
+ *              iterative refinement);
+ *            - dense-STORED inputs (nnz >= m n / 2: the paper's own workloads, section V-A, V-D P:366-371) on
+ *              many CTAs: every conditioning forms M = A~A~', its blocked Cholesky factor and the explicit inverse
+ *              M^-1 = L^-T L^-1 (hand-written fp64 kernels, csrc/cs_dense.cuh); every pass is w += M^-1 r followed by two
+ *              steps of iterative refinement against M -- dense matrix-vector products only.
+ *            No CG steps are counted.  Default: 128, or 4096 for a dense-stored input.  A Cholesky pivot below 1e-12
+ *            (the diagonal of A~A~' is 1: numerically rank-deficient A) falls back to CG for that scaling.
  * cs_set_params may be called at any time; mu, t, o_floor, precond, dense_m_threshold take effect at the next
  * cs_condition (or at the implicit first conditioning), cg_* at the next solve. */
 typedef struct {
@@ -120,7 +125,7 @@ typedef struct {
 /* Build a solver for (A,b,c,K): validates the input, copies it to the device, builds the CSC copy of A
  * and the work partitions.  b[m], c[n] live in `vec_where`.  Parameters start at mu=1, t=9.2 (n_soc=0)
  * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-16, cg_reduce=0, cg_max_iter=20000, precond=0,
- * dense_m_threshold=128; the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
+ * dense_m_threshold=128 (4096 for a dense-stored A); the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
  * mandatory first conditioning (l=1) the identity and s=0.  Synchronous.  On failure *out is NULL. */
 cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
                     const cs_cones *K, void *cuda_stream);

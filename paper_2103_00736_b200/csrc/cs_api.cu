@@ -347,12 +347,44 @@ void sync_params(cs_solver *S) {
     S->ctx.cg_max_iter = S->prm.cg_max_iter;
 }
 
+// Grid dense path: M = A~A~', its blocked Cholesky factor and the explicit inverse, from the values k_condition has
+// just rescaled (cs_dense.cuh).  Ordinary kernel launches on the handle's stream, no host synchronisation.
+cs_status dense_grid_factor(cs_solver *S) {
+    const Ctx &c = S->ctx;
+    const int m = c.m, n = c.n;
+    const size_t mm = (size_t)m * m;
+    const int tiles = (m + 63) / 64, n_tri = tiles * (tiles + 1) / 2, one = 1;
+    CS_CUDA(S, cudaMemsetAsync(c.gAd, 0, sizeof(double) * (size_t)m * n, S->stream));
+    CS_CUDA(S, cudaMemsetAsync(c.gZ, 0, sizeof(double) * mm, S->stream));
+    CS_CUDA(S, cudaMemcpyAsync(c.g_ok, &one, sizeof(int), cudaMemcpyHostToDevice, S->stream));
+    k_dense_scatter<<<148 * 4, 256, 0, S->stream>>>(c, c.gAd);
+    k_dense_aat<<<n_tri, 256, 0, S->stream>>>(c.gAd, m, n, c.gM);
+    CS_CUDA(S, cudaMemcpyAsync(c.gL, c.gM, sizeof(double) * mm, cudaMemcpyDeviceToDevice, S->stream));
+    S->launches += 2;
+    for (int kb = 0; kb < m; kb += kCholNB) {
+        k_chol_diag<<<1, kCholNB * kCholNB, 0, S->stream>>>(c.gL, m, kb, c.g_ok);
+        S->launches += 1;
+        const int rest = m - kb - kCholNB;
+        if (rest <= 0) break;
+        k_chol_panel<<<std::min(148 * 4, (rest + 7) / 8), 256, 0, S->stream>>>(c.gL, m, kb);
+        const int t = (rest + 63) / 64;
+        k_chol_update<<<t * (t + 1) / 2, 256, 0, S->stream>>>(c.gL, m, kb);
+        S->launches += 2;
+    }
+    k_dense_trinv<<<std::min(148 * 8, (m + 7) / 8), 256, 0, S->stream>>>(c.gL, m, c.gZ);
+    k_dense_aat<<<n_tri, 256, 0, S->stream>>>(c.gZ, m, m, c.gMinv);
+    S->launches += 2;
+    CS_CUDA(S, cudaGetLastError());
+    return CS_OK;
+}
+
 cs_status do_condition(cs_solver *S, int use_rule) {
     cs_status st = ensure_xz(S);
     if (st != CS_OK) return st;
     // automatic: FSAI(1) pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs);
     // with the SOCP setting t = 1.7 it saves ~10 % of the CG steps and costs 18 % per step (measured)
-    S->ctx.dense = S->grid == 1 && S->ctx.dM && S->ctx.m <= S->prm.dense_m_threshold;
+    S->ctx.dense = (S->grid == 1 && S->ctx.dM && S->ctx.m <= std::min(S->prm.dense_m_threshold, kDenseMax)) ? 1
+                 : (S->grid > 1 && S->ctx.gM && S->ctx.m <= S->prm.dense_m_threshold) ? 2 : 0;
     S->ctx.fsai = !S->ctx.dense && (S->prm.precond == 2 || (S->prm.precond == 0 && S->prm.t >= 4.0));
     S->ctx.mu = S->prm.mu;  // mu, t, o_floor, precond take effect here (cs.h)
     S->ctx.t = S->prm.t;
@@ -361,6 +393,7 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     void *args[] = {&S->ctx, &use_rule};
     st = launch_coop(S, (const void *)k_condition, args);
     if (st != CS_OK) return st;
+    if (S->ctx.dense == 2 && (st = dense_grid_factor(S)) != CS_OK) return st;
     S->conditioned = true;
     S->started = true;
     S->stall_at = -1;          // residuals of the old scaling do not compare with the new one's
@@ -695,6 +728,15 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         if ((st = dev_zeros(S, &x.dMd, (size_t)m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.dv, (size_t)2 * m)) != CS_OK) return st;
     }
+    // grid dense path (cs_dense.cuh): only for a dense-stored A (at least half of the m x n entries present) on many CTAs
+    if (S->grid > 1 && m <= kDenseGridMax && (double)nnz >= 0.5 * (double)m * (double)n) {
+        const size_t mm = (size_t)m * m;
+        if ((st = dev_zeros(S, &x.gAd, (size_t)m * n)) != CS_OK) return st;
+        double **gm[] = {&x.gM, &x.gL, &x.gZ, &x.gMinv};
+        for (double **q : gm) if ((st = dev_zeros(S, q, mm)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.dv, (size_t)4 * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.g_ok, 1)) != CS_OK) return st;
+    }
     if ((st = dev_zeros(S, &x.bar, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * kMaxGrid)) != CS_OK) return st;
     // ---- defaults (cs.h)
@@ -705,7 +747,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.cg_reduce = 0.0;
     S->prm.cg_max_iter = 20000;
     S->prm.precond = 0;
-    S->prm.dense_m_threshold = 128;
+    S->prm.dense_m_threshold = x.gM ? kDenseGridMax : 128;   // dense-stored input: the dense path is the default (cs.h)
     S->prm.reserved = 0;
     S->nnz = nnz;
     x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
@@ -737,8 +779,8 @@ cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const dou
 cs_status cs_set_params(cs_solver *S, const cs_params *p) {
     if (!S || !p) return CS_EINVAL;
     if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || !(p->cg_reduce >= 0.0 && p->cg_reduce < 1.0) || p->cg_max_iter < 1 ||
-        p->precond < 0 || p->precond > 2 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseMax) {
-        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2}, dense_m_threshold in [0,256]";
+        p->precond < 0 || p->precond > 2 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseGridMax) {
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2}, dense_m_threshold in [0,4096]";
         return CS_EINVAL;
     }
     S->prm = *p;

@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
     }
     gc.sync();
     if (c.fsai) fsai_build(c, gc);   // its own barriers; reads the rescaled values only
-    if (c.dense) dense_factor(c);    // one-CTA problems only (cs_api.cu): A~A~' and its Cholesky factor
+    if (c.dense == 1) dense_factor(c);    // one-CTA problems only (cs_api.cu): A~A~' and its Cholesky factor
     // Step 13's d is never formed: it is folded into the pass (cs_kernels.cuh), so a conditioning needs no
     // solve.  What remains is the recast of s (step 14) and g = A~'w in the new scaling.
     TermDot tw{c.w};

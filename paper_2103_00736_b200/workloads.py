@@ -276,6 +276,22 @@ def gaussian_dense_lp(seed, m=80, n=100, name="sec4a_gaussian_lp"):
                    x0=nanv(n), y0=nanv(m), s0=nanv(n), t=9.2, L_first=300, L_every=100)
 
 
+def dense_lp_sec5a(seed, n=100, name="sec5a_dense_lp"):
+    """PAPER.md:342-346 (section V-A): m = floor(0.8 n), A ~ U[-1,1] dense, b = A |xdot| with xdot ~ N(0,1),
+    c ~ N(0,1), K = R^n_+; schedule (17), t = 9.2, mu = 1.  No constructed optimum."""
+    rng = np.random.default_rng(seed)
+    m = int(0.8 * n)
+    M = rng.uniform(-1.0, 1.0, size=(m, n))
+    xdot = rng.standard_normal(n)
+    A = sp.csr_matrix(M)
+    A.sort_indices()
+    nanv = lambda k: np.full(k, np.nan)
+    return Problem(name=name, m=m, n=n, row_ptr=A.indptr.astype(np.int32),
+                   col_idx=A.indices.astype(np.int32), val=A.data.copy(), b=M @ np.abs(xdot),
+                   c=rng.standard_normal(n), n_lin=n, soc_size=np.zeros(0, np.int32),
+                   x0=nanv(n), y0=nanv(m), s0=nanv(n), t=9.2, L_first=300, L_every=100)
+
+
 def dense_socp_sec5d(seed, n=100, h=4, name="sec5d_dense_socp"):
     """PAPER.md:366-371 (section V-D) shape: m = floor(0.8 n), A ~ U[-1,1] dense, K = (K_h)^(n/h),
     c ~ U[0,1]; b = A * xfeas with xfeas in K.  The paper writes b = A*abs_K(xdot); here xfeas is

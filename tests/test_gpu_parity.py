@@ -504,7 +504,52 @@ def test_dense_factor_apply_matches_cg_and_oracle(name):
     _check_iterates(S, O)
     _check_resid(S, O)
     with pytest.raises(binding.CsError):
-        S.set_params(dense_m_threshold=257)
+        S.set_params(dense_m_threshold=4097)
+
+
+@pytest.mark.parametrize("name", ["sec5d_h4", "sec5d_h10", "sec5a_lp"])
+def test_grid_dense_factor_apply_on_the_papers_dense_shapes(name):
+    """S 8(f).3: the paper's own workloads (section V-D SOCP K = (K_h)^(n/h); section V-A dense LP)
+    at n = 1000, m = 800 through the grid dense path (csrc/cs_dense.cuh: explicit inverse of A~A~' rebuilt at every
+    conditioning, dense GEMVs + refinement per pass; the default for a dense-stored input): no CG steps, and the same
+    iterates as the CG path and as the oracle (dense Cholesky + refinement) to 1e-9 -- without a conditioning (protocol i)
+    and through a conditioning from identical bits (protocol ii-a)."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = {"sec5d_h4": lambda: W.dense_socp_sec5d(7, n=1000, h=4), "sec5d_h10": lambda: W.dense_socp_sec5d(8, n=1000, h=10),
+         "sec5a_lp": lambda: W.dense_lp_sec5a(9, n=1000)}[name]()
+    assert p.m == 800 and p.nnz == p.m * p.n
+    O = oracle.Oracle.from_problem(p, solve_mode=1)
+    O.run(15)
+    mid = O.get()
+    O2 = oracle.Oracle.from_problem(p, solve_mode=1)
+    O2.set_point(mid["x"], mid["z"])
+    O2.run(10, L=[1])
+    ref = O2.get()
+    sols = {}
+    for thr in (4096, 0):
+        S = binding.Solver.from_problem(p, device="cuda:0")
+        assert S.get_params()["dense_m_threshold"] == 4096          # dense-stored input: the default (cs.h)
+        S.set_params(dense_m_threshold=thr)
+        S.iterate(15)
+        got = S.solution()
+        for k in ("x", "z", "y", "s"):
+            assert rel(got[k], mid[k]) <= TOL_ITER, (thr, "leg 1", k, rel(got[k], mid[k]))
+        assert (S.residuals()["cg_steps_total"] == 0) == (thr > 0)
+        S.destroy()
+        S = binding.Solver.from_problem(p, device="cuda:0")
+        S.set_params(dense_m_threshold=thr)
+        S.set_point(mid["x"], mid["z"])
+        S.run(10, L=[1])
+        sols[thr], r = S.solution(), S.residuals()
+        assert rel(sols[thr]["O"], ref["O"]) <= 1e-12 and sols[thr]["O"].max() / sols[thr]["O"].min() > 1.5
+        for k in ("x", "z", "y", "s"):
+            assert rel(sols[thr][k], ref[k]) <= TOL_ITER, (thr, "leg 2", k, rel(sols[thr][k], ref[k]))
+        assert (r["cg_steps_total"] == 0) == (thr > 0) and r["n_conditionings"] == 1
+        q = O2.residuals()
+        for k in ("kkt_rel", "pres_abs", "dres_abs"):
+            assert abs(r[k] - q[k]) <= TOL_RES * abs(q[k]) + 1e-10 * (1 + np.linalg.norm(p.b)), (thr, k, r[k], q[k])
+        S.destroy()
 
 
 def test_dense_path_falls_back_to_cg_on_a_rank_deficient_matrix():
