@@ -120,7 +120,7 @@ struct HostSparse {
     uvec<int> idx;
     uvec<int> pos;                // compressed entry -> position in val/idx (for the plain compressed view, Csr in cs_device.cuh)
     uvec<double> val;
-    std::vector<unsigned> fmask;  // column-major copy with fused rows: [short slice][kFuseK] lane masks of the fused entries
+    std::vector<unsigned char> fmask;  // column-major copy with fused rows: [short slice][lane] bit k = entry k of the column is fused
     int n_chunk = 0, n_chunk_k2 = 0, n_slots = 0;
     bool too_big = false;         // padded storage would exceed 2^31 entries: nothing was filled
 };
@@ -237,7 +237,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
     h.pos.resize(idx.size());
     const int n_fuse = fuse ? fuse->rows() : 0, n_fa = fuse ? fuse->n_fa : 0;
     const int n_slice = (int)h.slices.size(), blk = 512;
-    if (n_fuse) h.fmask.assign((size_t)(n_slice - h.n_chunk) * kFuseK, 0u);
+    if (n_fuse) h.fmask.assign((size_t)(n_slice - h.n_chunk) * 32, (unsigned char)0);
     parallel_blocks((n_slice + blk - 1) / blk, nt, [&](int bi) {
         for (int si = bi * blk; si < std::min(n_slice, (bi + 1) * blk); ++si) {
             const int4 sl = h.slices[si];
@@ -278,7 +278,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
                             if (dup) continue;
                             seen[n_seen++] = i;
                         }
-                        h.fmask[(size_t)(si - h.n_chunk) * kFuseK + k] |= 1u << lane;
+                        h.fmask[(size_t)(si - h.n_chunk) * 32 + lane] |= (unsigned char)(1u << k);
                         (*fused_out)[ptr[seg] + k] = 1;
                         any_fused = true;
                     }
@@ -296,7 +296,7 @@ cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     if ((st = dev_upload(S, &p4, h.slices.data(), h.slices.size())) != CS_OK) return st; out->slices = p4;
     if ((st = dev_upload(S, &p4, h.multi.data(), h.multi.size())) != CS_OK) return st; out->multi = p4;
     if ((st = dev_upload(S, &p4, h.multi_k2.data(), h.multi_k2.size())) != CS_OK) return st; out->multi_k2 = p4;
-    unsigned *pu;
+    unsigned char *pu;
     if ((st = dev_upload(S, &pu, h.fmask.data(), h.fmask.size())) != CS_OK) return st; out->fmask = pu;
     if ((st = dev_upload(S, &pi, h.chunk_slot.data(), h.chunk_slot.size())) != CS_OK) return st; out->chunk_slot = pi;
     if ((st = dev_upload(S, &pi, h.idx.data(), h.idx.size())) != CS_OK) return st; out->idx = pi;
@@ -660,6 +660,15 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     x.norm_b = std::sqrt(nb); x.norm_c = std::sqrt(nc);
     int *ip; double *dp;
     if ((st = dev_upload(S, &ip, cone_off.data(), cone_off.size())) != CS_OK) return st; x.cone_off = ip;
+    {   // Lorentz blocks by size class (cone_sweep, cs_kernels.cuh): small (sub-warp), medium (warp), large (CTA)
+        std::vector<int> cls[3];
+        for (int i = 0; i < (int)K->n_soc; ++i) cls[K->soc_size[i] <= kConeSmall ? 0 : K->soc_size[i] <= kConeMedium ? 1 : 2].push_back(i);
+        x.n_cone_small = (int)cls[0].size(); x.n_cone_medium = (int)cls[1].size(); x.n_cone_large = (int)cls[2].size();
+        cls[0].insert(cls[0].end(), cls[1].begin(), cls[1].end());
+        cls[0].insert(cls[0].end(), cls[2].begin(), cls[2].end());
+        if ((st = dev_upload(S, &ip, cls[0].data(), cls[0].size())) != CS_OK) return st; x.cone_cls = ip;
+        CS_CUDA(S, cudaStreamSynchronize(S->stream));   // the staging vectors die here
+    }
     if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
     if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
     if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;      // x.R and x.Rc went up above

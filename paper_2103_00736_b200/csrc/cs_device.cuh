@@ -29,7 +29,9 @@ constexpr int kMaxRed = 8;           // scalars per grid reduction
 #endif
 constexpr int kShortMax = CS_SHORTMAX;        // segments up to this many non-zeros are "short" (1-8 lanes each inside a slice)
 constexpr int kChunk = CS_CHUNK;         // long segments are cut into warp-sized chunks of this many non-zeros
-constexpr int kConeLanes = 8;        // lanes cooperating on one Lorentz cone
+constexpr int kConeLanes = 8;        // lanes cooperating on one SMALL Lorentz cone (<= kConeSmall entries); see cone_sweep
+constexpr int kConeSmall = 64;       // up to here: sub-warp groups of kConeLanes lanes, 4 cones per warp
+constexpr int kConeMedium = 4096;    // up to here: one warp per cone; beyond: one CTA per cone
 constexpr int kDenseMax = 256;       // largest m of the dense factor-apply path (cs_params.dense_m_threshold)
 #ifndef CS_ROUNDK
 #define CS_ROUNDK 8
@@ -47,7 +49,8 @@ constexpr int kRoundK = CS_ROUNDK;   // slice rows per batch (8 values + 8 indic
 //            row in one instruction);
 //   class B: the next kFuseB rows    -- one accumulator per WARP and row; cs_create marks an entry as fused only if
 //            no lower lane of the same slice (32 columns) holds the same row, the others stay with K2.
-// Which entries are fused is a bit mask per slice row of the column-major copy (Sparse::fmask).
+// Which entries are fused is one byte per column of the column-major copy (Sparse::fmask), fetched with the slice's
+// epilogue operands before the batch.
 // Sizes: kFuseA * 6 KB + kFuseB * 192 B (one CTA of 768 threads per SM) must stay below ~96 KB, or the shared-memory
 // carve-out moves from 100 KB to 132 KB per SM and the gathers lose the L1 capacity they need.
 #ifndef CS_FUSE_A
@@ -94,8 +97,8 @@ struct Sparse {
     int n_chunk_k2, n_multi_k2;
     const int4 *multi_k2;
     const double *fpart;
-    // column-major copy only: fmask[(s - n_chunk) * kFuseK + k] = lanes of short slice s whose k-th entry is fused
-    const unsigned *fmask;
+    // column-major copy only: bit k of fmask[(s - n_chunk) * 32 + lane] = entry k of that lane's column in short slice s is fused
+    const unsigned char *fmask;
 };
 
 // Plain compressed view of one copy (segment s = entries [ptr[s], ptr[s+1]), minor index idx[e], value
@@ -117,6 +120,8 @@ enum { kPhCone = 0, kPhRhs = 1, kPhK1 = 2, kPhK2 = 3, kPhUpdate = 4, kPhReduce =
 struct Ctx {
     int m, n, n_lin, n_soc;
     const int *cone_off;    // [n_soc+1] absolute offsets of the Lorentz blocks (cone_off[0] = n_lin)
+    const int *cone_cls;    // [n_soc] cone ids by size class: small, then medium, then large (cone_sweep, cs_kernels.cuh)
+    int n_cone_small, n_cone_medium, n_cone_large;
     const int *perm_r, *perm_c;  // internal index -> caller's index (rows / columns sorted by length)
     Sparse R, C;            // row-major (segments = rows) and column-major (segments = columns) copies of A
     int n_fa, n_fb;         // heavy-row fusion: internal rows [0, n_fa) are class A, [n_fa, n_fa + n_fb) class B (0, 0: off)
@@ -286,7 +291,7 @@ __device__ void grid_reduce(double (&v)[NR], GridCtl &gc, double ident = 0.0) {
 // ---------------------------------------------------------------------------------------------
 struct NoFuse {
     static constexpr bool on = false;
-    template <int N> __device__ __forceinline__ void flags(const unsigned *, int, int, bool (&)[N]) const {}
+    template <int N> __device__ __forceinline__ void flags(unsigned, bool (&)[N]) const {}
     template <int N> __device__ __forceinline__ void scatter(const double (&)[N], const int (&)[N], const bool (&)[N], double) const {}
 };
 // Shared-memory accumulators of the heavy-row fusion (see kFuseA / kFuseB above), in the dynamic shared memory of
@@ -297,15 +302,12 @@ struct FuseAcc {
     static constexpr bool on = true;
     int n_fa;               // rows [0, n_fa) are class A, [n_fa, n_fa + n_fb) class B
     __device__ static double *smem() { extern __shared__ __align__(16) double fuse_smem[]; return fuse_smem; }
-    // which of the first kFuseK entries of this lane's column are fused: one warp-uniform 32-byte load of the slice's masks
+    // which of the first kFuseK entries of this lane's column are fused: bits of the byte fetched before the batch
     template <int N>
-    __device__ __forceinline__ void flags(const unsigned *fmask, int short_slice, int lane, bool (&f)[N]) const {
-        static_assert(N == kFuseK && N == 8, "the masks of a slice are two 16-byte loads");
-        const uint4 *mp = reinterpret_cast<const uint4 *>(fmask) + 2 * (size_t)short_slice;
-        const uint4 m0 = __ldg(mp), m1 = __ldg(mp + 1);
-        const unsigned m[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+    __device__ __forceinline__ void flags(unsigned fb, bool (&f)[N]) const {
+        static_assert(N == kFuseK && N == 8, "one byte per column");
 #pragma unroll
-        for (int q = 0; q < N; ++q) f[q] = (m[q] >> lane) & 1u;
+        for (int q = 0; q < N; ++q) f[q] = (fb >> q) & 1u;
     }
     // acc[row j[q]] += a[q] * uj for the fused entries (f[q]) among N entries of one column.  The read-modify-writes
     // are predicated, not branched around, and issued four at a time (loads, adds, stores), so that they overlap: the
@@ -356,6 +358,8 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
         const bool head = (lane >> lgT) < (sl.z & 255) && (lane & (T - 1)) == 0;
         const int cslot = CH ? __ldg(S.chunk_slot + s) : -1;  // fetched early, like `pre` (warp-uniform address)
         typename Epi::Pre pre = epi.pre(head ? seg : sl.y);
+        unsigned fb = 0;                                      // fused-entry bits of this lane's column (early, like `pre`)
+        if constexpr (Fuse::on && !CH) { if (sl.z >> 16) fb = __ldg(S.fmask + (size_t)(s - S.n_chunk) * 32 + lane); }
         double acc[NV];
 #pragma unroll
         for (int i = 0; i < NV; ++i) acc[i] = 0.0;
@@ -386,7 +390,7 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
                 if (head) uj = call_epi<Fuse::on>(epi, seg, acc, pre);   // T = 1 whenever the slice has fused entries (cs_create)
                 if (sl.z >> 16) {                            // warp-uniform: some entry of this slice is fused
                     bool f[UN];
-                    fuse.flags(S.fmask, s - S.n_chunk, lane, f);
+                    fuse.flags(fb, f);
                     fuse.scatter(a, j, f, uj);
                     __syncwarp();                            // the warp's next slice may hit the same class-B accumulators from other lanes
                 }
@@ -413,7 +417,7 @@ __device__ __forceinline__ void seg_reduce(const Sparse &S, Term &term, Epi &epi
             if (head) uj = call_epi<Fuse::on>(epi, seg, acc, pre);
             if (sl.z >> 16) {                                // longer columns: their first entries come back from L1 / L2
                 double a[UN]; int j[UN]; bool f[UN];
-                fuse.flags(S.fmask, s - S.n_chunk, lane, f);
+                fuse.flags(fb, f);
 #pragma unroll
                 for (int q = 0; q < UN; ++q) j[q] = f[q] ? __ldg(ip + 32 * q) : 0;
 #pragma unroll

@@ -14,28 +14,73 @@
 namespace csd {
 
 // ---------------------------------------------------------------------------------------------
-// abs_K on one Lorentz block handled by kConeLanes lanes (Def.1; closed form of the
-// projection onto {t >= ||u||}):  ||u|| <= t : v ;  ||u|| <= -t : -v ;  else (||u||, (t/||u||) u).
-// `f(j, s_j, p_j)` receives every coordinate.  All 32 lanes of a warp must call this together.
+// Lorentz blocks by size class (B north_star: "one warp or CTA per cone chosen by block size"; S 8(a) a1):
+//   small  (<= kConeSmall entries)  : kConeLanes = 8 lanes per block, 4 blocks per warp
+//   medium (<= kConeMedium entries) : one warp per block
+//   large                           : one CTA per block (block-wide sum through shared memory)
+// c.cone_cls lists the cone ids class by class (cs_create).  `sum(j, is_head, t)` adds coordinate j's contribution to
+// the double2 t; `apply(a, b, t, l, W)` is then called by all W lanes/threads of the group (l = 0..W-1) with the
+// complete sums of block [a, b).  All sums have a fixed order.  Every thread of the grid must call this together.
 // ---------------------------------------------------------------------------------------------
-template <class F>
-__device__ __forceinline__ void soc_abs_block(const double *s, int a, int b, int sl, bool active, F &f) {
-    double t = 0.0, nu2 = 0.0;
-    if (active) {
-        t = s[a];
-        for (int j = a + 1 + sl; j < b; j += kConeLanes) { const double x = s[j]; nu2 += x * x; }
+template <class Sum, class Apply>
+__device__ __forceinline__ void cone_sweep(const Ctx &c, Sum sum, Apply apply) {
+    const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gwarp = tid >> 5, nwarps = nth >> 5;
+    {   // small
+        const int sub = lane / kConeLanes, sl = lane % kConeLanes;
+        constexpr int CPW = 32 / kConeLanes;
+        for (int base = gwarp * CPW; base < c.n_cone_small; base += nwarps * CPW) {
+            const int q = base + sub;
+            const bool act = q < c.n_cone_small;
+            const int ci = act ? __ldg(c.cone_cls + q) : 0;
+            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
+            double2 t = make_double2(0.0, 0.0);
+            for (int j = a + sl; j < b; j += kConeLanes) sum(j, j == a, t);
+            t.x = group_reduce<kConeLanes>(t.x);
+            t.y = group_reduce<kConeLanes>(t.y);
+            if (act) apply(a, b, t, sl, kConeLanes);
+        }
     }
-    nu2 = group_reduce<kConeLanes>(nu2);
-    if (!active) return;
-    const double nu = sqrt(nu2);
+    for (int q = gwarp; q < c.n_cone_medium; q += nwarps) {   // medium: one warp per block
+        const int ci = __ldg(c.cone_cls + c.n_cone_small + q);
+        const int a = __ldg(c.cone_off + ci), b = __ldg(c.cone_off + ci + 1);
+        double2 t = make_double2(0.0, 0.0);
+        for (int j = a + lane; j < b; j += 32) sum(j, j == a, t);
+        t.x = group_reduce<32>(t.x);
+        t.y = group_reduce<32>(t.y);
+        apply(a, b, t, lane, 32);
+    }
+    if (c.n_cone_large) {                                     // large: one CTA per block
+        __shared__ double red[2][kWarps];
+        for (int q = blockIdx.x; q < c.n_cone_large; q += gridDim.x) {
+            const int ci = __ldg(c.cone_cls + c.n_cone_small + c.n_cone_medium + q);
+            const int a = __ldg(c.cone_off + ci), b = __ldg(c.cone_off + ci + 1);
+            double2 t = make_double2(0.0, 0.0);
+            for (int j = a + (int)threadIdx.x; j < b; j += kBlock) sum(j, j == a, t);
+            t.x = group_reduce<32>(t.x);
+            t.y = group_reduce<32>(t.y);
+            __syncthreads();                                  // the previous block's sums have been read
+            if (lane == 0) { red[0][warp] = t.x; red[1][warp] = t.y; }
+            __syncthreads();
+            t = make_double2(0.0, 0.0);
+            for (int w = 0; w < kWarps; ++w) { t.x += red[0][w]; t.y += red[1][w]; }
+            apply(a, b, t, (int)threadIdx.x, kBlock);
+        }
+    }
+}
+
+// abs_K on one Lorentz block (Def.1; closed form of the projection onto {t >= ||u||}):
+//   ||u|| <= t : v ;  ||u|| <= -t : -v ;  else (||u||, (t/||u||) u).   nu2 = ||u||^2; `f(j, p_j)` receives every coordinate.
+template <class F>
+__device__ __forceinline__ void soc_abs_apply(const double *s, int a, int b, double nu2, int l, int W, F &f) {
+    const double t = s[a], nu = sqrt(nu2);
     if (nu <= t) {
-        for (int j = a + sl; j < b; j += kConeLanes) f(j, s[j], s[j]);
+        for (int j = a + l; j < b; j += W) f(j, s[j]);
     } else if (nu <= -t) {
-        for (int j = a + sl; j < b; j += kConeLanes) f(j, s[j], -s[j]);
+        for (int j = a + l; j < b; j += W) f(j, -s[j]);
     } else {
         const double sc = t / nu;
-        if (sl == 0) f(a, t, nu);
-        for (int j = a + 1 + sl; j < b; j += kConeLanes) f(j, s[j], sc * s[j]);
+        for (int j = a + l; j < b; j += W) f(j, j == a ? nu : sc * s[j]);
     }
 }
 
@@ -44,30 +89,16 @@ __device__ __forceinline__ void soc_abs_block(const double *s, int a, int b, int
 //   e := p - mu c^ + g        (r0 = b~ - A~ e is its residual at the warm start w, g = A~'w kept from before)
 __device__ __forceinline__ void phase_cone_reflect(const Ctx &c) {
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
-    for (int j = tid; j < c.n_lin; j += nth) {
-        const double pj = fabs(c.s[j]);
+    auto put = [&](int j, double pj) {
         const double uj = pj - c.mu * c.chat[j];
         c.p[j] = pj;
         c.u[j] = uj;
         c.e[j] = uj + c.g[j];
-    }
-    if (c.n_soc) {
-        const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
-        constexpr int CPW = 32 / kConeLanes;
-        const int gwarp = tid >> 5, nwarps = nth >> 5;
-        auto put = [&](int j, double, double pj) {
-            const double uj = pj - c.mu * c.chat[j];
-            c.p[j] = pj;
-            c.u[j] = uj;
-            c.e[j] = uj + c.g[j];
-        };
-        for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
-            const int ci = base + sub;
-            const bool act = ci < c.n_soc;
-            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
-            soc_abs_block(c.s, a, b, sl, act, put);
-        }
-    }
+    };
+    for (int j = tid; j < c.n_lin; j += nth) put(j, fabs(c.s[j]));
+    if (c.n_soc)
+        cone_sweep(c, [&](int j, bool head, double2 &t) { if (!head) { const double x = c.s[j]; t.x += x * x; } },
+                   [&](int a, int b, double2 t, int l, int W) { soc_abs_apply(c.s, a, b, t.x, l, W, put); });
 }
 
 // ---------------------------------------------------------------------------------------------

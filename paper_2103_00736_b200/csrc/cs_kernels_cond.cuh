@@ -41,26 +41,15 @@ __device__ __forceinline__ void phase_cone_ratio(const Ctx &c, double &lmax, dou
         lmax = fmax(lmax, lo);
         lmin_neg = fmax(lmin_neg, -lo);
     }
-    if (c.n_soc) {
-        const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
-        constexpr int CPW = 32 / kConeLanes;
-        const int gwarp = tid >> 5, nwarps = nth >> 5;
-        for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
-            const int ci = base + sub;
-            const bool act = ci < c.n_soc;
-            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
-            double nu2 = 0.0;
-            for (int j = a + 1 + sl; j < b; j += kConeLanes) { const double x = c.xb[j]; nu2 += x * x; }
-            nu2 = group_reduce<kConeLanes>(nu2);
-            if (act) {
-                const double num = fmax(fabs(c.xb[a] - sqrt(nu2)), fl), den = fmax(fabs(c.zb[a]), fl);
-                const double lo = log(num / den);
-                for (int j = a + sl; j < b; j += kConeLanes) c.O[j] = lo;
-                lmax = fmax(lmax, lo);
-                lmin_neg = fmax(lmin_neg, -lo);
-            }
-        }
-    }
+    if (c.n_soc)
+        cone_sweep(c, [&](int j, bool head, double2 &t) { if (!head) { const double x = c.xb[j]; t.x += x * x; } },
+                   [&](int a, int b, double2 t, int l, int W) {
+                       const double num = fmax(fabs(c.xb[a] - sqrt(t.x)), fl), den = fmax(fabs(c.zb[a]), fl);
+                       const double lo = log(num / den);
+                       for (int j = a + l; j < b; j += W) c.O[j] = lo;
+                       lmax = fmax(lmax, lo);
+                       lmin_neg = fmax(lmin_neg, -lo);
+                   });
 }
 
 struct TermRowNorm {  // sum_j (A_ij O_j)^2   (traversed over the PRISTINE values)
@@ -325,24 +314,15 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_equilibrate(Ctx c, int n_sw
             const double v = c2[j];
             if (v > 0.0) E[j] = E[j] / sqrt(sqrt(v) / tau);
         }
-        if (c.n_soc) {   // one factor per Lorentz block: the block mean of c_j^2 (E must commute with K)
-            const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
-            constexpr int CPW = 32 / kConeLanes;
-            const int gwarp = tid >> 5, nwarps = nth >> 5;
-            for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
-                const int ci = base + sub;
-                const bool act = ci < c.n_soc;
-                const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
-                double sum = 0.0;
-                for (int j = a + sl; j < b; j += kConeLanes) sum += c2[j];
-                sum = group_reduce<kConeLanes>(sum);
-                const double mean = act ? sum / (double)(b - a) : 0.0;
-                if (mean > 0.0) {
-                    const double f = sqrt(sqrt(mean) / tau);
-                    for (int j = a + sl; j < b; j += kConeLanes) E[j] = E[j] / f;
-                }
-            }
-        }
+        if (c.n_soc)     // one factor per Lorentz block: the block mean of c_j^2 (E must commute with K)
+            cone_sweep(c, [&](int j, bool, double2 &t) { t.x += c2[j]; },
+                       [&](int a, int b, double2 t, int l, int W) {
+                           const double mean = t.x / (double)(b - a);
+                           if (mean > 0.0) {
+                               const double f = sqrt(sqrt(mean) / tau);
+                               for (int j = a + l; j < b; j += W) E[j] = E[j] / f;
+                           }
+                       });
         double *t = Dold; Dold = Dnew; Dnew = t;
         gc.sync();
     }
@@ -408,21 +388,9 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_residuals(Ctx c) {
         vx += a * a;
         vz += b * b;
     }
-    if (c.n_soc) {
-        const int lane = threadIdx.x & 31, sub = lane / kConeLanes, sl = lane % kConeLanes;
-        constexpr int CPW = 32 / kConeLanes;
-        const int gwarp = tid >> 5, nwarps = nth >> 5;
-        for (int base = gwarp * CPW; base < c.n_soc; base += nwarps * CPW) {
-            const int ci = base + sub;
-            const bool act = ci < c.n_soc;
-            const int a = act ? __ldg(c.cone_off + ci) : 0, b = act ? __ldg(c.cone_off + ci + 1) : 0;
-            double nx = 0.0, nz = 0.0;
-            for (int j = a + 1 + sl; j < b; j += kConeLanes) { nx += c.xb[j] * c.xb[j]; nz += c.zb[j] * c.zb[j]; }
-            nx = group_reduce<kConeLanes>(nx);
-            nz = group_reduce<kConeLanes>(nz);
-            if (act && sl == 0) { vx += soc_dist2(c.xb[a], nx); vz += soc_dist2(c.zb[a], nz); }
-        }
-    }
+    if (c.n_soc)
+        cone_sweep(c, [&](int j, bool head, double2 &t) { if (!head) { t.x += c.xb[j] * c.xb[j]; t.y += c.zb[j] * c.zb[j]; } },
+                   [&](int a, int, double2 t, int l, int) { if (l == 0) { vx += soc_dist2(c.xb[a], t.x); vz += soc_dist2(c.zb[a], t.y); } });
     double red[8] = {e1.pres2, e1.by, e2.dres2, e2.cx, e2.nx2, e2.nz2, vx, vz};
     grid_reduce<8>(red, gc);
     if (blockIdx.x == 0 && threadIdx.x == 0) {

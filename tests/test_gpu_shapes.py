@@ -31,9 +31,22 @@ SHAPES = {
     "socp_tiny_blocks": lambda: W.sparse_socp(16, 200, 900, 450, 4, lo=1, hi=3),
     "socp_large_blocks": lambda: W.sparse_socp(17, 300, 1500, 5, 5, lo=200, hi=400),
     "socp_plus_orthant": lambda: W.sparse_socp(18, 700, 2500, 60, 8, n_lin=1000, lo=2, hi=50),
+    # Lorentz blocks of all three size classes of cone_sweep (sub-warp <= 64 < warp <= 4096 < CTA) plus orthant coordinates
+    "socp_all_size_classes": lambda: _socp_with_sizes(23, 900, 150, [3, 40, 64, 65, 7, 300, 1000, 2, 4097, 33, 6000, 1, 12]),
     "one_cta_dense_path": lambda: W.sparse_socp(19, 60, 300, 20, 6, n_lin=100, lo=2, hi=20),
     "one_cta_cg_path": lambda: W.sparse_lp(20, 400, 1300, 5),
 }
+
+
+def _socp_with_sizes(seed, m, n_lin, sizes, per_col=6):
+    """Mixed-cone problem with the given Lorentz block sizes (constructed complementary optimum, as workloads.sparse_socp)."""
+    rng = np.random.default_rng(seed)
+    sizes = np.asarray(sizes, np.int32)
+    n = n_lin + int(sizes.sum())
+    A = W.sparse_fixed_per_column(rng, m, n, per_col)
+    xs, ss = W._soc_pair(rng, sizes)
+    xl, sl = W._lp_pair(rng, n_lin, 0.5)
+    return W._assemble("socp_sizes", A, np.concatenate([xl, xs]), np.concatenate([sl, ss]), rng, n_lin, sizes, t=1.7, L_first=200, L_every=100)
 
 
 def _with_dense_column(p):
