@@ -69,8 +69,9 @@ typedef struct {
  *   cg_tol   inner solve stops when ||residual||_2 <= cg_tol * ||rhs||_2, both measured on the
  *            row-equilibrated system (D A_hat)(D A_hat)' with D = diag(1/||row_i(A_hat)||_2).  The residual is
  *            the recurrence residual of CG, which keeps shrinking below the rounding level of the true one; the
- *            default 1e-16 takes the solve to that floor ("exact" projections, the parity setting: an in-run
- *            conditioning amplifies what is left of the solve error by 1e3-1e4)
+ *            default DBL_EPSILON = 2.22e-16 (the recurrence residual below one ulp of the right-hand side) takes the
+ *            solve to that floor ("exact" projections, the parity setting: an in-run conditioning amplifies what is
+ *            left of the solve error by 1e3-1e4)
  *   cg_reduce    inexact projections (0 = off, the default): the solve of a pass also stops once the residual of
  *            the WARM START has been reduced by this factor, ||residual||_2 <= max(cg_tol ||rhs||_2,
  *            cg_reduce ||residual at the warm start||_2).  The warm-start residual shrinks as the outer iteration
@@ -124,7 +125,7 @@ typedef struct {
 
 /* Build a solver for (A,b,c,K): validates the input, copies it to the device, builds the CSC copy of A
  * and the work partitions.  b[m], c[n] live in `vec_where`.  Parameters start at mu=1, t=9.2 (n_soc=0)
- * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=1e-16, cg_reduce=0, cg_max_iter=20000, precond=0,
+ * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=2.22e-16 (DBL_EPSILON), cg_reduce=0, cg_max_iter=20000, precond=0,
  * dense_m_threshold=128 (4096 for a dense-stored A); the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
  * mandatory first conditioning (l=1) the identity and s=0.  Synchronous.  On failure *out is NULL. */
 cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,

@@ -64,6 +64,17 @@ constexpr int kOneCtaNnz = 8192;   // problems up to this many non-zeros run on 
         }                                                                                        \
     } while (0)
 
+// A handle is bound to the device that was current at cs_create (cs.h): every entry point that takes a handle makes that
+// device current for the duration of the call and restores the caller's on exit.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const cs_solver *S) {
+        if (S && cudaGetDevice(&prev) == cudaSuccess && prev != S->device) cudaSetDevice(S->device);
+        else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 template <class T>
 cs_status dev_alloc(cs_solver *S, T **out, size_t count) {
     void *p = nullptr;
@@ -437,7 +448,7 @@ const char *cs_last_error(const cs_solver *S) { return S ? S->err.c_str() : g_cr
 
 void cs_destroy(cs_solver *S) {
     if (!S) return;
-    cudaSetDevice(S->device);
+    DeviceGuard guard(S);
     cudaStreamSynchronize(S->stream);
     for (void *p : S->allocs) cudaFree(p);
     delete S;
@@ -496,14 +507,19 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         std::atomic<int> bad{0};
         const int blk = 16384;
         parallel_blocks((m + blk - 1) / blk, host_threads(), [&](int bi) {
-            for (int i = bi * blk; i < std::min(m, (bi + 1) * blk); ++i)
+            for (int i = bi * blk; i < std::min(m, (bi + 1) * blk); ++i) {
+                double ss = 0.0;
                 for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
                     if (cidx[k] < 0 || cidx[k] >= n || (k > rptr[i] && cidx[k] <= cidx[k - 1])) bad.store(1);
                     else if (!std::isfinite(val[k])) bad.store(2);
+                    ss += val[k] * val[k];
                 }
+                if (!(ss > 0.0) && !bad.load()) bad.store(3);       // a row of stored zeros: A is not of full row rank
+            }
         });
         if (bad.load() == 1) { S->err = "col_idx out of range, unsorted or duplicated within a row"; return CS_EINVAL; }
         if (bad.load() == 2) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
+        if (bad.load() == 3) { S->err = "a row of A has zero norm (all stored entries are 0 or underflow when squared)"; return CS_EINVAL; }
     }
     double nb = 0.0, nc = 0.0;
     for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
@@ -520,6 +536,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         });
     }
     const std::vector<int> perm_r = order_by_length(rlen, m);
+    for (int i = 0; i < m && rlen[perm_r[i]] > kShortMax; ++i) S->ctx.n_long = i + 1;
     // (A lexicographic ordering of the columns by the heavy rows they touch was tried so that those rows'
     //  gathers run over contiguous stretches; it cost 3.4 s at config 4 and changed nothing measurable.)
     const std::vector<int> perm_c = order_by_length(clen, (int)K->n_lin);
@@ -752,7 +769,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.mu = 1.0;
     S->prm.t = K->n_soc > 0 ? 1.7 : 9.2;
     S->prm.o_floor = 1e-16;
-    S->prm.cg_tol = 1e-16;
+    S->prm.cg_tol = 2.220446049250313e-16;   // DBL_EPSILON: the recurrence residual below one ulp of the right-hand side (cs.h)
     S->prm.cg_reduce = 0.0;
     S->prm.cg_max_iter = 20000;
     S->prm.precond = 0;
@@ -805,6 +822,7 @@ cs_status cs_get_params(const cs_solver *S, cs_params *p) {
 
 cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem where) {
     if (!S || !x || !z) return CS_EINVAL;
+    DeviceGuard guard(S);
     if (S->started) { S->err = "cs_set_point after the iteration has started"; return CS_ESTATE; }
     cs_status st;
     if ((st = import_cols(S, S->ctx.xb, x, where)) != CS_OK) return st;
@@ -813,11 +831,13 @@ cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem wh
 
 cs_status cs_condition(cs_solver *S) {
     if (!S) return CS_EINVAL;
+    DeviceGuard guard(S);
     return do_condition(S, 1);
 }
 
 cs_status cs_set_scaling(cs_solver *S, const double *O, cs_mem where) {
     if (!S || !O) return CS_EINVAL;
+    DeviceGuard guard(S);
     cs_status st = ensure_xz(S);  // x,z of the OLD scaling, before O is overwritten
     if (st != CS_OK) return st;
     if ((st = import_cols(S, S->ctx.O, O, where)) != CS_OK) return st;
@@ -826,6 +846,7 @@ cs_status cs_set_scaling(cs_solver *S, const double *O, cs_mem where) {
 
 cs_status cs_iterate(cs_solver *S, int64_t k) {
     if (!S || k < 0) return CS_EINVAL;
+    DeviceGuard guard(S);
     if (k == 0) return CS_OK;
     cs_status st;
     if (!S->conditioned && (st = do_condition(S, 1)) != CS_OK) return st;  // step 4: l = 1
@@ -841,6 +862,7 @@ cs_status cs_iterate(cs_solver *S, int64_t k) {
 
 cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     if (!S || !out) return CS_EINVAL;
+    DeviceGuard guard(S);
     cs_status st;
     if (!S->conditioned && (st = do_condition(S, 1)) != CS_OK) return st;
     if ((st = ensure_xz(S)) != CS_OK) return st;
@@ -855,11 +877,16 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     out->pres_abs = h.resid[0]; out->pres_rel = h.resid[1]; out->dres_abs = h.resid[2]; out->dres_rel = h.resid[3];
     out->gap_abs = h.resid[4]; out->gap_rel = h.resid[5]; out->cone_viol_rel = h.resid[6]; out->kkt_rel = h.resid[7];
     out->pobj = h.resid[8]; out->dobj = h.resid[9]; out->fp_res = h.resid[10];
+    if (!std::isfinite(out->kkt_rel)) {
+        S->err = "non-finite KKT residual: the iteration has diverged or a scaling over/underflowed (t too large for this data?)";
+        return CS_ESTATE;
+    }
     return h.cg_hit_max ? CS_ECGMAX : CS_OK;
 }
 
 cs_status cs_equilibrate(cs_solver *S, int32_t n_sweeps) {
     if (!S || n_sweeps < 0) return CS_EINVAL;
+    DeviceGuard guard(S);
     cs_status st = ensure_xz(S);  // x,z of the OLD scaling, before O is overwritten
     if (st != CS_OK) return st;
     int ns = n_sweeps;
@@ -882,6 +909,7 @@ int64_t next_multiple(int64_t l, int64_t q) { return (l / q + 1) * q; }   // sma
 cs_status cs_solve(cs_solver *S, const cs_schedule *sch, cs_resid *out, int64_t *cond_iters, int64_t cond_cap,
                    int64_t *n_cond) {
     if (!S || !sch || !out || sch->max_iter < 0 || sch->check_every < 0 || cond_cap < 0) return CS_EINVAL;
+    DeviceGuard guard(S);
     const bool stall = sch->rule == CS_RULE_STALL;
     if (sch->rule != CS_RULE_SET && !stall) { S->err = "cs_solve: unknown rule"; return CS_EINVAL; }
     if (stall && (sch->window < 2 || sch->lag < 1 || sch->lag >= sch->window || !(sch->ratio >= 0.0))) {
@@ -949,6 +977,7 @@ cs_status cs_solve(cs_solver *S, const cs_schedule *sch, cs_resid *out, int64_t 
 
 cs_status cs_diag_phase_times(cs_solver *S, double out[8]) {
     if (!S || !out) return CS_EINVAL;
+    DeviceGuard guard(S);
     Scalars h;
     CS_CUDA(S, cudaMemcpyAsync(&h, S->ctx.sc, sizeof(h), cudaMemcpyDeviceToHost, S->stream));
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
@@ -1027,6 +1056,7 @@ cs_status cs_diag_l2_probe(int64_t bytes, int32_t reps, double *gbs) {
 
 cs_status cs_diag_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier) {
     if (!S || n < 1 || !us_per_barrier) return CS_EINVAL;
+    DeviceGuard guard(S);
     cudaEvent_t e0, e1;
     CS_CUDA(S, cudaEventCreate(&e0));
     CS_CUDA(S, cudaEventCreate(&e1));
@@ -1052,6 +1082,7 @@ cs_status cs_diag_barrier_probe(cs_solver *S, int32_t n, double *us_per_barrier)
 
 cs_status cs_solution(cs_solver *S, double *x, double *z, double *y, double *s, double *O, cs_mem where) {
     if (!S) return CS_EINVAL;
+    DeviceGuard guard(S);
     cs_status st;
     if ((st = ensure_xz(S)) != CS_OK) return st;
     const Ctx &c = S->ctx;

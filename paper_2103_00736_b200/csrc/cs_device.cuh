@@ -129,6 +129,7 @@ struct Ctx {
     Csr Rc, Cc;             // plain compressed views of the same two copies
     // FSAI(1) preconditioner G = diag(gd) + strictly-lower part with one entry gm[i] at column partner[i]
     int fsai;               // 0: off (plain Jacobi-equilibrated CG)
+    int n_long;             // internal rows [0, n_long) are longer than kShortMax: no FSAI partner, G = I there
     int *f_ctop;            // [n][3] strongest short rows of every column
     int *f_partner;         // [m] partner row (< i) or -1
     int *f_tptr, *f_tcur, *f_tidx, *f_blk;   // transposed lists: rows whose partner is k are f_tidx[f_tptr[k] .. f_tptr[k+1])

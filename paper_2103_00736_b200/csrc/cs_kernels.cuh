@@ -133,6 +133,8 @@ struct EpiK1 {
 };
 struct EpiK2 {       // z = preconditioned residual (== r when the FSAI preconditioner is off)
     double *v, *w, *r; const double *z; double alpha, beta; double rho;
+    double *z_long; int n_long;      // FSAI on: rows [0, n_long) (longer than kShortMax) have G = I, so z = r is written here
+    double rz_long;                  // ... and their share of r'z = ||r||^2 over them
     struct Pre { double r, z, v, w; };
     __device__ __forceinline__ Pre pre(int i) const { return Pre{r[i], z[i], v[i], w[i]}; }
     __device__ __forceinline__ void operator()(int i, const double (&a)[1], const Pre &q) {
@@ -141,6 +143,7 @@ struct EpiK2 {       // z = preconditioned residual (== r when the FSAI precondi
         w[i] = q.w + alpha * vi;
         const double rn = q.r - alpha * a[0];
         r[i] = rn;
+        if (i < n_long) { z_long[i] = rn; rz_long += rn * rn; }
         rho += rn * rn;
     }
 };
@@ -155,11 +158,12 @@ struct EpiK2 {       // z = preconditioned residual (== r when the FSAI precondi
 #endif
 // CS_FSAI_NB rows per thread at a time: the loads of a row form a dependent chain (partner / list bounds -> list
 // entry -> r), so the rows of a batch are interleaved by hand to keep several chains in flight (latency-bound).
-__device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
+// fsai_pass(c, k_begin): rows [k_begin, m), returns this thread's share of r'z (no grid reduction).
+__device__ __forceinline__ double fsai_pass(const Ctx &c, int k_begin) {
     const int tid = blockIdx.x * kBlock + threadIdx.x, nth = gridDim.x * kBlock;
     constexpr int NB = CS_FSAI_NB;
     double rz = 0.0;
-    for (int k0 = tid; k0 < c.m; k0 += NB * nth) {
+    for (int k0 = k_begin + tid; k0 < c.m; k0 += NB * nth) {
         int pk[NB], e0[NB], e1[NB];
         double rk[NB], acc[NB], rp[NB], ee[NB];
 #pragma unroll
@@ -195,7 +199,10 @@ __device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
             if (k < c.m) { c.z[k] = acc[q]; rz += rk[q] * acc[q]; }
         }
     }
-    double red[1] = {rz};
+    return rz;
+}
+__device__ __forceinline__ double apply_fsai(const Ctx &c, GridCtl &gc) {
+    double red[1] = {fsai_pass(c, 0)};
     grid_reduce<1>(red, gc);
     return red[0];
 }
@@ -373,15 +380,30 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, do
         if (!(sigma > 0.0)) break;
         const double alpha = rz / sigma;
         TermDot t2{c.u};
-        EpiK2 e2{c.v, c.w, c.r, zsrc, alpha, beta, 0.0};
+        EpiK2 e2{c.v, c.w, c.r, zsrc, alpha, beta, 0.0, c.z, c.fsai ? c.n_long : 0, 0.0};
         seg_reduce<1, false, 1>(c.R, t2, e2, gc);          // K2 view: without the entries the column pass has done
         gc.lap(kPhK2);
-        red[0] = e2.rho;
-        grid_reduce<1>(red, gc);
-        gc.lap(kPhReduce);
-        rr = red[0];
-        const double rz_new = c.fsai ? apply_fsai(c, gc) : rr;
-        if (c.fsai) gc.lap(kPhPrecond);
+        double rz_new;
+        if (c.fsai) {
+            // z = G'G r for the short rows in the same phase as K2's finishing step (the long rows, whose sums that step
+            // completes, have G = I and got z = r from the epilogue; no short row's z reads a long row's r): one barrier
+            // and one reduction for both ||r||^2 and r'z
+            if (!c.R.n_multi_k2) gc.sync();                // otherwise seg_reduce's own barrier has made r complete
+            double red2[2] = {e2.rho, 0.0};
+            red2[1] = fsai_pass(c, c.n_long);
+            gc.lap(kPhPrecond);
+            red2[1] += e2.rz_long;                         // the long rows' share, from K2's epilogue
+            grid_reduce<2>(red2, gc);
+            gc.lap(kPhReduce);
+            rr = red2[0];
+            rz_new = red2[1];
+        } else {
+            red[0] = e2.rho;
+            grid_reduce<1>(red, gc);
+            gc.lap(kPhReduce);
+            rr = red[0];
+            rz_new = rr;
+        }
         beta = rz_new / rz;
         rz = rz_new;
         ++steps;

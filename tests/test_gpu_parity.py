@@ -101,7 +101,7 @@ def test_iterates_one_early_conditioning(name):
     """Protocol (ii-b), S 8(c): conditioning at l=20 INSIDE a run, each side from its own iterate.  The rule
     o = |x|/|z| amplifies what the two sides' iterates differ by before it (1e-14 with the solves taken to their
     floor) by 1e3-1e4: x, z, y to 1e-9 (B north_star), s and O -- which the protocol holds to 1e-6 -- to 1e-8.
-    Measured (profiles/r02_parity_gaps.md): worst case cfg1 x 1.5e-10, O 3.5e-10; the oracle's own two solve modes
+    Measured: worst case cfg1 x 1.5e-10, O 3.5e-10; the oracle's own two solve modes
     differ by x 3.9e-10, O 9.7e-10 there."""
     make, k, okw = CASES[name]
     p = make()
@@ -130,7 +130,7 @@ def test_cfg2_replica_illconditioned():
     """Config 2 recipe (row 10^U(-3,3), column 10^U(-2,2)) at 1/100 scale, 30 passes, L = {}.  ||c|| is 2e4 x ||s||
     on this instance, so step 18's d = A^dagger b + ... cancels 5 digits and fp64 resolves the iterate to ~1e-9
     only: against an extended-precision rerun the oracle's Cholesky mode is 6e-10 off, its PCG mode 2e-9
-    (profiles/r02_parity_gaps.md).  Tolerance: 1e-9, or 3x the distance between the oracle's own two modes where
+    (DESIGN.md 7).  Tolerance: 1e-9, or 3x the distance between the oracle's own two modes where
     that is larger (measured in the test; 2.0e-9 on x, z, s here)."""
     p = W.config(2, 0.01)
     gap, ref = _oracle_mode_gap(p, lambda O: O.run(30), ("x", "z", "s"))
@@ -150,7 +150,7 @@ def test_conditioned_passes_on_midsize_replicas(cfg, scale):
     Config 4 (Zipf rows, heavy-row fusion active): x, z, y, s to 1e-9, O to 1e-12.
     Config 2: after a conditioning with t = 9.2 the scaled cost vector is ~1e7 x ||s||, and fp64 resolves a pass to
     ~3e-7 only -- both oracle modes are 3e-7 from an extended-precision rerun and from each other
-    (profiles/r02_parity_gaps.md) -- so the tolerance there is 3x the oracle's own mode-to-mode distance."""
+     -- so the tolerance there is 3x the oracle's own mode-to-mode distance."""
     import oracle
     from paper_2103_00736_b200 import binding
     p = W.config(cfg, scale)
