@@ -65,7 +65,11 @@ constexpr int kRoundK = CS_ROUNDK;   // slice rows per batch (8 values + 8 indic
 constexpr int kFuseA = CS_FUSE_A, kFuseB = CS_FUSE_B;
 constexpr int kFuseMinLen = CS_FUSE_MINLEN;     // rows shorter than this are never fused
 constexpr int kFuseSmem = (kFuseA * kBlock + kWarps * kFuseB) * 8;   // dynamic shared memory of k_iterate when rows are fused
-constexpr int kFuseK = CS_ROUNDK;          // only the first kFuseK entries of a column can be fused (the heavy rows come first)
+#ifndef CS_FUSE_K
+#define CS_FUSE_K 8
+#endif
+constexpr int kFuseK = CS_FUSE_K;          // only the first kFuseK entries of a column can be fused (the heavy rows come first)
+static_assert(kFuseK % 4 == 0 && kFuseK <= CS_ROUNDK, "scatter works on groups of 4 of a batch's entries");
 static_assert(kRoundK % 4 == 0 && kFuseA <= kMaxRed, "scatter works in groups of 4; fuse_flush borrows the reduction scratch");
 
 // One sparse format (rows of the row-major copy or columns of the column-major copy): a list of SLICES.
@@ -306,9 +310,9 @@ struct FuseAcc {
     // which of the first kFuseK entries of this lane's column are fused: bits of the byte fetched before the batch
     template <int N>
     __device__ __forceinline__ void flags(unsigned fb, bool (&f)[N]) const {
-        static_assert(N == kFuseK && N == 8, "one byte per column");
+        static_assert(N == 8, "one byte per column");
 #pragma unroll
-        for (int q = 0; q < N; ++q) f[q] = (fb >> q) & 1u;
+        for (int q = 0; q < N; ++q) f[q] = q < kFuseK && ((fb >> q) & 1u);
     }
     // acc[row j[q]] += a[q] * uj for the fused entries (f[q]) among N entries of one column.  The read-modify-writes
     // are predicated, not branched around, and issued four at a time (loads, adds, stores), so that they overlap: the
@@ -319,7 +323,7 @@ struct FuseAcc {
         double *sm = smem();
         const int my_a = threadIdx.x, my_b = kFuseOffB + (threadIdx.x >> 5) * kFuseB - n_fa;
 #pragma unroll
-        for (int h = 0; h < N; h += 4) {
+        for (int h = 0; h < kFuseK; h += 4) {
             int q[4];
             double v[4];
 #pragma unroll
