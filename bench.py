@@ -208,7 +208,7 @@ def main():
     ap.add_argument("--cg-reduce", type=float, default=0.0, help="--solve only: cs_params.cg_reduce (adaptive inexact projections)")
     ap.add_argument("--check-every", type=int, default=25)
     ap.add_argument("--max-iter", type=int, default=3000)
-    ap.add_argument("--precond", type=int, default=0, help="cs_params.precond: 0 auto, 1 none (Jacobi equilibration only), 2 FSAI(1)")
+    ap.add_argument("--precond", type=int, default=0, help="cs_params.precond: 0 auto, 1 none (Jacobi equilibration only), 2 FSAI(1), 3 FSAI(5)")
     ap.add_argument("--cg-max-iter", type=int, default=0, help="profiling only: cap CG steps per solve (0 = library default)")
     a = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -300,7 +300,7 @@ def main():
     # from the device counters (total minus those spent inside cs_condition).
     cg_steps = r1["cg_steps_total"] - r0["cg_steps_total"]
     cg_iter = cg_steps - (r1["cg_steps_cond"] - r0["cg_steps_cond"])
-    fsai_on = S.get_params()["precond"] == 2 or (S.get_params()["precond"] == 0 and p.t >= 4.0)
+    fsai_on = S.get_params()["precond"] in (2, 3) or (S.get_params()["precond"] == 0 and p.t >= 4.0)
     it_bytes, cg_bytes = algorithmic_bytes(p, n_it, cg_iter, 0, fsai_on)
     peaks = {}
     try:

@@ -78,10 +78,14 @@ typedef struct {
  *            converges (w converges to mu D^{-1} y), so the projection error shrinks with it -- an adaptive
  *            tolerance with the fixed point unchanged; 0 < cg_reduce < 1.
  *   cg_max_iter  cap on CG steps per solve
- *   precond  preconditioner of the inner CG beyond the Jacobi row equilibration: 0 = automatic (FSAI(1) when
- *            t >= 4, i.e. when a conditioning may spread O^2 over many decades), 1 = none, 2 = FSAI(1): a sparse
- *            approximate inverse factor with one off-diagonal entry per row, rebuilt on the device at every
- *            conditioning.  Changes the number of CG steps, not the solution of the solve.
+ *   precond  preconditioner of the inner CG beyond the Jacobi row equilibration: 0 = automatic (when t >= 4, i.e. when a
+ *            conditioning may spread O^2 over many decades: FSAI(5) if the two matrix copies fit in 100 MB, else FSAI(1)),
+ *            1 = none, 2 = FSAI(1): a sparse
+ *            approximate inverse factor with one off-diagonal entry per row, 3 = FSAI(5): up to five per row
+ *            (csrc/cs_fsaip.cuh; 35-55 % fewer CG steps than FSAI(1) on configs 1, 2 and on replicas of config 4, at
+ *            3-4x the cost of its application: it pays on configs 1 and 2, not on the full-size config 4).
+ *            Both are rebuilt on the device at every conditioning and change the number of CG steps, not
+ *            the solution of the solve.
  *   dense_m_threshold  dense factor-apply instead of CG where A is small enough that the solve truly is a dense
  *            contraction (B north_star; S 8(a) a3, S 8(f).3), for m <= dense_m_threshold (<= 4096; 0 = never):
  *            - problems that run on one CTA (nnz <= 8192) with m <= 256: every conditioning forms A~A~' (m x m, fp64) and

@@ -21,6 +21,9 @@
 #include "../../include/cs_diag.h"
 #include "cs_kernels_cond.cuh"
 
+#ifndef CS_AUTO_FSAIP_MB
+#define CS_AUTO_FSAIP_MB 100
+#endif
 #ifndef CS_STATIC_MAX_SOC
 #define CS_STATIC_MAX_SOC 32768
 #endif
@@ -53,6 +56,7 @@ namespace {
 
 thread_local std::string g_create_err;
 constexpr int kFuseCarveoutPct = CS_FUSE_CARVEOUT;   // percent of the SM's 228 KB of shared memory asked for when k_iterate fuses rows
+constexpr double kAutoFsaiPBytes = CS_AUTO_FSAIP_MB * 1e6;   // precond = 0 selects FSAI(5) up to this many bytes of matrix copies (L2-resident), FSAI(1) beyond
 constexpr int kOneCtaNnz = 8192;   // problems up to this many non-zeros run on ONE CTA
 
 #define CS_CUDA(S, call)                                                                         \
@@ -396,7 +400,11 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     // with the SOCP setting t = 1.7 it saves ~10 % of the CG steps and costs 18 % per step (measured)
     S->ctx.dense = (S->grid == 1 && S->ctx.dM && S->ctx.m <= std::min(S->prm.dense_m_threshold, kDenseMax)) ? 1
                  : (S->grid > 1 && S->ctx.gM && S->ctx.m <= S->prm.dense_m_threshold) ? 2 : 0;
-    S->ctx.fsai = !S->ctx.dense && (S->prm.precond == 2 || (S->prm.precond == 0 && S->prm.t >= 4.0));
+    // automatic: FSAI pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs); FSAI(5) where the
+    // matrix copies are L2-resident (its two gather passes cost 3-4x FSAI(1)'s: 1.2x faster per pass on configs 1, 2, slower
+    // on config 4), FSAI(1) otherwise
+    const int auto_fsai = 24.0 * (double)S->nnz <= kAutoFsaiPBytes ? 2 : 1;
+    S->ctx.fsai = S->ctx.dense ? 0 : S->prm.precond == 3 ? 2 : S->prm.precond == 2 ? 1 : (S->prm.precond == 0 && S->prm.t >= 4.0) ? auto_fsai : 0;
     S->ctx.mu = S->prm.mu;  // mu, t, o_floor, precond take effect here (cs.h)
     S->ctx.t = S->prm.t;
     S->ctx.o_floor = S->prm.o_floor;
@@ -697,6 +705,13 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         if ((st = dev_upload(S, &q, ri2.data(), ri2.size())) != CS_OK) return st; x.Cc.idx = q;
         if ((st = dev_upload(S, &q, hc2.pos.data(), hc2.pos.size())) != CS_OK) return st; x.Cc.pos = q;
         if ((st = dev_zeros(S, &x.f_ctop, (size_t)3 * n)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_ctop, (size_t)kFsTop * n)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_idx, (size_t)kFsP * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_tptr, (size_t)m + 1)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_tcnt, (size_t)m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_trow, (size_t)kFsP * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_val, (size_t)(kFsP + 1) * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_tval, (size_t)kFsP * m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_partner, (size_t)m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_tptr, (size_t)m + 1)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_tcur, (size_t)m)) != CS_OK) return st;
@@ -805,8 +820,8 @@ cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const dou
 cs_status cs_set_params(cs_solver *S, const cs_params *p) {
     if (!S || !p) return CS_EINVAL;
     if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || !(p->cg_reduce >= 0.0 && p->cg_reduce < 1.0) || p->cg_max_iter < 1 ||
-        p->precond < 0 || p->precond > 2 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseGridMax) {
-        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2}, dense_m_threshold in [0,4096]";
+        p->precond < 0 || p->precond > 3 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseGridMax) {
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2,3}, dense_m_threshold in [0,4096]";
         return CS_EINVAL;
     }
     S->prm = *p;

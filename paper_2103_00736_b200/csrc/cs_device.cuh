@@ -132,7 +132,9 @@ struct Ctx {
     double *fpart;          // [n_fa + n_fb][gridDim]: the column pass's partial sums of the fused rows, per CTA
     Csr Rc, Cc;             // plain compressed views of the same two copies
     // FSAI(1) preconditioner G = diag(gd) + strictly-lower part with one entry gm[i] at column partner[i]
-    int fsai;               // 0: off (plain Jacobi-equilibrated CG)
+    int fsai;               // 0: off (plain Jacobi-equilibrated CG), 1: FSAI(1) below, 2: FSAI(P) (cs_fsaip.cuh)
+    int *fp_ctop, *fp_idx, *fp_tptr, *fp_tcnt, *fp_trow;   // FSAI(P): [n][kFsTop], [kFsP][m], [m+1], [m], [kFsP*m]
+    double *fp_val, *fp_tval;                               // FSAI(P): [kFsP+1][m], [kFsP*m]
     int n_long;             // internal rows [0, n_long) are longer than kShortMax: no FSAI partner, G = I there
     int *f_ctop;            // [n][3] strongest short rows of every column
     int *f_partner;         // [m] partner row (< i) or -1

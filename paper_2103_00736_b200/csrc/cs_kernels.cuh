@@ -351,6 +351,20 @@ __device__ __forceinline__ void dense_apply_grid(const Ctx &c, GridCtl &gc) {
     gc.sync();
 }
 
+__device__ __forceinline__ void fsaip_pass_a(const Ctx &c, int k_begin);      // cs_fsaip.cuh
+__device__ __forceinline__ double fsaip_pass_b(const Ctx &c, int k_begin);
+// r'z with z = (preconditioner) r over ALL rows, one grid reduction (start of a solve)
+__device__ __forceinline__ double apply_precond(const Ctx &c, GridCtl &gc) {
+    if (c.fsai == 2) {
+        fsaip_pass_a(c, 0);
+        gc.sync();
+        double red[1] = {fsaip_pass_b(c, 0)};
+        grid_reduce<1>(red, gc);
+        return red[0];
+    }
+    return apply_fsai(c, gc);
+}
+
 __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, double qq, bool &hit_max) {
     // stop on ||r|| <= max(cg_tol ||q||, cg_reduce ||r at the warm start||) (equilibrated system; cs.h)
     const double thresh = fmax(c.cg_tol * c.cg_tol * qq, c.cg_reduce * c.cg_reduce * rr);
@@ -360,7 +374,7 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, do
     int steps = 0;
     hit_max = false;
     if (!(rr > thresh)) return 0;
-    double rz = c.fsai ? apply_fsai(c, gc) : rr;           // r'z, z = G'G r
+    double rz = c.fsai ? apply_precond(c, gc) : rr;        // r'z, z = G'G r
     while (rr > thresh) {
         if (steps >= c.cg_max_iter) { hit_max = true; break; }
         TermDot t1{zsrc};
@@ -390,7 +404,8 @@ __device__ __forceinline__ int cg_solve(const Ctx &c, GridCtl &gc, double rr, do
             // and one reduction for both ||r||^2 and r'z
             if (!c.R.n_multi_k2) gc.sync();                // otherwise seg_reduce's own barrier has made r complete
             double red2[2] = {e2.rho, 0.0};
-            red2[1] = fsai_pass(c, c.n_long);
+            if (c.fsai == 2) { fsaip_pass_a(c, c.n_long); gc.sync(); red2[1] = fsaip_pass_b(c, c.n_long); }   // FSAI(P): t = G r, z = G't
+            else red2[1] = fsai_pass(c, c.n_long);
             gc.lap(kPhPrecond);
             red2[1] += e2.rz_long;                         // the long rows' share, from K2's epilogue
             grid_reduce<2>(red2, gc);

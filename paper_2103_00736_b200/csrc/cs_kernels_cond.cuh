@@ -2,6 +2,7 @@
 // element-wise kernels around them.
 #pragma once
 #include "cs_kernels.cuh"
+#include "cs_fsaip.cuh"
 
 namespace csd {
 
@@ -259,7 +260,8 @@ __global__ void __launch_bounds__(kBlock, CS_MINB) k_condition(Ctx c, int use_ru
         seg_rescale(c.C, f2);
     }
     gc.sync();
-    if (c.fsai) fsai_build(c, gc);   // its own barriers; reads the rescaled values only
+    if (c.fsai == 1) fsai_build(c, gc);   // its own barriers; reads the rescaled values only
+    if (c.fsai == 2) fsaip_build(c, gc);
     if (c.dense == 1) dense_factor(c);    // one-CTA problems only (cs_api.cu): A~A~' and its Cholesky factor
     // Step 13's d is never formed: it is folded into the pass (cs_kernels.cuh), so a conditioning needs no
     // solve.  What remains is the recast of s (step 14) and g = A~'w in the new scaling.

@@ -436,8 +436,9 @@ def test_parameters_mu_and_t(mu, t):
 
 @pytest.mark.parametrize("name", ["cfg1_x0.3_pcg", "cfg4_x0.02_zipf_pcg", "mixed_cones"])
 def test_preconditioner_changes_the_steps_not_the_iterates(name):
-    """cs_params.precond: 1 = Jacobi equilibration only, 2 = FSAI(1).  Same passes (incl. a conditioning from
-    identical inputs) to 1e-9 against each other and against the oracle; fewer CG steps with FSAI on the LPs."""
+    """cs_params.precond: 1 = Jacobi equilibration only, 2 = FSAI(1), 3 = FSAI(5) (csrc/cs_fsaip.cuh).  Same passes (incl. a
+    conditioning from identical inputs) to 1e-9 against each other and against the oracle; fewer CG steps with FSAI on
+    the LPs, fewer still with FSAI(5)."""
     import oracle
     from paper_2103_00736_b200 import binding
     make, k, okw = CASES[name]
@@ -449,7 +450,7 @@ def test_preconditioner_changes_the_steps_not_the_iterates(name):
     O.set_point(start["x"], start["z"])
     O.run(8)
     ref, sols, steps = O.get(), {}, {}
-    for pc in (1, 2):
+    for pc in (1, 2, 3):
         S = binding.Solver.from_problem(p, device="cuda:0")
         S.set_params(precond=pc)
         assert S.get_params()["precond"] == pc
@@ -459,11 +460,11 @@ def test_preconditioner_changes_the_steps_not_the_iterates(name):
         for key in ("x", "z", "y", "s"):
             assert rel(sols[pc][key], ref[key]) <= TOL_ITER, (pc, key, rel(sols[pc][key], ref[key]))
     for key in ("x", "z", "y", "s"):
-        assert rel(sols[2][key], sols[1][key]) <= TOL_ITER
+        assert rel(sols[2][key], sols[1][key]) <= TOL_ITER and rel(sols[3][key], sols[1][key]) <= TOL_ITER
     if p.n_soc == 0:
-        assert steps[2] < 0.8 * steps[1], steps
+        assert steps[2] < 0.8 * steps[1] and steps[3] < 0.9 * steps[2], steps
     with pytest.raises(binding.CsError):
-        S.set_params(precond=3)
+        S.set_params(precond=4)
 
 
 @pytest.mark.parametrize("name", ["cfg0", "tiny_socp", "sec4a_gaussian"])
