@@ -79,7 +79,7 @@ typedef struct {
  *            tolerance with the fixed point unchanged; 0 < cg_reduce < 1.
  *   cg_max_iter  cap on CG steps per solve
  *   precond  preconditioner of the inner CG beyond the Jacobi row equilibration: 0 = automatic (when t >= 4, i.e. when a
- *            conditioning may spread O^2 over many decades: FSAI(5) if the two matrix copies fit in 100 MB, else FSAI(1)),
+ *            conditioning may spread O^2 over many decades: FSAI(5) if the two matrix copies take 16-100 MB, else FSAI(1)),
  *            1 = none, 2 = FSAI(1): a sparse
  *            approximate inverse factor with one off-diagonal entry per row, 3 = FSAI(5): up to five per row
  *            (csrc/cs_fsaip.cuh; 35-55 % fewer CG steps than FSAI(1) on configs 1, 2 and on replicas of config 4, at

@@ -56,6 +56,7 @@ namespace {
 
 thread_local std::string g_create_err;
 constexpr int kFuseCarveoutPct = CS_FUSE_CARVEOUT;   // percent of the SM's 228 KB of shared memory asked for when k_iterate fuses rows
+constexpr double kAutoFsaiPMinBytes = 16e6;
 constexpr double kAutoFsaiPBytes = CS_AUTO_FSAIP_MB * 1e6;   // precond = 0 selects FSAI(5) up to this many bytes of matrix copies (L2-resident), FSAI(1) beyond
 constexpr int kOneCtaNnz = 8192;   // problems up to this many non-zeros run on ONE CTA
 
@@ -401,9 +402,10 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     S->ctx.dense = (S->grid == 1 && S->ctx.dM && S->ctx.m <= std::min(S->prm.dense_m_threshold, kDenseMax)) ? 1
                  : (S->grid > 1 && S->ctx.gM && S->ctx.m <= S->prm.dense_m_threshold) ? 2 : 0;
     // automatic: FSAI pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs); FSAI(5) where the
-    // matrix copies are L2-resident (its two gather passes cost 3-4x FSAI(1)'s: 1.2x faster per pass on configs 1, 2, slower
-    // on config 4), FSAI(1) otherwise
-    const int auto_fsai = 24.0 * (double)S->nnz <= kAutoFsaiPBytes ? 2 : 1;
+    // matrix copies are L2-resident but the passes not yet latency-bound (config 2: 1.22x faster per pass; config 1: its two
+    // dependent gather passes and the heavier build cost what the saved steps gain; config 4: slower), FSAI(1) otherwise
+    const double mat_bytes = 24.0 * (double)S->nnz;
+    const int auto_fsai = mat_bytes >= kAutoFsaiPMinBytes && mat_bytes <= kAutoFsaiPBytes ? 2 : 1;
     S->ctx.fsai = S->ctx.dense ? 0 : S->prm.precond == 3 ? 2 : S->prm.precond == 2 ? 1 : (S->prm.precond == 0 && S->prm.t >= 4.0) ? auto_fsai : 0;
     S->ctx.mu = S->prm.mu;  // mu, t, o_floor, precond take effect here (cs.h)
     S->ctx.t = S->prm.t;
