@@ -204,7 +204,7 @@ def main():
     ap.add_argument("--solve", action="store_true",
                     help="extra mode: run the paper's schedule (17)/(18) to --tol and report the time to tolerance")
     ap.add_argument("--tol", type=float, default=1e-4)
-    ap.add_argument("--cg-tol", type=float, default=0.0, help="--solve only: inner CG tolerance (0 = library default 1e-15)")
+    ap.add_argument("--cg-tol", type=float, default=0.0, help="--solve only: inner CG tolerance (0 = library default DBL_EPSILON)")
     ap.add_argument("--cg-reduce", type=float, default=0.0, help="--solve only: cs_params.cg_reduce (adaptive inexact projections)")
     ap.add_argument("--check-every", type=int, default=25)
     ap.add_argument("--max-iter", type=int, default=3000)
@@ -512,7 +512,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
         except Exception as e:  # pragma: no cover
             line["secondary"] = {"error": str(e)}
         # B's third metric, "time to 1e-4 relative KKT residual", on the headline workload with the paper's
-        # schedule (17).  With the parity setting cg_tol = 1e-15 the conditioned solves take 1e4 CG steps per pass
+        # schedule (17).  With the parity setting (cg_tol = DBL_EPSILON) the conditioned solves take thousands of CG steps per pass
         # (DESIGN.md 9), so this leg uses inexact projections: cs_params.cg_reduce = 0.2, i.e. every pass's solve stops
         # once its warm-start residual has dropped 5x (measured at config 4: 7.3 s / 1350 passes / 21k CG steps; the
         # fixed tolerance cg_tol = 1e-7 needs 20 s / 825 passes / 63k CG steps, 1e-6 stalls at kkt 2e-4).

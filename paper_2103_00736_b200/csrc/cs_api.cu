@@ -1,6 +1,7 @@
-// cs_api.cu -- host side of libcs.so: the C ABI of include/cs.h.
-// Validation, CSR->CSC transposition and the work partition are one-off host work at cs_create;
-// every step of the iteration itself is a kernel in cs_kernels*.cuh.
+// cs_api.cu -- host side of libcs.so: the C ABI of include/cs.h (diagnostics: include/cs_diag.h).
+// Validation, the internal ordering, the CSR->CSC transposition, the slice layout and the heavy-row fusion plan are one-off
+// host work at cs_create; every step of the iteration itself is a kernel in cs_kernels*.cuh, cs_fsaip.cuh, cs_dense.cuh.
+// The handle-free, allocation-free entry point cs_cone_violation_static and its static scratch are at the end of the file.
 #include <cuda_runtime.h>
 
 #include <algorithm>
