@@ -388,7 +388,10 @@ cs_status dense_grid_factor(cs_solver *S) {
         k_chol_update<<<t * (t + 1) / 2, 256, 0, S->stream>>>(c.gL, m, kb);
         S->launches += 2;
     }
-    k_dense_trinv<<<std::min(148 * 8, (m + 7) / 8), 256, 0, S->stream>>>(c.gL, m, c.gZ);
+    // L' into gMinv (free until the last step), then the triangular inverse reads L by columns
+    k_dense_transpose_lower<<<dim3((m + 31) / 32, (m + 31) / 32), 256, 0, S->stream>>>(c.gL, m, c.gMinv);
+    k_dense_trinv<<<std::min(148 * 8, (m + 7) / 8), 256, 0, S->stream>>>(c.gMinv, m, c.gZ);
+    S->launches += 1;
     k_dense_aat<<<n_tri, 256, 0, S->stream>>>(c.gZ, m, m, c.gMinv);
     S->launches += 2;
     CS_CUDA(S, cudaGetLastError());
