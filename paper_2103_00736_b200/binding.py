@@ -202,7 +202,10 @@ class Solver:
 
     def destroy(self):
         if getattr(self, "_h", None):
-            lib().cs_destroy(self._h)
+            try:
+                lib().cs_destroy(self._h)
+            except TypeError:       # interpreter shutdown: the module globals are gone, the process frees the device memory
+                pass
             self._h = None
 
     __del__ = destroy

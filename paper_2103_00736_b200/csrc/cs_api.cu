@@ -344,6 +344,10 @@ std::vector<int> order_by_length(const std::vector<int> &len, int n_sort) {
 
 cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
     const size_t dyn = fn == (const void *)k_iterate ? S->dyn_smem : 0;
+    // the shared-memory carve-out is a property of the FUNCTION, shared by every handle of the process: a handle without
+    // fused rows must not inherit the 100 KB another handle asked for (its gathers would lose 100 KB of L1)
+    if (fn == (const void *)k_iterate)
+        CS_CUDA(S, cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, dyn ? kFuseCarveoutPct : (int)cudaSharedmemCarveoutDefault));
     CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, dyn, S->stream));
     S->launches += 1;
     return CS_OK;
