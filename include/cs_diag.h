@@ -23,6 +23,14 @@ cs_status cs_diag_phase_times(cs_solver *S, double out[8]);
  * LSU/L1TEX gather ceiling that bounds the sparse passes on irregular matrices. */
 cs_status cs_diag_gather_probe(int64_t n_vec, int64_t n_idx, double *us_gather, double *us_stream_only);
 
+/* cs_create with the layout build chosen by hand: build_mode 0 = as cs_create (on the device from 100,000 non-zeros on), 1 = on
+ * the host, 2 = on the device (csrc/cs_build.cuh).  The two builds produce identical layouts; the GPU test compares them with */
+cs_status cs_diag_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where, const cs_cones *K,
+                         void *cuda_stream, int32_t build_mode);
+/* ... FNV-1a digests of the handle's layout arrays (slices, indices, pristine values, chunk tables, compressed views, fusion
+ * marks, permutations, b, c) and its counters, 32 words.  Synchronous, copies the arrays to the host: small problems only. */
+cs_status cs_diag_layout_digest(cs_solver *S, uint64_t out[32]);
+
 /* Diagnostic (no handle, current device, default stream, synchronous): L2 -> SM read bandwidth in GB/s -- `reps` passes
  * of 16-byte loads over a `bytes`-sized buffer that stays in L2 (choose bytes well below the 126 MB of L2), best of 4. */
 cs_status cs_diag_l2_probe(int64_t bytes, int32_t reps, double *gbs);

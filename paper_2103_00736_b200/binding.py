@@ -54,7 +54,8 @@ CS_RULE_SET, CS_RULE_STALL = 0, 1
 
 _INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
                "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_diag_phase_times",
-               "cs_diag_gather_probe", "cs_diag_barrier_probe", "cs_diag_l2_probe", "cs_cone_violation_static")
+               "cs_diag_gather_probe", "cs_diag_barrier_probe", "cs_diag_l2_probe", "cs_diag_create", "cs_diag_layout_digest",
+               "cs_cone_violation_static")
 EXPORTS = _INT_STATUS + ("cs_kernel_launches", "cs_last_error", "cs_destroy")
 
 _lib = None
@@ -91,6 +92,8 @@ def lib():
         L.cs_solve.argtypes = [vp, C.POINTER(cs_schedule), C.POINTER(cs_resid), C.POINTER(C.c_int64), C.c_int64,
                                C.POINTER(C.c_int64)]
         L.cs_diag_l2_probe.argtypes = [C.c_int64, C.c_int32, C.POINTER(C.c_double)]
+        L.cs_diag_create.argtypes = [C.POINTER(vp), C.POINTER(cs_csr), vp, vp, C.c_int, C.POINTER(cs_cones), vp, C.c_int32]
+        L.cs_diag_layout_digest.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.cs_cone_violation_static.argtypes = [vp, vp, C.c_int64, C.POINTER(cs_cones), vp, C.c_int, vp]
         for name in _INT_STATUS:
             getattr(L, name).restype = C.c_int
@@ -166,7 +169,8 @@ def cone_violation_static(x, z, n_lin, soc_size=None, out=None, stream=None):
 class Solver:
     """One ``cs_solver`` handle.  Method names mirror the C ABI without the ``cs_`` prefix."""
 
-    def __init__(self, m, n, row_ptr, col_idx, val, b, c, n_lin, soc_size=None, stream=None):
+    def __init__(self, m, n, row_ptr, col_idx, val, b, c, n_lin, soc_size=None, stream=None, build_mode=None):
+        """build_mode (diagnostic, cs_diag_create): None = cs_create, 1 = layout built on the host, 2 = on the device."""
         L = lib()
         rp, ci, va = _ptr(row_ptr, np.int32), _ptr(col_idx, np.int32), _ptr(val, np.float64)
         where_A = _same_space(rp, ci, va)
@@ -177,21 +181,24 @@ class Solver:
         soc = np.ascontiguousarray(soc_size if soc_size is not None else [], dtype=np.int32)
         K = cs_cones(int(n_lin), int(soc.shape[0]), soc.ctypes.data if soc.size else None)
         h = C.c_void_p()
-        st = L.cs_create(C.byref(h), C.byref(A), bp[0], cp[0], where_v, C.byref(K),
-                         C.c_void_p(int(stream)) if stream else None)
+        sp = C.c_void_p(int(stream)) if stream else None
+        if build_mode is None:
+            st = L.cs_create(C.byref(h), C.byref(A), bp[0], cp[0], where_v, C.byref(K), sp)
+        else:
+            st = L.cs_diag_create(C.byref(h), C.byref(A), bp[0], cp[0], where_v, C.byref(K), sp, int(build_mode))
         if st != CS_OK:
             raise CsError(st, L.cs_last_error(None).decode())
         self._h, self.m, self.n = h, int(m), int(n)
 
     @classmethod
-    def from_problem(cls, p, device=None, stream=None):
+    def from_problem(cls, p, device=None, stream=None, build_mode=None):
         """Build from a ``workloads.Problem``; ``device`` = torch device to stage the inputs on first
         (inputs resident in HBM), None = pass the host arrays."""
         arrs = [p.row_ptr, p.col_idx, p.val, p.b, p.c]
         if device is not None:
             import torch
             arrs = [torch.from_numpy(np.ascontiguousarray(a)).to(device) for a in arrs]
-        S = cls(p.m, p.n, arrs[0], arrs[1], arrs[2], arrs[3], arrs[4], p.n_lin, p.soc_size, stream=stream)
+        S = cls(p.m, p.n, arrs[0], arrs[1], arrs[2], arrs[3], arrs[4], p.n_lin, p.soc_size, stream=stream, build_mode=build_mode)
         S.set_params(mu=p.mu, t=p.t)
         return S
 
@@ -287,6 +294,12 @@ class Solver:
         us = C.c_double()
         self._check(lib().cs_diag_barrier_probe(self._h, int(n), C.byref(us)))
         return us.value
+
+    def layout_digest(self):
+        """cs_diag_layout_digest: 32 words identifying the handle's layout (diagnostic; copies the arrays to the host)."""
+        a = (C.c_uint64 * 32)()
+        self._check(lib().cs_diag_layout_digest(self._h, a))
+        return [int(v) for v in a]
 
     def kernel_launches(self):
         return int(lib().cs_kernel_launches(self._h))

@@ -21,6 +21,7 @@
 
 #include "../../include/cs_diag.h"
 #include "cs_kernels_cond.cuh"
+#include "cs_build.cuh"
 
 #ifndef CS_AUTO_FSAIP_MB
 #define CS_AUTO_FSAIP_MB 100
@@ -46,6 +47,8 @@ struct cs_solver {
     bool conditioned = false;  // the l=1 conditioning of step 4 has run
     bool xz_stale = false;     // xb, zb older than (p, s)
     bool started = false;      // some pass or conditioning has run (cs_set_point no longer allowed)
+    int build_mode = 0;        // layout build: 0 automatic, 1 host, 2 device (cs_diag_create)
+    size_t tot_r = 0, tot_c = 0;   // padded entries of the two sliced copies (cs_diag_layout_digest)
     int64_t launches = 0;
     int64_t iter = 0;          // passes done (Algorithm 2's l), mirrors Scalars::iter
     double stall_f = 0.0;      // cs_solve, stall rule: fixed-point residual sampled after pass stall_at (-1: none)
@@ -59,6 +62,7 @@ thread_local std::string g_create_err;
 constexpr int kFuseCarveoutPct = CS_FUSE_CARVEOUT;   // percent of the SM's 228 KB of shared memory asked for when k_iterate fuses rows
 constexpr double kAutoFsaiPMinBytes = 16e6;
 constexpr double kAutoFsaiPBytes = CS_AUTO_FSAIP_MB * 1e6;   // precond = 0 selects FSAI(5) up to this many bytes of matrix copies (L2-resident), FSAI(1) beyond
+constexpr int kDeviceBuildMinNnz = 100000;   // smaller problems are laid out on the host (a few ms either way)
 constexpr int kOneCtaNnz = 8192;   // problems up to this many non-zeros run on ONE CTA
 
 #define CS_CUDA(S, call)                                                                         \
@@ -139,6 +143,8 @@ struct HostSparse {
     uvec<double> val;
     std::vector<unsigned char> fmask;  // column-major copy with fused rows: [short slice][lane] bit k = entry k of the column is fused
     int n_chunk = 0, n_chunk_k2 = 0, n_slots = 0;
+    std::vector<int> chunk_src, chunk_len;   // first source entry and length of every chunk slice (the fill needs them)
+    size_t total = 0;             // padded entries
     bool too_big = false;         // padded storage would exceed 2^31 entries: nothing was filled
 };
 
@@ -175,17 +181,18 @@ struct FusePlan { int n_fa = 0, n_fb = 0; int rows() const { return n_fa + n_fb;
 //     are per warp); only the first kFuseK entries of a column qualify.
 //   Row-major copy (split != nullptr): the first split[s] entries of fused row s stay with the row pass of a CG step
 //     (K2 view), the rest have been taken over by the column pass; each part gets its own chunk slices.
+//   plan_only: stop after the plan (the device build fills the arrays with kernels, cs_build.cuh).
 HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const uvec<double> &val, int nt,
                        const FusePlan *fuse = nullptr, uvec<unsigned char> *fused_out = nullptr,
-                       const std::vector<int> *split = nullptr) {
+                       const std::vector<int> *split = nullptr, bool plan_only = false) {
     HostSparse h;
+    std::vector<int> &chunk_src = h.chunk_src, &chunk_len = h.chunk_len;
     const int nseg = (int)ptr.size() - 1;
     // several lanes per segment only pay when there are too few segments to fill the machine (measured:
     // T>1 is slower once every warp has >= 2 thread-per-segment slices)
     const bool split_lanes = nseg < 300000;
     auto lg_lanes = [split_lanes](int len) { return (!split_lanes || len <= 8) ? 0 : len <= 16 ? 1 : len <= 32 ? 2 : 3; };  // T = 1,2,4,8 lanes
     size_t total = 0;
-    std::vector<int> chunk_src, chunk_len;       // first source entry and length of every chunk slice
     auto plan_slice = [&](int seg0, int meta, int width) {
         h.slices.push_back(make_int4((int)std::min<size_t>(total, INT32_MAX), seg0, meta, width));
         total += 32u * (size_t)width;
@@ -247,7 +254,9 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
         run = s + 1;
     }
     plan_run(run, nseg);
+    h.total = total;
     if (total >= (size_t)INT32_MAX) { h.too_big = true; return h; }   // offsets are int32: refuse before anything is filled
+    if (plan_only) return h;
     // fill (padding: val = 0, a valid index replicated)
     h.val.resize(total);          // no zero-fill: the fill below writes every slot (padding values = 0)
     h.idx.resize(total);
@@ -309,6 +318,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
 
 cs_status upload_sparse(cs_solver *S, const HostSparse &h, Sparse *out) {
     cs_status st;
+    (out == &S->ctx.R ? S->tot_r : S->tot_c) = h.val.size();
     int4 *p4; int *pi; double *pd;
     if ((st = dev_upload(S, &p4, h.slices.data(), h.slices.size())) != CS_OK) return st; out->slices = p4;
     if ((st = dev_upload(S, &p4, h.multi.data(), h.multi.size())) != CS_OK) return st; out->multi = p4;
@@ -340,6 +350,256 @@ std::vector<int> order_by_length(const std::vector<int> &len, int n_sort) {
     for (int i = 0; i < n_sort; ++i) perm[start[maxlen - len[i]]++] = i;
     for (int i = n_sort; i < n; ++i) perm[i] = i;
     return perm;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// cs_create on the device (cs_build.cuh): the O(nnz) work -- validation, the two ordered compressed copies (one radix sort
+// each), the slice fill, the fusion marks, the fused rows' partition -- runs as kernels on the uploaded CSR; the host does
+// the O(m + n) part (length ordering, prefix sums, slice plans).  Same layouts as the host build, bit for bit.
+// ---------------------------------------------------------------------------------------------------------------------
+int ew_blocks(int n) { return std::max(1, std::min((n + 255) / 256, 148 * 8)); }
+
+struct DevTmp {                                   // scratch of the build: stream-ordered allocations, released on every path
+    std::vector<void *> p;
+    cudaStream_t stream = nullptr;
+    ~DevTmp() { for (void *q : p) cudaFreeAsync(q, stream); }
+    template <class T>
+    cs_status alloc(cs_solver *S, T **out, size_t count, bool zero = false) {
+        void *q = nullptr;
+        stream = S->stream;
+        CS_CUDA(S, cudaMallocAsync(&q, std::max<size_t>(count, 1) * sizeof(T), S->stream));
+        p.push_back(q);
+        *out = static_cast<T *>(q);
+        if (zero) CS_CUDA(S, cudaMemsetAsync(q, 0, std::max<size_t>(count, 1) * sizeof(T), S->stream));
+        return CS_OK;
+    }
+};
+
+// plan -> device Sparse: uploads the descriptors, allocates the slice storage; chunk_src / chunk_len go to scratch
+cs_status upload_plan(cs_solver *S, DevTmp &tmp, const HostSparse &h, Sparse *out, int4 **d_slices, int **d_csrc, int **d_clen, int **d_idx,
+                      double **d_val0, bool with_fmask) {
+    cs_status st;
+    (out == &S->ctx.R ? S->tot_r : S->tot_c) = h.total;
+    int4 *p4; int *pi;
+    if ((st = dev_upload(S, d_slices, h.slices.data(), h.slices.size())) != CS_OK) return st; out->slices = *d_slices;
+    if ((st = dev_upload(S, &p4, h.multi.data(), h.multi.size())) != CS_OK) return st; out->multi = p4;
+    if ((st = dev_upload(S, &p4, h.multi_k2.data(), h.multi_k2.size())) != CS_OK) return st; out->multi_k2 = p4;
+    if ((st = dev_upload(S, &pi, h.chunk_slot.data(), h.chunk_slot.size())) != CS_OK) return st; out->chunk_slot = pi;
+    if ((st = tmp.alloc(S, d_csrc, h.chunk_src.size())) != CS_OK) return st;
+    if ((st = tmp.alloc(S, d_clen, h.chunk_len.size())) != CS_OK) return st;
+    if (!h.chunk_src.empty()) {
+        CS_CUDA(S, cudaMemcpyAsync(*d_csrc, h.chunk_src.data(), sizeof(int) * h.chunk_src.size(), cudaMemcpyHostToDevice, S->stream));
+        CS_CUDA(S, cudaMemcpyAsync(*d_clen, h.chunk_len.data(), sizeof(int) * h.chunk_len.size(), cudaMemcpyHostToDevice, S->stream));
+    }
+    if ((st = dev_alloc(S, d_idx, h.total)) != CS_OK) return st; out->idx = *d_idx;
+    if ((st = dev_alloc(S, d_val0, h.total)) != CS_OK) return st; out->val0 = *d_val0;
+    if ((st = dev_alloc(S, &out->val, h.total)) != CS_OK) return st;
+    unsigned char *pu = nullptr;
+    const size_t nmask = with_fmask ? (h.slices.size() - (size_t)h.n_chunk) * 32 : 0;
+    if ((st = dev_zeros(S, &pu, nmask)) != CS_OK) return st; out->fmask = pu;
+    out->n_slice = (int)h.slices.size();
+    out->n_chunk = h.n_chunk;
+    out->n_chunk_k2 = h.n_chunk_k2;
+    out->n_multi = (int)h.multi.size();
+    out->n_multi_k2 = (int)h.multi_k2.size();
+    return dev_zeros(S, &out->partial, (size_t)h.n_slots * 2);
+}
+
+template <class LapFn>
+cs_status layout_device(cs_solver *S, const cs_csr *A, const double *b, const double *c, cs_mem vec_where, const cs_cones *K, int m, int n,
+                        int nnz, std::vector<int> &perm_r, std::vector<int> &perm_c, std::vector<double> &hb, std::vector<double> &hc,
+                        double &nb, double &nc, LapFn lap) {
+    DevTmp tmp;
+    cs_status st;
+    Ctx &x = S->ctx;
+    const int grid = 148 * 8;
+    // ---- the caller's CSR on the device
+    const int *d_rptr = A->row_ptr, *d_cidx = A->col_idx;
+    const double *d_val = A->val;
+    std::vector<int> rptr_v;
+    const int *rptr = A->row_ptr;
+    if (A->where == CS_HOST) {
+        int *q; double *qd;
+        if ((st = tmp.alloc(S, &q, (size_t)m + 1)) != CS_OK) return st;
+        CS_CUDA(S, cudaMemcpyAsync(q, A->row_ptr, sizeof(int) * ((size_t)m + 1), cudaMemcpyHostToDevice, S->stream)); d_rptr = q;
+        if ((st = tmp.alloc(S, &q, (size_t)nnz)) != CS_OK) return st;
+        CS_CUDA(S, cudaMemcpyAsync(q, A->col_idx, sizeof(int) * (size_t)nnz, cudaMemcpyHostToDevice, S->stream)); d_cidx = q;
+        if ((st = tmp.alloc(S, &qd, (size_t)nnz)) != CS_OK) return st;
+        CS_CUDA(S, cudaMemcpyAsync(qd, A->val, sizeof(double) * (size_t)nnz, cudaMemcpyHostToDevice, S->stream)); d_val = qd;
+    } else {
+        if ((st = fetch(S, rptr_v, A->row_ptr, (size_t)m + 1, A->where)) != CS_OK) return st;
+        rptr = rptr_v.data();
+    }
+    // b, c: raw copies on the device (permuted there once the ordering is known); the host reads them for the norms
+    const double *hb_p = b, *hc_p = c, *d_braw = b, *d_craw = c;
+    if (vec_where == CS_HOST) {
+        double *qd;
+        if ((st = tmp.alloc(S, &qd, (size_t)m)) != CS_OK) return st;
+        CS_CUDA(S, cudaMemcpyAsync(qd, b, sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, S->stream)); d_braw = qd;
+        if ((st = tmp.alloc(S, &qd, (size_t)n)) != CS_OK) return st;
+        CS_CUDA(S, cudaMemcpyAsync(qd, c, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, S->stream)); d_craw = qd;
+    } else {
+        if ((st = fetch(S, hb, b, (size_t)m, vec_where)) != CS_OK) return st;
+        if ((st = fetch(S, hc, c, (size_t)n, vec_where)) != CS_OK) return st;
+        hb_p = hb.data(); hc_p = hc.data();
+    }
+    if (rptr[0] != 0 || rptr[m] != nnz) { S->err = "row_ptr[0] != 0 or row_ptr[m] != nnz"; return CS_EINVAL; }
+    for (int i = 0; i < m; ++i) {
+        if (rptr[i + 1] <= rptr[i]) { S->err = "row_ptr not increasing (empty rows are not allowed)"; return CS_EINVAL; }
+        if (rptr[i + 1] > nnz) { S->err = "row_ptr out of range"; return CS_EINVAL; }
+    }
+    // ---- validation + column counts (device)
+    int *d_clen, *d_status;
+    if ((st = tmp.alloc(S, &d_clen, (size_t)n, true)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &d_status, 1, true)) != CS_OK) return st;
+    csb::k_validate<<<grid, 256, 0, S->stream>>>(d_rptr, d_cidx, d_val, m, n, d_clen, d_status);
+    int status = 0;
+    CS_CUDA(S, cudaMemcpyAsync(&status, d_status, sizeof(int), cudaMemcpyDeviceToHost, S->stream));
+    nb = 0.0; nc = 0.0;                                                // meanwhile on the host: b, c
+    for (int i = 0; i < m; ++i) { if (!std::isfinite(hb_p[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb_p[i] * hb_p[i]; }
+    for (int j = 0; j < n; ++j) { if (!std::isfinite(hc_p[j])) { S->err = "non-finite c"; return CS_EINVAL; } nc += hc_p[j] * hc_p[j]; }
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    S->launches += 1;
+    if (status & csb::kBadIndex) { S->err = "col_idx out of range, unsorted or duplicated within a row"; return CS_EINVAL; }
+    if (status & csb::kBadValue) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
+    if (status & csb::kZeroRow) { S->err = "a row of A has zero norm (all stored entries are 0 or underflow when squared)"; return CS_EINVAL; }
+    lap("upload + validate (device)");
+    // ---- internal ordering: stable sorts by decreasing length (rows; the orthant columns), inverse permutations, new pointers
+    const int n_lin = (int)K->n_lin, nmax = std::max(m, n);
+    unsigned *lk, *lk_s, *io;
+    int *d_perm_r, *d_perm_c, *d_inv_r, *d_inv_c, *d_rp2, *d_cp2, *d_len;
+    if ((st = tmp.alloc(S, &lk, (size_t)nmax)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &lk_s, (size_t)nmax)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &io, (size_t)nmax)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &d_len, (size_t)nmax + 1)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &d_inv_r, (size_t)m)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &d_inv_c, (size_t)n)) != CS_OK) return st;
+    if ((st = dev_alloc(S, &d_perm_r, (size_t)m)) != CS_OK) return st; x.perm_r = d_perm_r;
+    if ((st = dev_alloc(S, &d_perm_c, (size_t)n)) != CS_OK) return st; x.perm_c = d_perm_c;
+    if ((st = dev_alloc(S, &d_rp2, (size_t)m + 1)) != CS_OK) return st; x.Rc.ptr = d_rp2;
+    if ((st = dev_alloc(S, &d_cp2, (size_t)n + 1)) != CS_OK) return st; x.Cc.ptr = d_cp2;
+    size_t ob1 = 0, ob2 = 0;
+    CS_CUDA(S, cub::DeviceRadixSort::SortPairs(nullptr, ob1, lk, lk_s, io, reinterpret_cast<unsigned *>(d_perm_r), nmax, 0, 32, S->stream));
+    CS_CUDA(S, cub::DeviceScan::ExclusiveSum(nullptr, ob2, d_len, d_rp2, nmax + 1, S->stream));
+    unsigned char *otmp;
+    const size_t ob = std::max(ob1, ob2) + 16;
+    if ((st = tmp.alloc(S, &otmp, ob)) != CS_OK) return st;
+    size_t obq = ob;
+    csb::k_len_keys<<<grid, 256, 0, S->stream>>>(d_rptr, 1, m, lk, io);
+    CS_CUDA(S, cub::DeviceRadixSort::SortPairs(otmp, obq, lk, lk_s, io, reinterpret_cast<unsigned *>(d_perm_r), m, 0, 32, S->stream));
+    csb::k_invert_and_len<<<grid, 256, 0, S->stream>>>(d_perm_r, d_rptr, 1, m, d_inv_r, d_len);
+    obq = ob;
+    CS_CUDA(S, cub::DeviceScan::ExclusiveSum(otmp, obq, d_len, d_rp2, m + 1, S->stream));
+    if (n_lin > 0) {
+        csb::k_len_keys<<<grid, 256, 0, S->stream>>>(d_clen, 0, n_lin, lk, io);
+        obq = ob;
+        CS_CUDA(S, cub::DeviceRadixSort::SortPairs(otmp, obq, lk, lk_s, io, reinterpret_cast<unsigned *>(d_perm_c), n_lin, 0, 32, S->stream));
+    }
+    csb::k_iota_tail<<<grid, 256, 0, S->stream>>>(d_perm_c, n_lin, n);
+    csb::k_invert_and_len<<<grid, 256, 0, S->stream>>>(d_perm_c, d_clen, 0, n, d_inv_c, d_len);
+    obq = ob;
+    CS_CUDA(S, cub::DeviceScan::ExclusiveSum(otmp, obq, d_len, d_cp2, n + 1, S->stream));
+    // b, c in internal order
+    double *d_b, *d_c;
+    if ((st = dev_alloc(S, &d_b, (size_t)m)) != CS_OK) return st; x.b = d_b;
+    if ((st = dev_alloc(S, &d_c, (size_t)n)) != CS_OK) return st; x.c = d_c;
+    k_gather_perm<<<ew_blocks(m), 256, 0, S->stream>>>(d_b, d_braw, d_perm_r, m);
+    k_gather_perm<<<ew_blocks(n), 256, 0, S->stream>>>(d_c, d_craw, d_perm_c, n);
+    std::vector<int> rp2((size_t)m + 1), cp2((size_t)n + 1);        // the slice plans are made on the host
+    CS_CUDA(S, cudaMemcpyAsync(rp2.data(), d_rp2, sizeof(int) * ((size_t)m + 1), cudaMemcpyDeviceToHost, S->stream));
+    CS_CUDA(S, cudaMemcpyAsync(cp2.data(), d_cp2, sizeof(int) * ((size_t)n + 1), cudaMemcpyDeviceToHost, S->stream));
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    S->launches += 9;
+    for (int i = 0; i < m && rp2[(size_t)i + 1] - rp2[i] > kShortMax; ++i) x.n_long = i + 1;
+    lap("row/column ordering");
+    // ---- the two compressed copies: one radix sort each
+    unsigned long long *key_c, *key_r, *key_s;
+    unsigned int *pay, *pay_s;
+    if ((st = tmp.alloc(S, &key_c, (size_t)nnz)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &key_r, (size_t)nnz)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &key_s, (size_t)nnz)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &pay, (size_t)nnz)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &pay_s, (size_t)nnz)) != CS_OK) return st;
+    csb::k_keys<<<grid, 256, 0, S->stream>>>(d_rptr, d_cidx, m, d_inv_r, d_inv_c, key_c, key_r, pay);
+    auto bits = [](int v) { int b = 1; while ((1ll << b) < (long long)v) ++b; return b; };
+    const int end_c = 32 + bits(n), end_r = 32 + bits(m);       // the high word holds an internal column / row number
+    size_t cub_bytes = 0;
+    CS_CUDA(S, cub::DeviceRadixSort::SortPairs(nullptr, cub_bytes, key_c, key_s, pay, pay_s, nnz, 0, 64, S->stream));
+    unsigned char *cub_tmp;
+    if ((st = tmp.alloc(S, &cub_tmp, cub_bytes + 16)) != CS_OK) return st;
+    int *ri2, *ci2;
+    double *cv2, *va2;
+    if ((st = dev_alloc(S, &ri2, (size_t)nnz)) != CS_OK) return st; x.Cc.idx = ri2;
+    if ((st = dev_alloc(S, &ci2, (size_t)nnz)) != CS_OK) return st; x.Rc.idx = ci2;
+    if ((st = tmp.alloc(S, &cv2, (size_t)nnz)) != CS_OK) return st;
+    if ((st = tmp.alloc(S, &va2, (size_t)nnz)) != CS_OK) return st;
+    CS_CUDA(S, cub::DeviceRadixSort::SortPairs(cub_tmp, cub_bytes, key_c, key_s, pay, pay_s, nnz, 0, end_c, S->stream));
+    csb::k_gather_c<<<grid, 256, 0, S->stream>>>(key_s, pay_s, d_val, nnz, ri2, cv2);
+    CS_CUDA(S, cub::DeviceRadixSort::SortPairs(cub_tmp, cub_bytes, key_r, key_s, pay, pay_s, nnz, 0, end_r, S->stream));
+    csb::k_gather_r<<<grid, 256, 0, S->stream>>>(pay_s, d_cidx, d_val, d_inv_c, nnz, ci2, va2);
+    S->launches += 5;
+    CS_CUDA(S, cudaGetLastError());
+    lap("compressed copies (2 radix sorts)");
+    // ---- column-major copy: plan (host), fill + fusion marks (device)
+    const int nt = host_threads();
+    const uvec<int> no_idx;
+    const uvec<double> no_val;
+    FusePlan fuse;
+    if (nnz > kOneCtaNnz)
+        for (int i = 0; i < std::min(m, kFuseA + kFuseB) && rp2[(size_t)i + 1] - rp2[i] >= kFuseMinLen; ++i)
+            (i < kFuseA ? fuse.n_fa : fuse.n_fb) += 1;
+    const HostSparse hc2 = make_sparse(cp2, no_idx, no_val, nt, nullptr, nullptr, nullptr, true);
+    if (hc2.too_big) { S->err = "padded slice storage exceeds 2^31 entries"; return CS_EINVAL; }
+    int4 *d_sl; int *d_csrc, *d_clen2, *d_idx, *d_pos;
+    double *d_val0;
+    if ((st = upload_plan(S, tmp, hc2, &x.C, &d_sl, &d_csrc, &d_clen2, &d_idx, &d_val0, fuse.rows() > 0)) != CS_OK) return st;
+    if ((st = dev_alloc(S, &d_pos, (size_t)nnz)) != CS_OK) return st; x.Cc.pos = d_pos;
+    unsigned char *fused_c;
+    if ((st = tmp.alloc(S, &fused_c, (size_t)nnz, fuse.rows() > 0)) != CS_OK) return st;
+    csb::k_fill_slices<<<grid, 256, 0, S->stream>>>(d_sl, x.C.n_slice, x.C.n_chunk, d_csrc, d_clen2, d_cp2, ri2, cv2, d_idx, d_val0, d_pos,
+                                                    fuse.rows(), fuse.n_fa, const_cast<unsigned char *>(x.C.fmask), fused_c);
+    CS_CUDA(S, cudaMemcpyAsync(x.C.val, d_val0, sizeof(double) * hc2.total, cudaMemcpyDeviceToDevice, S->stream));
+    S->launches += 1;
+    // ---- fused rows of the row-major copy: unfused entries first
+    std::vector<int> split((size_t)fuse.rows());
+    if (fuse.rows()) {
+        const int nf = fuse.rows(), region = rp2[nf];
+        int *flag, *sc, *ci2_o, *d_split;
+        double *va2_o;
+        if ((st = tmp.alloc(S, &flag, (size_t)region + 1)) != CS_OK) return st;
+        if ((st = tmp.alloc(S, &sc, (size_t)region + 1)) != CS_OK) return st;
+        if ((st = tmp.alloc(S, &ci2_o, (size_t)region)) != CS_OK) return st;
+        if ((st = tmp.alloc(S, &va2_o, (size_t)region)) != CS_OK) return st;
+        if ((st = tmp.alloc(S, &d_split, (size_t)nf)) != CS_OK) return st;
+        csb::k_fused_flags<<<grid, 256, 0, S->stream>>>(d_rp2, ci2, d_cp2, ri2, fused_c, nf, flag);
+        size_t scan_bytes = 0;
+        CS_CUDA(S, cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, flag, sc, region + 1, S->stream));
+        unsigned char *scan_tmp;
+        if ((st = tmp.alloc(S, &scan_tmp, scan_bytes + 16)) != CS_OK) return st;
+        CS_CUDA(S, cub::DeviceScan::ExclusiveSum(scan_tmp, scan_bytes, flag, sc, region + 1, S->stream));
+        csb::k_fused_partition<<<grid, 256, 0, S->stream>>>(d_rp2, flag, sc, nf, ci2, va2, ci2_o, va2_o, d_split);
+        CS_CUDA(S, cudaMemcpyAsync(ci2, ci2_o, sizeof(int) * (size_t)region, cudaMemcpyDeviceToDevice, S->stream));
+        CS_CUDA(S, cudaMemcpyAsync(va2, va2_o, sizeof(double) * (size_t)region, cudaMemcpyDeviceToDevice, S->stream));
+        CS_CUDA(S, cudaMemcpyAsync(split.data(), d_split, sizeof(int) * (size_t)nf, cudaMemcpyDeviceToHost, S->stream));
+        CS_CUDA(S, cudaStreamSynchronize(S->stream));
+        S->launches += 3;
+        x.n_fa = fuse.n_fa;
+        x.n_fb = fuse.n_fb;
+    }
+    lap("column-major slices + fused rows");
+    // ---- row-major copy: plan (host, needs the split), fill (device)
+    const HostSparse hr = make_sparse(rp2, no_idx, no_val, nt, nullptr, nullptr, fuse.rows() ? &split : nullptr, true);
+    if (hr.too_big) { S->err = "padded slice storage exceeds 2^31 entries"; return CS_EINVAL; }
+    if ((st = upload_plan(S, tmp, hr, &x.R, &d_sl, &d_csrc, &d_clen2, &d_idx, &d_val0, false)) != CS_OK) return st;
+    if ((st = dev_alloc(S, &d_pos, (size_t)nnz)) != CS_OK) return st; x.Rc.pos = d_pos;
+    csb::k_fill_slices<<<grid, 256, 0, S->stream>>>(d_sl, x.R.n_slice, x.R.n_chunk, d_csrc, d_clen2, d_rp2, ci2, va2, d_idx, d_val0, d_pos, 0, 0,
+                                                    nullptr, nullptr);
+    CS_CUDA(S, cudaMemcpyAsync(x.R.val, d_val0, sizeof(double) * hr.total, cudaMemcpyDeviceToDevice, S->stream));
+    S->launches += 1;
+    CS_CUDA(S, cudaGetLastError());
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));    // the scratch (DevTmp) is freed on return
+    lap("row-major slices");
+    return CS_OK;
 }
 
 cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
@@ -429,7 +689,6 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     return CS_OK;
 }
 
-int ew_blocks(int n) { return std::max(1, std::min((n + 255) / 256, 148 * 8)); }
 
 // caller's n-vector (host or device) -> internal order, into dst (device)
 cs_status import_cols(cs_solver *S, double *dst, const double *src, cs_mem where) {
@@ -502,192 +761,210 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     }
     if (off != n64) { S->err = "n_lin + sum(soc_size) != n"; return CS_EINVAL; }
     cone_off[K->n_soc] = n;
-    // ---- fetch and validate A
-    std::vector<int> rptr_v, cidx_v;
-    std::vector<double> val_v, hb, hc;
-    const int *rptr = A->row_ptr, *cidx = A->col_idx;      // host inputs are read in place (they are only read)
-    const double *val = A->val;
+    // ---- the layout: internal ordering, the two sliced copies, the fusion plan -- built on the device (cs_build.cuh) for
+    //      all but small problems, on the host otherwise (and on request: cs_diag_create, for the layout-identity test)
     cs_status st;
-    if (A->where != CS_HOST) {
-        if ((st = fetch(S, rptr_v, A->row_ptr, (size_t)m + 1, A->where)) != CS_OK) return st;
-        if ((st = fetch(S, cidx_v, A->col_idx, (size_t)nnz, A->where)) != CS_OK) return st;
-        if ((st = fetch(S, val_v, A->val, (size_t)nnz, A->where)) != CS_OK) return st;
-        rptr = rptr_v.data(); cidx = cidx_v.data(); val = val_v.data();
-    }
-    if ((st = fetch(S, hb, b, (size_t)m, vec_where)) != CS_OK) return st;
-    if ((st = fetch(S, hc, c, (size_t)n, vec_where)) != CS_OK) return st;
-    if (rptr[0] != 0 || rptr[m] != nnz) { S->err = "row_ptr[0] != 0 or row_ptr[m] != nnz"; return CS_EINVAL; }
-    for (int i = 0; i < m; ++i) {
-        if (rptr[i + 1] <= rptr[i]) { S->err = "row_ptr not increasing (empty rows are not allowed)"; return CS_EINVAL; }
-        if (rptr[i + 1] > nnz) { S->err = "row_ptr out of range"; return CS_EINVAL; }
-    }
-    {
-        std::atomic<int> bad{0};
-        const int blk = 16384;
-        parallel_blocks((m + blk - 1) / blk, host_threads(), [&](int bi) {
-            for (int i = bi * blk; i < std::min(m, (bi + 1) * blk); ++i) {
-                double ss = 0.0;
-                for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
-                    if (cidx[k] < 0 || cidx[k] >= n || (k > rptr[i] && cidx[k] <= cidx[k - 1])) bad.store(1);
-                    else if (!std::isfinite(val[k])) bad.store(2);
-                    ss += val[k] * val[k];
-                }
-                if (!(ss > 0.0) && !bad.load()) bad.store(3);       // a row of stored zeros: A is not of full row rank
-            }
-        });
-        if (bad.load() == 1) { S->err = "col_idx out of range, unsorted or duplicated within a row"; return CS_EINVAL; }
-        if (bad.load() == 2) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
-        if (bad.load() == 3) { S->err = "a row of A has zero norm (all stored entries are 0 or underflow when squared)"; return CS_EINVAL; }
-    }
+    std::vector<int> perm_r, perm_c;
+    std::vector<double> hb, hc;
     double nb = 0.0, nc = 0.0;
-    for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
-    for (int j = 0; j < n; ++j) { if (!std::isfinite(hc[j])) { S->err = "non-finite c"; return CS_EINVAL; } nc += hc[j] * hc[j]; }
-    lap("fetch + validate");
-    // ---- internal ordering: rows sorted by decreasing length, orthant columns likewise (Lorentz blocks
-    //      keep their place so that cones stay contiguous).  perm[internal] = caller's index.
-    std::vector<int> rlen((size_t)m), clen((size_t)n, 0);
-    for (int i = 0; i < m; ++i) rlen[i] = rptr[i + 1] - rptr[i];
-    {
-        const int blk = 1 << 20;
-        parallel_blocks((nnz + blk - 1) / blk, host_threads(), [&](int bi) {
-            for (int k = bi * blk; k < std::min(nnz, (bi + 1) * blk); ++k) __atomic_fetch_add(&clen[cidx[k]], 1, __ATOMIC_RELAXED);
-        });
-    }
-    const std::vector<int> perm_r = order_by_length(rlen, m);
-    for (int i = 0; i < m && rlen[perm_r[i]] > kShortMax; ++i) S->ctx.n_long = i + 1;
-    // (A lexicographic ordering of the columns by the heavy rows they touch was tried so that those rows'
-    //  gathers run over contiguous stretches; it cost 3.4 s at config 4 and changed nothing measurable.)
-    const std::vector<int> perm_c = order_by_length(clen, (int)K->n_lin);
-    std::vector<int> inv_c((size_t)n);
-    for (int j = 0; j < n; ++j) inv_c[perm_c[j]] = j;
-    lap("row/column ordering");
-    // row-major copy in internal numbering (entries of a row sorted by internal column)
-    std::vector<int> rp2((size_t)m + 1, 0);
-    uvec<int> ci2((size_t)nnz);
-    uvec<double> va2((size_t)nnz);
-    for (int i = 0; i < m; ++i) rp2[(size_t)i + 1] = rp2[i] + rlen[perm_r[i]];
-    {
-        auto fill_rows = [&](int i0, int i1) {
-            std::vector<std::pair<int, double>> tmp;
-            for (int i = i0; i < i1; ++i) {
-                const int src = perm_r[i], a0 = rptr[src], len = rlen[src], dst = rp2[i];
-                if (len <= kShortMax) {     // order inside a short row is irrelevant
-                    for (int k = 0; k < len; ++k) { ci2[dst + k] = inv_c[cidx[a0 + k]]; va2[dst + k] = val[a0 + k]; }
-                    continue;
-                }
-                if (len > n / 16) {         // nearly dense row: bucket by internal column instead of sorting (O(n))
-                    std::vector<double> dense((size_t)n, 0.0);
-                    std::vector<unsigned char> mark((size_t)n, 0);
-                    for (int k = 0; k < len; ++k) { const int j = inv_c[cidx[a0 + k]]; dense[j] = val[a0 + k]; mark[j] = 1; }
-                    int q = dst;
-                    for (int j = 0; j < n; ++j) if (mark[j]) { ci2[q] = j; va2[q] = dense[j]; ++q; }
-                    continue;
-                }
-                tmp.resize(len);            // long rows: ascending internal column, so their gathers stay as local as they were
-                for (int k = 0; k < len; ++k) tmp[k] = {inv_c[cidx[a0 + k]], val[a0 + k]};
-                std::sort(tmp.begin(), tmp.end(), [](const std::pair<int, double> &u, const std::pair<int, double> &v) { return u.first < v.first; });
-                for (int k = 0; k < len; ++k) { ci2[dst + k] = tmp[k].first; va2[dst + k] = tmp[k].second; }
-            }
-        };
-        // blocks of rows with at most ~256k entries (the heavy rows come first and get blocks of their own)
-        std::vector<int> cut{0};
-        for (int i = 0, acc = 0; i < m; ++i) {
-            acc += rlen[perm_r[i]];
-            if (acc >= (1 << 18) || i + 1 == m) { cut.push_back(i + 1); acc = 0; }
+    const bool device_build = S->build_mode == 2 || (S->build_mode == 0 && nnz >= kDeviceBuildMinNnz);
+    if (device_build) {
+        if ((st = layout_device(S, A, b, c, vec_where, K, m, n, nnz, perm_r, perm_c, hb, hc, nb, nc, lap)) != CS_OK) return st;
+    } else {
+        // ---- fetch and validate A
+        std::vector<int> rptr_v, cidx_v;
+        std::vector<double> val_v;
+        const int *rptr = A->row_ptr, *cidx = A->col_idx;      // host inputs are read in place (they are only read)
+        const double *val = A->val;
+        if (A->where != CS_HOST) {
+            if ((st = fetch(S, rptr_v, A->row_ptr, (size_t)m + 1, A->where)) != CS_OK) return st;
+            if ((st = fetch(S, cidx_v, A->col_idx, (size_t)nnz, A->where)) != CS_OK) return st;
+            if ((st = fetch(S, val_v, A->val, (size_t)nnz, A->where)) != CS_OK) return st;
+            rptr = rptr_v.data(); cidx = cidx_v.data(); val = val_v.data();
         }
-        parallel_blocks((int)cut.size() - 1, host_threads(), [&](int bi) { fill_rows(cut[bi], cut[bi + 1]); });
-    }
-    lap("row-major copy");
-    // column-major copy (counting sort by internal column; rows come out sorted within a column)
-    HostSparse hr, hc2;
-    std::vector<int> cp2((size_t)n + 1, 0);
-    uvec<int> ri2((size_t)nnz);
-    const int nt = host_threads();
-    {
-        uvec<double> cv2((size_t)nnz);
-        for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] = cp2[j] + clen[perm_c[j]];   // internal column j = caller's perm_c[j]
-        std::vector<int> fill(cp2.begin(), cp2.end() - 1);
-        // every helper scans all entries in row order but places only those of its own column range:
-        // sequential reads, writes confined to the range, order within a column = row order (deterministic)
-        const int parts = std::max(1, nt);
-        parallel_blocks(parts, parts, [&](int part) {
-            const int j0 = (int)((long long)n * part / parts), j1 = (int)((long long)n * (part + 1) / parts);
-            for (int i = 0; i < m; ++i)
-                for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
-                    const int j = ci2[k];
-                    if (j < j0 || j >= j1) continue;
-                    const int q = fill[j]++;
-                    ri2[q] = i;
-                    cv2[q] = va2[k];
-                }
-        });
-        lap("column-major copy");
-        // Heavy-row fusion plan: the longest rows (internal rows come sorted by decreasing length), if they are long
-        // enough to be worth it and the problem runs on more than one CTA.
-        FusePlan fuse;
-        if (nnz > kOneCtaNnz)
-            for (int i = 0; i < std::min(m, kFuseA + kFuseB) && rp2[(size_t)i + 1] - rp2[i] >= kFuseMinLen; ++i)
-                (i < kFuseA ? fuse.n_fa : fuse.n_fb) += 1;
-        uvec<unsigned char> fused;
-        if (fuse.rows()) {
-            fused.resize((size_t)nnz);
-            std::memset(fused.data(), 0, (size_t)nnz);
+        if ((st = fetch(S, hb, b, (size_t)m, vec_where)) != CS_OK) return st;
+        if ((st = fetch(S, hc, c, (size_t)n, vec_where)) != CS_OK) return st;
+        if (rptr[0] != 0 || rptr[m] != nnz) { S->err = "row_ptr[0] != 0 or row_ptr[m] != nnz"; return CS_EINVAL; }
+        for (int i = 0; i < m; ++i) {
+            if (rptr[i + 1] <= rptr[i]) { S->err = "row_ptr not increasing (empty rows are not allowed)"; return CS_EINVAL; }
+            if (rptr[i + 1] > nnz) { S->err = "row_ptr out of range"; return CS_EINVAL; }
         }
-        hc2 = make_sparse(cp2, ri2, cv2, nt, fuse.rows() ? &fuse : nullptr, fuse.rows() ? &fused : nullptr);
-        lap("column-major slices");
-        // fused rows: entries that stay with the row pass first, the fused ones after them (each part keeps its
-        // ascending column order); split[s] = size of the first part.  The rows are rebuilt from the column-major copy
-        // by two sequential scans over the columns (count, then place): the fused rows are the first entries of a
-        // column (rows ascend), so a column is left as soon as a row >= fuse.rows() shows up -- no searching.
-        std::vector<int> split((size_t)fuse.rows());
-        if (fuse.rows() && !hc2.too_big) {
-            const int nf = fuse.rows(), cblk = 1 << 16, nblk = (n + cblk - 1) / cblk;
-            std::vector<int> cnt((size_t)nblk * nf * 2, 0);      // [block][row][unfused, fused]
-            parallel_blocks(nblk, nt, [&](int bi) {
-                int *c = cnt.data() + (size_t)bi * nf * 2;
-                for (int j = bi * cblk; j < std::min(n, (bi + 1) * cblk); ++j)
-                    for (int e = cp2[j]; e < cp2[(size_t)j + 1] && ri2[e] < nf; ++e) c[2 * ri2[e] + fused[e]] += 1;
+        {
+            std::atomic<int> bad{0};
+            const int blk = 16384;
+            parallel_blocks((m + blk - 1) / blk, host_threads(), [&](int bi) {
+                for (int i = bi * blk; i < std::min(m, (bi + 1) * blk); ++i) {
+                    double ss = 0.0;
+                    for (int k = rptr[i]; k < rptr[i + 1]; ++k) {
+                        if (cidx[k] < 0 || cidx[k] >= n || (k > rptr[i] && cidx[k] <= cidx[k - 1])) bad.store(1);
+                        else if (!std::isfinite(val[k])) bad.store(2);
+                        ss += val[k] * val[k];
+                    }
+                    if (!(ss > 0.0) && !bad.load()) bad.store(3);       // a row of stored zeros: A is not of full row rank
+                }
             });
-            std::vector<int> off((size_t)nblk * nf * 2);
-            for (int r = 0; r < nf; ++r) {
-                int u = rp2[r];
-                for (int bi = 0; bi < nblk; ++bi) { off[((size_t)bi * nf + r) * 2] = u; u += cnt[((size_t)bi * nf + r) * 2]; }
-                split[r] = u - rp2[r];
-                for (int bi = 0; bi < nblk; ++bi) { off[((size_t)bi * nf + r) * 2 + 1] = u; u += cnt[((size_t)bi * nf + r) * 2 + 1]; }
+            if (bad.load() == 1) { S->err = "col_idx out of range, unsorted or duplicated within a row"; return CS_EINVAL; }
+            if (bad.load() == 2) { S->err = "non-finite matrix entry"; return CS_EINVAL; }
+            if (bad.load() == 3) { S->err = "a row of A has zero norm (all stored entries are 0 or underflow when squared)"; return CS_EINVAL; }
+        }
+        nb = 0.0; nc = 0.0;
+        for (int i = 0; i < m; ++i) { if (!std::isfinite(hb[i])) { S->err = "non-finite b"; return CS_EINVAL; } nb += hb[i] * hb[i]; }
+        for (int j = 0; j < n; ++j) { if (!std::isfinite(hc[j])) { S->err = "non-finite c"; return CS_EINVAL; } nc += hc[j] * hc[j]; }
+        lap("fetch + validate");
+        // ---- internal ordering: rows sorted by decreasing length, orthant columns likewise (Lorentz blocks
+        //      keep their place so that cones stay contiguous).  perm[internal] = caller's index.
+        std::vector<int> rlen((size_t)m), clen((size_t)n, 0);
+        for (int i = 0; i < m; ++i) rlen[i] = rptr[i + 1] - rptr[i];
+        {
+            const int blk = 1 << 20;
+            parallel_blocks((nnz + blk - 1) / blk, host_threads(), [&](int bi) {
+                for (int k = bi * blk; k < std::min(nnz, (bi + 1) * blk); ++k) __atomic_fetch_add(&clen[cidx[k]], 1, __ATOMIC_RELAXED);
+            });
+        }
+        perm_r = order_by_length(rlen, m);
+        for (int i = 0; i < m && rlen[perm_r[i]] > kShortMax; ++i) S->ctx.n_long = i + 1;
+        // (A lexicographic ordering of the columns by the heavy rows they touch was tried so that those rows'
+        //  gathers run over contiguous stretches; it cost 3.4 s at config 4 and changed nothing measurable.)
+        perm_c = order_by_length(clen, (int)K->n_lin);
+        std::vector<int> inv_c((size_t)n);
+        for (int j = 0; j < n; ++j) inv_c[perm_c[j]] = j;
+        lap("row/column ordering");
+        // row-major copy in internal numbering (entries of a row sorted by internal column)
+        std::vector<int> rp2((size_t)m + 1, 0);
+        uvec<int> ci2((size_t)nnz);
+        uvec<double> va2((size_t)nnz);
+        for (int i = 0; i < m; ++i) rp2[(size_t)i + 1] = rp2[i] + rlen[perm_r[i]];
+        {
+            auto fill_rows = [&](int i0, int i1) {
+                std::vector<std::pair<int, double>> tmp;
+                for (int i = i0; i < i1; ++i) {
+                    const int src = perm_r[i], a0 = rptr[src], len = rlen[src], dst = rp2[i];
+                    if (len <= kShortMax) {     // order inside a short row is irrelevant
+                        for (int k = 0; k < len; ++k) { ci2[dst + k] = inv_c[cidx[a0 + k]]; va2[dst + k] = val[a0 + k]; }
+                        continue;
+                    }
+                    if (len > n / 16) {         // nearly dense row: bucket by internal column instead of sorting (O(n))
+                        std::vector<double> dense((size_t)n, 0.0);
+                        std::vector<unsigned char> mark((size_t)n, 0);
+                        for (int k = 0; k < len; ++k) { const int j = inv_c[cidx[a0 + k]]; dense[j] = val[a0 + k]; mark[j] = 1; }
+                        int q = dst;
+                        for (int j = 0; j < n; ++j) if (mark[j]) { ci2[q] = j; va2[q] = dense[j]; ++q; }
+                        continue;
+                    }
+                    tmp.resize(len);            // long rows: ascending internal column, so their gathers stay as local as they were
+                    for (int k = 0; k < len; ++k) tmp[k] = {inv_c[cidx[a0 + k]], val[a0 + k]};
+                    std::sort(tmp.begin(), tmp.end(), [](const std::pair<int, double> &u, const std::pair<int, double> &v) { return u.first < v.first; });
+                    for (int k = 0; k < len; ++k) { ci2[dst + k] = tmp[k].first; va2[dst + k] = tmp[k].second; }
+                }
+            };
+            // blocks of rows with at most ~256k entries (the heavy rows come first and get blocks of their own)
+            std::vector<int> cut{0};
+            for (int i = 0, acc = 0; i < m; ++i) {
+                acc += rlen[perm_r[i]];
+                if (acc >= (1 << 18) || i + 1 == m) { cut.push_back(i + 1); acc = 0; }
             }
-            parallel_blocks(nblk, nt, [&](int bi) {
-                int *o = off.data() + (size_t)bi * nf * 2;
-                for (int j = bi * cblk; j < std::min(n, (bi + 1) * cblk); ++j)
-                    for (int e = cp2[j]; e < cp2[(size_t)j + 1] && ri2[e] < nf; ++e) {
-                        const int q = o[2 * ri2[e] + fused[e]]++;
-                        ci2[q] = j;
-                        va2[q] = cv2[e];
+            parallel_blocks((int)cut.size() - 1, host_threads(), [&](int bi) { fill_rows(cut[bi], cut[bi + 1]); });
+        }
+        lap("row-major copy");
+        // column-major copy (counting sort by internal column; rows come out sorted within a column)
+        HostSparse hr, hc2;
+        std::vector<int> cp2((size_t)n + 1, 0);
+        uvec<int> ri2((size_t)nnz);
+        const int nt = host_threads();
+        {
+            uvec<double> cv2((size_t)nnz);
+            for (int j = 0; j < n; ++j) cp2[(size_t)j + 1] = cp2[j] + clen[perm_c[j]];   // internal column j = caller's perm_c[j]
+            std::vector<int> fill(cp2.begin(), cp2.end() - 1);
+            // every helper scans all entries in row order but places only those of its own column range:
+            // sequential reads, writes confined to the range, order within a column = row order (deterministic)
+            const int parts = std::max(1, nt);
+            parallel_blocks(parts, parts, [&](int part) {
+                const int j0 = (int)((long long)n * part / parts), j1 = (int)((long long)n * (part + 1) / parts);
+                for (int i = 0; i < m; ++i)
+                    for (int k = rp2[i]; k < rp2[i + 1]; ++k) {
+                        const int j = ci2[k];
+                        if (j < j0 || j >= j1) continue;
+                        const int q = fill[j]++;
+                        ri2[q] = i;
+                        cv2[q] = va2[k];
                     }
             });
-            S->ctx.n_fa = fuse.n_fa;
-            S->ctx.n_fb = fuse.n_fb;
-            lap("fused rows: partition");
+            lap("column-major copy");
+            // Heavy-row fusion plan: the longest rows (internal rows come sorted by decreasing length), if they are long
+            // enough to be worth it and the problem runs on more than one CTA.
+            FusePlan fuse;
+            if (nnz > kOneCtaNnz)
+                for (int i = 0; i < std::min(m, kFuseA + kFuseB) && rp2[(size_t)i + 1] - rp2[i] >= kFuseMinLen; ++i)
+                    (i < kFuseA ? fuse.n_fa : fuse.n_fb) += 1;
+            uvec<unsigned char> fused;
+            if (fuse.rows()) {
+                fused.resize((size_t)nnz);
+                std::memset(fused.data(), 0, (size_t)nnz);
+            }
+            hc2 = make_sparse(cp2, ri2, cv2, nt, fuse.rows() ? &fuse : nullptr, fuse.rows() ? &fused : nullptr);
+            lap("column-major slices");
+            // fused rows: entries that stay with the row pass first, the fused ones after them (each part keeps its
+            // ascending column order); split[s] = size of the first part.  The rows are rebuilt from the column-major copy
+            // by two sequential scans over the columns (count, then place): the fused rows are the first entries of a
+            // column (rows ascend), so a column is left as soon as a row >= fuse.rows() shows up -- no searching.
+            std::vector<int> split((size_t)fuse.rows());
+            if (fuse.rows() && !hc2.too_big) {
+                const int nf = fuse.rows(), cblk = 1 << 16, nblk = (n + cblk - 1) / cblk;
+                std::vector<int> cnt((size_t)nblk * nf * 2, 0);      // [block][row][unfused, fused]
+                parallel_blocks(nblk, nt, [&](int bi) {
+                    int *c = cnt.data() + (size_t)bi * nf * 2;
+                    for (int j = bi * cblk; j < std::min(n, (bi + 1) * cblk); ++j)
+                        for (int e = cp2[j]; e < cp2[(size_t)j + 1] && ri2[e] < nf; ++e) c[2 * ri2[e] + fused[e]] += 1;
+                });
+                std::vector<int> off((size_t)nblk * nf * 2);
+                for (int r = 0; r < nf; ++r) {
+                    int u = rp2[r];
+                    for (int bi = 0; bi < nblk; ++bi) { off[((size_t)bi * nf + r) * 2] = u; u += cnt[((size_t)bi * nf + r) * 2]; }
+                    split[r] = u - rp2[r];
+                    for (int bi = 0; bi < nblk; ++bi) { off[((size_t)bi * nf + r) * 2 + 1] = u; u += cnt[((size_t)bi * nf + r) * 2 + 1]; }
+                }
+                parallel_blocks(nblk, nt, [&](int bi) {
+                    int *o = off.data() + (size_t)bi * nf * 2;
+                    for (int j = bi * cblk; j < std::min(n, (bi + 1) * cblk); ++j)
+                        for (int e = cp2[j]; e < cp2[(size_t)j + 1] && ri2[e] < nf; ++e) {
+                            const int q = o[2 * ri2[e] + fused[e]]++;
+                            ci2[q] = j;
+                            va2[q] = cv2[e];
+                        }
+                });
+                S->ctx.n_fa = fuse.n_fa;
+                S->ctx.n_fb = fuse.n_fb;
+                lap("fused rows: partition");
+            }
+            hr = make_sparse(rp2, ci2, va2, nt, nullptr, nullptr, fuse.rows() ? &split : nullptr);
         }
-        hr = make_sparse(rp2, ci2, va2, nt, nullptr, nullptr, fuse.rows() ? &split : nullptr);
-    }
-    lap("row-major slices");
-    if (hr.too_big || hc2.too_big) {
-        S->err = "padded slice storage exceeds 2^31 entries";
-        return CS_EINVAL;
-    }
-    {
-        int *q;
-        if ((st = upload_sparse(S, hr, &S->ctx.R)) != CS_OK) return st;
-        if ((st = dev_upload(S, &q, rp2.data(), rp2.size())) != CS_OK) return st; S->ctx.Rc.ptr = q;
-        if ((st = dev_upload(S, &q, ci2.data(), ci2.size())) != CS_OK) return st; S->ctx.Rc.idx = q;
-        if ((st = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) != CS_OK) return st; S->ctx.Rc.pos = q;
-    }
-    {   // b, c in internal order
-        std::vector<double> t((size_t)std::max(m, n));
-        for (int i = 0; i < m; ++i) t[i] = hb[perm_r[i]];
-        std::copy(t.begin(), t.begin() + m, hb.begin());
-        for (int j = 0; j < n; ++j) t[j] = hc[perm_c[j]];
-        std::copy(t.begin(), t.begin() + n, hc.begin());
+        lap("row-major slices");
+        if (hr.too_big || hc2.too_big) {
+            S->err = "padded slice storage exceeds 2^31 entries";
+            return CS_EINVAL;
+        }
+        {
+            int *q;
+            if ((st = upload_sparse(S, hr, &S->ctx.R)) != CS_OK) return st;
+            if ((st = dev_upload(S, &q, rp2.data(), rp2.size())) != CS_OK) return st; S->ctx.Rc.ptr = q;
+            if ((st = dev_upload(S, &q, ci2.data(), ci2.size())) != CS_OK) return st; S->ctx.Rc.idx = q;
+            if ((st = dev_upload(S, &q, hr.pos.data(), hr.pos.size())) != CS_OK) return st; S->ctx.Rc.pos = q;
+        }
+        {   // b, c in internal order
+            std::vector<double> t((size_t)std::max(m, n));
+            for (int i = 0; i < m; ++i) t[i] = hb[perm_r[i]];
+            std::copy(t.begin(), t.begin() + m, hb.begin());
+            for (int j = 0; j < n; ++j) t[j] = hc[perm_c[j]];
+            std::copy(t.begin(), t.begin() + n, hc.begin());
+        }
+        {   // the column-major copy and the plain compressed views of the same entries (the FSAI build and the dense path walk them)
+            int *q;
+            if ((st = upload_sparse(S, hc2, &S->ctx.C)) != CS_OK) return st;
+            if ((st = dev_upload(S, &q, cp2.data(), cp2.size())) != CS_OK) return st; S->ctx.Cc.ptr = q;
+            if ((st = dev_upload(S, &q, ri2.data(), ri2.size())) != CS_OK) return st; S->ctx.Cc.idx = q;
+            if ((st = dev_upload(S, &q, hc2.pos.data(), hc2.pos.size())) != CS_OK) return st; S->ctx.Cc.pos = q;
+            CS_CUDA(S, cudaStreamSynchronize(S->stream));   // the host images die at the end of this block
+        }
     }
     // ---- device state
     Ctx &x = S->ctx;
@@ -704,16 +981,13 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         if ((st = dev_upload(S, &ip, cls[0].data(), cls[0].size())) != CS_OK) return st; x.cone_cls = ip;
         CS_CUDA(S, cudaStreamSynchronize(S->stream));   // the staging vectors die here
     }
-    if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
-    if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
-    if ((st = upload_sparse(S, hc2, &x.C)) != CS_OK) return st;      // x.R and x.Rc went up above
+    if (!x.perm_r) {   // (the device build has made them on the device)
+        if ((st = dev_upload(S, &ip, perm_r.data(), perm_r.size())) != CS_OK) return st; x.perm_r = ip;
+        if ((st = dev_upload(S, &ip, perm_c.data(), perm_c.size())) != CS_OK) return st; x.perm_c = ip;
+    }
     if ((st = dev_zeros(S, &x.fpart, (size_t)(x.n_fa + x.n_fb) * kMaxGrid)) != CS_OK) return st;
     x.R.fpart = x.fpart;
-    {   // plain compressed views of the same entries (the FSAI build and the dense factor path walk them)
-        int *q;
-        if ((st = dev_upload(S, &q, cp2.data(), cp2.size())) != CS_OK) return st; x.Cc.ptr = q;
-        if ((st = dev_upload(S, &q, ri2.data(), ri2.size())) != CS_OK) return st; x.Cc.idx = q;
-        if ((st = dev_upload(S, &q, hc2.pos.data(), hc2.pos.size())) != CS_OK) return st; x.Cc.pos = q;
+    {   // scratch of the FSAI builds
         if ((st = dev_zeros(S, &x.f_ctop, (size_t)3 * n)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.fp_ctop, (size_t)kFsTop * n)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.fp_idx, (size_t)kFsP * m)) != CS_OK) return st;
@@ -732,21 +1006,25 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     }
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
     lap("upload");
-    if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
-    if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
+    if (!x.b) {   // (the device build has already permuted b, c on the device)
+        if ((st = dev_upload(S, &dp, hb.data(), hb.size())) != CS_OK) return st; x.b = dp;
+        if ((st = dev_upload(S, &dp, hc.data(), hc.size())) != CS_OK) return st; x.c = dp;
+    }
     double **nv[] = {&x.s, &x.p, &x.g, &x.e, &x.u, &x.chat};
     for (double **q : nv) if ((st = dev_zeros(S, q, (size_t)n)) != CS_OK) return st;
     double **mv[] = {&x.w, &x.r, &x.v, &x.btil};
     for (double **q : mv) if ((st = dev_zeros(S, q, (size_t)m)) != CS_OK) return st;
     {   // O = 1, D = 1, x = z = e_K
-        std::vector<double> ones((size_t)std::max(m, n), 1.0), ek((size_t)n, 0.0);
-        for (int j = 0; j < x.n_lin; ++j) ek[j] = 1.0;
-        for (int i = 0; i < x.n_soc; ++i) ek[cone_off[i]] = 1.0;
-        if ((st = dev_upload(S, &x.O, ones.data(), (size_t)n)) != CS_OK) return st;
-        if ((st = dev_upload(S, &x.D, ones.data(), (size_t)m)) != CS_OK) return st;
-        if ((st = dev_upload(S, &x.xb, ek.data(), (size_t)n)) != CS_OK) return st;
-        if ((st = dev_upload(S, &x.zb, ek.data(), (size_t)n)) != CS_OK) return st;
-        CS_CUDA(S, cudaStreamSynchronize(S->stream));  // host staging buffers die at scope end
+        if ((st = dev_alloc(S, &x.O, (size_t)n)) != CS_OK) return st;
+        if ((st = dev_alloc(S, &x.D, (size_t)m)) != CS_OK) return st;
+        if ((st = dev_alloc(S, &x.xb, (size_t)n)) != CS_OK) return st;
+        if ((st = dev_alloc(S, &x.zb, (size_t)n)) != CS_OK) return st;
+        csb::k_fill<<<ew_blocks(n), 256, 0, S->stream>>>(x.O, n, 1.0);
+        csb::k_fill<<<ew_blocks(m), 256, 0, S->stream>>>(x.D, m, 1.0);
+        csb::k_unit_cone_point<<<ew_blocks(n), 256, 0, S->stream>>>(x.xb, x.zb, n, x.n_lin, x.cone_off, x.n_soc);
+        if (x.n_soc) csb::k_unit_cone_heads<<<ew_blocks(x.n_soc), 256, 0, S->stream>>>(x.xb, x.zb, x.cone_off, x.n_soc);
+        CS_CUDA(S, cudaGetLastError());
+        S->launches += 4;
     }
     if ((st = dev_zeros(S, &x.sc, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partial_probe, 1)) != CS_OK) return st;
@@ -808,14 +1086,15 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     return CS_OK;
 }
 
-cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
-                    const cs_cones *K, void *cuda_stream) {
+static cs_status create_common(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
+                               const cs_cones *K, void *cuda_stream, int build_mode) {
     if (!out) return CS_EINVAL;
     *out = nullptr;
     if (!A || !b || !c || !K || !A->row_ptr || !A->col_idx || !A->val) { g_create_err = "NULL argument"; return CS_EINVAL; }
     cs_solver *S = new (std::nothrow) cs_solver;
     if (!S) return CS_ENOMEM;
     S->stream = static_cast<cudaStream_t>(cuda_stream);
+    S->build_mode = build_mode;
     cs_status st = CS_OK;
     if (cudaGetDevice(&S->device) != cudaSuccess) { S->err = "no CUDA device"; st = CS_ECUDA; }
     if (st == CS_OK) {
@@ -824,6 +1103,59 @@ cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const dou
     }
     if (st != CS_OK) { g_create_err = S->err; cs_destroy(S); return st; }
     *out = S;
+    return CS_OK;
+}
+
+cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
+                    const cs_cones *K, void *cuda_stream) {
+    return create_common(out, A, b, c, vec_where, K, cuda_stream, 0);
+}
+
+cs_status cs_diag_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
+                         const cs_cones *K, void *cuda_stream, int32_t build_mode) {
+    if (build_mode < 0 || build_mode > 2) return CS_EINVAL;
+    return create_common(out, A, b, c, vec_where, K, cuda_stream, build_mode);
+}
+
+cs_status cs_diag_layout_digest(cs_solver *S, uint64_t out[32]) {
+    if (!S || !out) return CS_EINVAL;
+    DeviceGuard guard(S);
+    const Ctx &c = S->ctx;
+    std::vector<unsigned char> h;
+    int k = 0;
+    auto digest = [&](const void *dev, size_t bytes) -> cs_status {       // FNV-1a over a device array
+        h.resize(bytes);
+        if (bytes) CS_CUDA(S, cudaMemcpy(h.data(), dev, bytes, cudaMemcpyDeviceToHost));
+        uint64_t f = 1469598103934665603ull;
+        for (size_t i = 0; i < bytes; ++i) { f ^= h[i]; f *= 1099511628211ull; }
+        out[k++] = f;
+        return CS_OK;
+    };
+    CS_CUDA(S, cudaStreamSynchronize(S->stream));
+    cs_status st;
+    const Sparse *sp[2] = {&c.R, &c.C};
+    const Csr *cv[2] = {&c.Rc, &c.Cc};
+    const size_t tot[2] = {S->tot_r, S->tot_c};
+    const int nseg[2] = {c.m, c.n};
+    for (int q = 0; q < 2; ++q) {
+        if ((st = digest(sp[q]->slices, sizeof(int4) * (size_t)sp[q]->n_slice)) != CS_OK) return st;
+        if ((st = digest(sp[q]->idx, sizeof(int) * tot[q])) != CS_OK) return st;
+        if ((st = digest(sp[q]->val0, sizeof(double) * tot[q])) != CS_OK) return st;
+        if ((st = digest(sp[q]->chunk_slot, sizeof(int) * (size_t)sp[q]->n_chunk)) != CS_OK) return st;
+        if ((st = digest(sp[q]->multi, sizeof(int4) * (size_t)sp[q]->n_multi)) != CS_OK) return st;
+        if ((st = digest(sp[q]->multi_k2, sizeof(int4) * (size_t)sp[q]->n_multi_k2)) != CS_OK) return st;
+        if ((st = digest(cv[q]->ptr, sizeof(int) * ((size_t)nseg[q] + 1))) != CS_OK) return st;
+        if ((st = digest(cv[q]->idx, sizeof(int) * (size_t)S->nnz)) != CS_OK) return st;
+        if ((st = digest(cv[q]->pos, sizeof(int) * (size_t)S->nnz)) != CS_OK) return st;
+    }
+    if ((st = digest(c.C.fmask, c.n_fa + c.n_fb ? (size_t)(c.C.n_slice - c.C.n_chunk) * 32 : 0)) != CS_OK) return st;
+    if ((st = digest(c.perm_r, sizeof(int) * (size_t)c.m)) != CS_OK) return st;
+    if ((st = digest(c.perm_c, sizeof(int) * (size_t)c.n)) != CS_OK) return st;
+    if ((st = digest(c.b, sizeof(double) * (size_t)c.m)) != CS_OK) return st;
+    if ((st = digest(c.c, sizeof(double) * (size_t)c.n)) != CS_OK) return st;
+    out[k++] = ((uint64_t)(unsigned)c.R.n_chunk_k2 << 32) | (unsigned)c.R.n_chunk;
+    out[k++] = ((uint64_t)(unsigned)c.n_fa << 40) | ((uint64_t)(unsigned)c.n_fb << 20) | (unsigned)c.n_long;
+    while (k < 32) out[k++] = 0;
     return CS_OK;
 }
 

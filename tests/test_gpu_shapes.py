@@ -90,3 +90,48 @@ def test_shape_sweep_against_the_oracle(name):
     for k in ("pres_abs", "dres_abs", "gap_abs", "kkt_rel"):
         assert abs(r[k] - q[k]) <= 1e-6 * abs(q[k]) + 1e-10 * (1 + np.linalg.norm(p.b)), (name, k, r[k], q[k])
     S.destroy()
+
+
+LAYOUT_CASES = dict(SHAPES)
+LAYOUT_CASES.update({"cfg4_x0.02_fused_rows": lambda: W.config(4, 0.02), "cfg3_x0.1": lambda: W.config(3, 0.1), "cfg0": lambda: W.config(0),
+                     "dense_sec5d_n400": lambda: W.dense_socp_sec5d(3, n=400, h=4)})
+
+
+@pytest.mark.parametrize("name", list(LAYOUT_CASES))
+def test_device_build_lays_the_matrix_out_exactly_as_the_host_build(name):
+    """cs_create builds its layout on the device (csrc/cs_build.cuh: validation, two radix sorts, slice fill, fusion marks,
+    fused rows' partition; automatic from 100,000 non-zeros on) or on the host.  Both, from host and from device inputs,
+    must give the same bits in every layout array (slices, indices, pristine values, chunk tables, compressed views,
+    fusion marks, permutations, b, c: cs_diag_layout_digest), and the same iterates bit for bit."""
+    from paper_2103_00736_b200 import binding
+    p = LAYOUT_CASES[name]()
+    ref, sols = None, []
+    for mode in (1, 2):
+        for dev in (None, "cuda:0"):
+            S = binding.Solver.from_problem(p, device=dev, build_mode=mode)
+            d = S.layout_digest()
+            ref = ref or d
+            assert d == ref, (name, mode, dev, [i for i in range(32) if d[i] != ref[i]])
+            if dev is None:
+                S.run(5, L=[3])
+                sols.append(S.solution())
+            S.destroy()
+    for k in sols[0]:
+        assert np.array_equal(sols[0][k], sols[1][k]), (name, k)
+
+
+def test_device_build_rejects_what_the_host_build_rejects():
+    from paper_2103_00736_b200 import binding
+    p = W.config(1, 0.05)
+    bad_cols = p.col_idx.copy()
+    bad_cols[[0, 1]] = bad_cols[[1, 0]]
+    zero_row = p.val.copy()
+    zero_row[p.row_ptr[7]:p.row_ptr[8]] = 0.0
+    for kw in (dict(col_idx=bad_cols), dict(val=np.where(np.arange(p.nnz) == 3, np.nan, p.val)), dict(val=zero_row),
+               dict(b=np.where(np.arange(p.m) == 2, np.inf, p.b))):
+        for mode in (1, 2):
+            a = dict(m=p.m, n=p.n, row_ptr=p.row_ptr, col_idx=p.col_idx, val=p.val, b=p.b, c=p.c, n_lin=p.n_lin, soc_size=p.soc_size)
+            a.update(kw)
+            with pytest.raises(binding.CsError) as ei:
+                binding.Solver(build_mode=mode, **a)
+            assert ei.value.status == binding.CS_EINVAL, (mode, list(kw))
