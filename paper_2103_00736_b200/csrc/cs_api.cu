@@ -201,21 +201,23 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
     // every traversal walks (the K2 view), pass 1 the fused tails of the fused rows; slots are numbered per segment,
     // K2 part first, so that a chunk has the same slot in both views.
     const int n_split = split ? (int)split->size() : 0;
-    std::vector<int> first_slot((size_t)nseg, -1);
+    std::vector<int> long_seg, first_slot;                 // the long segments (few) and the first slot of each (-1: none)
     for (int s = 0; s < nseg; ++s) {
         const int len = ptr[s + 1] - ptr[s];
         if (len <= kShortMax) continue;
         const int nu = s < n_split ? (*split)[s] : len, nf = len - nu;
         const int nch_u = (nu + kChunk - 1) / kChunk, nch_f = (nf + kChunk - 1) / kChunk;
-        if (nch_u + nch_f > 1 || nf > 0) { first_slot[s] = h.n_slots; h.n_slots += nch_u + nch_f; }
-        if (nch_u + nch_f > 1) h.multi.push_back(make_int4(s, first_slot[s], nch_u + nch_f, 0));
-        if (nf > 0) h.multi_k2.push_back(make_int4(s, first_slot[s], nch_u, s + 1));
-        else if (nch_u > 1) h.multi_k2.push_back(make_int4(s, first_slot[s], nch_u, 0));
+        int fs = -1;
+        if (nch_u + nch_f > 1 || nf > 0) { fs = h.n_slots; h.n_slots += nch_u + nch_f; }
+        long_seg.push_back(s);
+        first_slot.push_back(fs);
+        if (nch_u + nch_f > 1) h.multi.push_back(make_int4(s, fs, nch_u + nch_f, 0));
+        if (nf > 0) h.multi_k2.push_back(make_int4(s, fs, nch_u, s + 1));
+        else if (nch_u > 1) h.multi_k2.push_back(make_int4(s, fs, nch_u, 0));
     }
     for (int pass = 0; pass < 2; ++pass) {
-        for (int s = 0; s < nseg; ++s) {
-            const int len = ptr[s + 1] - ptr[s];
-            if (len <= kShortMax) continue;
+        for (size_t li = 0; li < long_seg.size(); ++li) {
+            const int s = long_seg[li], len = ptr[s + 1] - ptr[s];
             const int nu = s < n_split ? (*split)[s] : len, nf = len - nu;
             const int nch_u = (nu + kChunk - 1) / kChunk;
             const int beg = pass ? ptr[s] + nu : ptr[s], cnt = pass ? nf : nu, nch = (cnt + kChunk - 1) / kChunk;
@@ -225,7 +227,7 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
                 plan_slice(s, 1 | (5 << 8), (clen + 31) / 32);
                 chunk_src.push_back(a);
                 chunk_len.push_back(clen);
-                int slot = direct ? -1 : first_slot[s] + (pass ? nch_u : 0) + q;
+                int slot = direct ? -1 : first_slot[li] + (pass ? nch_u : 0) + q;
                 if (pass && nu == 0 && nch == 1) slot = -1;  // all entries fused, one chunk: the full view completes it directly
                 h.chunk_slot.push_back(slot);
             }
@@ -247,9 +249,9 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
             s0 += cnt;
         }
     };
+    h.slices.reserve(h.slices.size() + (size_t)nseg / 32 + long_seg.size() + 2);
     int run = 0;
-    for (int s = 0; s < nseg; ++s) {
-        if (ptr[s + 1] - ptr[s] <= kShortMax) continue;
+    for (int s : long_seg) {                                // the short segments between two long ones form a run
         plan_run(run, s);
         run = s + 1;
     }
@@ -444,15 +446,24 @@ cs_status layout_device(cs_solver *S, const cs_csr *A, const double *b, const do
         hb_p = hb.data(); hc_p = hc.data();
     }
     if (rptr[0] != 0 || rptr[m] != nnz) { S->err = "row_ptr[0] != 0 or row_ptr[m] != nnz"; return CS_EINVAL; }
+    std::vector<int> long_rows;                                       // validated by one CTA each
     for (int i = 0; i < m; ++i) {
         if (rptr[i + 1] <= rptr[i]) { S->err = "row_ptr not increasing (empty rows are not allowed)"; return CS_EINVAL; }
         if (rptr[i + 1] > nnz) { S->err = "row_ptr out of range"; return CS_EINVAL; }
+        if (rptr[i + 1] - rptr[i] > csb::kValidateLong) long_rows.push_back(i);
     }
     // ---- validation + column counts (device)
     int *d_clen, *d_status;
     if ((st = tmp.alloc(S, &d_clen, (size_t)n, true)) != CS_OK) return st;
     if ((st = tmp.alloc(S, &d_status, 1, true)) != CS_OK) return st;
     csb::k_validate<<<grid, 256, 0, S->stream>>>(d_rptr, d_cidx, d_val, m, n, d_clen, d_status);
+    if (!long_rows.empty()) {
+        int *d_long;
+        if ((st = tmp.alloc(S, &d_long, long_rows.size())) != CS_OK) return st;
+        CS_CUDA(S, cudaMemcpyAsync(d_long, long_rows.data(), sizeof(int) * long_rows.size(), cudaMemcpyHostToDevice, S->stream));
+        csb::k_validate_long<<<std::min((int)long_rows.size(), grid), 256, 0, S->stream>>>(d_rptr, d_cidx, d_val, d_long, (int)long_rows.size(), n,
+                                                                                       d_clen, d_status);
+    }
     int status = 0;
     CS_CUDA(S, cudaMemcpyAsync(&status, d_status, sizeof(int), cudaMemcpyDeviceToHost, S->stream));
     nb = 0.0; nc = 0.0;                                                // meanwhile on the host: b, c
@@ -549,11 +560,13 @@ cs_status layout_device(cs_solver *S, const cs_csr *A, const double *b, const do
         for (int i = 0; i < std::min(m, kFuseA + kFuseB) && rp2[(size_t)i + 1] - rp2[i] >= kFuseMinLen; ++i)
             (i < kFuseA ? fuse.n_fa : fuse.n_fb) += 1;
     const HostSparse hc2 = make_sparse(cp2, no_idx, no_val, nt, nullptr, nullptr, nullptr, true);
+    lap("  column-major plan (host)");
     if (hc2.too_big) { S->err = "padded slice storage exceeds 2^31 entries"; return CS_EINVAL; }
     int4 *d_sl; int *d_csrc, *d_clen2, *d_idx, *d_pos;
     double *d_val0;
     if ((st = upload_plan(S, tmp, hc2, &x.C, &d_sl, &d_csrc, &d_clen2, &d_idx, &d_val0, fuse.rows() > 0)) != CS_OK) return st;
     if ((st = dev_alloc(S, &d_pos, (size_t)nnz)) != CS_OK) return st; x.Cc.pos = d_pos;
+    lap("  column-major allocations + plan upload");
     unsigned char *fused_c;
     if ((st = tmp.alloc(S, &fused_c, (size_t)nnz, fuse.rows() > 0)) != CS_OK) return st;
     csb::k_fill_slices<<<grid, 256, 0, S->stream>>>(d_sl, x.C.n_slice, x.C.n_chunk, d_csrc, d_clen2, d_cp2, ri2, cv2, d_idx, d_val0, d_pos,

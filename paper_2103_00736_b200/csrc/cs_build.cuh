@@ -20,7 +20,20 @@ using csd::kShortMax;
 // status bits of the validation
 enum { kBadIndex = 1, kBadValue = 2, kZeroRow = 4, kEmptyRow = 8 };
 
-// One warp per row of the caller's CSR: indices in range, strictly ascending, values finite, row norm > 0; column counts.
+// One warp per row of the caller's CSR (one CTA per row for the rows of the list `long_rows`, which the warp kernel skips):
+// indices in range, strictly ascending, values finite, row norm > 0; column counts.
+constexpr int kValidateLong = 8192;
+__device__ __forceinline__ void validate_entries(const int *cidx, const double *val, int a, int b, int first, int stride, int n, int *clen,
+                                                 int &bad, double &ss) {
+    for (int e = a + first; e < b; e += stride) {
+        const int j = cidx[e];
+        const double v = val[e];
+        if (j < 0 || j >= n || (e > a && j <= cidx[e - 1])) bad |= kBadIndex;
+        else atomicAdd(clen + j, 1);
+        if (!isfinite(v)) bad |= kBadValue;
+        ss += v * v;
+    }
+}
 __global__ void __launch_bounds__(256) k_validate(const int *rptr, const int *cidx, const double *val, int m, int n, int *clen, int *status) {
     const int lane = threadIdx.x & 31;
     const int gwarp = (blockIdx.x * 256 + threadIdx.x) >> 5, nwarps = (gridDim.x * 256) >> 5;
@@ -28,19 +41,33 @@ __global__ void __launch_bounds__(256) k_validate(const int *rptr, const int *ci
     for (int i = gwarp; i < m; i += nwarps) {
         const int a = rptr[i], b = rptr[i + 1];
         if (b <= a) { bad |= kEmptyRow; continue; }
+        if (b - a > kValidateLong) continue;                         // k_validate_long
         double ss = 0.0;
-        for (int e = a + lane; e < b; e += 32) {
-            const int j = cidx[e];
-            const double v = val[e];
-            if (j < 0 || j >= n || (e > a && j <= cidx[e - 1])) bad |= kBadIndex;
-            else atomicAdd(clen + j, 1);
-            if (!isfinite(v)) bad |= kBadValue;
-            ss += v * v;
-        }
+        validate_entries(cidx, val, a, b, lane, 32, n, clen, bad, ss);
         ss = csd::group_reduce<32>(ss);
         if (!(ss > 0.0)) bad |= kZeroRow;
     }
     if (bad) atomicOr(status, bad);
+}
+__global__ void __launch_bounds__(256) k_validate_long(const int *rptr, const int *cidx, const double *val, const int *long_rows, int n_long,
+                                                       int n, int *clen, int *status) {
+    __shared__ double red[8];
+    for (int q = blockIdx.x; q < n_long; q += gridDim.x) {
+        const int i = long_rows[q], a = rptr[i], b = rptr[i + 1];
+        int bad = 0;
+        double ss = 0.0;
+        validate_entries(cidx, val, a, b, (int)threadIdx.x, 256, n, clen, bad, ss);
+        ss = csd::group_reduce<32>(ss);
+        __syncthreads();
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int w = 0; w < 8; ++w) t += red[w];
+            if (!(t > 0.0)) bad |= kZeroRow;
+        }
+        if (bad) atomicOr(status, bad);
+    }
 }
 
 // length ordering: segments sorted by DECREASING length, stable (ties keep their index order) = an ascending stable radix sort of
