@@ -688,6 +688,17 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     const double mat_bytes = 24.0 * (double)S->nnz;
     const int auto_fsai = mat_bytes >= kAutoFsaiPMinBytes && mat_bytes <= kAutoFsaiPBytes ? 2 : 1;
     S->ctx.fsai = S->ctx.dense ? 0 : S->prm.precond == 3 ? 2 : S->prm.precond == 2 ? 1 : (S->prm.precond == 0 && S->prm.t >= 4.0) ? auto_fsai : 0;
+    if (S->ctx.fsai == 2 && !S->ctx.fp_ctop) {   // the tables of FSAI(5) (~76 bytes per row + 24 per column) are allocated on first use
+        Ctx &x = S->ctx;
+        const size_t m = (size_t)x.m, n = (size_t)x.n;
+        if ((st = dev_zeros(S, &x.fp_idx, kFsP * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_tptr, m + 1)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_tcnt, m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_trow, kFsP * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_val, (kFsP + 1) * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_tval, kFsP * m)) != CS_OK) return st;
+        if ((st = dev_zeros(S, &x.fp_ctop, kFsTop * n)) != CS_OK) return st;
+    }
     S->ctx.mu = S->prm.mu;  // mu, t, o_floor, precond take effect here (cs.h)
     S->ctx.t = S->prm.t;
     S->ctx.o_floor = S->prm.o_floor;
@@ -1002,13 +1013,6 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     x.R.fpart = x.fpart;
     {   // scratch of the FSAI builds
         if ((st = dev_zeros(S, &x.f_ctop, (size_t)3 * n)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_ctop, (size_t)kFsTop * n)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_idx, (size_t)kFsP * m)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_tptr, (size_t)m + 1)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_tcnt, (size_t)m)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_trow, (size_t)kFsP * m)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_val, (size_t)(kFsP + 1) * m)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.fp_tval, (size_t)kFsP * m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_partner, (size_t)m)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_tptr, (size_t)m + 1)) != CS_OK) return st;
         if ((st = dev_zeros(S, &x.f_tcur, (size_t)m)) != CS_OK) return st;

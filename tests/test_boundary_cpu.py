@@ -145,8 +145,8 @@ def test_bench_byte_accounting():
     assert total == 10 * per_cg + 2 * (24 * p.nnz + 92 * p.n + 24 * p.m)
     sv_total, sv_cg = bench.survey_bytes(p, k_iter=2, cg_steps=10)          # SURVEY.md 8(d) as written
     assert sv_cg == 24 * p.nnz + 20 * p.n + 100 * p.m and sv_total == (10 + 2) * sv_cg + 2 * 40 * p.n
-    for cfg in (3, 4):                                                      # the committed ncu exports bench.py reads
+    for cfg in (1, 3, 4):                                                   # the committed ncu exports bench.py reads
         cap = bench.ncu_capture(cfg)
-        assert cap and cap["cg_steps_in_launch"] > 0 and cap["dram__bytes_read.sum"] > 1e8 and cap["lts__t_bytes.sum"] > 1e8
+        assert cap and cap["cg_steps_in_launch"] > 0 and cap["dram__bytes_read.sum"] > 1e6 and cap["lts__t_bytes.sum"] > 1e8
         assert cap["launch__registers_per_thread"] <= 80
     assert bench.max_over_ranks(3.5) == 3.5                  # no process group: identity

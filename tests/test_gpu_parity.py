@@ -275,6 +275,28 @@ def test_fixed_scaling_and_set_point():
     assert ei.value.status == binding.CS_ESTATE
 
 
+def test_checkpoint_and_resume_through_solution_and_set_point():
+    """S 5 (checkpoint / resume): the state of Algorithm 2 is (x, z, O) -- s is recast from them by step 14 and
+    the multiplier w is only a warm start.  cs_solution -> new handle -> cs_set_point + cs_set_scaling continues the run:
+    after 10 more passes the resumed handle and the original agree to the parity tolerance."""
+    from paper_2103_00736_b200 import binding
+    p = W.sparse_socp(41, 600, 1500, 40, 6, n_lin=400, lo=2, hi=50)
+    S1 = binding.Solver.from_problem(p, device="cuda:0")
+    S1.run(30, L=[20])
+    ck = S1.solution()
+    S2 = binding.Solver.from_problem(p, device="cuda:0")
+    S2.set_point(ck["x"], ck["z"])
+    S2.set_scaling(ck["O"])
+    assert rel(S2.solution()["s"], ck["s"]) <= 1e-13
+    S1.iterate(10)
+    S2.iterate(10)
+    a, b = S1.solution(), S2.solution()
+    for k in ("x", "z", "y", "s", "O"):
+        assert rel(b[k], a[k]) <= TOL_ITER, (k, rel(b[k], a[k]))
+    r1, r2 = S1.residuals(), S2.residuals()
+    assert abs(r1["kkt_rel"] - r2["kkt_rel"]) <= TOL_RES * r1["kkt_rel"] and abs(r1["pobj"] - r2["pobj"]) <= TOL_RES * (1 + abs(r1["pobj"]))
+
+
 def test_host_and_device_inputs_agree_bitwise():
     from paper_2103_00736_b200 import binding
     p = W.config(1, 0.05)
