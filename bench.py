@@ -372,12 +372,13 @@ def main():
     return finish(a, p, S, line, rank, world, dev, stream)
 
 
-def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
+def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None, scale=1.0):
     """The same step on another config, reported inside the one JSON line (north_star names the largest LP
-    AND the SOCP): value, us per CG step and the roofline fraction, no e2e / CPU legs."""
+    AND the SOCP): value, us per CG step and the roofline fraction, no e2e / CPU legs. scale > 1 grows the config
+    (same recipe, m, n and the cone count times scale) past the L2 so that its HBM fraction means something."""
     import torch
     from paper_2103_00736_b200 import binding
-    p = W.config(cfg)
+    p = W.config(cfg, scale=scale)
     S = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     for _ in range(a.warmup):
         S.condition(); S.iterate(a.k); S.residuals()
@@ -405,7 +406,7 @@ def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
     # L2 roofline (configs 1-3 are L2-resident, "report L2 throughput for them"): achieved = bytes the
     # kernel pulls through L2 per CG step (lts__t_bytes of the committed ncu capture) / time, against an L2-resident copy
     # measured live (l2_read_peak)
-    cap = ncu_capture(cfg)
+    cap = ncu_capture(cfg) if scale == 1.0 else None
     l2 = None
     if cap and cap.get("cg_steps_in_launch") and l2_peak:
         lts_per_cg = cap["lts__t_bytes.sum"] / (cap["cg_steps_in_launch"] + 1)
@@ -417,8 +418,9 @@ def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
            "steps": steps, "k_per_step": a.k, "cg_steps_per_iter": cg_iter / (steps * a.k),
            "us_per_cg_step": 1e3 * ms_iter / max(1, cg_iter), "cg_steps_per_s": cg_iter / (ms_iter * 1e-3), "bytes_per_cg_step": sv_cg,
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                        "note": "matrix copies of %d MB: (partly) resident in the 126 MB L2, so the HBM fraction is not the yardstick "
-                                "here; see roofline_l2" % (24 * p.nnz // 10**6)},
+                        "note": ("matrix copies of %d MB: (partly) resident in the 126 MB L2, so the HBM fraction is not the "
+                                 "yardstick here; see roofline_l2" if 24 * p.nnz < 2.5e8 else
+                                 "matrix copies of %d MB: HBM-bound like the headline workload") % (24 * p.nnz // 10**6)},
            "roofline_l2": l2,
            "gather_ceiling_frac": (2 * p.nnz * cg_iter / (ms_iter * 1e-3)) / (p.nnz / (us_g * 1e-6)), "phases": phases,
            "kkt_rel": r1["kkt_rel"]}
@@ -426,6 +428,8 @@ def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None):
     # B's third metric on this workload: paper schedule, exact projections (the parity setting) and cg_reduce = 0.3
     import argparse as _ap
     for tag, prm in (("time_to_kkt_1e-4_exact", {}), ("time_to_kkt_1e-4", {"cg_tol": 1e-12, "cg_reduce": 0.3})):
+        if scale != 1.0 and not prm:
+            continue                       # the scaled workload: the inexact run only (keeps the default bench short)
         try:
             a2 = _ap.Namespace(**{**vars(a), "tol": 1e-4, "check_every": 25, "max_iter": 3000, "time_cap_s": 60.0})
             S2 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
@@ -508,6 +512,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
             line["secondary"] = {"l2_read_peak": l2p,
                                  "cfg3_socp": secondary_workload(3, a, dev, stream, line["roofline"]["peak"], l2p),
                                  "cfg1_lp": secondary_workload(1, a, dev, stream, line["roofline"]["peak"], l2p),
+                                 "cfg3_socp_x8": secondary_workload(3, a, dev, stream, line["roofline"]["peak"], None, 8.0),
                                  "dense_sec5d": dense_workload(a, dev, stream, line["roofline"]["peak"])}
         except Exception as e:  # pragma: no cover
             line["secondary"] = {"error": str(e)}
@@ -553,19 +558,27 @@ def finish(a, p, S, line, rank, world, dev, stream):
     hx, hz = torch.empty(p.n, dtype=torch.float64).pin_memory(), torch.empty(p.n, dtype=torch.float64).pin_memory()
     h2d = sum(t.numel() * t.element_size() for t in hin) + 16 * p.n
     d2h = 16 * p.n + 128
+    e2e_log = {"step_s": [], "create_s": [], "cg_steps": []}
     def e2e_step():
+        ta = time.perf_counter()
         S2 = binding.Solver(p.m, p.n, hin[0].numpy(), hin[1].numpy(), hin[2].numpy(), hin[3].numpy(), hin[4].numpy(),
                             p.n_lin, p.soc_size, stream=stream.cuda_stream)
+        tb = time.perf_counter()               # cs_create returns with the layouts built (it synchronises itself)
         S2.set_params(mu=p.mu, t=p.t, precond=a.precond, **({"cg_max_iter": a.cg_max_iter} if a.cg_max_iter else {}))
         S2.set_point(hx0.numpy(), hz0.numpy())
         S2.condition()
         S2.iterate(a.k)
-        S2.residuals()
+        r2 = S2.residuals()
         S2.solution_into(x=hx.numpy(), z=hz.numpy())
         S2.destroy()
+        e2e_log["step_s"].append(time.perf_counter() - ta)
+        e2e_log["create_s"].append(tb - ta)
+        e2e_log["cg_steps"].append(int(r2["cg_steps_total"]))
     dt = float("nan")
     if a.e2e_steps > 0:
         e2e_step()  # warm-up
+        for v in e2e_log.values():
+            v.clear()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         for _ in range(a.e2e_steps):
@@ -574,7 +587,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
         dt = time.perf_counter() - t0
     dt_max = max_over_ranks(dt, dev)
     line["e2e"] = {"value": whole_job_value(a.e2e_steps * a.k, world, dt_max * 1e3) if a.e2e_steps else None, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-                   "d2h_bytes_per_step": int(d2h), "steps": a.e2e_steps,
+                   "d2h_bytes_per_step": int(d2h), "steps": a.e2e_steps, **e2e_log,
                    "step": "cs_create(host A,b,c) + cs_set_point(host x,z of the last timed step) + cs_condition + cs_iterate(k) + "
                            "cs_residuals + cs_solution(host x,z)"}
     if rank == 0:

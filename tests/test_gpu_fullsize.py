@@ -56,10 +56,11 @@ def test_fullsize_against_oracle(cfg, k):
         assert abs(r[key] - q[key]) <= 1e-6 * abs(q[key]) + 1e-11, (key, r[key], q[key])
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
-def test_fullsize_pass_identities(cfg):
+@pytest.mark.parametrize("cfg,scale", [(1, 1.0), (2, 1.0), (3, 1.0), (4, 1.0), (3, 8.0)])
+def test_fullsize_pass_identities(cfg, scale):
+    """(3, 8.0) is bench.py's HBM-scale SOCP block (config 3's recipe at 8x: 160,000 cones, 32 M stored entries)."""
     from paper_2103_00736_b200 import binding
-    p = W.config(cfg)
+    p = W.config(cfg, scale=scale)
     S = binding.Solver.from_problem(p, device="cuda:0")
     s_opt = p.x0 - p.mu * p.s0
     S.iterate(2)
