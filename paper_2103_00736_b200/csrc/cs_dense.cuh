@@ -4,7 +4,7 @@
 //   at every conditioning   Ad = A~ (m x n, row-major)          k_dense_scatter
 //                           M  = Ad Ad'                          k_dense_aat        (unit diagonal: A~ is row-equilibrated)
 //                           M  = L L'   (blocked, right-looking) k_chol_diag / k_chol_panel / k_chol_update
-//                           Z  = L^-T   (row j = column j of L^-1)  k_dense_transpose_lower, k_dense_trinv
+//                           Z  = L^-T   (row j = column j of L^-1)  k_dense_diag_inv, k_dense_trinv_blk
 //                           Minv = Z Z' = M^-1                   k_dense_aat
 //   at every pass           w += M^-1 r by dense_apply_grid (cs_kernels.cuh): x = Minv r, then kDenseRefine steps of
 //                           iterative refinement x += Minv (r - M x) against the stored M -- dense GEMVs only.
@@ -29,7 +29,8 @@ __global__ void k_dense_scatter(Ctx c, double *Ad) {
 
 // C = A A' for a row-major A [r][k]; C [r][r] full (both triangles written).  One CTA of 256 threads per 64 x 64 tile
 // of the lower triangle, 4 x 4 outputs per thread, the k range consumed 16 at a time through shared memory.
-__global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k, double *C) {
+// tri != 0: A is upper triangular (A[a][i] = 0 for i < a, k = r), so the sum starts at the tile's first row (Minv = Z Z').
+__global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k, double *C, int tri) {
     __shared__ double sa[16][65], sb[16][65];
     // tile (ti, tj) with tj <= ti from the linear block index
     int ti = (int)((sqrt(8.0 * blockIdx.x + 1.0) - 1.0) * 0.5);
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k
     const int tj = blockIdx.x - ti * (ti + 1) / 2;
     const int a0 = ti * 64, b0 = tj * 64, tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
     double acc[4][4] = {};
-    for (int k0 = 0; k0 < k; k0 += 16) {
+    for (int k0 = tri ? a0 : 0; k0 < k; k0 += 16) {              // a0 >= b0: both operands are zero before column a0
         for (int q = threadIdx.x; q < 64 * 16; q += 256) {       // rows of the tile x 16 columns: 128-byte row pieces
             const int row = q >> 4, col = q & 15;
             const bool okc = k0 + col < k;
@@ -148,56 +149,85 @@ __global__ void __launch_bounds__(256) k_chol_update(double *L, int m, int kb) {
         }
 }
 
-// Lt = L' (upper triangle, row-major): the triangular inverse below reads L by columns
-__global__ void __launch_bounds__(256) k_dense_transpose_lower(const double *L, int m, double *Lt) {
-    __shared__ double tile[32][33];
-    const int bx = blockIdx.x * 32, by = blockIdx.y * 32, tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    if (bx > by + 31) return;                                    // tile entirely above the diagonal of L: nothing stored there
-    for (int r = ty; r < 32; r += 8) {
-        const int i = by + r, k = bx + tx;
-        tile[r][tx] = (i < m && k < m && k <= i) ? L[(size_t)i * m + k] : 0.0;
+// ---- Z = L^-T (row j of Z = column j of L^-1), blocked ---------------------------------------------------------------
+// Column j of X = L^-1 depends on L only, so column groups are independent; inside a group the block rows follow one
+// another:  X_JJ = (L_JJ)^-1,   X_IJ = -(L_II)^-1 sum_{K=J}^{I-1} L_IK X_KJ   (64 x 64 blocks of L).
+// k_dense_diag_inv inverts every diagonal block once; k_dense_trinv_blk gives one CTA a group of kTriCW columns and walks
+// the block rows with 64 x 64 tiles of L in shared memory (each tile serves 64 x kTriCW x 64 multiply-adds, so L is read
+// m / (3 kTriCW) times from L2 instead of m / 3 times: 6.9 -> ~1 ms at m = 2320).  Heaviest groups (J = 0) have the
+// lowest block indices and start first.  Fixed summation order; Z zeroed by the caller (x_i = 0 for i < j's block).
+constexpr int kTriNB = 64, kTriCW = 8;
+
+__global__ void __launch_bounds__(kTriNB) k_dense_diag_inv(const double *L, int m, double *Dinv) {
+    constexpr int kTri = kTriNB * (kTriNB + 1) / 2;              // packed lower triangles: (i, k) at i (i + 1) / 2 + k
+    __shared__ double sl[kTri], sx[kTri];
+    const int I = blockIdx.x, b0 = I * kTriNB, j = threadIdx.x;
+    for (int r = j; r < kTriNB; ++r) {                           // thread j loads column j; identity-padded past m
+        const int gi = b0 + r, gj = b0 + j;
+        sl[r * (r + 1) / 2 + j] = (gi < m && gj < m) ? L[(size_t)gi * m + gj] : (r == j ? 1.0 : 0.0);
     }
     __syncthreads();
-    for (int r = ty; r < 32; r += 8) {
-        const int k = bx + r, i = by + tx;
-        if (k < m && i < m) Lt[(size_t)k * m + i] = tile[tx][r];
+    for (int i = j; i < kTriNB; ++i) {                           // thread j: column j of the inverse, forward substitution
+        double s = i == j ? 1.0 : 0.0;
+        for (int k = j; k < i; ++k) s -= sl[i * (i + 1) / 2 + k] * sx[k * (k + 1) / 2 + j];
+        sx[i * (i + 1) / 2 + j] = s / sl[i * (i + 1) / 2 + i];
     }
+    for (int r = 0; r < kTriNB; ++r) Dinv[((size_t)I * kTriNB + r) * kTriNB + j] = j <= r ? sx[r * (r + 1) / 2 + j] : 0.0;
 }
 
-// Z = L^-T, row j = column j of L^-1: one warp per column j solves L x = e_j forwards, 32 rows at a time.  Lane r owns
-// row i = i0 + r of the block: first s_r = sum_{k < i0} L[i][k] x[k] -- a loop over k with no dependence between its
-// iterations (Lt[k][i0 + lane] is one coalesced load, x[k] a broadcast) -- then the 32 x 32 diagonal block is solved inside
-// the warp with shuffles.  The dependent chain through memory is m/32 steps long instead of m (14.7 -> 6.9 ms at m = 2320;
-// what is left is L2 traffic: every column streams the part of L' below it, 4 m^3 / 3 bytes in all -- a tile-sharing blocked
-// inverse is the next step).  Z zeroed by the caller (x_k = 0 for k < j).  Fixed summation order.
-__global__ void __launch_bounds__(256) k_dense_trinv(const double *Lt, int m, double *Z) {
-    const int lane = threadIdx.x & 31;
-    const int gwarp = (blockIdx.x * 256 + threadIdx.x) >> 5, nwarps = (gridDim.x * 256) >> 5;
-    for (int j = gwarp; j < m; j += nwarps) {
-        double *x = Z + (size_t)j * m;
-        for (int i0 = j & ~31; i0 < m; i0 += 32) {
-            const int i = i0 + lane;
-            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-            int k = j;
-            if (i < m) {
-                for (; k + 3 < i0; k += 4) {
-                    s0 += Lt[(size_t)k * m + i] * __ldcg(x + k);
-                    s1 += Lt[(size_t)(k + 1) * m + i] * __ldcg(x + k + 1);
-                    s2 += Lt[(size_t)(k + 2) * m + i] * __ldcg(x + k + 2);
-                    s3 += Lt[(size_t)(k + 3) * m + i] * __ldcg(x + k + 3);
-                }
-                for (; k < i0; ++k) s0 += Lt[(size_t)k * m + i] * __ldcg(x + k);
+__global__ void __launch_bounds__(128) k_dense_trinv_blk(const double *L, const double *Dinv, int m, double *Z) {
+    __shared__ __align__(16) double sl[kTriNB][kTriNB + 2];      // a tile of L, or (L_II)^-1
+    __shared__ double sx[kTriNB][kTriCW + 1];                    // the matching rows of X for this group's columns, or T
+    const int c0 = blockIdx.x * kTriCW, J = c0 / kTriNB, nblk = (m + kTriNB - 1) / kTriNB;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, cc = lane & (kTriCW - 1), rh = lane / kTriCW;
+    const int gc = c0 + cc;                                      // this thread's column of L^-1 = row of Z
+    int row[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) row[q] = 16 * w + rh + 4 * q;    // its four rows of the block row
+    for (int I = J; I < nblk; ++I) {
+        double acc[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int K = J; K < I; ++K) {                            // T = sum_K L_IK X_KJ
+            for (int t = threadIdx.x; t < kTriNB * kTriNB; t += 128) {
+                const int r = t >> 6, k = t & 63, gi = I * kTriNB + r;
+                sl[r][k] = gi < m ? L[(size_t)gi * m + K * kTriNB + k] : 0.0;
             }
-            double rhs = (i == j ? 1.0 : 0.0) - ((s0 + s1) + (s2 + s3));
-            const double dg = i < m ? Lt[(size_t)i * m + i] : 1.0;
-            for (int cidx = 0; cidx < 32 && i0 + cidx < m; ++cidx) {     // x_c = rhs_c / L_cc ; rhs_r -= L[r][c] x_c for r > c
-                const double xc = __shfl_sync(0xffffffffu, rhs, cidx) / __shfl_sync(0xffffffffu, dg, cidx);
-                if (lane == cidx) rhs = xc;
-                else if (lane > cidx && i < m) rhs -= Lt[(size_t)(i0 + cidx) * m + i] * xc;
+            for (int t = threadIdx.x; t < kTriNB * kTriCW; t += 128) {
+                const int c = t >> 6, k = t & 63;
+                sx[k][c] = c0 + c < m ? __ldcg(Z + (size_t)(c0 + c) * m + K * kTriNB + k) : 0.0;
             }
-            if (i < m && i >= j) __stcg(x + i, rhs);
-            __syncwarp();                                        // the next block reads x[i0 .. i0+32) (through L2: __stcg / __ldcg)
+            __syncthreads();
+#pragma unroll 8
+            for (int k = 0; k < kTriNB; ++k) {
+                const double x = sx[k][cc];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[q] += sl[row[q]][k] * x;
+            }
+            __syncthreads();
         }
+        for (int t = threadIdx.x; t < kTriNB * kTriNB; t += 128)
+            sl[t >> 6][t & 63] = Dinv[(size_t)I * kTriNB * kTriNB + t];
+        double xo[4] = {0.0, 0.0, 0.0, 0.0};
+        if (I == J) {                                            // X_JJ: the group's columns of (L_JJ)^-1
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < 4; ++q) xo[q] = sl[row[q]][gc - J * kTriNB];
+        } else {                                                 // X_IJ = -(L_II)^-1 T
+#pragma unroll
+            for (int q = 0; q < 4; ++q) sx[row[q]][cc] = acc[q];
+            __syncthreads();
+#pragma unroll 8
+            for (int k = 0; k < kTriNB; ++k) {
+                const double x = sx[k][cc];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) xo[q] -= sl[row[q]][k] * x;
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int gi = I * kTriNB + row[q];
+            if (gi < m && gc < m) __stcg(Z + (size_t)gc * m + gi, xo[q]);
+        }
+        __syncthreads();                                         // the group's later block rows read these (through L2)
     }
 }
 
