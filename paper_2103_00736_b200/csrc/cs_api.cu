@@ -651,7 +651,7 @@ cs_status dense_grid_factor(cs_solver *S) {
     const Ctx &c = S->ctx;
     const int m = c.m, n = c.n;
     const size_t mm = (size_t)m * m;
-    const int tiles = (m + 63) / 64, n_tri = tiles * (tiles + 1) / 2, one = 1;
+    const int tiles = (m + kGemmT - 1) / kGemmT, n_tri = tiles * (tiles + 1) / 2, one = 1;
     CS_CUDA(S, cudaMemsetAsync(c.gAd, 0, sizeof(double) * (size_t)m * n, S->stream));
     CS_CUDA(S, cudaMemsetAsync(c.gZ, 0, sizeof(double) * mm, S->stream));
     CS_CUDA(S, cudaMemcpyAsync(c.g_ok, &one, sizeof(int), cudaMemcpyHostToDevice, S->stream));
@@ -671,7 +671,8 @@ cs_status dense_grid_factor(cs_solver *S) {
     }
     // Z = L^-T by column groups (inverses of the diagonal blocks first), then Minv = Z Z'
     k_dense_diag_inv<<<(m + kTriNB - 1) / kTriNB, kTriNB, 0, S->stream>>>(c.gL, m, c.gDinv);
-    k_dense_trinv_blk<<<(m + kTriCW - 1) / kTriCW, 128, 0, S->stream>>>(c.gL, c.gDinv, m, c.gZ);
+    CS_CUDA(S, cudaFuncSetAttribute((const void *)k_dense_trinv_blk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TrinvSmem)));
+    k_dense_trinv_blk<<<(m + kTriCW - 1) / kTriCW, 128, sizeof(TrinvSmem), S->stream>>>(c.gL, c.gDinv, m, c.gZ);
     k_dense_aat<<<n_tri, 256, 0, S->stream>>>(c.gZ, m, m, c.gMinv, 1);
     S->launches += 3;
     CS_CUDA(S, cudaGetLastError());

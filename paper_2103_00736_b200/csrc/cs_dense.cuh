@@ -27,43 +27,80 @@ __global__ void k_dense_scatter(Ctx c, double *Ad) {
         for (int e = c.Rc.ptr[i] + lane; e < c.Rc.ptr[i + 1]; e += 32) Ad[(size_t)i * c.n + c.Rc.idx[e]] = c.R.val[c.Rc.pos[e]];
 }
 
-// C = A A' for a row-major A [r][k]; C [r][r] full (both triangles written).  One CTA of 256 threads per 64 x 64 tile
-// of the lower triangle, 4 x 4 outputs per thread, the k range consumed 16 at a time through shared memory.
-// tri != 0: A is upper triangular (A[a][i] = 0 for i < a, k = r), so the sum starts at the tile's first row (Minv = Z Z').
-__global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k, double *C, int tri) {
-    __shared__ double sa[16][65], sb[16][65];
-    // tile (ti, tj) with tj <= ti from the linear block index
-    int ti = (int)((sqrt(8.0 * blockIdx.x + 1.0) - 1.0) * 0.5);
-    while ((ti + 1) * (ti + 2) / 2 <= (int)blockIdx.x) ++ti;
-    while (ti * (ti + 1) / 2 > (int)blockIdx.x) --ti;
-    const int tj = blockIdx.x - ti * (ti + 1) / 2;
-    const int a0 = ti * 64, b0 = tj * 64, tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-    double acc[4][4] = {};
-    for (int k0 = tri ? a0 : 0; k0 < k; k0 += 16) {              // a0 >= b0: both operands are zero before column a0
-        for (int q = threadIdx.x; q < 64 * 16; q += 256) {       // rows of the tile x 16 columns: 128-byte row pieces
-            const int row = q >> 4, col = q & 15;
-            const bool okc = k0 + col < k;
-            sa[col][row] = (okc && a0 + row < r) ? A[(size_t)(a0 + row) * k + k0 + col] : 0.0;
-            sb[col][row] = (okc && b0 + row < r) ? A[(size_t)(b0 + row) * k + k0 + col] : 0.0;
+// ---- the dense contraction core: a 128 x 128 tile of sum_k A[a0+i][k] B[b0+j][k] ("NT": both operands row-major along k) --
+// 256 threads, 8 x 8 outputs per thread in registers (rows ty*4+{0..3} and 64+ty*4+{0..3}, columns likewise with tx: the
+// shared-memory reads are 16-byte loads without bank conflicts), operands staged k-major 16 columns at a time, the next
+// stage fetched into registers while the current one is consumed.  Plain DFMA: per k a thread does 64 multiply-adds on 8
+// 16-byte shared loads, so the FP64 pipe is the bound (B200's fp64 tensor rate equals its vector rate).  Fixed summation order.
+constexpr int kGemmT = 128, kGemmK = 16;
+struct GemmSmem { double a[kGemmK][kGemmT + 2], b[kGemmK][kGemmT + 2]; };
+
+__device__ __forceinline__ void gemm_nt_tile(const double *A, size_t lda, int ra, int a0, const double *B, size_t ldb, int rb, int b0,
+                                             int k0, int k1, GemmSmem &sm, double (&acc)[8][8]) {
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int lr = tid >> 3, lc = (tid & 7) * 2;                 // loader: rows lr + 32 i, columns lc, lc + 1 of the stage
+    double pa[4][2], pb[4][2];
+    auto fetch = [&](int kk) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int r = a0 + lr + 32 * i, q = b0 + lr + 32 * i, k = kk + lc;
+            pa[i][0] = (r < ra && k < k1) ? A[(size_t)r * lda + k] : 0.0;
+            pa[i][1] = (r < ra && k + 1 < k1) ? A[(size_t)r * lda + k + 1] : 0.0;
+            pb[i][0] = (q < rb && k < k1) ? B[(size_t)q * ldb + k] : 0.0;
+            pb[i][1] = (q < rb && k + 1 < k1) ? B[(size_t)q * ldb + k + 1] : 0.0;
+        }
+    };
+    fetch(k0);
+    for (int kk0 = k0; kk0 < k1; kk0 += kGemmK) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            sm.a[lc][lr + 32 * i] = pa[i][0]; sm.a[lc + 1][lr + 32 * i] = pa[i][1];
+            sm.b[lc][lr + 32 * i] = pb[i][0]; sm.b[lc + 1][lr + 32 * i] = pb[i][1];
         }
         __syncthreads();
+        if (kk0 + kGemmK < k1) fetch(kk0 + kGemmK);
 #pragma unroll
-        for (int kk = 0; kk < 16; ++kk) {
-            double va[4], vb[4];
+        for (int kk = 0; kk < kGemmK; ++kk) {
+            double va[8], vb[8];
+            *reinterpret_cast<double2 *>(va + 0) = *reinterpret_cast<const double2 *>(&sm.a[kk][ty * 4]);
+            *reinterpret_cast<double2 *>(va + 2) = *reinterpret_cast<const double2 *>(&sm.a[kk][ty * 4 + 2]);
+            *reinterpret_cast<double2 *>(va + 4) = *reinterpret_cast<const double2 *>(&sm.a[kk][64 + ty * 4]);
+            *reinterpret_cast<double2 *>(va + 6) = *reinterpret_cast<const double2 *>(&sm.a[kk][64 + ty * 4 + 2]);
+            *reinterpret_cast<double2 *>(vb + 0) = *reinterpret_cast<const double2 *>(&sm.b[kk][tx * 4]);
+            *reinterpret_cast<double2 *>(vb + 2) = *reinterpret_cast<const double2 *>(&sm.b[kk][tx * 4 + 2]);
+            *reinterpret_cast<double2 *>(vb + 4) = *reinterpret_cast<const double2 *>(&sm.b[kk][64 + tx * 4]);
+            *reinterpret_cast<double2 *>(vb + 6) = *reinterpret_cast<const double2 *>(&sm.b[kk][64 + tx * 4 + 2]);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) { va[i] = sa[kk][ty * 4 + i]; vb[i] = sb[kk][tx * 4 + i]; }
+            for (int i = 0; i < 8; ++i)
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) acc[i][j] += va[i] * vb[j];
+                for (int j = 0; j < 8; ++j) acc[i][j] += va[i] * vb[j];
         }
         __syncthreads();
     }
+}
+// tile (ti, tj), tj <= ti, of the lower triangle from the linear block index
+__device__ __forceinline__ void tri_tile(int b, int &ti, int &tj) {
+    ti = (int)((sqrt(8.0 * b + 1.0) - 1.0) * 0.5);
+    while ((ti + 1) * (ti + 2) / 2 <= b) ++ti;
+    while (ti * (ti + 1) / 2 > b) --ti;
+    tj = b - ti * (ti + 1) / 2;
+}
+__device__ __forceinline__ int gemm_row(int t, int i) { return (i < 4 ? 0 : 60) + t * 4 + i; }   // output i of thread coordinate t
+
+// C = A A' for a row-major A [r][k]; C [r][r] full (both triangles written).  One CTA per 128 x 128 tile of the lower triangle.
+// tri != 0: A is upper triangular (A[a][i] = 0 for i < a, k = r), so the sum starts at the tile's first row (Minv = Z Z').
+__global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k, double *C, int tri) {
+    __shared__ __align__(16) GemmSmem sm;
+    int ti, tj;
+    tri_tile(blockIdx.x, ti, tj);
+    const int a0 = ti * kGemmT, b0 = tj * kGemmT, tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    double acc[8][8] = {};
+    gemm_nt_tile(A, (size_t)k, r, a0, A, (size_t)k, r, b0, tri ? a0 : 0, k, sm, acc);   // a0 >= b0: both operands are zero before column a0
 #pragma unroll
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 8; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int a = a0 + ty * 4 + i, b = b0 + tx * 4 + j;
+        for (int j = 0; j < 8; ++j) {
+            const int a = a0 + gemm_row(ty, i), b = b0 + gemm_row(tx, j);
             if (a < r && b < r) {
                 C[(size_t)a * r + b] = acc[i][j];
                 if (ti != tj) C[(size_t)b * r + a] = acc[i][j];
@@ -75,7 +112,8 @@ __global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k
 // step kb: (1) k_chol_diag factors the nb x nb diagonal block in shared memory (one CTA); a pivot <= 1e-12 (diag(M) = 1:
 //              a relative test) clears *ok and is replaced by 1 so that the run stays finite (the caller falls back to CG)
 //          (2) k_chol_panel: rows below the block, X D' = L[i][kb:kb+nb] -- one warp per row, lane c owns column c
-//          (3) k_chol_update: trailing L[i][j] -= sum_c P[i][c] P[j][c] (j <= i), 64 x 64 tiles, 4 x 4 per thread
+//          (3) k_chol_update: trailing L[i][j] -= sum_c P[i][c] P[j][c] (j <= i), 64 x 64 tiles, 4 x 4 per thread (a rank-32
+//              update is bound by reading and writing L: the 128 x 128 core above is slower here, 27 vs 20 us per panel)
 __global__ void __launch_bounds__(kCholNB * kCholNB) k_chol_diag(double *L, int m, int kb, int *ok) {
     __shared__ double d[kCholNB][kCholNB + 1];
     const int nb = min(kCholNB, m - kb), r = threadIdx.x / kCholNB, cc = threadIdx.x % kCholNB;
@@ -175,59 +213,90 @@ __global__ void __launch_bounds__(kTriNB) k_dense_diag_inv(const double *L, int 
     for (int r = 0; r < kTriNB; ++r) Dinv[((size_t)I * kTriNB + r) * kTriNB + j] = j <= r ? sx[r * (r + 1) / 2 + j] : 0.0;
 }
 
+// shared memory of k_dense_trinv_blk (dynamic: ~79 KB, two CTAs per SM): two stages of {tile of L or (L_II)^-1, rows of X}
+// filled by cp.async one step ahead, and the block row of X computed last (the next block row's first-hand operand)
+struct TrinvSmem {
+    double l[2][kTriNB][kTriNB + 2];
+    double x[2][kTriCW][kTriNB + 2];     // [column of the group][k]
+    double fresh[kTriCW][kTriNB + 2];
+};
+__device__ __forceinline__ void cp_async8(void *dst, const void *src, bool ok) {   // 8 bytes global -> shared, zero-filled if !ok
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    const int n = ok ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
+}
+
 __global__ void __launch_bounds__(128) k_dense_trinv_blk(const double *L, const double *Dinv, int m, double *Z) {
-    __shared__ __align__(16) double sl[kTriNB][kTriNB + 2];      // a tile of L, or (L_II)^-1
-    __shared__ double sx[kTriNB][kTriCW + 1];                    // the matching rows of X for this group's columns, or T
+    extern __shared__ __align__(16) unsigned char trinv_raw[];
+    TrinvSmem &sm = *reinterpret_cast<TrinvSmem *>(trinv_raw);
     const int c0 = blockIdx.x * kTriCW, J = c0 / kTriNB, nblk = (m + kTriNB - 1) / kTriNB;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, cc = lane & (kTriCW - 1), rh = lane / kTriCW;
     const int gc = c0 + cc;                                      // this thread's column of L^-1 = row of Z
     int row[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) row[q] = 16 * w + rh + 4 * q;    // its four rows of the block row
-    for (int I = J; I < nblk; ++I) {
-        double acc[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int K = J; K < I; ++K) {                            // T = sum_K L_IK X_KJ
-            for (int t = threadIdx.x; t < kTriNB * kTriNB; t += 128) {
-                const int r = t >> 6, k = t & 63, gi = I * kTriNB + r;
-                sl[r][k] = gi < m ? L[(size_t)gi * m + K * kTriNB + k] : 0.0;
-            }
+    // step (I, K): K < I multiplies the tile L_IK with X_K; K == I multiplies (L_II)^-1 with the finished sum.  The loads of
+    // a step are issued one step ahead; X_{I-1} comes from sm.fresh (it was computed in the previous block row).
+    auto issue = [&](int I, int K, int buf) {
+        for (int t = threadIdx.x; t < kTriNB * kTriNB; t += 128) {
+            const int r = t >> 6, k = t & 63, gi = I * kTriNB + r;
+            const bool ok = K == I || gi < m;
+            const double *src = K == I ? Dinv + (size_t)I * kTriNB * kTriNB + t : L + (size_t)(ok ? gi : 0) * m + K * kTriNB + k;
+            cp_async8(&sm.l[buf][r][k], src, ok);
+        }
+        if (K < I - 1)
             for (int t = threadIdx.x; t < kTriNB * kTriCW; t += 128) {
                 const int c = t >> 6, k = t & 63;
-                sx[k][c] = c0 + c < m ? __ldcg(Z + (size_t)(c0 + c) * m + K * kTriNB + k) : 0.0;
+                const bool ok = c0 + c < m;
+                cp_async8(&sm.x[buf][c][k], Z + (size_t)(ok ? c0 + c : 0) * m + K * kTriNB + k, ok);
+            }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int buf = 0;
+    issue(J, J, 0);
+    for (int I = J; I < nblk; ++I) {
+        double acc[4] = {0.0, 0.0, 0.0, 0.0}, xo[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int K = J; K <= I; ++K) {
+            const bool more = K < I || I + 1 < nblk;
+            if (more) issue(K < I ? I : I + 1, K < I ? K + 1 : J, buf ^ 1);
+            if (more) asm volatile("cp.async.wait_group 1;" ::: "memory");
+            else asm volatile("cp.async.wait_group 0;" ::: "memory");
+            if (K == I && I > J) {                               // the finished sum T becomes the operand of (L_II)^-1
+#pragma unroll
+                for (int q = 0; q < 4; ++q) sm.x[buf][cc][row[q]] = acc[q];
             }
             __syncthreads();
+            if (K == I && I == J) {                              // X_JJ: the group's columns of (L_JJ)^-1
+#pragma unroll
+                for (int q = 0; q < 4; ++q) xo[q] = sm.l[buf][row[q]][gc - J * kTriNB];
+            } else {
+                const double *xs = K == I - 1 ? sm.fresh[cc] : sm.x[buf][cc];
+                if (K < I) {
 #pragma unroll 8
-            for (int k = 0; k < kTriNB; ++k) {
-                const double x = sx[k][cc];
+                    for (int k = 0; k < kTriNB; ++k) {
+                        const double x = xs[k];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) acc[q] += sl[row[q]][k] * x;
-            }
-            __syncthreads();
-        }
-        for (int t = threadIdx.x; t < kTriNB * kTriNB; t += 128)
-            sl[t >> 6][t & 63] = Dinv[(size_t)I * kTriNB * kTriNB + t];
-        double xo[4] = {0.0, 0.0, 0.0, 0.0};
-        if (I == J) {                                            // X_JJ: the group's columns of (L_JJ)^-1
-            __syncthreads();
-#pragma unroll
-            for (int q = 0; q < 4; ++q) xo[q] = sl[row[q]][gc - J * kTriNB];
-        } else {                                                 // X_IJ = -(L_II)^-1 T
-#pragma unroll
-            for (int q = 0; q < 4; ++q) sx[row[q]][cc] = acc[q];
-            __syncthreads();
+                        for (int q = 0; q < 4; ++q) acc[q] += sm.l[buf][row[q]][k] * x;
+                    }
+                } else {                                         // X_IJ = -(L_II)^-1 T
 #pragma unroll 8
-            for (int k = 0; k < kTriNB; ++k) {
-                const double x = sx[k][cc];
+                    for (int k = 0; k < kTriNB; ++k) {
+                        const double x = xs[k];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) xo[q] -= sl[row[q]][k] * x;
+                        for (int q = 0; q < 4; ++q) xo[q] -= sm.l[buf][row[q]][k] * x;
+                    }
+                }
             }
+            __syncthreads();                                     // stage `buf` is free for the loads of the step after next
+            buf ^= 1;
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const int gi = I * kTriNB + row[q];
+            sm.fresh[cc][row[q]] = xo[q];                        // read next as X_I (no reader is left from the previous block row)
             if (gi < m && gc < m) __stcg(Z + (size_t)gc * m + gi, xo[q]);
         }
-        __syncthreads();                                         // the group's later block rows read these (through L2)
+        __syncthreads();                                         // the group's later block rows read Z (through L2) and sm.fresh
     }
 }
 
