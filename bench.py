@@ -200,6 +200,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 (SOCP) block")
+    ap.add_argument("--dense-n", type=int, default=10000, help="n of the section V-A dense LP block (the paper goes to 30000)")
     ap.add_argument("--no-time-to-tol", action="store_true", help="skip the time-to-1e-4-KKT leg of the default run")
     ap.add_argument("--solve", action="store_true",
                     help="extra mode: run the paper's schedule (17)/(18) to --tol and report the time to tolerance")
@@ -443,15 +444,15 @@ def secondary_workload(cfg, a, dev, stream, peak, l2_peak=None, scale=1.0):
     return out
 
 
-def dense_workload(a, dev, stream, peak):
-    """Secondary block for the paper's own dense shape (section V-D: SOCP, K = (K_4)^(n/4), n = 2900, m = 2320)
-    through the grid dense factor-apply path (csrc/cs_dense.cuh): time per pass (k = 100 passes per launch, schedule (18)),
+def dense_workload(a, dev, stream, peak, kind="sec5d", n=2900):
+    """Secondary block for the paper's own dense shapes (section V-D: SOCP, K = (K_4)^(n/4), n = 2900, m = 2320, P:366-371;
+    section V-A: LP, n up to 30000, m = 0.8 n) through the grid dense factor-apply path (csrc/cs_dense.cuh): time per pass (k = 100 passes per launch, schedule (18)),
     per conditioning (incl. the m x m factorisation and explicit inverse), and time to kkt_rel <= 1e-4.
     Rooflines: the per-pass apply is 2*refine+1 = 5 dense m x m GEMVs (HBM/L2 bytes); the factorisation is fp64 FMA work
     against 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s."""
     import torch
     from paper_2103_00736_b200 import binding
-    p = W.dense_socp_sec5d(BASE_DENSE_SEED, n=2900, h=4)
+    p = W.dense_socp_sec5d(BASE_DENSE_SEED, n=n, h=4) if kind == "sec5d" else W.dense_lp_sec5a(BASE_DENSE_SEED + 1, n=n)
     S = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     S.iterate(50)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
@@ -466,25 +467,27 @@ def dense_workload(a, dev, stream, peak):
     m, n = p.m, p.n
     us_pass = 1e3 * ms_i / (reps * 100)
     gemv_bytes = 5 * m * m * 8 + 2 * 12 * p.nnz              # the apply + the rhs and update passes over the stored A~
-    flops = m * m * n + 5.0 * m ** 3 / 3.0                    # SYRK + Cholesky + L^-T + Z Z'
+    flops = m * m * n + 1.0 * m ** 3                          # SYRK + Cholesky + L^-T + Z Z' (triangular operands), m^3 / 3 each
     S2 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     r2, conds = S2.solve(20000, tol=1e-4, check_every=25, first=p.L_first, every=p.L_every)
     dt = time.perf_counter() - t0
     S2.destroy()
-    return {"workload": "sec5d_dense_socp n=2900 h=4 (P:366-371)", "m": m, "n": n, "nnz": p.nnz, "n_soc": p.n_soc,
-            "path": "grid dense factor-apply (cs_params.dense_m_threshold = 4096: default for a dense-stored A)",
+    return {"workload": f"sec5d_dense_socp n={n} h=4 (P:366-371)" if kind == "sec5d" else f"sec5a_dense_lp n={n} (P:342-346)",
+            "m": m, "n": n, "nnz": p.nnz, "n_soc": p.n_soc,
+            "path": "grid dense factor-apply (cs_params.dense_m_threshold = 24576: default for a dense-stored A)",
             "us_per_pass": us_pass, "value": 1e6 / us_pass, "unit": UNIT, "cg_steps_total": r["cg_steps_total"],
             "ms_per_conditioning": ms_c / reps,
             "roofline_pass": {"bound": "hbm", "achieved": gemv_bytes / (us_pass * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
                               "frac": gemv_bytes / (us_pass * 1e-6) / 1e9 / peak,
-                              "bytes": "5 m^2 x 8 (M^-1, M, M^-1, M, M^-1) + 24 nnz (rhs and update passes); 86 MB of matrices: partly L2-resident"},
+                              "bytes": "5 m^2 x 8 (M^-1, M, M^-1, M, M^-1) + 24 nnz (rhs and update passes); %d MB of matrices" % (16 * m * m // 10**6)},
             "roofline_factor": {"bound": "alu", "achieved": flops / (ms_c / reps * 1e-3) / 1e12, "peak": 37.2, "unit": "TFLOP/s",
-                                "frac": flops / (ms_c / reps * 1e-3) / 1e12 / 37.2, "flops": "m^2 n + 5 m^3 / 3 (SYRK, Cholesky, L^-T, Z Z')",
+                                "frac": flops / (ms_c / reps * 1e-3) / 1e12 / 37.2, "flops": "m^2 n + m^3 (SYRK; Cholesky, L^-T, Z Z' at m^3 / 3 each)",
                                 "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 8)"},
             "time_to_kkt_1e-4": {"time_to_tol_s": dt, "reached": bool(r2["kkt_rel"] <= 1e-4), "iterations": r2["iter"],
-                                 "n_conditionings": len(conds), "kkt_rel": r2["kkt_rel"], "schedule": "L = {200, 300, ...}, t = 1.7, mu = 1 (18)"}}
+                                 "n_conditionings": len(conds), "kkt_rel": r2["kkt_rel"],
+                                 "schedule": "L = {200, 300, ...}, t = 1.7, mu = 1 (18)" if kind == "sec5d" else "L = {300, 400, ...}, t = 9.2, mu = 1 (17)"}}
 
 
 BASE_DENSE_SEED = 210300736 + 50
@@ -513,7 +516,8 @@ def finish(a, p, S, line, rank, world, dev, stream):
                                  "cfg3_socp": secondary_workload(3, a, dev, stream, line["roofline"]["peak"], l2p),
                                  "cfg1_lp": secondary_workload(1, a, dev, stream, line["roofline"]["peak"], l2p),
                                  "cfg3_socp_x8": secondary_workload(3, a, dev, stream, line["roofline"]["peak"], None, 8.0),
-                                 "dense_sec5d": dense_workload(a, dev, stream, line["roofline"]["peak"])}
+                                 "dense_sec5d": dense_workload(a, dev, stream, line["roofline"]["peak"]),
+                                 "dense_sec5a": dense_workload(a, dev, stream, line["roofline"]["peak"], "sec5a", a.dense_n)}
         except Exception as e:  # pragma: no cover
             line["secondary"] = {"error": str(e)}
         # B's third metric, "time to 1e-4 relative KKT residual", on the headline workload with the paper's

@@ -87,7 +87,7 @@ typedef struct {
  *            Both are rebuilt on the device at every conditioning and change the number of CG steps, not
  *            the solution of the solve.
  *   dense_m_threshold  dense factor-apply instead of CG where A is small enough that the solve truly is a dense
- *            contraction (B north_star; S 8(a) a3, S 8(f).3), for m <= dense_m_threshold (<= 4096; 0 = never):
+ *            contraction (B north_star; S 8(a) a3, S 8(f).3), for m <= dense_m_threshold (<= 24576; 0 = never):
  *            - problems that run on one CTA (nnz <= 8192) with m <= 256: every conditioning forms A~A~' (m x m, fp64) and
  *              factors it by Cholesky in that CTA; every pass applies the factor (two triangular solves + one step of
  *              iterative refinement);
@@ -95,7 +95,10 @@ typedef struct {
  *              many CTAs: every conditioning forms M = A~A~', its blocked Cholesky factor and the explicit inverse
  *              M^-1 = L^-T L^-1 (hand-written fp64 kernels, csrc/cs_dense.cuh); every pass is w += M^-1 r followed by two
  *              steps of iterative refinement against M -- dense matrix-vector products only.
- *            No CG steps are counted.  Default: 128, or 4096 for a dense-stored input.  A Cholesky pivot below 1e-12
+ *              The limit 24576 covers the paper's largest dense LP (n = 30000, m = 24000); the path's buffers
+ *              (A~ as [m][n] and four m x m matrices: 24 GB there) are allocated at the first conditioning that uses it,
+ *              and if the device cannot hold them the solve stays with CG (not an error).
+ *            No CG steps are counted.  Default: 128, or 24576 for a dense-stored input.  A Cholesky pivot below 1e-12
  *            (the diagonal of A~A~' is 1: numerically rank-deficient A) falls back to CG for that scaling.
  * cs_set_params may be called at any time; mu, t, o_floor, precond, dense_m_threshold take effect at the next
  * cs_condition (or at the implicit first conditioning), cg_* at the next solve. */
@@ -130,7 +133,7 @@ typedef struct {
 /* Build a solver for (A,b,c,K): validates the input, copies it to the device, builds the CSC copy of A
  * and the work partitions.  b[m], c[n] live in `vec_where`.  Parameters start at mu=1, t=9.2 (n_soc=0)
  * or 1.7 (n_soc>0), o_floor=1e-16, cg_tol=2.22e-16 (DBL_EPSILON), cg_reduce=0, cg_max_iter=20000, precond=0,
- * dense_m_threshold=128 (4096 for a dense-stored A); the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
+ * dense_m_threshold=128 (24576 for a dense-stored A); the starting point is x=z=e_K (1 on each cone's first coordinate), which makes the
  * mandatory first conditioning (l=1) the identity and s=0.  Synchronous.  On failure *out is NULL. */
 cs_status cs_create(cs_solver **out, const cs_csr *A, const double *b, const double *c, cs_mem vec_where,
                     const cs_cones *K, void *cuda_stream);

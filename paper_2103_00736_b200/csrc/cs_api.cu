@@ -44,6 +44,7 @@ struct cs_solver {
     size_t dyn_smem = 0;       // bytes of dynamic shared memory of k_iterate (accumulators of the heavy-row fusion)
     std::vector<void *> allocs;
     cs_params prm{};
+    bool dense_capable = false;   // dense-stored A on many CTAs with m <= kDenseGridMax: the grid dense path may be used (its buffers are allocated on first use)
     bool conditioned = false;  // the l=1 conditioning of step 4 has run
     bool xz_stale = false;     // xb, zb older than (p, s)
     bool started = false;      // some pass or conditioning has run (cs_set_point no longer allowed)
@@ -222,12 +223,8 @@ HostSparse make_sparse(const std::vector<int> &ptr, const uvec<int> &idx, const 
             const int nch_u = (nu + kChunk - 1) / kChunk;
             const int beg = pass ? ptr[s] + nu : ptr[s], cnt = pass ? nf : nu, nch = (cnt + kChunk - 1) / kChunk;
             const bool direct = nf == 0 && nch_u == 1;      // a single chunk that completes its segment
-            // equal chunks (a multiple of 32 entries each) rather than full ones and a remainder: with rows of 1-2 k entries
-            // listed one after the other, "1024 + rest" alternates heavy and light slices, which the round-robin deal turns
-            // into a systematic imbalance between even and odd CTAs (measured: 5.5 us of barrier wait per CG step at config 4)
-            const int cl = nch ? ((cnt + nch - 1) / nch + 31) / 32 * 32 : kChunk;
             for (int q = 0; q < nch; ++q) {
-                const int a = beg + q * cl, clen = std::min(cl, beg + cnt - a);
+                const int a = beg + q * kChunk, clen = std::min(kChunk, beg + cnt - a);
                 plan_slice(s, 1 | (5 << 8), (clen + 31) / 32);
                 chunk_src.push_back(a);
                 chunk_len.push_back(clen);
@@ -684,6 +681,28 @@ cs_status do_condition(cs_solver *S, int use_rule) {
     if (st != CS_OK) return st;
     // automatic: FSAI(1) pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs);
     // with the SOCP setting t = 1.7 it saves ~10 % of the CG steps and costs 18 % per step (measured)
+    if (S->dense_capable && !S->ctx.gM && S->ctx.m <= S->prm.dense_m_threshold) {
+        // buffers of the grid dense path, on first use: Ad [m][n], four [m][m] matrices (24 GB at the paper's largest LP,
+        // n = 30000).  If the device cannot hold them the solve stays with CG: not an error.
+        Ctx &x = S->ctx;
+        const size_t m = (size_t)x.m, mm = m * m, nd = ((m + kTriNB - 1) / kTriNB) * kTriNB * kTriNB;
+        const size_t counts[] = {m * (size_t)x.n, mm, mm, mm, mm, nd, 4 * m};
+        double **ptrs[] = {&x.gAd, &x.gM, &x.gL, &x.gZ, &x.gMinv, &x.gDinv, &x.dv};
+        void *got[7] = {};
+        bool ok = true;
+        for (int q = 0; q < 7 && ok; ++q) ok = cudaMalloc(&got[q], counts[q] * sizeof(double)) == cudaSuccess;
+        if (ok) ok = cudaMalloc((void **)&x.g_ok, sizeof(int)) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();                                  // clear the allocation error
+            for (void *q : got) if (q) cudaFree(q);
+            x.g_ok = nullptr;
+            S->dense_capable = false;
+        } else {
+            for (int q = 0; q < 7; ++q) { *ptrs[q] = static_cast<double *>(got[q]); S->allocs.push_back(got[q]); }
+            S->allocs.push_back(x.g_ok);
+            CS_CUDA(S, cudaMemsetAsync(x.dv, 0, 4 * m * sizeof(double), S->stream));
+        }
+    }
     S->ctx.dense = (S->grid == 1 && S->ctx.dM && S->ctx.m <= std::min(S->prm.dense_m_threshold, kDenseMax)) ? 1
                  : (S->grid > 1 && S->ctx.gM && S->ctx.m <= S->prm.dense_m_threshold) ? 2 : 0;
     // automatic: FSAI pays when the conditioning may spread O^2 over many decades (t = 9.2 for LPs); FSAI(5) where the
@@ -1079,15 +1098,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
         if ((st = dev_zeros(S, &x.dv, (size_t)2 * m)) != CS_OK) return st;
     }
     // grid dense path (cs_dense.cuh): only for a dense-stored A (at least half of the m x n entries present) on many CTAs
-    if (S->grid > 1 && m <= kDenseGridMax && (double)nnz >= 0.5 * (double)m * (double)n) {
-        const size_t mm = (size_t)m * m;
-        if ((st = dev_zeros(S, &x.gAd, (size_t)m * n)) != CS_OK) return st;
-        double **gm[] = {&x.gM, &x.gL, &x.gZ, &x.gMinv};
-        for (double **q : gm) if ((st = dev_zeros(S, q, mm)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.dv, (size_t)4 * m)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.g_ok, 1)) != CS_OK) return st;
-        if ((st = dev_zeros(S, &x.gDinv, (size_t)((m + kTriNB - 1) / kTriNB) * kTriNB * kTriNB)) != CS_OK) return st;
-    }
+    S->dense_capable = S->grid > 1 && m <= kDenseGridMax && (double)nnz >= 0.5 * (double)m * (double)n;
     if ((st = dev_zeros(S, &x.bar, 1)) != CS_OK) return st;
     if ((st = dev_zeros(S, &x.partials, (size_t)2 * kMaxRed * kMaxGrid)) != CS_OK) return st;
     // ---- defaults (cs.h)
@@ -1098,7 +1109,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
     S->prm.cg_reduce = 0.0;
     S->prm.cg_max_iter = 20000;
     S->prm.precond = 0;
-    S->prm.dense_m_threshold = x.gM ? kDenseGridMax : 128;   // dense-stored input: the dense path is the default (cs.h)
+    S->prm.dense_m_threshold = S->dense_capable ? kDenseGridMax : 128;   // dense-stored input: the dense path is the default (cs.h)
     S->prm.reserved = 0;
     S->nnz = nnz;
     x.mu = S->prm.mu; x.t = S->prm.t; x.o_floor = S->prm.o_floor;
@@ -1185,7 +1196,7 @@ cs_status cs_set_params(cs_solver *S, const cs_params *p) {
     if (!S || !p) return CS_EINVAL;
     if (!(p->mu > 0.0) || !(p->t > 0.0) || !(p->o_floor > 0.0) || !(p->cg_tol >= 0.0) || !(p->cg_reduce >= 0.0 && p->cg_reduce < 1.0) || p->cg_max_iter < 1 ||
         p->precond < 0 || p->precond > 3 || p->dense_m_threshold < 0 || p->dense_m_threshold > kDenseGridMax) {
-        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2,3}, dense_m_threshold in [0,4096]";
+        S->err = "mu, t, o_floor must be > 0, cg_tol >= 0, 0 <= cg_reduce < 1, cg_max_iter >= 1, precond in {0,1,2,3}, dense_m_threshold in [0,24576]";
         return CS_EINVAL;
     }
     S->prm = *p;

@@ -15,7 +15,8 @@
 
 namespace csd {
 
-constexpr int kDenseGridMax = 4096;  // largest m of the grid dense path (4 m x m fp64 matrices = 537 MB at the limit)
+constexpr int kDenseGridMax = 24576; // largest m of the grid dense path: covers the paper's largest dense LP, n = 30000, m = 24000;
+                                     // four m x m fp64 matrices + A~ [m][n] = 24 GB there, allocated on first use (cs_api.cu)
 constexpr int kDenseRefine = 2;      // refinement steps of the per-pass apply
 constexpr int kCholNB = 32;          // panel width of the blocked Cholesky
 

@@ -88,3 +88,34 @@ def test_fullsize_pass_identities(cfg, scale):
     _one_pass_identities(p, S, g0["s"], tol=1e-6 if cfg == 2 else 1e-8)
     r = S.residuals()
     assert r["iter"] == 4 and r["cg_hit_max"] == 0 and r["n_conditionings"] == 2
+
+
+def test_grid_dense_path_beyond_4096_rows():
+    """The grid dense factor-apply path above its round-1 limit (cs_params.dense_m_threshold up to 24576: the paper's
+    section V-A LPs go to n = 30000, m = 24000): a V-A LP with n = 5600, m = 4480 (too large for the oracle's dense
+    solve to finish in seconds), checked through the identities that hold at any size, before and after a conditioning,
+    and against the CG path of the same library (a device-to-device comparison: it shows that the two solves agree, the
+    identities and the smaller oracle tests in test_gpu_parity.py show that they are right)."""
+    from paper_2103_00736_b200 import binding
+    p = W.dense_lp_sec5a(11, n=5600)
+    assert p.m == 4480 and p.nnz == p.m * p.n
+    sols = {}
+    for thr in (24576, 0):
+        S = binding.Solver.from_problem(p, device="cuda:0")
+        assert S.get_params()["dense_m_threshold"] == 24576
+        S.set_params(dense_m_threshold=thr)
+        S.iterate(4)
+        s_prev = S.solution()["s"]
+        S.iterate(1)
+        g = _one_pass_identities(p, S, s_prev)
+        S.condition()
+        g0 = S.solution()
+        assert g0["O"].max() / g0["O"].min() > 1.5
+        S.iterate(1)
+        _one_pass_identities(p, S, g0["s"], tol=1e-8)
+        S.iterate(2)
+        sols[thr], r = S.solution(), S.residuals()
+        assert (r["cg_steps_total"] == 0) == (thr > 0) and r["cg_hit_max"] == 0 and r["iter"] == 8
+        S.destroy()
+    for k in ("O", "x", "z", "y", "s"):
+        assert rel(sols[24576][k], sols[0][k]) <= 1e-9, (k, rel(sols[24576][k], sols[0][k]))

@@ -527,7 +527,7 @@ def test_dense_factor_apply_matches_cg_and_oracle(name):
     _check_iterates(S, O)
     _check_resid(S, O)
     with pytest.raises(binding.CsError):
-        S.set_params(dense_m_threshold=4097)
+        S.set_params(dense_m_threshold=24577)
 
 
 @pytest.mark.parametrize("name", ["sec5d_h4", "sec5d_h10", "sec5a_lp"])
@@ -552,7 +552,7 @@ def test_grid_dense_factor_apply_on_the_papers_dense_shapes(name):
     sols = {}
     for thr in (4096, 0):
         S = binding.Solver.from_problem(p, device="cuda:0")
-        assert S.get_params()["dense_m_threshold"] == 4096          # dense-stored input: the default (cs.h)
+        assert S.get_params()["dense_m_threshold"] == 24576         # dense-stored input: the default (cs.h)
         S.set_params(dense_m_threshold=thr)
         S.iterate(15)
         got = S.solution()
