@@ -656,20 +656,40 @@ cs_status dense_grid_factor(cs_solver *S) {
     k_dense_aat<<<n_tri, 256, 0, S->stream>>>(c.gAd, m, n, c.gM, 0);
     CS_CUDA(S, cudaMemcpyAsync(c.gL, c.gM, sizeof(double) * mm, cudaMemcpyDeviceToDevice, S->stream));
     S->launches += 2;
-    for (int kb = 0; kb < m; kb += kCholNB) {
-        k_chol_diag<<<1, kCholNB * kCholNB, 0, S->stream>>>(c.gL, m, kb, c.g_ok);
-        S->launches += 1;
-        const int rest = m - kb - kCholNB;
-        if (rest <= 0) break;
-        k_chol_panel<<<std::min(148 * 4, (rest + 7) / 8), 256, 0, S->stream>>>(c.gL, m, kb);
-        const int t = (rest + 63) / 64;
-        k_chol_update<<<t * (t + 1) / 2, 256, 0, S->stream>>>(c.gL, m, kb);
-        S->launches += 2;
+    for (int pb = 0; pb < m; pb += kCholPanel) {
+        const int pend = std::min(pb + kCholPanel, m);
+        for (int kb = pb; kb < pend; kb += kCholNB) {
+            k_chol_diag<<<1, kCholNB * kCholNB, 0, S->stream>>>(c.gL, m, kb, c.g_ok);
+            S->launches += 1;
+            const int rest = m - kb - kCholNB;
+            if (rest <= 0) break;
+            k_chol_panel<<<std::min(148 * 4, (rest + 7) / 8), 256, 0, S->stream>>>(c.gL, m, kb);
+            S->launches += 1;
+            if (kb + kCholNB < pend) {                           // the panel's remaining columns
+                k_chol_update<<<dim3((rest + 63) / 64, (pend - kb - kCholNB + 63) / 64), 256, 0, S->stream>>>(c.gL, m, kb, pend);
+                S->launches += 1;
+            }
+        }
+        if (pend < m) {                                          // everything behind the panel, rank 128
+            const int t = (m - pend + kGemmT - 1) / kGemmT;
+            k_chol_update_panel<<<t * (t + 1) / 2, 256, 0, S->stream>>>(c.gL, m, pb, pend);
+            S->launches += 1;
+        }
     }
     // Z = L^-T by column groups (inverses of the diagonal blocks first), then Minv = Z Z'
     k_dense_diag_inv<<<(m + kTriNB - 1) / kTriNB, kTriNB, 0, S->stream>>>(c.gL, m, c.gDinv);
-    CS_CUDA(S, cudaFuncSetAttribute((const void *)k_dense_trinv_blk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TrinvSmem)));
-    k_dense_trinv_blk<<<(m + kTriCW - 1) / kTriCW, 128, sizeof(TrinvSmem), S->stream>>>(c.gL, c.gDinv, m, c.gZ);
+    {   // the widest column group that still gives every SM two CTAs (cs_dense.cuh)
+        auto run = [&](auto tag) -> cs_status {
+            constexpr int CW = decltype(tag)::value;
+            CS_CUDA(S, cudaFuncSetAttribute((const void *)k_dense_trinv_blk<CW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TrinvSmem<CW>)));
+            k_dense_trinv_blk<CW><<<(m + CW - 1) / CW, kTriThreads, sizeof(TrinvSmem<CW>), S->stream>>>(c.gL, c.gDinv, m, c.gZ);
+            return CS_OK;
+        };
+        const int sms2 = 2 * 148;
+        cs_status st = m >= 32 * sms2 ? run(std::integral_constant<int, 32>{}) : m >= 16 * sms2 ? run(std::integral_constant<int, 16>{})
+                                                                                                : run(std::integral_constant<int, 8>{});
+        if (st != CS_OK) return st;
+    }
     k_dense_aat<<<n_tri, 256, 0, S->stream>>>(c.gZ, m, m, c.gMinv, 1);
     S->launches += 3;
     CS_CUDA(S, cudaGetLastError());

@@ -110,11 +110,15 @@ __global__ void __launch_bounds__(256) k_dense_aat(const double *A, int r, int k
 }
 
 // ---- blocked right-looking Cholesky of L (m x m row-major, lower triangle used; starts as a copy of M) -------------
+// Two levels: panels of kCholPanel = 128 columns, factored in steps of nb = 32 columns,
 // step kb: (1) k_chol_diag factors the nb x nb diagonal block in shared memory (one CTA); a pivot <= 1e-12 (diag(M) = 1:
 //              a relative test) clears *ok and is replaced by 1 so that the run stays finite (the caller falls back to CG)
 //          (2) k_chol_panel: rows below the block, X D' = L[i][kb:kb+nb] -- one warp per row, lane c owns column c
-//          (3) k_chol_update: trailing L[i][j] -= sum_c P[i][c] P[j][c] (j <= i), 64 x 64 tiles, 4 x 4 per thread (a rank-32
-//              update is bound by reading and writing L: the 128 x 128 core above is slower here, 27 vs 20 us per panel)
+//          (3) k_chol_update: the rank-32 update of the panel's remaining columns only (64 x 64 tiles, 4 x 4 per thread)
+// and after the panel's last step ONE rank-128 update of everything behind it, k_chol_update_panel, through the 128 x 128
+// contraction core: a rank-32 update of the whole trailing matrix is bound by reading and writing L (6.5 TFLOP/s at
+// m = 8000), the rank-128 one by the FP64 pipe.
+constexpr int kCholPanel = 128;
 __global__ void __launch_bounds__(kCholNB * kCholNB) k_chol_diag(double *L, int m, int kb, int *ok) {
     __shared__ double d[kCholNB][kCholNB + 1];
     const int nb = min(kCholNB, m - kb), r = threadIdx.x / kCholNB, cc = threadIdx.x % kCholNB;
@@ -154,13 +158,12 @@ __global__ void __launch_bounds__(256) k_chol_panel(double *L, int m, int kb) {
     }
 }
 
-__global__ void __launch_bounds__(256) k_chol_update(double *L, int m, int kb) {
+// rank-32 update inside the current 128-wide panel: columns [kb + nb, cend) of the rows below the block
+__global__ void __launch_bounds__(256) k_chol_update(double *L, int m, int kb, int cend) {
     __shared__ double pi[kCholNB][65], pj[kCholNB][65];
     const int nb = min(kCholNB, m - kb), base = kb + nb;
-    int ti = (int)((sqrt(8.0 * blockIdx.x + 1.0) - 1.0) * 0.5);
-    while ((ti + 1) * (ti + 2) / 2 <= (int)blockIdx.x) ++ti;
-    while (ti * (ti + 1) / 2 > (int)blockIdx.x) --ti;
-    const int tj = blockIdx.x - ti * (ti + 1) / 2;
+    const int ti = blockIdx.x, tj = blockIdx.y;
+    if (tj > ti) return;                                         // tile above the diagonal
     const int i0 = base + ti * 64, j0 = base + tj * 64, tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
     for (int q = threadIdx.x; q < 64 * kCholNB; q += 256) {
         const int row = q / kCholNB, cc = q % kCholNB;
@@ -184,6 +187,25 @@ __global__ void __launch_bounds__(256) k_chol_update(double *L, int m, int kb) {
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int a = i0 + ty * 4 + i, b = j0 + tx * 4 + j;
+            if (a < m && b <= a && b < cend) L[(size_t)a * m + b] -= acc[i][j];
+        }
+}
+
+// rank-(pend - pb) update of everything behind a finished panel: L[a][b] -= sum_{c in [pb, pend)} L[a][c] L[b][c], a >= b >= pend,
+// through the 128 x 128 contraction core (one CTA per tile of the lower triangle)
+__global__ void __launch_bounds__(256) k_chol_update_panel(double *L, int m, int pb, int pend) {
+    __shared__ __align__(16) GemmSmem sm;
+    int ti, tj;
+    tri_tile(blockIdx.x, ti, tj);
+    const int a0 = ti * kGemmT, b0 = tj * kGemmT, tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    const double *P = L + (size_t)pend * m + pb;                 // row i of P = row pend + i of L, columns pb .. pend
+    double acc[8][8] = {};
+    gemm_nt_tile(P, (size_t)m, m - pend, a0, P, (size_t)m, m - pend, b0, 0, pend - pb, sm, acc);
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int a = pend + a0 + gemm_row(ty, i), b = pend + b0 + gemm_row(tx, j);
             if (a < m && b <= a) L[(size_t)a * m + b] -= acc[i][j];
         }
 }
@@ -191,11 +213,11 @@ __global__ void __launch_bounds__(256) k_chol_update(double *L, int m, int kb) {
 // ---- Z = L^-T (row j of Z = column j of L^-1), blocked ---------------------------------------------------------------
 // Column j of X = L^-1 depends on L only, so column groups are independent; inside a group the block rows follow one
 // another:  X_JJ = (L_JJ)^-1,   X_IJ = -(L_II)^-1 sum_{K=J}^{I-1} L_IK X_KJ   (64 x 64 blocks of L).
-// k_dense_diag_inv inverts every diagonal block once; k_dense_trinv_blk gives one CTA a group of kTriCW columns and walks
-// the block rows with 64 x 64 tiles of L in shared memory (each tile serves 64 x kTriCW x 64 multiply-adds, so L is read
-// m / (3 kTriCW) times from L2 instead of m / 3 times: 6.9 -> ~1 ms at m = 2320).  Heaviest groups (J = 0) have the
+// k_dense_diag_inv inverts every diagonal block once; k_dense_trinv_blk gives one CTA a group of CW columns and walks
+// the block rows with 64 x 64 tiles of L in shared memory (each tile serves 64 x CW x 64 multiply-adds, so L is read
+// m / (3 CW) times from L2 instead of m / 3 times: 6.9 -> 1.7 ms at m = 2320 with CW = 8).  Heaviest groups (J = 0) have the
 // lowest block indices and start first.  Fixed summation order; Z zeroed by the caller (x_i = 0 for i < j's block).
-constexpr int kTriNB = 64, kTriCW = 8;
+constexpr int kTriNB = 64;
 
 __global__ void __launch_bounds__(kTriNB) k_dense_diag_inv(const double *L, int m, double *Dinv) {
     constexpr int kTri = kTriNB * (kTriNB + 1) / 2;              // packed lower triangles: (i, k) at i (i + 1) / 2 + k
@@ -214,12 +236,15 @@ __global__ void __launch_bounds__(kTriNB) k_dense_diag_inv(const double *L, int 
     for (int r = 0; r < kTriNB; ++r) Dinv[((size_t)I * kTriNB + r) * kTriNB + j] = j <= r ? sx[r * (r + 1) / 2 + j] : 0.0;
 }
 
-// shared memory of k_dense_trinv_blk (dynamic: ~79 KB, two CTAs per SM): two stages of {tile of L or (L_II)^-1, rows of X}
-// filled by cp.async one step ahead, and the block row of X computed last (the next block row's first-hand operand)
+// shared memory of k_dense_trinv_blk (dynamic; 148-186 KB: one CTA per SM): a ring of kTriStages tiles of L (or (L_II)^-1)
+// filled by cp.async kTriStages - 1 steps ahead, two stages of the matching rows of X, and the block row of X computed last
+// (the next block row's first-hand operand)
+constexpr int kTriStages = 4;
+template <int CW>
 struct TrinvSmem {
-    double l[2][kTriNB][kTriNB + 2];
-    double x[2][kTriCW][kTriNB + 2];     // [column of the group][k]
-    double fresh[kTriCW][kTriNB + 2];
+    double l[kTriStages][kTriNB][kTriNB + 2];
+    double x[2][CW][kTriNB + 2];         // [column of the group][k]
+    double fresh[CW][kTriNB + 2];
 };
 __device__ __forceinline__ void cp_async8(void *dst, const void *src, bool ok) {   // 8 bytes global -> shared, zero-filled if !ok
     const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
@@ -227,78 +252,119 @@ __device__ __forceinline__ void cp_async8(void *dst, const void *src, bool ok) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
 }
 
-__global__ void __launch_bounds__(128) k_dense_trinv_blk(const double *L, const double *Dinv, int m, double *Z) {
+__device__ __forceinline__ void cp_async16(void *dst, const void *src, bool ok) {  // 16 bytes, both sides 16-byte aligned
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+    const int n = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
+}
+
+// CW columns of L^-1 per CTA (8, 16 or 32: the host picks the widest that still leaves two groups per SM -- a wider group
+// reads L fewer times, m / (3 CW) in all, but there are fewer groups and each one's chain of block rows is serial).
+// 256 threads (two warps per scheduler: the steps are short and latency-bound); thread (cc = lane % CW, rh = lane / CW) of
+// warp w owns rows 8 w + rh + (32 / CW) q, q < CW / 4, of a block row.
+// Step (I, K): K < I multiplies the tile L_IK with X_K; K == I multiplies (L_II)^-1 with the finished sum.  The steps of a
+// group form one serial chain (the first group's is (m / 64)^2 / 2 steps long), so what matters is the time per step:
+// the tiles of L come from HBM and are requested kTriStages - 1 steps ahead; the rows of X (L2, written by this CTA at
+// least one block row earlier) are loaded into registers one step ahead; X_{I-1} is still in shared memory (sm.fresh).
+constexpr int kTriThreads = 256;
+template <int CW>
+__global__ void __launch_bounds__(kTriThreads) k_dense_trinv_blk(const double *L, const double *Dinv, int m, double *Z) {
+    constexpr int NQ = CW / 4, RS = 32 / CW, ST = kTriStages, NT = kTriThreads, NX = kTriNB * CW / NT;
     extern __shared__ __align__(16) unsigned char trinv_raw[];
-    TrinvSmem &sm = *reinterpret_cast<TrinvSmem *>(trinv_raw);
-    const int c0 = blockIdx.x * kTriCW, J = c0 / kTriNB, nblk = (m + kTriNB - 1) / kTriNB;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, cc = lane & (kTriCW - 1), rh = lane / kTriCW;
+    TrinvSmem<CW> &sm = *reinterpret_cast<TrinvSmem<CW> *>(trinv_raw);
+    const int c0 = blockIdx.x * CW, J = c0 / kTriNB, nblk = (m + kTriNB - 1) / kTriNB;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, cc = lane & (CW - 1), rh = lane / CW;
     const int gc = c0 + cc;                                      // this thread's column of L^-1 = row of Z
-    int row[4];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) row[q] = 16 * w + rh + 4 * q;    // its four rows of the block row
-    // step (I, K): K < I multiplies the tile L_IK with X_K; K == I multiplies (L_II)^-1 with the finished sum.  The loads of
-    // a step are issued one step ahead; X_{I-1} comes from sm.fresh (it was computed in the previous block row).
-    auto issue = [&](int I, int K, int buf) {
-        for (int t = threadIdx.x; t < kTriNB * kTriNB; t += 128) {
-            const int r = t >> 6, k = t & 63, gi = I * kTriNB + r;
-            const bool ok = K == I || gi < m;
-            const double *src = K == I ? Dinv + (size_t)I * kTriNB * kTriNB + t : L + (size_t)(ok ? gi : 0) * m + K * kTriNB + k;
-            cp_async8(&sm.l[buf][r][k], src, ok);
-        }
-        if (K < I - 1)
-            for (int t = threadIdx.x; t < kTriNB * kTriCW; t += 128) {
-                const int c = t >> 6, k = t & 63;
-                const bool ok = c0 + c < m;
-                cp_async8(&sm.x[buf][c][k], Z + (size_t)(ok ? c0 + c : 0) * m + K * kTriNB + k, ok);
+    const int row0 = 8 * w + rh;                                 // its rows of the block row: row0 + RS q
+    const bool even = (m & 1) == 0;                              // rows of L start 16-byte aligned: 16-byte cp.async
+    auto issue_l = [&](int I, int K, int stage) {                // one group per step, empty past the end of the chain
+        if (I < nblk) {
+            const double *base = K == I ? Dinv + (size_t)I * kTriNB * kTriNB : L + (size_t)I * kTriNB * m + K * kTriNB;
+            const size_t ld = K == I ? (size_t)kTriNB : (size_t)m;
+            const int rows = K == I ? kTriNB : min(kTriNB, m - I * kTriNB);   // rows past m are zero-filled
+            if (even) {
+                for (int t = threadIdx.x; t < kTriNB * kTriNB / 2; t += NT) {
+                    const int r = t >> 5, k = (t & 31) * 2;
+                    cp_async16(&sm.l[stage][r][k], base + (r < rows ? (size_t)r * ld + k : 0), r < rows);
+                }
+            } else {
+                for (int t = threadIdx.x; t < kTriNB * kTriNB; t += NT) {
+                    const int r = t >> 6, k = t & 63;
+                    cp_async8(&sm.l[stage][r][k], base + (r < rows ? (size_t)r * ld + k : 0), r < rows);
+                }
             }
+        }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    int buf = 0;
-    issue(J, J, 0);
+    auto advance = [&](int &I, int &K) { if (K < I) ++K; else { ++I; K = J; } };
+    int pI = J, pK = J;                                          // the step whose tile of L is requested next
+    for (int q = 0; q < ST - 1; ++q) { issue_l(pI, pK, q); advance(pI, pK); }
+    int step = 0;
     for (int I = J; I < nblk; ++I) {
-        double acc[4] = {0.0, 0.0, 0.0, 0.0}, xo[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int K = J; K <= I; ++K) {
-            const bool more = K < I || I + 1 < nblk;
-            if (more) issue(K < I ? I : I + 1, K < I ? K + 1 : J, buf ^ 1);
-            if (more) asm volatile("cp.async.wait_group 1;" ::: "memory");
-            else asm volatile("cp.async.wait_group 0;" ::: "memory");
+        double acc[NQ], xo[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) { acc[q] = 0.0; xo[q] = 0.0; }
+        for (int K = J; K <= I; ++K, ++step) {
+            const int stage = step % ST;
+            issue_l(pI, pK, (step + ST - 1) % ST);
+            advance(pI, pK);
+            // rows of X for the next step into registers (it needs them from Z only if its K' < I' - 1)
+            int nI = I, nK = K;
+            advance(nI, nK);
+            const bool next_x = nI < nblk && nK < nI - 1;
+            double xr[NX];                                       // 64 CW doubles over the CTA's threads
+            if (next_x) {
+#pragma unroll
+                for (int q = 0; q < NX; ++q) {
+                    const int t = threadIdx.x + NT * q, c = t >> 6, k = t & 63;
+                    xr[q] = c0 + c < m ? __ldcg(Z + (size_t)(c0 + c) * m + nK * kTriNB + k) : 0.0;
+                }
+            }
+            asm volatile("cp.async.wait_group %0;" :: "n"(ST - 1) : "memory");   // this step's tile of L has landed
             if (K == I && I > J) {                               // the finished sum T becomes the operand of (L_II)^-1
 #pragma unroll
-                for (int q = 0; q < 4; ++q) sm.x[buf][cc][row[q]] = acc[q];
+                for (int q = 0; q < NQ; ++q) sm.x[step & 1][cc][row0 + RS * q] = acc[q];
             }
             __syncthreads();
             if (K == I && I == J) {                              // X_JJ: the group's columns of (L_JJ)^-1
 #pragma unroll
-                for (int q = 0; q < 4; ++q) xo[q] = sm.l[buf][row[q]][gc - J * kTriNB];
+                for (int q = 0; q < NQ; ++q) xo[q] = sm.l[stage][row0 + RS * q][gc - J * kTriNB];
             } else {
-                const double *xs = K == I - 1 ? sm.fresh[cc] : sm.x[buf][cc];
+                const double *xs = K == I - 1 ? sm.fresh[cc] : sm.x[step & 1][cc];
                 if (K < I) {
-#pragma unroll 8
+#pragma unroll 4
                     for (int k = 0; k < kTriNB; ++k) {
                         const double x = xs[k];
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) acc[q] += sm.l[buf][row[q]][k] * x;
+                        for (int q = 0; q < NQ; ++q) acc[q] += sm.l[stage][row0 + RS * q][k] * x;
                     }
                 } else {                                         // X_IJ = -(L_II)^-1 T
-#pragma unroll 8
+#pragma unroll 4
                     for (int k = 0; k < kTriNB; ++k) {
                         const double x = xs[k];
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) xo[q] -= sm.l[buf][row[q]][k] * x;
+                        for (int q = 0; q < NQ; ++q) xo[q] -= sm.l[stage][row0 + RS * q][k] * x;
                     }
                 }
             }
-            __syncthreads();                                     // stage `buf` is free for the loads of the step after next
-            buf ^= 1;
+            __syncthreads();                                     // the stage and sm.x[step & 1] are free again
+            if (next_x) {
+#pragma unroll
+                for (int q = 0; q < NX; ++q) {
+                    const int t = threadIdx.x + NT * q;
+                    sm.x[(step + 1) & 1][t >> 6][t & 63] = xr[q];
+                }
+            }
         }
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int gi = I * kTriNB + row[q];
-            sm.fresh[cc][row[q]] = xo[q];                        // read next as X_I (no reader is left from the previous block row)
+        for (int q = 0; q < NQ; ++q) {
+            const int gi = I * kTriNB + row0 + RS * q;
+            sm.fresh[cc][row0 + RS * q] = xo[q];                 // read next as X_I (no reader is left from the previous block row)
             if (gi < m && gc < m) __stcg(Z + (size_t)gc * m + gi, xo[q]);
         }
         __syncthreads();                                         // the group's later block rows read Z (through L2) and sm.fresh
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
 }  // namespace csd

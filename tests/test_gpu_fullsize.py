@@ -90,15 +90,17 @@ def test_fullsize_pass_identities(cfg, scale):
     assert r["iter"] == 4 and r["cg_hit_max"] == 0 and r["n_conditionings"] == 2
 
 
-def test_grid_dense_path_beyond_4096_rows():
-    """The grid dense factor-apply path above its round-1 limit (cs_params.dense_m_threshold up to 24576: the paper's
-    section V-A LPs go to n = 30000, m = 24000): a V-A LP with n = 5600, m = 4480 (too large for the oracle's dense
-    solve to finish in seconds), checked through the identities that hold at any size, before and after a conditioning,
-    and against the CG path of the same library (a device-to-device comparison: it shows that the two solves agree, the
-    identities and the smaller oracle tests in test_gpu_parity.py show that they are right)."""
+@pytest.mark.parametrize("n", [6000, 12000])
+def test_grid_dense_path_beyond_4096_rows(n):
+    """The grid dense factor-apply path above m = 4096 (cs_params.dense_m_threshold up to 24576: the paper's section V-A
+    LPs go to n = 30000, m = 24000): V-A LPs with m = 4800 and m = 9600 (too large for the oracle's dense solve to
+    finish in seconds; the two sizes take the 16- and the 32-column variant of the triangular inverse), checked through the
+    identities that hold at any size, before and after a conditioning, and against the CG path of the same library (a
+    device-to-device comparison: it shows that the two solves agree, the identities and the smaller oracle tests in
+    test_gpu_parity.py show that they are right)."""
     from paper_2103_00736_b200 import binding
-    p = W.dense_lp_sec5a(11, n=5600)
-    assert p.m == 4480 and p.nnz == p.m * p.n
+    p = W.dense_lp_sec5a(11, n=n)
+    assert p.m == 4 * n // 5 and p.nnz == p.m * p.n
     sols = {}
     for thr in (24576, 0):
         S = binding.Solver.from_problem(p, device="cuda:0")
@@ -114,8 +116,12 @@ def test_grid_dense_path_beyond_4096_rows():
         S.iterate(1)
         _one_pass_identities(p, S, g0["s"], tol=1e-8)
         S.iterate(2)
-        sols[thr], r = S.solution(), S.residuals()
+        sols[thr], r = (g, S.solution()), S.residuals()
         assert (r["cg_steps_total"] == 0) == (thr > 0) and r["cg_hit_max"] == 0 and r["iter"] == 8
         S.destroy()
+    for k in ("x", "z", "y", "s"):                               # before the conditioning: protocol (i)
+        assert rel(sols[24576][0][k], sols[0][0][k]) <= 1e-9, (k, rel(sols[24576][0][k], sols[0][0][k]))
+    # after a conditioning from each run's OWN iterate the rule o = |x| / |z| (step 7) amplifies the 1e-11 the two solves
+    # differ by (protocol ii-b; measured 3.4e-9 on O at m = 9600): looser here, on a device-to-device check
     for k in ("O", "x", "z", "y", "s"):
-        assert rel(sols[24576][k], sols[0][k]) <= 1e-9, (k, rel(sols[24576][k], sols[0][k]))
+        assert rel(sols[24576][1][k], sols[0][1][k]) <= 5e-8, (k, rel(sols[24576][1][k], sols[0][1][k]))
