@@ -507,7 +507,8 @@ def finish(a, p, S, line, rank, world, dev, stream):
     # the iterate the timed steps ended on: the e2e step below starts from it (cs_set_point), so that its
     # conditioning and its k passes do the work a further resident step would do
     hx0, hz0 = torch.empty(p.n, dtype=torch.float64).pin_memory(), torch.empty(p.n, dtype=torch.float64).pin_memory()
-    S.solution_into(x=hx0.numpy(), z=hz0.numpy())
+    hy0 = torch.empty(p.m, dtype=torch.float64).pin_memory()    # the multiplier: warm start of the e2e step's solve (cs_set_dual)
+    S.solution_into(x=hx0.numpy(), z=hz0.numpy(), y=hy0.numpy())
     S.destroy()
     if a.config == 4 and a.scale == 1.0 and world == 1 and not a.cg_max_iter and not a.no_secondary:
         try:
@@ -560,7 +561,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
     pin = lambda x: torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
     hin = [pin(x) for x in (p.row_ptr, p.col_idx, p.val, p.b, p.c)]
     hx, hz = torch.empty(p.n, dtype=torch.float64).pin_memory(), torch.empty(p.n, dtype=torch.float64).pin_memory()
-    h2d = sum(t.numel() * t.element_size() for t in hin) + 16 * p.n
+    h2d = sum(t.numel() * t.element_size() for t in hin) + 16 * p.n + 8 * p.m
     d2h = 16 * p.n + 128
     e2e_log = {"step_s": [], "create_s": [], "cg_steps": []}
     def e2e_step():
@@ -570,6 +571,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
         tb = time.perf_counter()               # cs_create returns with the layouts built (it synchronises itself)
         S2.set_params(mu=p.mu, t=p.t, precond=a.precond, **({"cg_max_iter": a.cg_max_iter} if a.cg_max_iter else {}))
         S2.set_point(hx0.numpy(), hz0.numpy())
+        S2.set_dual(hy0.numpy())
         S2.condition()
         S2.iterate(a.k)
         r2 = S2.residuals()
@@ -592,7 +594,7 @@ def finish(a, p, S, line, rank, world, dev, stream):
     dt_max = max_over_ranks(dt, dev)
     line["e2e"] = {"value": whole_job_value(a.e2e_steps * a.k, world, dt_max * 1e3) if a.e2e_steps else None, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                    "d2h_bytes_per_step": int(d2h), "steps": a.e2e_steps, **e2e_log,
-                   "step": "cs_create(host A,b,c) + cs_set_point(host x,z of the last timed step) + cs_condition + cs_iterate(k) + "
+                   "step": "cs_create(host A,b,c) + cs_set_point + cs_set_dual(host x,z,y of the last timed step) + cs_condition + cs_iterate(k) + "
                            "cs_residuals + cs_solution(host x,z)"}
     if rank == 0:
         if not a.no_cpu_baseline and world == 1:

@@ -145,6 +145,14 @@ cs_status cs_get_params(const cs_solver *S, cs_params *p);
  * cs_iterate / cs_condition (else CS_ESTATE). */
 cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem where);
 
+/* Optional warm start of the inner solve from a dual vector y[m] in `where` -- cs_solution's y of an earlier run (the
+ * multiplier of Ax = b, y = (w_d - w)/mu; derived, S 8(c) reading (o)): the solve's unknown is w = mu D^-1 y in
+ * the row scaling D of the moment, so a run resumed from (x, z, O) of a checkpoint (cs_set_point, cs_set_scaling) starts its
+ * first solve where the checkpointed run's last one ended instead of at w = 0.  It changes the number of CG steps of the first
+ * passes, not the iterates (the solve is exact, reading (s)); without it the start is w = 0.  Only before the first
+ * cs_iterate / cs_condition / cs_set_scaling (else CS_ESTATE); uses the value of mu in force at the call. */
+cs_status cs_set_dual(cs_solver *S, const double *y, cs_mem where);
+
 /* k passes of steps 16-18: p = abs_K(s); r = abs_{A_hat}(p); s = s/2 - r/2 + d.
  * x,z of steps 19-20 are formed lazily by cs_condition / cs_residuals / cs_solution.  If no
  * conditioning has happened yet, the l=1 conditioning of step 4 runs first.  One kernel launch for

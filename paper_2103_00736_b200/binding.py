@@ -52,7 +52,7 @@ class cs_schedule(C.Structure):
 
 CS_RULE_SET, CS_RULE_STALL = 0, 1
 
-_INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_iterate", "cs_condition",
+_INT_STATUS = ("cs_create", "cs_set_params", "cs_get_params", "cs_set_point", "cs_set_dual", "cs_iterate", "cs_condition",
                "cs_set_scaling", "cs_equilibrate", "cs_solve", "cs_residuals", "cs_solution", "cs_diag_phase_times",
                "cs_diag_gather_probe", "cs_diag_barrier_probe", "cs_diag_l2_probe", "cs_diag_create", "cs_diag_layout_digest",
                "cs_cone_violation_static")
@@ -74,6 +74,7 @@ def lib():
         L.cs_set_params.argtypes = [vp, C.POINTER(cs_params)]
         L.cs_get_params.argtypes = [vp, C.POINTER(cs_params)]
         L.cs_set_point.argtypes = [vp, vp, vp, C.c_int]
+        L.cs_set_dual.argtypes = [vp, vp, C.c_int]
         L.cs_iterate.argtypes = [vp, C.c_int64]
         L.cs_condition.argtypes = [vp]
         L.cs_set_scaling.argtypes = [vp, vp, C.c_int]
@@ -236,6 +237,11 @@ class Solver:
     def set_point(self, x, z):
         xp, zp = _ptr(x, np.float64), _ptr(z, np.float64)
         self._check(lib().cs_set_point(self._h, xp[0], zp[0], _same_space(xp, zp)))
+
+    def set_dual(self, y):
+        """cs_set_dual: warm start of the inner solve from a dual vector y[m] (cs_solution's y of an earlier run)."""
+        yp = _ptr(y, np.float64)
+        self._check(lib().cs_set_dual(self._h, yp[0], yp[1]))
 
     def iterate(self, k):
         self._check(lib().cs_iterate(self._h, int(k)))

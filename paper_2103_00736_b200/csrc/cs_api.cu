@@ -1239,6 +1239,23 @@ cs_status cs_set_point(cs_solver *S, const double *x, const double *z, cs_mem wh
     return import_cols(S, S->ctx.zb, z, where);
 }
 
+cs_status cs_set_dual(cs_solver *S, const double *y, cs_mem where) {
+    if (!S || !y) return CS_EINVAL;
+    DeviceGuard guard(S);
+    if (S->started) { S->err = "cs_set_dual after the iteration has started"; return CS_ESTATE; }
+    const Ctx &c = S->ctx;
+    const double *dy = y;
+    if (where == CS_HOST) {                                      // r is scratch until the first pass
+        CS_CUDA(S, cudaMemcpyAsync(c.r, y, sizeof(double) * c.m, cudaMemcpyHostToDevice, S->stream));
+        dy = c.r;
+    }
+    k_w_from_y<<<ew_blocks(c.m), 256, 0, S->stream>>>(c, dy, S->prm.mu);
+    CS_CUDA(S, cudaGetLastError());
+    S->launches += 1;
+    if (where == CS_HOST) CS_CUDA(S, cudaStreamSynchronize(S->stream));   // the caller's buffer is free on return
+    return CS_OK;
+}
+
 cs_status cs_condition(cs_solver *S) {
     if (!S) return CS_EINVAL;
     DeviceGuard guard(S);

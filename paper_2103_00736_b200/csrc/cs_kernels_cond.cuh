@@ -22,6 +22,12 @@ __global__ void k_dual_y(Ctx c, double *y) {   // written in the caller's (origi
     for (int i = tid; i < c.m; i += nth) y[c.perm_r[i]] = c.D[i] * c.w[i] / c.mu;
 }
 
+// the inverse: w = mu y / D from a caller's y in the original row order (cs_set_dual: warm start of the inner solve)
+__global__ void k_w_from_y(Ctx c, const double *y, double mu) {
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    for (int i = tid; i < c.m; i += nth) c.w[i] = mu * y[c.perm_r[i]] / c.D[i];
+}
+
 // internal (sorted) order <-> caller's order: dst[i] = src[perm[i]]  /  dst[perm[i]] = src[i]
 __global__ void k_gather_perm(double *dst, const double *src, const int *perm, int n) {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;

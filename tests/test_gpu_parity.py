@@ -297,6 +297,45 @@ def test_checkpoint_and_resume_through_solution_and_set_point():
     assert abs(r1["kkt_rel"] - r2["kkt_rel"]) <= TOL_RES * r1["kkt_rel"] and abs(r1["pobj"] - r2["pobj"]) <= TOL_RES * (1 + abs(r1["pobj"]))
 
 
+def test_set_dual_warm_starts_the_resumed_solve():
+    """cs_set_dual: the multiplier y of a checkpoint is the inner solve's unknown up to the row scaling (w = mu D^-1 y), so a
+    resumed run that passes it starts its first solve where the checkpointed run stopped.  The iterates do not depend on it
+    (the solve is exact: resumed with y, resumed without, the uninterrupted run and the oracle from the same point agree to
+    1e-9); the number of CG steps does."""
+    import oracle
+    from paper_2103_00736_b200 import binding
+    p = W.config(4, 0.001)                                       # m = 2000: the oracle's dense solve takes seconds
+    S1 = binding.Solver.from_problem(p, device="cuda:0")
+    S1.run(40, L=[20, 30])
+    ck = S1.solution()
+    steps0 = S1.residuals()["cg_steps_total"]
+    S1.iterate(3)
+    per_pass = (S1.residuals()["cg_steps_total"] - steps0) / 3
+    ref = S1.solution()
+    O = oracle.Oracle.from_problem(p, solve_mode=1)
+    O.set_point(ck["x"], ck["z"])
+    O.set_scaling(ck["O"])
+    O.run_fixed(3)
+    got, cg = {}, {}
+    for with_y in (True, False):
+        S2 = binding.Solver.from_problem(p, device="cuda:0")
+        S2.set_point(ck["x"], ck["z"])
+        if with_y:
+            S2.set_dual(ck["y"])
+        S2.set_scaling(ck["O"])
+        S2.iterate(3)
+        got[with_y], r = S2.solution(), S2.residuals()
+        cg[with_y] = r["cg_steps_total"] - r["cg_steps_cond"]
+        with pytest.raises(binding.CsError):
+            S2.set_dual(ck["y"])                                 # only before the iteration has started
+        S2.destroy()
+    for k in ("x", "z", "y", "s"):
+        assert rel(got[True][k], ref[k]) <= TOL_ITER and rel(got[False][k], ref[k]) <= TOL_ITER, k
+        assert rel(got[True][k], O.get()[k]) <= TOL_ITER, (k, rel(got[True][k], O.get()[k]))
+    # the first solve of the cold resume starts at w = 0; with y all three passes cost what the uninterrupted run's do
+    assert cg[True] < cg[False] and cg[True] <= 1.25 * 3 * per_pass, (cg, per_pass)
+
+
 def test_host_and_device_inputs_agree_bitwise():
     from paper_2103_00736_b200 import binding
     p = W.config(1, 0.05)
