@@ -201,6 +201,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 (SOCP) block")
     ap.add_argument("--dense-n", type=int, default=10000, help="n of the section V-A dense LP block (the paper goes to 30000)")
+    ap.add_argument("--dense-only", action="store_true",
+                    help="extra mode: only the section V-A dense LP block (--dense-n) through the grid dense factor-apply path")
     ap.add_argument("--no-time-to-tol", action="store_true", help="skip the time-to-1e-4-KKT leg of the default run")
     ap.add_argument("--solve", action="store_true",
                     help="extra mode: run the paper's schedule (17)/(18) to --tol and report the time to tolerance")
@@ -240,6 +242,14 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    if a.dense_only:
+        try:
+            peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+        except Exception:
+            peak = 6650.0                                        # B200_PROFILING.md fallback
+        print(json.dumps({"dense_sec5a": dense_workload(a, dev, torch.cuda.current_stream(), peak, "sec5a", a.dense_n)}))
+        return 0
 
     t_gen = time.perf_counter()
     p = W.config(a.config, a.scale)

@@ -33,6 +33,10 @@ SHAPES = {
     "socp_plus_orthant": lambda: W.sparse_socp(18, 700, 2500, 60, 8, n_lin=1000, lo=2, hi=50),
     # Lorentz blocks of all three size classes of cone_sweep (sub-warp <= 64 < warp <= 4096 < CTA) plus orthant coordinates
     "socp_all_size_classes": lambda: _socp_with_sizes(23, 900, 150, [3, 40, 64, 65, 7, 300, 1000, 2, 4097, 33, 6000, 1, 12]),
+    # dense-stored inputs on many CTAs: the grid dense factor-apply path (csrc/cs_dense.cuh) with ragged sizes -- fewer rows
+    # than one 64-row block; an odd m that is no multiple of any tile size (8-byte copies in the triangular inverse)
+    "dense_grid_m40_wide": lambda: W.gaussian_dense_lp(24, m=40, n=400),
+    "dense_grid_m203_ragged": lambda: W.gaussian_dense_lp(25, m=203, n=261),
     "one_cta_dense_path": lambda: W.sparse_socp(19, 60, 300, 20, 6, n_lin=100, lo=2, hi=20),
     "one_cta_cg_path": lambda: W.sparse_lp(20, 400, 1300, 5),
 }
@@ -78,6 +82,8 @@ def test_shape_sweep_against_the_oracle(name):
     got = S.solution()
     for k in ("x", "z", "y", "s"):
         assert rel(got[k], mid[k]) <= 1e-9, (name, "leg 1", k, rel(got[k], mid[k]))
+    if name.startswith("dense_grid"):
+        assert S.residuals()["cg_steps_total"] == 0            # the dense path ran, not CG
     S.destroy()
     S = binding.Solver.from_problem(p, device="cuda:0")
     S.set_point(mid["x"], mid["z"])
