@@ -3,13 +3,13 @@
 // P:342-346 and V-D P:366-371).  For a dense-stored A with m <= kDenseGridMax:
 //   at every conditioning   Ad = A~ (m x n, row-major)          k_dense_scatter
 //                           M  = Ad Ad'                          k_dense_aat        (unit diagonal: A~ is row-equilibrated)
-//                           M  = L L'   (blocked, right-looking) k_chol_diag / k_chol_panel / k_chol_update
+//                           M  = L L'   (blocked, right-looking) k_chol_diag / k_chol_panel / k_chol_update / k_chol_update_panel
 //                           Z  = L^-T   (row j = column j of L^-1)  k_dense_diag_inv, k_dense_trinv_blk
 //                           Minv = Z Z' = M^-1                   k_dense_aat
 //   at every pass           w += M^-1 r by dense_apply_grid (cs_kernels.cuh): x = Minv r, then kDenseRefine steps of
 //                           iterative refinement x += Minv (r - M x) against the stored M -- dense GEMVs only.
 // All sums have a fixed order (no atomics).  fp64 throughout; plain DFMA (no tensor cores: B200's fp64 tensor rate equals
-// its vector rate and the matrices are a few thousand wide).
+// its vector rate).  Measured from m = 2320 to m = 24000 (the paper's largest LP): DESIGN.md 10.
 #pragma once
 #include "cs_device.cuh"
 
