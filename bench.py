@@ -476,7 +476,7 @@ def dense_workload(a, dev, stream, peak, kind="sec5d", n=2900):
     S.destroy()
     m, n = p.m, p.n
     us_pass = 1e3 * ms_i / (reps * 100)
-    gemv_bytes = 5 * m * m * 8 + 2 * 12 * p.nnz              # the apply + the rhs and update passes over the stored A~
+    gemv_bytes = 5 * m * m * 8 + 2 * 8 * m * n               # the apply + the rhs and update passes over the dense copy of A~
     flops = m * m * n + 1.0 * m ** 3                          # SYRK + Cholesky + L^-T + Z Z' (triangular operands), m^3 / 3 each
     S2 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     torch.cuda.synchronize()
@@ -491,7 +491,7 @@ def dense_workload(a, dev, stream, peak, kind="sec5d", n=2900):
             "ms_per_conditioning": ms_c / reps,
             "roofline_pass": {"bound": "hbm", "achieved": gemv_bytes / (us_pass * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
                               "frac": gemv_bytes / (us_pass * 1e-6) / 1e9 / peak,
-                              "bytes": "5 m^2 x 8 (M^-1, M, M^-1, M, M^-1) + 24 nnz (rhs and update passes); %d MB of matrices" % (16 * m * m // 10**6)},
+                              "bytes": "5 m^2 x 8 (M^-1, M, M^-1, M, M^-1) + 16 m n (rhs and update passes over the dense copy of A~); %d MB of matrices" % ((16 * m * m + 8 * m * n) // 10**6)},
             "roofline_factor": {"bound": "alu", "achieved": flops / (ms_c / reps * 1e-3) / 1e12, "peak": 37.2, "unit": "TFLOP/s",
                                 "frac": flops / (ms_c / reps * 1e-3) / 1e12 / 37.2, "flops": "m^2 n + m^3 (SYRK; Cholesky, L^-T, Z Z' at m^3 / 3 each)",
                                 "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 8)"},

@@ -706,11 +706,13 @@ cs_status do_condition(cs_solver *S, int use_rule) {
         // n = 30000).  If the device cannot hold them the solve stays with CG: not an error.
         Ctx &x = S->ctx;
         const size_t m = (size_t)x.m, mm = m * m, nd = ((m + kTriNB - 1) / kTriNB) * kTriNB * kTriNB;
-        const size_t counts[] = {m * (size_t)x.n, mm, mm, mm, mm, nd, 4 * m};
-        double **ptrs[] = {&x.gAd, &x.gM, &x.gL, &x.gZ, &x.gMinv, &x.gDinv, &x.dv};
-        void *got[7] = {};
+        const size_t npart = std::max<size_t>((size_t)x.n, (size_t)kMaxGrid * (kBlock / 32) * 64);   // [row ranges][n], ranges * n <= warps * 64
+        const size_t counts[] = {m * (size_t)x.n, mm, mm, mm, mm, nd, 4 * m, npart};
+        double **ptrs[] = {&x.gAd, &x.gM, &x.gL, &x.gZ, &x.gMinv, &x.gDinv, &x.dv, &x.gpart};
+        constexpr int NB = 8;
+        void *got[NB] = {};
         bool ok = true;
-        for (int q = 0; q < 7 && ok; ++q) ok = cudaMalloc(&got[q], counts[q] * sizeof(double)) == cudaSuccess;
+        for (int q = 0; q < NB && ok; ++q) ok = cudaMalloc(&got[q], counts[q] * sizeof(double)) == cudaSuccess;
         if (ok) ok = cudaMalloc((void **)&x.g_ok, sizeof(int)) == cudaSuccess;
         if (!ok) {
             cudaGetLastError();                                  // clear the allocation error
@@ -718,7 +720,7 @@ cs_status do_condition(cs_solver *S, int use_rule) {
             x.g_ok = nullptr;
             S->dense_capable = false;
         } else {
-            for (int q = 0; q < 7; ++q) { *ptrs[q] = static_cast<double *>(got[q]); S->allocs.push_back(got[q]); }
+            for (int q = 0; q < NB; ++q) { *ptrs[q] = static_cast<double *>(got[q]); S->allocs.push_back(got[q]); }
             S->allocs.push_back(x.g_ok);
             CS_CUDA(S, cudaMemsetAsync(x.dv, 0, 4 * m * sizeof(double), S->stream));
         }

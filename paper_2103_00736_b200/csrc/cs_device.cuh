@@ -146,6 +146,7 @@ struct Ctx {
     int dense;              // 0: off, 1: one-CTA factor-apply below, 2: grid path (cs_dense.cuh): gM = A~A~', gMinv = its inverse
     double *gAd, *gM, *gL, *gZ, *gMinv;   // grid dense path: [m][n], then four [m][m] row-major matrices
     double *gDinv;          // inverses of L's 64 x 64 diagonal blocks (cs_dense.cuh)
+    double *gpart;          // partial column sums of the dense update pass [row range][n] (cs_kernels.cuh dense_cols)
     int *g_ok;              // grid dense path: 0 if a Cholesky pivot failed (written by k_chol_diag)
     double *dM;             // [m][m] row-major: lower triangle incl. diagonal = Cholesky factor L, strict upper = A~A~'
     double *dMd;            // [m] diagonal of A~A~'

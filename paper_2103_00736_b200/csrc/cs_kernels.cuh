@@ -351,6 +351,74 @@ __device__ __forceinline__ void dense_apply_grid(const Ctx &c, GridCtl &gc) {
     gc.sync();
 }
 
+// The two passes over A~ of a dense-path iteration (the right-hand side and steps 17-18) read the row-major dense copy
+// Ad [m][n] that the conditioning has scattered (cs_dense.cuh) instead of the sliced sparse copies: 8 bytes per entry instead
+// of 12, contiguous vector reads instead of gathers.  Fixed summation orders.
+//   dense_rows_pair: (sum_j Ad[i][j] x[j], sum_j Ad[i][j] y[j]) per row i -> epi(i, .): one warp per row, lanes along the row
+template <class Epi>
+__device__ __forceinline__ void dense_rows_pair(const Ctx &c, const double *x, const double *y, Epi &epi) {
+    const int lane = threadIdx.x & 31, gwarp = blockIdx.x + gridDim.x * (threadIdx.x >> 5), nwarps = (gridDim.x * kBlock) >> 5;
+    const int n = c.n;
+    for (int i = gwarp; i < c.m; i += nwarps) {
+        const double *row = c.gAd + (size_t)i * n;
+        double a0 = 0.0, a1 = 0.0;
+        int j = lane;
+        for (; j + 224 < n; j += 256) {                          // 8 independent row loads in flight
+            double v[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = __ldcs(row + j + 32 * q);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { a0 += v[q] * x[j + 32 * q]; a1 += v[q] * y[j + 32 * q]; }
+        }
+        for (; j < n; j += 32) { const double v = __ldcs(row + j); a0 += v * x[j]; a1 += v * y[j]; }
+        a0 = group_reduce<32>(a0);
+        a1 = group_reduce<32>(a1);
+        if (lane == 0) { const double acc[2] = {a0, a1}; epi(i, acc, epi.pre(i)); }
+    }
+}
+//   dense_cols: sum_i Ad[i][j] w[i] per column j -> epi(j, .).  Work items (64 columns, a range of rows), one warp each, two
+//   columns per lane; the items' partial sums go through c.gpart [row range][n] and are added in range order after a barrier.
+template <class Epi>
+__device__ __forceinline__ void dense_cols(const Ctx &c, const double *w, Epi &epi, GridCtl &gc) {
+    const int lane = threadIdx.x & 31, gwarp = blockIdx.x + gridDim.x * (threadIdx.x >> 5), nwarps = (gridDim.x * kBlock) >> 5;
+    const int n = c.n, m = c.m, G = (n + 63) / 64;
+    const int nsplit = max(1, min(nwarps / G, m));               // row ranges: as many as fill the machine
+    const int per = (m + nsplit - 1) / nsplit;
+    for (int t = gwarp; t < G * nsplit; t += nwarps) {
+        const int g = t % G, rs = t / G, r0 = rs * per, r1 = min(m, r0 + per);
+        const int j0 = g * 64 + lane, j1 = j0 + 32;              // this lane's two columns
+        double a0 = 0.0, a1 = 0.0;
+        const double *col = c.gAd + (size_t)r0 * n;
+        int i = r0;
+        for (; i + 3 < r1; i += 4) {                             // 8 independent loads in flight
+            double v0[4], v1[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                v0[q] = j0 < n ? __ldcs(col + (size_t)q * n + j0) : 0.0;
+                v1[q] = j1 < n ? __ldcs(col + (size_t)q * n + j1) : 0.0;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { const double wi = w[i + q]; a0 += v0[q] * wi; a1 += v1[q] * wi; }
+            col += (size_t)4 * n;
+        }
+        for (; i < r1; ++i, col += n) {
+            const double wi = w[i];
+            if (j0 < n) a0 += __ldcs(col + j0) * wi;
+            if (j1 < n) a1 += __ldcs(col + j1) * wi;
+        }
+        if (j0 < n) __stcg(c.gpart + (size_t)rs * n + j0, a0);
+        if (j1 < n) __stcg(c.gpart + (size_t)rs * n + j1, a1);
+    }
+    gc.sync();
+    for (int j = blockIdx.x * kBlock + threadIdx.x; j < n; j += gridDim.x * kBlock) {
+        typename Epi::Pre pre = epi.pre(j);
+        double a = 0.0;
+        for (int rs = 0; rs < nsplit; ++rs) a += __ldcg(c.gpart + (size_t)rs * n + j);
+        const double acc[1] = {a};
+        epi(j, acc, pre);
+    }
+}
+
 __device__ __forceinline__ void fsaip_pass_a(const Ctx &c, int k_begin);      // cs_fsaip.cuh
 __device__ __forceinline__ double fsaip_pass_b(const Ctx &c, int k_begin);
 // r'z with z = (preconditioner) r over ALL rows, one grid reduction (start of a solve)
@@ -479,7 +547,8 @@ __device__ __forceinline__ void iterate_body(const Ctx &c, long long k_iter) {
         gc.lap(kPhCone);
         TermPair tq{c.u, c.e};
         EpiRhs eq{c.r, c.btil, 0.0, 0.0};
-        seg_reduce<2, false>(c.R, tq, eq, gc);
+        if (DENSE && c.dense == 2) dense_rows_pair(c, c.u, c.e, eq);   // the dense copy of A~ (grid dense path)
+        else seg_reduce<2, false>(c.R, tq, eq, gc);
         gc.lap(kPhRhs);
         double red[2] = {eq.qq, eq.rho};
         grid_reduce<2>(red, gc);
@@ -492,7 +561,8 @@ __device__ __forceinline__ void iterate_body(const Ctx &c, long long k_iter) {
         cg_total += cg_last;
         TermDot tw{c.w};
         EpiUpdate eu{c.s, c.g, c.p, c.chat, c.mu, 0.0};
-        seg_reduce<1, false>(c.C, tw, eu, gc);                   // steps 17-18
+        if (DENSE && c.dense == 2) dense_cols(c, c.w, eu, gc);   // steps 17-18 over the dense copy
+        else seg_reduce<1, false>(c.C, tw, eu, gc);              // steps 17-18
         gc.lap(kPhUpdate);
         double rf[1] = {eu.fp2};
         grid_reduce<1>(rf, gc);
