@@ -458,7 +458,7 @@ def dense_workload(a, dev, stream, peak, kind="sec5d", n=2900):
     """Secondary block for the paper's own dense shapes (section V-D: SOCP, K = (K_4)^(n/4), n = 2900, m = 2320, P:366-371;
     section V-A: LP, n up to 30000, m = 0.8 n) through the grid dense factor-apply path (csrc/cs_dense.cuh): time per pass (k = 100 passes per launch, schedule (18)),
     per conditioning (incl. the m x m factorisation and explicit inverse), and time to kkt_rel <= 1e-4.
-    Rooflines: the per-pass apply is 2*refine+1 = 5 dense m x m GEMVs (HBM/L2 bytes); the factorisation is fp64 FMA work
+    Rooflines: the per-pass apply is 3 dense m x m GEMVs (5 with the second refinement step; HBM/L2 bytes); the factorisation is fp64 FMA work
     against 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s."""
     import torch
     from paper_2103_00736_b200 import binding
@@ -476,7 +476,7 @@ def dense_workload(a, dev, stream, peak, kind="sec5d", n=2900):
     S.destroy()
     m, n = p.m, p.n
     us_pass = 1e3 * ms_i / (reps * 100)
-    gemv_bytes = 5 * m * m * 8 + 2 * 8 * m * n               # the apply + the rhs and update passes over the dense copy of A~
+    gemv_bytes = 3 * m * m * 8 + 2 * 8 * m * n               # the apply (3 GEMVs; 5 when a second refinement step runs) + the two passes over the dense copy of A~
     flops = m * m * n + 1.0 * m ** 3                          # SYRK + Cholesky + L^-T + Z Z' (triangular operands), m^3 / 3 each
     S2 = binding.Solver.from_problem(p, device=dev, stream=stream.cuda_stream)
     torch.cuda.synchronize()
@@ -491,7 +491,8 @@ def dense_workload(a, dev, stream, peak, kind="sec5d", n=2900):
             "ms_per_conditioning": ms_c / reps,
             "roofline_pass": {"bound": "hbm", "achieved": gemv_bytes / (us_pass * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
                               "frac": gemv_bytes / (us_pass * 1e-6) / 1e9 / peak,
-                              "bytes": "5 m^2 x 8 (M^-1, M, M^-1, M, M^-1) + 16 m n (rhs and update passes over the dense copy of A~); %d MB of matrices" % ((16 * m * m + 8 * m * n) // 10**6)},
+                              "bytes": "3 m^2 x 8 (M^-1, M, M^-1; a second refinement step, two more, runs only when the first one's residual is above 1.5e-9) "
+                                       "+ 16 m n (rhs and update passes over the dense copy of A~); %d MB of matrices" % ((16 * m * m + 8 * m * n) // 10**6)},
             "roofline_factor": {"bound": "alu", "achieved": flops / (ms_c / reps * 1e-3) / 1e12, "peak": 37.2, "unit": "TFLOP/s",
                                 "frac": flops / (ms_c / reps * 1e-3) / 1e12 / 37.2, "flops": "m^2 n + m^3 (SYRK; Cholesky, L^-T, Z Z' at m^3 / 3 each)",
                                 "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 2 x 1.965 GHz (DESIGN.md 8)"},

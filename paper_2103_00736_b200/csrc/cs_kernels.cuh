@@ -317,11 +317,16 @@ __device__ __forceinline__ void fuse_flush(const Ctx &c, double *scratch /* [kFu
     __syncthreads();
 }
 
-// Grid dense path (cs_dense.cuh): w += M^-1 r with the explicit inverse and kDenseRefine steps of iterative refinement
+// Grid dense path (cs_dense.cuh): w += M^-1 r with the explicit inverse and up to kDenseRefine steps of iterative refinement
 // against the stored M = A~A~'.  Dense GEMVs: one warp per row, lanes along the row (coalesced), butterfly reduction.
 //   x = Minv r ;  repeat: t = r - M x ; x += Minv t        (x in dv[0..m), t in dv[m..2m))
-__device__ __forceinline__ void dense_gemv_rows(const double *A, const double *v, int m, int gwarp, int nwarps, int lane,
-                                                double *out, const double *base, double sign, const double *add) {
+// The first refinement step always runs.  Its residual t measures what the explicit inverse leaves, eps0 = ||t|| / ||r||, and
+// a step shrinks the residual by about that factor again; the second step runs unless eps0^2 is already a hundred times below
+// cg_tol -- the criterion the CG path stops on (cs.h), with a margin for eps0 underestimating ||I - M Minv||.
+// dense_gemv_rows returns this thread's share of sum_i out_i^2.
+__device__ __forceinline__ double dense_gemv_rows(const double *A, const double *v, int m, int gwarp, int nwarps, int lane,
+                                                  double *out, const double *base, double sign, const double *add) {
+    double ss = 0.0;
     for (int i = gwarp; i < m; i += nwarps) {                 // out_i = (base ? base_i : 0) + sign * <A_i, v> + (add ? add_i : 0)
         const double *Ai = A + (size_t)i * m;
         double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
@@ -331,21 +336,27 @@ __device__ __forceinline__ void dense_gemv_rows(const double *A, const double *v
         }
         for (; k < m; k += 32) s0 += Ai[k] * v[k];
         const double s = group_reduce<32>((s0 + s1) + (s2 + s3));
-        if (lane == 0) out[i] = (base ? base[i] : 0.0) + sign * s + (add ? add[i] : 0.0);
+        if (lane == 0) {
+            const double o = (base ? base[i] : 0.0) + sign * s + (add ? add[i] : 0.0);
+            out[i] = o;
+            ss += o * o;
+        }
     }
+    return ss;
 }
-__device__ __forceinline__ void dense_apply_grid(const Ctx &c, GridCtl &gc) {
+__device__ __forceinline__ void dense_apply_grid(const Ctx &c, GridCtl &gc, double rr /* ||r||^2 */) {
     const int lane = threadIdx.x & 31, gwarp = blockIdx.x + gridDim.x * (threadIdx.x >> 5), nwarps = (gridDim.x * kBlock) >> 5;
     double *x = c.dv, *t = c.dv + c.m;
     dense_gemv_rows(c.gMinv, c.r, c.m, gwarp, nwarps, lane, x, nullptr, 1.0, nullptr);          // x = Minv r
     gc.sync();
     for (int it = 0; it < kDenseRefine; ++it) {
-        dense_gemv_rows(c.gM, x, c.m, gwarp, nwarps, lane, t, c.r, -1.0, nullptr);              // t = r - M x
-        gc.sync();
+        double tt[1] = {dense_gemv_rows(c.gM, x, c.m, gwarp, nwarps, lane, t, c.r, -1.0, nullptr)};   // t = r - M x
+        grid_reduce<1>(tt, gc);                                                                  // ||t||^2, and the barrier
         double *xn = c.dv + 2 * c.m + (it & 1) * c.m;                                           // ping-pong: x is read by every warp
         dense_gemv_rows(c.gMinv, t, c.m, gwarp, nwarps, lane, xn, x, 1.0, nullptr);             // x' = x + Minv t
         gc.sync();
         x = xn;
+        if (!(tt[0] > 0.01 * c.cg_tol * rr)) break;            // uniform over the grid (grid_reduce returns the same bits everywhere)
     }
     for (int i = blockIdx.x * kBlock + threadIdx.x; i < c.m; i += gridDim.x * kBlock) c.w[i] += x[i];
     gc.sync();
@@ -554,7 +565,7 @@ __device__ __forceinline__ void iterate_body(const Ctx &c, long long k_iter) {
         grid_reduce<2>(red, gc);
         gc.lap(kPhReduce);
         bool hm;
-        if (DENSE && c.dense == 2 && *c.g_ok) { dense_apply_grid(c, gc); cg_last = 0; hm = false; }   // dense factor-apply (grid)
+        if (DENSE && c.dense == 2 && *c.g_ok) { dense_apply_grid(c, gc, red[1]); cg_last = 0; hm = false; }   // dense factor-apply (grid)
         else if (DENSE && c.dense == 1 && c.sc->dense_ok) { dense_solve(c); cg_last = 0; hm = false; }   // dense factor-apply (one CTA)
         else cg_last = cg_solve(c, gc, red[1], red[0], hm);      // w = (A~A~')^{-1} (b~ - A~(p - mu c^)) = w_d - w_p
         any_max |= hm;
