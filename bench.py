@@ -197,7 +197,7 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--k", type=int, default=1, help="outer iterations per step (1 = continuous conditioning, P:313)")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the config-3 (SOCP) block")
     ap.add_argument("--dense-n", type=int, default=10000, help="n of the section V-A dense LP block (the paper goes to 30000)")

@@ -93,8 +93,9 @@ typedef struct {
  *              iterative refinement);
  *            - dense-STORED inputs (nnz >= m n / 2: the paper's own workloads, section V-A, V-D P:366-371) on
  *              many CTAs: every conditioning forms M = A~A~', its blocked Cholesky factor and the explicit inverse
- *              M^-1 = L^-T L^-1 (hand-written fp64 kernels, csrc/cs_dense.cuh); every pass is w += M^-1 r followed by two
- *              steps of iterative refinement against M -- dense matrix-vector products only.
+ *              M^-1 = L^-T L^-1 (hand-written fp64 kernels, csrc/cs_dense.cuh); every pass is w += M^-1 r followed by one
+ *              or two steps of iterative refinement against M (the second only when the first one's residual is not yet a
+ *              hundred times below cg_tol, squared) -- dense matrix-vector products only.
  *              The limit 24576 covers the paper's largest dense LP (n = 30000, m = 24000); the path's buffers
  *              (A~ as [m][n] and four m x m matrices: 24 GB there) are allocated at the first conditioning that uses it,
  *              and if the device cannot hold them the solve stays with CG (not an error).

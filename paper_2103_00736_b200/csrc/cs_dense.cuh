@@ -6,7 +6,7 @@
 //                           M  = L L'   (blocked, right-looking) k_chol_diag / k_chol_panel / k_chol_update / k_chol_update_panel
 //                           Z  = L^-T   (row j = column j of L^-1)  k_dense_diag_inv, k_dense_trinv_blk
 //                           Minv = Z Z' = M^-1                   k_dense_aat
-//   at every pass           w += M^-1 r by dense_apply_grid (cs_kernels.cuh): x = Minv r, then kDenseRefine steps of
+//   at every pass           w += M^-1 r by dense_apply_grid (cs_kernels.cuh): x = Minv r, then up to kDenseRefine steps of
 //                           iterative refinement x += Minv (r - M x) against the stored M -- dense GEMVs only.
 // All sums have a fixed order (no atomics).  fp64 throughout; plain DFMA (no tensor cores: B200's fp64 tensor rate equals
 // its vector rate).  Measured from m = 2320 to m = 24000 (the paper's largest LP): DESIGN.md 10.
@@ -17,7 +17,7 @@ namespace csd {
 
 constexpr int kDenseGridMax = 24576; // largest m of the grid dense path: covers the paper's largest dense LP, n = 30000, m = 24000;
                                      // four m x m fp64 matrices + A~ [m][n] = 24 GB there, allocated on first use (cs_api.cu)
-constexpr int kDenseRefine = 2;      // refinement steps of the per-pass apply
+constexpr int kDenseRefine = 2;      // most refinement steps of the per-pass apply (the second runs only when needed)
 constexpr int kCholNB = 32;          // panel width of the blocked Cholesky
 
 // Ad[i][j] = A~_ij from the row-major slice copy (Ad zeroed by the caller)
