@@ -127,7 +127,7 @@ typedef struct {
     int32_t cg_steps_last;  /* CG steps of the most recent solve                     */
     int32_t n_conditionings;
     int32_t cg_hit_max;     /* 1 if some solve hit cg_max_iter since the last cs_residuals */
-    int32_t reserved;
+    int32_t dense_refine2;  /* passes so far whose dense factor-apply took its second refinement step (dense_m_threshold) */
     double pres_abs, pres_rel, dres_abs, dres_rel, gap_abs, gap_rel, cone_viol_rel, kkt_rel, pobj, dobj, fp_res;
 } cs_resid;
 

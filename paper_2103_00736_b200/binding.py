@@ -36,7 +36,7 @@ class cs_params(C.Structure):
 
 class cs_resid(C.Structure):
     _fields_ = [("iter", C.c_int64), ("cg_steps_total", C.c_int64), ("cg_steps_cond", C.c_int64), ("cg_steps_last", C.c_int32),
-                ("n_conditionings", C.c_int32), ("cg_hit_max", C.c_int32), ("reserved", C.c_int32)] + \
+                ("n_conditionings", C.c_int32), ("cg_hit_max", C.c_int32), ("dense_refine2", C.c_int32)] + \
                [(k, C.c_double) for k in ("pres_abs", "pres_rel", "dres_abs", "dres_rel", "gap_abs", "gap_rel",
                                           "cone_viol_rel", "kkt_rel", "pobj", "dobj", "fp_res")]
 

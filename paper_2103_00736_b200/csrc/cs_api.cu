@@ -1302,7 +1302,7 @@ cs_status cs_residuals(cs_solver *S, cs_resid *out) {
     CS_CUDA(S, cudaMemsetAsync(&S->ctx.sc->cg_hit_max, 0, sizeof(int), S->stream));
     CS_CUDA(S, cudaStreamSynchronize(S->stream));
     out->iter = h.iter; out->cg_steps_total = h.cg_steps_total; out->cg_steps_cond = h.cg_steps_cond; out->cg_steps_last = h.cg_steps_last;
-    out->n_conditionings = h.n_cond; out->cg_hit_max = h.cg_hit_max; out->reserved = 0;
+    out->n_conditionings = h.n_cond; out->cg_hit_max = h.cg_hit_max; out->dense_refine2 = h.dense_refine2;
     out->pres_abs = h.resid[0]; out->pres_rel = h.resid[1]; out->dres_abs = h.resid[2]; out->dres_rel = h.resid[3];
     out->gap_abs = h.resid[4]; out->gap_rel = h.resid[5]; out->cone_viol_rel = h.resid[6]; out->kkt_rel = h.resid[7];
     out->pobj = h.resid[8]; out->dobj = h.resid[9]; out->fp_res = h.resid[10];

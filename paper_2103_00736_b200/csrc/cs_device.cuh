@@ -116,6 +116,7 @@ struct Scalars {            // device-resident state scalars (read back only by 
     long long iter, cg_steps_total, cg_steps_cond;
     int cg_steps_last, n_cond, cg_hit_max, dense_ok;   // dense_ok: the Cholesky factor of the current scaling is usable
     double fp_res2;         // ||s_new - s||^2 of the last pass
+    int dense_refine2;      // passes whose dense apply needed the second refinement step (grid dense path)
     unsigned long long phase_ns[8];  // time spent per phase id (kPh*), measured by CTA 0 between grid barriers
 };
 

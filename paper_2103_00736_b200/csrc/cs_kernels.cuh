@@ -357,6 +357,7 @@ __device__ __forceinline__ void dense_apply_grid(const Ctx &c, GridCtl &gc, doub
         gc.sync();
         x = xn;
         if (!(tt[0] > 0.01 * c.cg_tol * rr)) break;            // uniform over the grid (grid_reduce returns the same bits everywhere)
+        if (it == 0 && blockIdx.x == 0 && threadIdx.x == 0) c.sc->dense_refine2 += 1;
     }
     for (int i = blockIdx.x * kBlock + threadIdx.x; i < c.m; i += gridDim.x * kBlock) c.w[i] += x[i];
     gc.sync();

@@ -614,6 +614,34 @@ def test_grid_dense_factor_apply_on_the_papers_dense_shapes(name):
         S.destroy()
 
 
+def test_dense_apply_takes_its_second_refinement_step_when_the_inverse_needs_it():
+    """The grid dense path refines x = M^-1 r once, and a second time only if the first step's residual says so
+    (eps0^2 > cg_tol / 100, csrc/cs_kernels.cuh dense_apply_grid; counted in cs_resid.dense_refine2).  A V-A LP whose
+    columns are scaled over four decades makes A~A~' ill-conditioned enough for the second step; the iterates still match the
+    oracle (dense Cholesky + refinement) to 1e-9.  The well-conditioned original never needs it."""
+    import oracle
+    import scipy.sparse as sp
+    from paper_2103_00736_b200 import binding
+    p0 = W.dense_lp_sec5a(13, n=400)
+    rng = np.random.default_rng(5)
+    A = sp.csr_matrix(p0.csr() @ sp.diags(10.0 ** rng.uniform(-2.0, 2.0, p0.n)))
+    A.sort_indices()
+    xdot = np.abs(rng.standard_normal(p0.n))
+    p = W.Problem(name="sec5a_cols_scaled", m=p0.m, n=p0.n, row_ptr=A.indptr.astype(np.int32), col_idx=A.indices.astype(np.int32),
+                  val=A.data.copy(), b=A @ xdot, c=p0.c, n_lin=p0.n, soc_size=p0.soc_size, x0=p0.x0, y0=p0.y0, s0=p0.s0,
+                  t=p0.t, L_first=p0.L_first, L_every=p0.L_every)
+    for q, expect_second in ((p0, False), (p, True)):
+        O = oracle.Oracle.from_problem(q, solve_mode=1)
+        O.run(15)
+        S = binding.Solver.from_problem(q, device="cuda:0")
+        S.iterate(15)
+        r = S.residuals()
+        assert r["cg_steps_total"] == 0
+        assert (r["dense_refine2"] > 0) == expect_second, (q.name, r["dense_refine2"])
+        _check_iterates(S, O)
+        S.destroy()
+
+
 def test_dense_path_falls_back_to_cg_on_a_rank_deficient_matrix():
     """A duplicated row makes A~A~' singular: the Cholesky pivot test fails and the pass's solve goes through CG (which
     handles the consistent singular system, DESIGN.md 3 reading (r)); the run still converges to the same optimum."""
