@@ -617,10 +617,12 @@ cs_status layout_device(cs_solver *S, const cs_csr *A, const double *b, const do
 }
 
 cs_status launch_coop(cs_solver *S, const void *fn, void **args) {
-    const size_t dyn = fn == (const void *)k_iterate ? S->dyn_smem : 0;
+    // k_iterate_dense runs the same CG (fused column pass included) when a Cholesky pivot fails, so it gets the same shared memory
+    const bool iter = fn == (const void *)k_iterate || fn == (const void *)k_iterate_dense;
+    const size_t dyn = iter ? S->dyn_smem : 0;
     // the shared-memory carve-out is a property of the FUNCTION, shared by every handle of the process: a handle without
     // fused rows must not inherit the 100 KB another handle asked for (its gathers would lose 100 KB of L1)
-    if (fn == (const void *)k_iterate)
+    if (iter)
         CS_CUDA(S, cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, dyn ? kFuseCarveoutPct : (int)cudaSharedmemCarveoutDefault));
     CS_CUDA(S, cudaLaunchCooperativeKernel(fn, dim3(S->grid), dim3(kBlock), args, dyn, S->stream));
     S->launches += 1;
@@ -1099,7 +1101,7 @@ static cs_status create_impl(cs_solver *S, const cs_csr *A, const double *b, con
                              (const void *)k_equilibrate, (const void *)k_barrier_probe};
     S->dyn_smem = x.n_fa + x.n_fb > 0 ? (size_t)kFuseSmem : 0;
     for (const void *k : kernels) {
-        const size_t dyn = k == (const void *)k_iterate ? S->dyn_smem : 0;
+        const size_t dyn = k == (const void *)k_iterate || k == (const void *)k_iterate_dense ? S->dyn_smem : 0;
         if (dyn) {
             CS_CUDA(S, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
             // < 96 KB: ask for the 100 KB carve-out, so that the gathers keep ~128 KB of L1 (they collapse below ~90 KB,

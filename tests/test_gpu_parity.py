@@ -662,6 +662,31 @@ def test_dense_path_falls_back_to_cg_on_a_rank_deficient_matrix():
     S.destroy()
 
 
+def test_grid_dense_path_falls_back_to_cg_with_fused_rows():
+    """The same on many CTAs, with rows long enough (4,200 entries) for the heavy-row fusion: a duplicated row makes the
+    blocked Cholesky refuse the factor (g_ok = 0) and the pass's solve runs the CG of k_iterate_dense -- fused column pass
+    and its shared-memory accumulators included.  The iterates match the CG-only run of the same handle type."""
+    import scipy.sparse as sp
+    from paper_2103_00736_b200 import binding
+    p = W.gaussian_dense_lp(33, m=120, n=4200)
+    A = p.csr()
+    A2 = sp.vstack([A, A[7]]).tocsr()
+    A2.sort_indices()
+    b2 = np.concatenate([p.b, p.b[7:8]])
+    sols = {}
+    for thr in (24576, 0):
+        S = binding.Solver(p.m + 1, p.n, A2.indptr.astype(np.int32), A2.indices.astype(np.int32), A2.data.copy(), b2, p.c,
+                           p.n_lin, p.soc_size)
+        S.set_params(dense_m_threshold=thr)
+        S.run(30, L=[10, 20])
+        r = S.residuals()
+        assert r["cg_steps_total"] > 0 and r["cg_hit_max"] == 0 and np.isfinite(r["kkt_rel"])
+        sols[thr] = S.solution()
+        S.destroy()
+    for k in ("x", "z", "s", "O"):
+        assert rel(sols[24576][k], sols[0][k]) <= 1e-7, (k, rel(sols[24576][k], sols[0][k]))
+
+
 # ------------------------------------------------------------------ S 8(f) rows 2, 3: schedules, fixed equilibration
 @pytest.mark.parametrize("name", ["lp_scaled", "mixed_cones", "cfg4_zipf"])
 def test_equilibrate_matches_oracle_ruiz(name):
