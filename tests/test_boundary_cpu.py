@@ -28,6 +28,15 @@ def test_library_exports_every_declared_symbol():
     assert ctypes.sizeof(binding.cs_params) == 56
     assert ctypes.sizeof(binding.cs_resid) == 3 * 8 + 4 * 4 + 11 * 8
     assert ctypes.sizeof(binding.cs_csr) == 56 and ctypes.sizeof(binding.cs_cones) == 24
+    # ... and the field names, in order (the binding reads the structs by position)
+    for cname, cls in (("cs_params", binding.cs_params), ("cs_resid", binding.cs_resid), ("cs_schedule", binding.cs_schedule)):
+        body = re.search(r"typedef struct \{([^}]*)\}\s*" + cname + r"\s*;", header, flags=re.S).group(1)
+        names = []
+        for decl in body.split(";"):
+            decl = decl.strip()
+            if decl:
+                names += [v.strip() for v in re.sub(r"^\w+\s+", "", decl).split(",")]
+        assert names == [k for k, _ in cls._fields_], (cname, names)
 
 
 def test_hot_kernel_sass_is_what_design_md_says():
